@@ -1,0 +1,338 @@
+"""paper_0908_4421_b200 -- Python binding of libimrtgp (include/imrtgp.h).
+
+Argument marshalling only: every step of the optimiser (dose SpMV, penalty / residual / objective reduction,
+transpose SpMV, projection, Armijo line search, stop test -- PAPER.md:51-114) runs in the CUDA kernels of
+csrc/.  PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback: if the shared
+library cannot be loaded, importing the binding's functions raises.
+
+Module-level functions carry the C names (imrt_plan_create, imrt_plan_run_iters, ...) and take torch CUDA
+tensors where the C-ABI takes device pointers; `Plan` is a small convenience wrapper around them.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+__all__ = ["Plan", "ImrtError", "lib", "Params", "STATUS_NAMES", "STOP_NAMES", "EXPORTS"]
+
+STATUS_NAMES = ("OK", "INVALID_ARG", "BAD_CSR", "BAD_STRUCTURE", "WORKSPACE_TOO_SMALL", "CUDA_ERROR",
+                "UNSUPPORTED_DEVICE", "UNSUPPORTED", "BAD_X", "NOT_READY")
+STOP_NAMES = ("MAX_ITERS", "TOLERANCE", "STATIONARY", "LINESEARCH_STALLED")
+DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
+
+# every symbol include/imrtgp.h declares
+EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
+           "imrt_plan_eval", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
+           "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_last_error", "imrt_plan_destroy",
+           "imrt_version")
+
+
+class ImrtError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        self.status = status
+        self.status_name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        super().__init__("libimrtgp: %s: %s" % (self.status_name, message))
+
+
+class Params(ctypes.Structure):
+    """imrt_params."""
+    _fields_ = [("eps", ctypes.c_double), ("alpha", ctypes.c_double), ("lambda0", ctypes.c_double),
+                ("max_ls", ctypes.c_int32), ("max_iters", ctypes.c_int32), ("driver", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
+
+
+_lib = None
+_P = ctypes.c_void_p
+
+
+def lib() -> ctypes.CDLL:
+    """Load libimrtgp.so (building it in-tree first if it is missing or older than its sources)."""
+    global _lib
+    if _lib is None:
+        try:
+            path = _build.build()
+        except Exception as exc:  # no nvcc and no prebuilt library: there is nothing to fall back to
+            if not os.path.exists(_build.LIB):
+                raise ImportError("libimrtgp.so is not built and could not be built (%s); run "
+                                  "`python -m paper_0908_4421_b200.build` where nvcc is available" % exc) from exc
+            path = _build.LIB
+        L = ctypes.CDLL(path)
+        i64, i32, dbl = ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+        L.imrt_workspace_bytes.argtypes = [i64, i64, i64, i32, i32, ctypes.POINTER(ctypes.c_size_t)]
+        L.imrt_plan_create.argtypes = [ctypes.POINTER(_P), i64, i64, i64, _P, _P, _P, _P, i32, _P, _P, _P, _P,
+                                       ctypes.POINTER(Params), _P, ctypes.c_size_t, _P]
+        L.imrt_plan_set_x.argtypes = [_P, _P]
+        L.imrt_plan_run_iters.argtypes = [_P, i32]
+        L.imrt_plan_run_to_tol.argtypes = [_P, dbl, i32]
+        L.imrt_plan_eval.argtypes = [_P, _P, _P, _P, _P, ctypes.POINTER(dbl)]
+        L.imrt_plan_get_x.argtypes = [_P, _P]
+        L.imrt_plan_get_dose.argtypes = [_P, _P]
+        L.imrt_plan_dvh.argtypes = [_P, _P, i32, _P, _P]
+        L.imrt_plan_get_trace.argtypes = [_P, ctypes.POINTER(i32), ctypes.POINTER(i32), _P, _P, _P, _P, i32]
+        L.imrt_plan_get_counters.argtypes = [_P, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+        L.imrt_plan_get_info.argtypes = [_P, _P, i32, _P, _P, _P]
+        L.imrt_plan_launch_pass.argtypes = [_P, i32, i32]
+        L.imrt_plan_destroy.argtypes = [_P]
+        L.imrt_last_error.argtypes = [_P]
+        L.imrt_last_error.restype = ctypes.c_char_p
+        L.imrt_version.argtypes = []
+        L.imrt_version.restype = ctypes.c_char_p
+        for name in EXPORTS:
+            if name not in ("imrt_last_error", "imrt_version"):
+                getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _check(status: int, plan=None):
+    if status != 0:
+        msg = lib().imrt_last_error(plan)
+        raise ImrtError(status, msg.decode() if msg else "")
+
+
+def _dptr(t, dtype=None, n=None):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError("expected dtype %s, got %s" % (dtype, t.dtype))
+    if n is not None and t.numel() < n:
+        raise ValueError("tensor too small: %d < %d" % (t.numel(), n))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _hptr(a):
+    return a.ctypes.data_as(_P)
+
+
+# ------------------------------------------------------------------------------------------------ C names
+def imrt_version() -> str:
+    return lib().imrt_version().decode()
+
+
+def imrt_workspace_bytes(n_v: int, n_b: int, nnz: int, n_structures: int, max_iters: int) -> int:
+    out = ctypes.c_size_t(0)
+    _check(lib().imrt_workspace_bytes(n_v, n_b, nnz, n_structures, max_iters, ctypes.byref(out)))
+    return out.value
+
+
+def imrt_plan_create(n_v, n_b, nnz, row_ptr, col_idx, val, structure_id, t_under, t_over, w_under, w_over, params: Params,
+                     workspace, stream_ptr: int = 0):
+    """Returns the opaque plan handle (a ctypes.c_void_p).  Tensors are borrowed: keep them alive."""
+    import torch
+    tabs = [np.ascontiguousarray(a, dtype=np.float32) for a in (t_under, t_over, w_under, w_over)]
+    n_s = tabs[0].shape[0]
+    handle = _P()
+    st = lib().imrt_plan_create(ctypes.byref(handle), n_v, n_b, nnz, _dptr(row_ptr, torch.int32, n_v + 1),
+                                _dptr(col_idx, torch.int32, nnz), _dptr(val, torch.float32, nnz),
+                                _dptr(structure_id, torch.uint8, n_v), n_s, _hptr(tabs[0]), _hptr(tabs[1]), _hptr(tabs[2]),
+                                _hptr(tabs[3]), ctypes.byref(params), _dptr(workspace), workspace.numel() * workspace.element_size(),
+                                ctypes.c_void_p(stream_ptr))
+    _check(st, None)
+    return handle
+
+
+def imrt_plan_set_x(plan, x0):
+    import torch
+    _check(lib().imrt_plan_set_x(plan, _dptr(x0, torch.float32)), plan)
+
+
+def imrt_plan_run_iters(plan, n_iters: int):
+    _check(lib().imrt_plan_run_iters(plan, n_iters), plan)
+
+
+def imrt_plan_run_to_tol(plan, delta: float, max_iters: int):
+    _check(lib().imrt_plan_run_to_tol(plan, delta, max_iters), plan)
+
+
+def imrt_plan_eval(plan, x, d=None, r=None, g=None) -> float:
+    import torch
+    obj = ctypes.c_double(0.0)
+    _check(lib().imrt_plan_eval(plan, _dptr(x, torch.float32), _dptr(d, torch.float32), _dptr(r, torch.float32),
+                                _dptr(g, torch.float32), ctypes.byref(obj)), plan)
+    return obj.value
+
+
+def imrt_plan_get_x(plan, x):
+    import torch
+    _check(lib().imrt_plan_get_x(plan, _dptr(x, torch.float32)), plan)
+
+
+def imrt_plan_get_dose(plan, d):
+    import torch
+    _check(lib().imrt_plan_get_dose(plan, _dptr(d, torch.float32)), plan)
+
+
+def imrt_plan_dvh(plan, pcts, n_structures: int):
+    pc = np.ascontiguousarray(pcts, dtype=np.float64)
+    dp = np.empty((n_structures, pc.shape[0]), np.float64)
+    mean = np.empty(n_structures, np.float64)
+    _check(lib().imrt_plan_dvh(plan, _hptr(pc), pc.shape[0], _hptr(dp), _hptr(mean)), plan)
+    return dp, mean
+
+
+@dataclass
+class Trace:
+    n_iters: int
+    stop_reason: int
+    obj: np.ndarray        # float64 [n+1]
+    lam: np.ndarray        # float64 [n]
+    n_trials: np.ndarray   # int32 [n]
+    step_sq: np.ndarray    # float64 [n]
+
+
+def imrt_plan_get_trace(plan, capacity: int) -> Trace:
+    n = ctypes.c_int32(0)
+    reason = ctypes.c_int32(0)
+    obj = np.zeros(capacity + 1, np.float64)
+    lam = np.zeros(max(capacity, 1), np.float64)
+    ntr = np.zeros(max(capacity, 1), np.int32)
+    ssq = np.zeros(max(capacity, 1), np.float64)
+    _check(lib().imrt_plan_get_trace(plan, ctypes.byref(n), ctypes.byref(reason), _hptr(obj), _hptr(lam), _hptr(ntr),
+                                     _hptr(ssq), capacity), plan)
+    k = min(n.value, capacity)
+    return Trace(n.value, reason.value, obj[:k + 1].copy(), lam[:k].copy(), ntr[:k].copy(), ssq[:k].copy())
+
+
+def imrt_plan_get_counters(plan):
+    f, t = ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(lib().imrt_plan_get_counters(plan, ctypes.byref(f), ctypes.byref(t)), plan)
+    return f.value, t.value
+
+
+INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "fwd_smem", "tr_smem", "g_slots", "nonempty_rows", "n_sm", "x_in_smem")
+
+
+def imrt_plan_get_info(plan, rowT_ptr=None, colT=None, valT=None) -> dict:
+    import torch
+    info = np.zeros(10, np.int64)
+    _check(lib().imrt_plan_get_info(plan, _hptr(info), 10, _dptr(rowT_ptr, torch.int32), _dptr(colT, torch.int32),
+                                    _dptr(valT, torch.float32)), plan)
+    return dict(zip(INFO_KEYS, (int(v) for v in info)))
+
+
+def imrt_plan_launch_pass(plan, kind: int, n_repeat: int):
+    _check(lib().imrt_plan_launch_pass(plan, kind, n_repeat), plan)
+
+
+def imrt_plan_destroy(plan):
+    _check(lib().imrt_plan_destroy(plan))
+
+
+# ------------------------------------------------------------------------------------------------ convenience
+class Plan:
+    """Owns the device copies of a problem, the workspace and the plan handle.
+
+    `prob` is any object with the fields n_v, n_b, row_ptr, col, val, sid, t_under, t_over, w_under, w_over,
+    eps, alpha, lambda0, max_ls (numpy arrays / scalars); arrays may also already be torch CUDA tensors.
+    """
+
+    def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_0908_4421_b200 needs a CUDA device (sm_100a); there is no CPU path")
+        lib()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+
+        def dev(a, dt):
+            if isinstance(a, torch.Tensor):
+                return a.to(device=self.device, dtype=dt).contiguous()
+            return torch.from_numpy(np.ascontiguousarray(a)).to(device=self.device, dtype=dt)
+
+        self.n_v, self.n_b = int(prob.n_v), int(prob.n_b)
+        self.row_ptr = dev(prob.row_ptr, torch.int32)
+        self.nnz = int(self.row_ptr[-1].item()) if self.n_v > 0 else 0
+        self.col = dev(prob.col, torch.int32) if self.nnz else torch.zeros(4, dtype=torch.int32, device=self.device)
+        self.val = dev(prob.val, torch.float32) if self.nnz else torch.zeros(4, dtype=torch.float32, device=self.device)
+        self.sid = dev(prob.sid, torch.uint8)
+        self.n_structures = int(len(prob.t_under))
+        self.max_iters = int(max_iters)
+        self.params = Params(float(prob.eps), float(prob.alpha), float(prob.lambda0), int(prob.max_ls), self.max_iters,
+                             int(driver), 0)
+        nbytes = imrt_workspace_bytes(self.n_v, self.n_b, self.nnz, self.n_structures, self.max_iters)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.handle = imrt_plan_create(self.n_v, self.n_b, self.nnz, self.row_ptr, self.col, self.val, self.sid,
+                                       prob.t_under, prob.t_over, prob.w_under, prob.w_over, self.params, self.workspace,
+                                       self.stream.cuda_stream)
+
+    # -- the calls of the C-ABI
+    def set_x(self, x0):
+        import torch
+        if not isinstance(x0, torch.Tensor):
+            x0 = torch.from_numpy(np.ascontiguousarray(x0, dtype=np.float32))
+        self._x0 = x0.to(device=self.device, dtype=torch.float32).contiguous()
+        imrt_plan_set_x(self.handle, self._x0)
+
+    def run_iters(self, n: int):
+        imrt_plan_run_iters(self.handle, int(n))
+
+    def run_to_tol(self, delta: float, max_iters: int):
+        imrt_plan_run_to_tol(self.handle, float(delta), int(max_iters))
+
+    def eval(self, x, want_d=True, want_r=True, want_g=True):
+        """(d, r, g, G) at x -- tensors on the device (None where not wanted)."""
+        import torch
+        if not isinstance(x, torch.Tensor):
+            x = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32))
+        x = x.to(device=self.device, dtype=torch.float32).contiguous()
+        d = torch.empty(self.n_v, dtype=torch.float32, device=self.device) if want_d else None
+        r = torch.empty(self.n_v, dtype=torch.float32, device=self.device) if want_r else None
+        g = torch.empty(self.n_b, dtype=torch.float32, device=self.device) if want_g else None
+        G = imrt_plan_eval(self.handle, x, d, r, g)
+        return d, r, g, G
+
+    def get_x(self):
+        import torch
+        x = torch.empty(self.n_b, dtype=torch.float32, device=self.device)
+        imrt_plan_get_x(self.handle, x)
+        return x
+
+    def get_dose(self):
+        import torch
+        d = torch.empty(self.n_v, dtype=torch.float32, device=self.device)
+        imrt_plan_get_dose(self.handle, d)
+        return d
+
+    def dvh(self, pcts):
+        return imrt_plan_dvh(self.handle, pcts, self.n_structures)
+
+    def trace(self) -> Trace:
+        return imrt_plan_get_trace(self.handle, self.max_iters)
+
+    def counters(self):
+        return imrt_plan_get_counters(self.handle)
+
+    def info(self) -> dict:
+        return imrt_plan_get_info(self.handle)
+
+    def transpose_csr(self):
+        """(rowT_ptr, colT, valT) copies of the library-built D^T."""
+        import torch
+        rp = torch.empty(self.n_b + 1, dtype=torch.int32, device=self.device)
+        c = torch.empty(max(self.nnz, 1), dtype=torch.int32, device=self.device)
+        v = torch.empty(max(self.nnz, 1), dtype=torch.float32, device=self.device)
+        imrt_plan_get_info(self.handle, rp, c, v)
+        return rp, c[:self.nnz], v[:self.nnz]
+
+    def launch_pass(self, kind: int, n_repeat: int = 1):
+        imrt_plan_launch_pass(self.handle, int(kind), int(n_repeat))
+
+    def close(self):
+        if getattr(self, "handle", None):
+            imrt_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

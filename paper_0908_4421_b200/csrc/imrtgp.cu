@@ -1,0 +1,846 @@
+// imrtgp.cu -- host side of libimrtgp: the C-ABI of include/imrtgp.h, plan construction (validation, explicit
+// transpose, row blocks, nnz ranges), the three loop drivers and the read-backs.  Kernels live in kernels.cuh.
+//
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -shared -Xcompiler -fPIC (see ../build.py).
+#include "../../include/imrtgp.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <cub/device/device_radix_sort.cuh>
+
+#include "dvh.cuh"
+#include "kernels.cuh"
+
+using namespace imrt;
+
+// ------------------------------------------------------------------------------------------------ errors
+static thread_local std::string g_create_error;
+
+struct imrt_plan {
+    DevPlan P;
+    imrt_params prm;
+    cudaStream_t stream;
+    int n_sm;
+    size_t smem_bytes;
+    int grid_p;                       // persistent kernel grid
+    bool has_x;
+    int64_t n_blk, n_nonempty, n_skipped;
+    // borrowed inputs
+    const int32_t* row_ptr;
+    const uint8_t* sid;
+    // workspace pieces the host needs by name
+    float* r_scratch;
+    float* g_scratch;
+    float* d_scratch;
+    int* rowT_ptr_w;
+    int* colT_w;
+    float* valT_w;
+    DvhWork dvh;
+    // conditional graph (driver 0)
+    cudaGraph_t graph;
+    cudaGraphExec_t graph_exec;
+    std::string err;
+};
+
+static imrt_status fail(imrt_plan* p, imrt_status s, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->err = buf; else g_create_error = buf;
+    return s;
+}
+
+#define CUDA_TRY(plan, expr)                                                                                       \
+    do {                                                                                                           \
+        cudaError_t e_ = (expr);                                                                                   \
+        if (e_ != cudaSuccess)                                                                                     \
+            return fail(plan, IMRT_STATUS_CUDA_ERROR, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__,  \
+                        __LINE__);                                                                                 \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------ workspace
+namespace {
+
+struct Bump {                           // the same walk sizes the workspace and places the arrays
+    unsigned char* base;
+    size_t off;
+    template <typename T>
+    T* take(size_t n) {
+        off = (off + 255) & ~(size_t)255;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+struct Bounds {
+    int64_t max_blk, max_meta, max_ranges, max_slots, nnz_pad;
+    size_t sort_temp;
+};
+
+Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
+    Bounds b;
+    b.max_blk = 2 * (nnz / (CHUNK_F - 3) + 1) + 2 * (n_v / MAXROWS_F + 1) + n_v / 32 + 4;
+    b.max_meta = n_v + b.max_blk * (META_HDR + 1 + 3) + 8;
+    b.max_ranges = 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
+    b.max_slots = n_b + b.max_ranges + 4;
+    b.nnz_pad = ((nnz + 3) & ~(int64_t)3) + 8;
+    b.sort_temp = (size_t)(16 << 20) + (size_t)nnz;
+    return b;
+}
+
+struct Layout {
+    State* st;
+    float4* table;
+    int4* blk;
+    uint32_t* rowmeta;
+    int* cta_blk;
+    int* rowT_ptr;
+    int* colT;
+    float* valT;
+    TrRange* tr_range;
+    int* rowslot_ptr;
+    float* xbuf[2];
+    float* g;
+    float* rbuf[2];
+    double* Gpart[2];
+    double* gslot[2];
+    double* tr_obj;
+    double* tr_lambda;
+    double* tr_step_sq;
+    int* tr_trials;
+    float* r_scratch;
+    float* g_scratch;
+    float* d_scratch;
+    int* flags;
+    DvhWork dvh;
+    // build scratch
+    unsigned int* keysA;
+    unsigned int* keysB;
+    unsigned int* valsA;
+    unsigned int* valsB;
+    void* sort_temp;
+    size_t total;
+};
+
+Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, int max_iters) {
+    const Bounds B = bounds_for(n_v, n_b, nnz);
+    Bump w{static_cast<unsigned char*>(base), 0};
+    Layout L;
+    L.st = w.take<State>(1);
+    L.table = w.take<float4>(MAX_STRUCTURES);
+    L.blk = w.take<int4>(B.max_blk);
+    L.rowmeta = w.take<uint32_t>(B.max_meta);
+    L.cta_blk = w.take<int>(1024 + 1);
+    L.rowT_ptr = w.take<int>(n_b + 1);
+    L.colT = w.take<int>(B.nnz_pad);
+    L.valT = w.take<float>(B.nnz_pad);
+    L.tr_range = w.take<TrRange>(B.max_ranges);
+    L.rowslot_ptr = w.take<int>(n_b + 1);
+    for (int i = 0; i < 2; ++i) L.xbuf[i] = w.take<float>(n_b + 4);
+    L.g = w.take<float>(n_b + 4);
+    L.rbuf[0] = w.take<float>(2 * (n_v + 4));   // the two residual buffers are contiguous (one L2 window)
+    L.rbuf[1] = L.rbuf[0] ? L.rbuf[0] + (n_v + 4) : nullptr;
+    for (int i = 0; i < 2; ++i) L.Gpart[i] = w.take<double>(1024);
+    for (int i = 0; i < 2; ++i) L.gslot[i] = w.take<double>(B.max_slots);
+    L.tr_obj = w.take<double>((size_t)max_iters + 1);
+    L.tr_lambda = w.take<double>((size_t)max_iters + 1);
+    L.tr_step_sq = w.take<double>((size_t)max_iters + 1);
+    L.tr_trials = w.take<int>((size_t)max_iters + 1);
+    L.r_scratch = w.take<float>(n_v + 4);
+    L.g_scratch = w.take<float>(n_b + 4);
+    L.d_scratch = w.take<float>(n_v + 4);
+    L.flags = w.take<int>(16);
+    L.dvh.hist = w.take<unsigned int>((size_t)n_s * DVH_MAX_PCTS * DVH_BINS);
+    L.dvh.cnt = w.take<unsigned int>((size_t)MAX_STRUCTURES);
+    L.dvh.sum = w.take<double>((size_t)MAX_STRUCTURES);
+    L.dvh.query = w.take<DvhQuery>((size_t)MAX_STRUCTURES * DVH_MAX_PCTS);
+    L.keysA = w.take<unsigned int>(nnz + 4);
+    L.keysB = w.take<unsigned int>(nnz + 4);
+    L.valsA = w.take<unsigned int>(nnz + 4);
+    L.valsB = w.take<unsigned int>(nnz + 4);
+    L.sort_temp = w.take<unsigned char>(B.sort_temp);
+    L.total = (w.off + 255) & ~(size_t)255;
+    return L;
+}
+
+// ------------------------------------------------------------------------------------------------ build kernels
+__global__ void k_validate(const int* __restrict__ col, const float* __restrict__ val, long long nnz, int n_b, int* flags) {
+    int bad_col = 0, bad_val = 0;
+    for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < nnz; p += (long long)gridDim.x * blockDim.x) {
+        const int c = col[p];
+        bad_col |= (c < 0) | (c >= n_b);
+        bad_val |= !isfinite(val[p]);
+    }
+    if (bad_col) flags[0] = 1;
+    if (bad_val) flags[1] = 1;
+}
+
+__global__ void k_iota_keys(const int* __restrict__ col, unsigned int* keys, unsigned int* vals, long long nnz) {
+    for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < nnz; p += (long long)gridDim.x * blockDim.x) {
+        keys[p] = (unsigned int)col[p];
+        vals[p] = (unsigned int)p;
+    }
+}
+
+// rowT_ptr[i] = first position of the sorted column keys that is >= i
+__global__ void k_rowT_ptr(const unsigned int* __restrict__ keys, long long nnz, int n_b, int* rowT_ptr) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n_b) return;
+    long long lo = 0, hi = nnz;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (keys[mid] < (unsigned int)i) lo = mid + 1; else hi = mid;
+    }
+    rowT_ptr[i] = (int)lo;
+}
+
+// entry q of D^T comes from entry p = perm[q] of D: its column is the row of D holding p (upper_bound on row_ptr)
+__global__ void k_fill_transpose(const unsigned int* __restrict__ perm, const int* __restrict__ row_ptr, int n_v,
+                                 const float* __restrict__ val, long long nnz, int* colT, float* valT) {
+    for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < nnz; q += (long long)gridDim.x * blockDim.x) {
+        const int p = (int)perm[q];
+        int lo = 0, hi = n_v;   // largest j with row_ptr[j] <= p
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (row_ptr[mid] <= p) lo = mid; else hi = mid - 1;
+        }
+        colT[q] = lo;
+        valT[q] = val[p];
+    }
+}
+
+// d = 0 and the matching constant residual on every row; the dose pass then overwrites the rows its blocks cover.
+__global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, int n_v, float* r0,
+                                      float* r1, float* d) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_v) return;
+    const float4 t = table[sid[j]];
+    const float u = fmaxf(0.0f, t.x), o = fmaxf(0.0f, -t.y);
+    const float r = 2.0f * (t.w * o - t.z * u);
+    if (r0) r0[j] = r;
+    if (r1) r1[j] = r;
+    if (d) d[j] = 0.0f;
+}
+
+__global__ void k_check_x(const float* __restrict__ x, int n_b, State* st) {
+    int bad = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_b; i += gridDim.x * blockDim.x) {
+        const float v = x[i];
+        bad |= !(v >= 0.0f) | !isfinite(v);
+    }
+    if (bad) st->bad_x = 1;
+}
+
+__global__ void k_reset_state(State* st) {
+    st->G_k = 0.0; st->lambda = st->lambda0; st->step_sq = 0.0;
+    st->fwd_passes = 0; st->tr_passes = 0;
+    st->iter = 0; st->iter_target = 0; st->m = 0; st->stop_reason = STOP_MAX_ITERS;
+    st->xi = 1; st->ri = 1;   // the MODE_INIT dose pass reads xbuf[0], writes rbuf[0] and flips both
+    st->cont_outer = 0; st->cont_inner = 0; st->bad_x = 0;
+    st->ticket_f = 0u; st->ticket_t = 0u; st->gridbar = 0u;
+}
+
+__global__ void k_copy_current_x(const DevPlan P, float* x) {
+    const float* src = P.xbuf[P.st->xi];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n_b; i += gridDim.x * blockDim.x) x[i] = src[i];
+}
+
+inline int grid_for(long long n, int block) {
+    long long g = (n + block - 1) / block;
+    return (int)std::max<long long>(1, std::min<long long>(g, 148 * 16));
+}
+
+// ------------------------------------------------------------------------------------------------ host builders
+// Row-aligned blocks of D for the dose pass (each fits one pipeline stage) and their packed row metadata.
+imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::vector<uint8_t>& sid, const float4* table_h,
+                         std::vector<int4>& blk, std::vector<uint32_t>& meta, double& G_skip, int64_t& n_skipped,
+                         int64_t& n_nonempty) {
+    const int n_v = (int)sid.size();
+    G_skip = 0.0;
+    n_skipped = 0;
+    n_nonempty = 0;
+    auto skip_row = [&](int j) {   // d = 0 on a row without entries: a constant of the objective
+        const float4 t = table_h[sid[j]];
+        const double u = std::max(0.0, (double)t.x), o = std::max(0.0, -(double)t.y);
+        G_skip += (double)t.z * u * u + (double)t.w * o * o;
+        ++n_skipped;
+    };
+    int j = 0;
+    while (j < n_v) {
+        if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
+        const int r0 = j, p0a = rp[j] & ~3;
+        if (rp[j + 1] - p0a > CHUNK_F)
+            return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
+                        rp[j + 1] - rp[j], CHUNK_F - 3);
+        int last = j, empties = 0, jj = j + 1;
+        long long len_sum = rp[j + 1] - rp[j];
+        int n_full = 1;
+        while (jj < n_v && jj - r0 < MAXROWS_F) {
+            const int len = rp[jj + 1] - rp[jj];
+            if (len == 0) {
+                if (++empties > 32) break;
+                ++jj;
+                continue;
+            }
+            if (rp[jj + 1] - p0a > CHUNK_F) break;
+            empties = 0;
+            last = jj;
+            len_sum += len;
+            ++n_full;
+            ++jj;
+        }
+        const int r1 = last + 1, nrows = r1 - r0;
+        n_nonempty += n_full;
+        const double mean = (double)len_sum / n_full;
+        const uint32_t lv = mean >= 96.0 ? 5u : mean >= 32.0 ? 4u : mean >= 12.0 ? 3u : 2u;
+        const int mo = (int)meta.size();
+        meta.push_back((uint32_t)nrows);
+        meta.push_back((uint32_t)r0);
+        meta.push_back(lv);
+        meta.push_back(0u);
+        for (int row = r0; row < r1; ++row) meta.push_back((uint32_t)(rp[row] - p0a) | ((uint32_t)sid[row] << 16));
+        meta.push_back((uint32_t)(rp[r1] - p0a));
+        while (meta.size() & 3) meta.push_back(0u);
+        blk.push_back(make_int4(p0a, rp[r1] - p0a, mo, (int)meta.size() - mo));
+        j = r1;
+    }
+    return IMRT_STATUS_OK;
+}
+
+// Equal-nnz ranges of the D^T stream, each spanning at most RL_MAX rows, and the gradient partial slots.
+void build_ranges(const std::vector<int>& rpT, int n_b, int n_sm, std::vector<TrRange>& ranges, std::vector<int>& rowslot_ptr) {
+    const long long nnz = rpT[n_b];
+    ranges.clear();
+    rowslot_ptr.assign(n_b + 1, 0);
+    if (nnz == 0) return;
+    long long per = (nnz + n_sm - 1) / n_sm;
+    per = (per + 3) & ~3LL;
+    std::vector<int> cnt(n_b, 0);
+    long long e = 0;
+    int row = 0, slot = 0;
+    while (e < nnz) {
+        while (rpT[row + 1] <= e) ++row;
+        TrRange R;
+        memset(&R, 0, sizeof R);
+        R.e_begin = (int)e;
+        R.first_row = row;
+        long long e_end = std::min(nnz, e + per);
+        e_end = std::min<long long>(e_end, rpT[std::min(n_b, row + RL_MAX)]);
+        R.e_end = (int)e_end;
+        int last = row;
+        while (rpT[last + 1] < e_end) ++last;
+        R.n_rows = last - row + 1;
+        R.slot_base = slot;
+        for (int i = row; i <= last; ++i) ++cnt[i];
+        slot += R.n_rows;
+        ranges.push_back(R);
+        e = e_end;
+    }
+    for (int i = 0; i < n_b; ++i) rowslot_ptr[i + 1] = rowslot_ptr[i] + cnt[i];
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ launch helpers
+static cudaError_t launch_dose(imrt_plan* pl, const PassArgs& A) {
+    k_dose<<<pl->P.grid_f, NTHREADS, pl->smem_bytes, pl->stream>>>(pl->P, A);
+    return cudaGetLastError();
+}
+static cudaError_t launch_transpose(imrt_plan* pl, const PassArgs& A) {
+    k_transpose<<<pl->P.grid_t, NTHREADS, pl->smem_bytes, pl->stream>>>(pl->P, A);
+    return cudaGetLastError();
+}
+static cudaError_t launch_persistent(imrt_plan* pl) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3(pl->grid_p);
+    cfg.blockDim = dim3(NTHREADS);
+    cfg.dynamicSmemBytes = pl->smem_bytes;
+    cfg.stream = pl->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;   // co-residency of all CTAs is required by the grid barrier
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_persistent, pl->P);
+}
+
+// graph:  k_begin -> WHILE(outer){ k_transpose -> WHILE(inner){ k_dose } }
+static imrt_status build_graph(imrt_plan* pl) {
+    CUDA_TRY(pl, cudaGraphCreate(&pl->graph, 0));
+    cudaGraphConditionalHandle h_outer, h_inner;
+    CUDA_TRY(pl, cudaGraphConditionalHandleCreate(&h_outer, pl->graph, 0, 0));
+    CUDA_TRY(pl, cudaGraphConditionalHandleCreate(&h_inner, pl->graph, 0, 0));
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_TRIAL;
+    A.use_handles = 1;
+    A.h_outer = h_outer;
+    A.h_inner = h_inner;
+
+    cudaGraphNode_t n_begin, n_outer, n_tr, n_inner, n_dose;
+    {
+        State* st = pl->P.st;
+        int use = 1;
+        void* args[] = {&st, &use, &h_outer};
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeKernel;
+        np.kernel.func = (void*)k_begin;
+        np.kernel.gridDim = dim3(1);
+        np.kernel.blockDim = dim3(1);
+        np.kernel.kernelParams = args;
+        CUDA_TRY(pl, cudaGraphAddNode(&n_begin, pl->graph, nullptr, 0, &np));
+    }
+    cudaGraph_t body_outer, body_inner;
+    {
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = h_outer;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        CUDA_TRY(pl, cudaGraphAddNode(&n_outer, pl->graph, &n_begin, 1, &np));
+        body_outer = np.conditional.phGraph_out[0];
+    }
+    {
+        void* args[] = {&pl->P, &A};
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeKernel;
+        np.kernel.func = (void*)k_transpose;
+        np.kernel.gridDim = dim3(pl->P.grid_t);
+        np.kernel.blockDim = dim3(NTHREADS);
+        np.kernel.sharedMemBytes = (unsigned int)pl->smem_bytes;
+        np.kernel.kernelParams = args;
+        CUDA_TRY(pl, cudaGraphAddNode(&n_tr, body_outer, nullptr, 0, &np));
+    }
+    {
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = h_inner;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        CUDA_TRY(pl, cudaGraphAddNode(&n_inner, body_outer, &n_tr, 1, &np));
+        body_inner = np.conditional.phGraph_out[0];
+    }
+    {
+        void* args[] = {&pl->P, &A};
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeKernel;
+        np.kernel.func = (void*)k_dose;
+        np.kernel.gridDim = dim3(pl->P.grid_f);
+        np.kernel.blockDim = dim3(NTHREADS);
+        np.kernel.sharedMemBytes = (unsigned int)pl->smem_bytes;
+        np.kernel.kernelParams = args;
+        CUDA_TRY(pl, cudaGraphAddNode(&n_dose, body_inner, nullptr, 0, &np));
+    }
+    CUDA_TRY(pl, cudaGraphInstantiate(&pl->graph_exec, pl->graph, 0));
+    return IMRT_STATUS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ C-ABI
+extern "C" {
+
+const char* imrt_version(void) { return "imrtgp 0.1 (sm_100a)"; }
+
+const char* imrt_last_error(const imrt_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+imrt_status imrt_workspace_bytes(int64_t n_v, int64_t n_b, int64_t nnz, int32_t n_structures, int32_t max_iters,
+                                 size_t* host_bytes) {
+    if (!host_bytes || n_v < 0 || n_b < 0 || nnz < 0 || n_structures < 1 || n_structures > MAX_STRUCTURES || max_iters < 0)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_workspace_bytes: bad argument");
+    if (nnz >= (1LL << 31) - 16 || n_v >= (1LL << 31) - 16 || n_b >= (1LL << 31) - 16)
+        return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "sizes must fit int32");
+    *host_bytes = make_layout(nullptr, n_v, n_b, nnz, n_structures, max_iters).total;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t nnz, const int32_t* row_ptr,
+                             const int32_t* col_idx, const float* val, const uint8_t* structure_id, int32_t n_structures,
+                             const float* host_t_under, const float* host_t_over, const float* host_w_under,
+                             const float* host_w_over, const imrt_params* prm, void* workspace, size_t workspace_bytes,
+                             void* stream) {
+    if (out) *out = nullptr;
+    if (!out || !row_ptr || !structure_id || !host_t_under || !host_t_over || !host_w_under || !host_w_over || !prm || !workspace)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: null argument");
+    if ((nnz > 0 && (!col_idx || !val)) || n_v < 1 || n_b < 1 || nnz < 0 || n_structures < 1 || n_structures > MAX_STRUCTURES)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad size (n_v %lld, n_b %lld, nnz %lld, n_structures %d)",
+                    (long long)n_v, (long long)n_b, (long long)nnz, n_structures);
+    if (nnz >= (1LL << 31) - 16 || n_v >= (1LL << 31) - 16 || n_b >= (1LL << 31) - 16)
+        return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "sizes must fit int32");
+    if (!(prm->eps > 0.0 && prm->eps < 1.0) || !(prm->alpha > 1.0) || !(prm->lambda0 > 0.0) || !std::isfinite(prm->lambda0) ||
+        prm->max_ls < 0 || prm->max_iters < 0 || prm->driver < 0 || prm->driver > 2 || prm->reserved != 0)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad imrt_params (need 0<eps<1, alpha>1, lambda0>0, driver in 0..2)");
+    if (((uintptr_t)row_ptr | (uintptr_t)col_idx | (uintptr_t)val | (uintptr_t)workspace) & 15)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: device arrays must be 16-byte aligned");
+    for (int s = 0; s < n_structures; ++s) {
+        const float v[4] = {host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]};
+        for (float f : v)
+            if (!std::isfinite(f)) return fail(nullptr, IMRT_STATUS_BAD_STRUCTURE, "structure %d: non-finite limit or weight", s);
+        if (v[2] < 0.0f || v[3] < 0.0f) return fail(nullptr, IMRT_STATUS_BAD_STRUCTURE, "structure %d: negative weight", s);
+    }
+    const Layout L = make_layout(workspace, n_v, n_b, nnz, n_structures, prm->max_iters);
+    if (workspace_bytes < L.total)
+        return fail(nullptr, IMRT_STATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", workspace_bytes, L.total);
+
+    int dev = 0, cc_major = 0, n_sm = 0, smem_optin = 0;
+    CUDA_TRY(nullptr, cudaGetDevice(&dev));
+    CUDA_TRY(nullptr, cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+    CUDA_TRY(nullptr, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    CUDA_TRY(nullptr, cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    if (cc_major != 10)
+        return fail(nullptr, IMRT_STATUS_UNSUPPORTED_DEVICE, "device has compute capability %d.x; libimrtgp is built for sm_100a only", cc_major);
+    if (n_sm > 1024) n_sm = 1024;
+
+    imrt_plan* pl = new imrt_plan();
+    pl->prm = *prm;
+    pl->stream = (cudaStream_t)stream;
+    pl->n_sm = n_sm;
+    pl->has_x = false;
+    pl->graph = nullptr;
+    pl->graph_exec = nullptr;
+    pl->row_ptr = row_ptr;
+    pl->sid = structure_id;
+    cudaStream_t st = pl->stream;
+    // every early return below releases the handle
+    struct Guard { imrt_plan* p; ~Guard() { if (p) { g_create_error = p->err; delete p; } } } guard{pl};
+
+    // ---- validate what the host can see: row_ptr and structure ids
+    std::vector<int> rp((size_t)n_v + 1);
+    std::vector<uint8_t> sid((size_t)n_v);
+    CUDA_TRY(pl, cudaMemcpyAsync(rp.data(), row_ptr, sizeof(int) * (n_v + 1), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(sid.data(), structure_id, (size_t)n_v, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.flags, 0, 16 * sizeof(int), st));
+    if (nnz > 0) k_validate<<<grid_for(nnz, 256), 256, 0, st>>>(col_idx, val, nnz, (int)n_b, L.flags);
+    int flags_h[16];
+    CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    if (rp[0] != 0 || rp[n_v] != nnz) return fail(pl, IMRT_STATUS_BAD_CSR, "row_ptr[0] = %d, row_ptr[n_v] = %d, nnz = %lld", rp[0], rp[n_v], (long long)nnz);
+    for (int64_t j = 0; j < n_v; ++j)
+        if (rp[j + 1] < rp[j]) return fail(pl, IMRT_STATUS_BAD_CSR, "row_ptr decreases at row %lld", (long long)j);
+    if (flags_h[0]) return fail(pl, IMRT_STATUS_BAD_CSR, "a column index is outside [0, n_b)");
+    if (flags_h[1]) return fail(pl, IMRT_STATUS_BAD_CSR, "a value of D is not finite");
+    for (int64_t j = 0; j < n_v; ++j)
+        if (sid[j] >= n_structures) return fail(pl, IMRT_STATUS_BAD_STRUCTURE, "structure_id[%lld] = %d >= n_structures", (long long)j, sid[j]);
+
+    // ---- penalty table
+    std::vector<float4> table_h(MAX_STRUCTURES, make_float4(0, 0, 0, 0));
+    for (int s = 0; s < n_structures; ++s) table_h[s] = make_float4(host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]);
+    CUDA_TRY(pl, cudaMemcpyAsync(L.table, table_h.data(), sizeof(float4) * MAX_STRUCTURES, cudaMemcpyHostToDevice, st));
+
+    // ---- dose-pass blocks
+    std::vector<int4> blk;
+    std::vector<uint32_t> meta;
+    double G_skip = 0.0;
+    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), blk, meta, G_skip, pl->n_skipped, pl->n_nonempty);
+    if (s != IMRT_STATUS_OK) return s;
+    const Bounds B = bounds_for(n_v, n_b, nnz);
+    if ((int64_t)blk.size() > B.max_blk || (int64_t)meta.size() > B.max_meta)
+        return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %zu words)", blk.size(), meta.size());
+    pl->n_blk = (int64_t)blk.size();
+    const int grid_f = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, blk.size()));
+    std::vector<int> cta_blk(grid_f + 1, 0);
+    {
+        std::vector<double> pre(blk.size() + 1, 0.0);
+        for (size_t b = 0; b < blk.size(); ++b) pre[b + 1] = pre[b] + 8.0 * blk[b].y + 4.0 * blk[b].w + 64.0;
+        size_t b = 0;
+        for (int c = 0; c < grid_f; ++c) {
+            const double want = pre[blk.size()] * c / grid_f;
+            while (b < blk.size() && pre[b] < want) ++b;
+            cta_blk[c] = (int)b;
+        }
+        cta_blk[grid_f] = (int)blk.size();
+    }
+    if (!blk.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.blk, blk.data(), sizeof(int4) * blk.size(), cudaMemcpyHostToDevice, st));
+    if (!meta.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.rowmeta, meta.data(), sizeof(uint32_t) * meta.size(), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(L.cta_blk, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
+
+    // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1)
+    CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.valT, 0, sizeof(float) * B.nnz_pad, st));
+    std::vector<int> rpT((size_t)n_b + 1, 0);
+    if (nnz > 0) {
+        k_iota_keys<<<grid_for(nnz, 256), 256, 0, st>>>(col_idx, L.keysA, L.valsA, nnz);
+        cub::DoubleBuffer<unsigned int> dk(L.keysA, L.keysB), dv(L.valsA, L.valsB);
+        int end_bit = 1;
+        while ((1LL << end_bit) < n_b) ++end_bit;
+        size_t temp = 0;
+        CUDA_TRY(pl, cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)nnz, 0, end_bit, st));
+        if (temp > B.sort_temp) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: radix sort needs %zu temp bytes, %zu reserved", temp, B.sort_temp);
+        CUDA_TRY(pl, cub::DeviceRadixSort::SortPairs(L.sort_temp, temp, dk, dv, (int)nnz, 0, end_bit, st));
+        k_rowT_ptr<<<(int)((n_b + 1 + 255) / 256), 256, 0, st>>>(dk.Current(), nnz, (int)n_b, L.rowT_ptr);
+        k_fill_transpose<<<grid_for(nnz, 256), 256, 0, st>>>(dv.Current(), row_ptr, (int)n_v, val, nnz, L.colT, L.valT);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(rpT.data(), L.rowT_ptr, sizeof(int) * (n_b + 1), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+    } else {
+        CUDA_TRY(pl, cudaMemsetAsync(L.rowT_ptr, 0, sizeof(int) * (n_b + 1), st));
+    }
+
+    // ---- transpose-pass ranges and gradient slots
+    std::vector<TrRange> ranges;
+    std::vector<int> rowslot;
+    build_ranges(rpT, (int)n_b, n_sm, ranges, rowslot);
+    if ((int64_t)ranges.size() > B.max_ranges) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: %zu transpose ranges exceed the bound", ranges.size());
+    const int n_slots = rowslot[n_b];
+    if (!ranges.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.tr_range, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
+
+    // ---- shared-memory layout (one layout for the three kernels)
+    const int nb_pad = (int)((n_b + 31) & ~31LL);
+    int off = SMEM_HEADER + SMEM_TABLE + SMEM_WPART;
+    DevPlan& P = pl->P;
+    memset(&P, 0, sizeof P);
+    P.x_off = off; off += nb_pad * 4;
+    P.g_off = off; off += nb_pad * 4;
+    P.xt_off = off; off += nb_pad * 4;
+    off = (off + 127) & ~127;
+    P.stage_off = off;
+    const int avail = smem_optin - off;
+    const int sf = std::min(MAX_STAGES, avail / STAGE_F_BYTES), stt = std::min(MAX_STAGES, avail / STAGE_T_BYTES);
+    if (avail < 0 || sf < 2 || stt < 2)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets do not fit in shared memory next to the pipeline stages", (long long)n_b);
+    pl->smem_bytes = (size_t)off + (size_t)std::max(sf * STAGE_F_BYTES, stt * STAGE_T_BYTES);
+
+    P.col = col_idx; P.val = val; P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
+    P.blk = L.blk; P.rowmeta = L.rowmeta; P.cta_blk = L.cta_blk; P.grid_f = grid_f; P.n_stages_f = sf;
+    P.rowT_ptr = L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
+    P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr;
+    P.n_ranges = (int)ranges.size(); P.grid_t = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, ranges.size()));
+    P.n_stages_t = stt; P.n_slots = n_slots;
+    P.table = L.table; P.n_structures = n_structures; P.G_skip = G_skip;
+    P.xbuf[0] = L.xbuf[0]; P.xbuf[1] = L.xbuf[1]; P.g = L.g; P.rbuf[0] = L.rbuf[0]; P.rbuf[1] = L.rbuf[1];
+    P.Gpart[0] = L.Gpart[0]; P.Gpart[1] = L.Gpart[1]; P.gslot[0] = L.gslot[0]; P.gslot[1] = L.gslot[1];
+    P.st = L.st; P.tr_obj = L.tr_obj; P.tr_lambda = L.tr_lambda; P.tr_step_sq = L.tr_step_sq; P.tr_trials = L.tr_trials;
+    pl->r_scratch = L.r_scratch; pl->g_scratch = L.g_scratch; pl->d_scratch = L.d_scratch;
+    pl->rowT_ptr_w = L.rowT_ptr; pl->colT_w = L.colT; pl->valT_w = L.valT;
+    pl->dvh = L.dvh;
+    pl->grid_p = n_sm;
+
+    CUDA_TRY(pl, cudaFuncSetAttribute(k_dose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
+    CUDA_TRY(pl, cudaFuncSetAttribute(k_transpose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
+    CUDA_TRY(pl, cudaFuncSetAttribute(k_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
+
+    // ---- device state, constant residual of the zero-dose rows
+    State st_h;
+    memset(&st_h, 0, sizeof st_h);
+    st_h.eps = prm->eps; st_h.alpha = prm->alpha; st_h.lambda0 = prm->lambda0; st_h.lambda = prm->lambda0;
+    st_h.max_ls = prm->max_ls; st_h.trace_cap = prm->max_iters; st_h.xi = 1; st_h.ri = 1;
+    CUDA_TRY(pl, cudaMemcpyAsync(L.st, &st_h, sizeof st_h, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.gslot[0], 0, sizeof(double) * B.max_slots, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.gslot[1], 0, sizeof(double) * B.max_slots, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[0], 0, sizeof(double) * 1024, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[1], 0, sizeof(double) * 1024, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.g, 0, sizeof(float) * (n_b + 4), st));
+    k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, (int)n_v, L.rbuf[0], L.rbuf[1], nullptr);
+    CUDA_TRY(pl, cudaGetLastError());
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+
+    if (prm->driver == 0) {
+        s = build_graph(pl);
+        if (s != IMRT_STATUS_OK) return s;
+    }
+    guard.p = nullptr;
+    *out = pl;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_destroy(imrt_plan* pl) {
+    if (!pl) return IMRT_STATUS_INVALID_ARG;
+    cudaStreamSynchronize(pl->stream);
+    if (pl->graph_exec) cudaGraphExecDestroy(pl->graph_exec);
+    if (pl->graph) cudaGraphDestroy(pl->graph);
+    delete pl;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_set_x(imrt_plan* pl, const float* x0) {
+    if (!pl || !x0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_x: null argument");
+    cudaStream_t st = pl->stream;
+    k_reset_state<<<1, 1, 0, st>>>(pl->P.st);
+    k_check_x<<<grid_for(pl->P.n_b, 256), 256, 0, st>>>(x0, pl->P.n_b, pl->P.st);
+    int bad = 0;
+    CUDA_TRY(pl, cudaMemcpyAsync(&bad, &pl->P.st->bad_x, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    if (bad) { pl->has_x = false; return fail(pl, IMRT_STATUS_BAD_X, "x0 has a negative or non-finite entry"); }
+    CUDA_TRY(pl, cudaMemcpyAsync(pl->P.xbuf[0], x0, sizeof(float) * pl->P.n_b, cudaMemcpyDeviceToDevice, st));
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_INIT;   // G(x_1), r(x_1): reads xbuf[0], writes rbuf[0], flips xi / ri to 0
+    CUDA_TRY(pl, launch_dose(pl, A));
+    pl->has_x = true;
+    return IMRT_STATUS_OK;
+}
+
+static imrt_status run_common(imrt_plan* pl, int32_t n_iters, double delta) {
+    if (!pl) return IMRT_STATUS_INVALID_ARG;
+    if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    if (n_iters < 0 || !(delta >= 0.0)) return fail(pl, IMRT_STATUS_INVALID_ARG, "run: n_iters and delta must be >= 0");
+    cudaStream_t st = pl->stream;
+    k_set_target<<<1, 1, 0, st>>>(pl->P.st, n_iters, delta);
+    CUDA_TRY(pl, cudaGetLastError());
+    if (pl->prm.driver == 0) {
+        CUDA_TRY(pl, cudaGraphLaunch(pl->graph_exec, st));
+    } else if (pl->prm.driver == 2) {
+        CUDA_TRY(pl, launch_persistent(pl));
+    } else {
+        // host-driven: the loop conditions come back after every pass (one sync per trial)
+        PassArgs A;
+        memset(&A, 0, sizeof A);
+        A.mode = MODE_TRIAL;
+        cudaGraphConditionalHandle none = 0;
+        k_begin<<<1, 1, 0, st>>>(pl->P.st, 0, none);
+        int cont[2];
+        auto fetch = [&]() -> cudaError_t {
+            cudaError_t e = cudaMemcpyAsync(cont, &pl->P.st->cont_outer, 2 * sizeof(int), cudaMemcpyDeviceToHost, st);
+            return e != cudaSuccess ? e : cudaStreamSynchronize(st);
+        };
+        CUDA_TRY(pl, fetch());
+        while (cont[0]) {
+            CUDA_TRY(pl, launch_transpose(pl, A));
+            CUDA_TRY(pl, fetch());
+            while (cont[1]) {
+                CUDA_TRY(pl, launch_dose(pl, A));
+                CUDA_TRY(pl, fetch());
+            }
+        }
+    }
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_run_iters(imrt_plan* pl, int32_t n_iters) { return run_common(pl, n_iters, 0.0); }
+
+imrt_status imrt_plan_run_to_tol(imrt_plan* pl, double delta, int32_t max_iters) {
+    if (pl && !(delta > 0.0)) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_to_tol: delta must be > 0");
+    return run_common(pl, max_iters, delta);
+}
+
+imrt_status imrt_plan_eval(imrt_plan* pl, const float* x, float* d, float* r, float* g, double* host_obj) {
+    if (!pl || !x) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_eval: null argument");
+    cudaStream_t st = pl->stream;
+    float* r_used = r ? r : pl->r_scratch;
+    const int n_v = pl->P.n_v;
+    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, st>>>(pl->sid, pl->P.table, n_v, r_used, nullptr, d);
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_EVAL;
+    A.x_in = x;
+    A.r_out = r_used;
+    A.d_out = d;
+    CUDA_TRY(pl, launch_dose(pl, A));
+    if (g) {
+        PassArgs T;
+        memset(&T, 0, sizeof T);
+        T.mode = MODE_EVAL;
+        T.r_in = r_used;
+        T.g_out = g;
+        CUDA_TRY(pl, launch_transpose(pl, T));
+    }
+    double obj = 0.0;
+    CUDA_TRY(pl, cudaMemcpyAsync(&obj, &pl->P.st->eval_obj, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    if (host_obj) *host_obj = obj;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_x(imrt_plan* pl, float* x) {
+    if (!pl || !x) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_x: null argument");
+    if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    k_copy_current_x<<<grid_for(pl->P.n_b, 256), 256, 0, pl->stream>>>(pl->P, x);
+    CUDA_TRY(pl, cudaGetLastError());
+    return IMRT_STATUS_OK;
+}
+
+static imrt_status dose_of_current_x(imrt_plan* pl, float* d) {
+    const int n_v = pl->P.n_v;
+    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, pl->stream>>>(pl->sid, pl->P.table, n_v, nullptr, nullptr, d);
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_EVAL;   // x_in NULL: the current iterate
+    A.r_out = pl->r_scratch;
+    A.d_out = d;
+    CUDA_TRY(pl, launch_dose(pl, A));
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_dose(imrt_plan* pl, float* d) {
+    if (!pl || !d) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_dose: null argument");
+    if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    return dose_of_current_x(pl, d);
+}
+
+imrt_status imrt_plan_dvh(imrt_plan* pl, const double* host_pcts, int32_t n_pcts, double* host_dp, double* host_mean) {
+    if (!pl || !host_pcts || !host_dp || !host_mean || n_pcts < 1 || n_pcts > DVH_MAX_PCTS)
+        return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_dvh: bad argument (1 <= n_pcts <= %d)", DVH_MAX_PCTS);
+    if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    imrt_status s = dose_of_current_x(pl, pl->d_scratch);
+    if (s != IMRT_STATUS_OK) return s;
+    const char* msg = nullptr;
+    cudaError_t e = dvh_points(pl->dvh, pl->d_scratch, pl->sid, pl->P.n_v, pl->P.n_structures, host_pcts, n_pcts, host_dp, host_mean,
+                               pl->stream, &msg);
+    if (e != cudaSuccess) return fail(pl, IMRT_STATUS_CUDA_ERROR, "dvh: %s (%s)", cudaGetErrorString(e), msg ? msg : "");
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_trace(imrt_plan* pl, int32_t* host_n_iters_done, int32_t* host_stop_reason, double* host_obj,
+                                double* host_lambda, int32_t* host_n_trials, double* host_step_sq, int32_t capacity) {
+    if (!pl || capacity < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_trace: bad argument");
+    if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    cudaStream_t st = pl->stream;
+    State s;
+    CUDA_TRY(pl, cudaMemcpyAsync(&s, pl->P.st, sizeof s, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    const int n = std::min(s.iter, capacity);
+    if (host_n_iters_done) *host_n_iters_done = s.iter;
+    if (host_stop_reason) *host_stop_reason = s.stop_reason;
+    if (host_obj) CUDA_TRY(pl, cudaMemcpyAsync(host_obj, pl->P.tr_obj, sizeof(double) * (n + 1), cudaMemcpyDeviceToHost, st));
+    if (host_lambda && n) CUDA_TRY(pl, cudaMemcpyAsync(host_lambda, pl->P.tr_lambda, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (host_n_trials && n) CUDA_TRY(pl, cudaMemcpyAsync(host_n_trials, pl->P.tr_trials, sizeof(int) * n, cudaMemcpyDeviceToHost, st));
+    if (host_step_sq && n) CUDA_TRY(pl, cudaMemcpyAsync(host_step_sq, pl->P.tr_step_sq, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_counters(imrt_plan* pl, int64_t* host_fwd_passes, int64_t* host_tr_passes) {
+    if (!pl) return IMRT_STATUS_INVALID_ARG;
+    State s;
+    CUDA_TRY(pl, cudaMemcpyAsync(&s, pl->P.st, sizeof s, cudaMemcpyDeviceToHost, pl->stream));
+    CUDA_TRY(pl, cudaStreamSynchronize(pl->stream));
+    if (host_fwd_passes) *host_fwd_passes = s.fwd_passes;
+    if (host_tr_passes) *host_tr_passes = s.tr_passes;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info, int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT) {
+    if (!pl) return IMRT_STATUS_INVALID_ARG;
+    const int64_t info[10] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, (int64_t)pl->smem_bytes,
+                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, 1};
+    for (int i = 0; i < n_info && i < 10 && host_info; ++i) host_info[i] = info[i];
+    cudaStream_t st = pl->stream;
+    if (d_rowT_ptr) CUDA_TRY(pl, cudaMemcpyAsync(d_rowT_ptr, pl->rowT_ptr_w, sizeof(int) * (pl->P.n_b + 1), cudaMemcpyDeviceToDevice, st));
+    if (d_colT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_colT, pl->colT_w, sizeof(int) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));
+    if (d_valT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_valT, pl->valT_w, sizeof(float) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_launch_pass(imrt_plan* pl, int32_t kind, int32_t n_repeat) {
+    if (!pl || kind < 0 || kind > 1 || n_repeat < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_launch_pass: bad argument");
+    if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_EVAL;
+    A.r_out = pl->r_scratch;    // dose pass: at the current iterate, outputs to scratch
+    A.g_out = pl->g_scratch;    // transpose pass: on r(x_k), output to scratch
+    for (int i = 0; i < n_repeat; ++i) CUDA_TRY(pl, kind == 0 ? launch_dose(pl, A) : launch_transpose(pl, A));
+    return IMRT_STATUS_OK;
+}
+
+}  // extern "C"

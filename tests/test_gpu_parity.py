@@ -1,0 +1,268 @@
+"""GPU parity: libimrtgp (through its C-ABI binding) against the fp64 CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star):
+  per-kernel   d, r, g: ||a-b||_inf / ||b||_inf and ||a-b||_2 / ||b||_2 <= 1e-5;  G: |a-b|/|b| <= 1e-5
+  trajectory   same accepted-iteration count, oracle in follow mode (slack 1e-6 G_k on the Armijo margin):
+               final G within 1e-4 relative; DVH points within 0.5 % of the 70 Gy prescription (0.35 Gy)
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synth_inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_KERNEL = 1e-5
+TOL_G_FINAL = 1e-4
+TOL_DVH_GY = 0.005 * 70.0
+
+
+@pytest.fixture(scope="module")
+def m():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_0908_4421_b200 as mod
+    mod.lib()
+    return mod
+
+
+_phantoms = {}
+
+
+def phantom(i):
+    if i not in _phantoms:
+        _phantoms[i] = synth_inputs.make_phantom(i)
+    return _phantoms[i]
+
+
+def relerr(a, b):
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    ninf = np.abs(b).max() if b.size else 0.0
+    n2 = np.linalg.norm(b)
+    einf = np.abs(a - b).max() / ninf if ninf > 0 else np.abs(a - b).max(initial=0.0)
+    e2 = np.linalg.norm(a - b) / n2 if n2 > 0 else np.linalg.norm(a - b)
+    return max(einf, e2)
+
+
+def check_eval(m, plan, prob, x):
+    d, r, g, G = plan.eval(x)
+    x64 = np.asarray(x, np.float32).astype(np.float64)
+    d_o, r_o, G_o = oracle.eval_objective(prob, x64)
+    g_o = oracle.gradient(prob, r_o)
+    assert relerr(d.cpu().numpy(), d_o) <= TOL_KERNEL
+    assert relerr(r.cpu().numpy(), r_o) <= TOL_KERNEL
+    assert relerr(g.cpu().numpy(), g_o) <= TOL_KERNEL
+    assert abs(G - G_o) <= TOL_KERNEL * abs(G_o) + 1e-300
+    # the transpose kernel alone: feed it the ORACLE's residual (rounded to fp32) instead of the GPU's
+    return d, r, g, G
+
+
+# ---------------------------------------------------------------------------------------------- D^T construction
+@pytest.mark.parametrize("case", ["cfg0", "rand_a", "rand_b"])
+def test_transpose_csr_is_exact(m, case):
+    import scipy.sparse as sp
+    prob = phantom(0) if case == "cfg0" else synth_inputs.make_random(7 if case == "rand_a" else 8, n_v=777, n_b=53,
+                                                                      density=0.3, empty_row_frac=0.2, full_rows=3)
+    plan = m.Plan(prob, max_iters=4)
+    rpT, cT, vT = (t.cpu().numpy() for t in plan.transpose_csr())
+    A = sp.csr_matrix((prob.val, prob.col, prob.row_ptr), shape=(prob.n_v, prob.n_b))
+    T = A.T.tocsr()
+    T.sort_indices()
+    np.testing.assert_array_equal(rpT, T.indptr)
+    np.testing.assert_array_equal(cT, T.indices)
+    np.testing.assert_array_equal(vT, T.data)
+    plan.close()
+
+
+# ---------------------------------------------------------------------------------------------- per-kernel parity
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_eval_parity_phantoms(m, cfg):
+    prob = phantom(cfg)
+    plan = m.Plan(prob, max_iters=8)
+    check_eval(m, plan, prob, prob.x0)
+    # also at the oracle's iterate after 1 and 10 iterations (x rounded to fp32 is what both sides see)
+    for n in (1, 10):
+        xo = oracle.run(prob, n_iters=n).x.astype(np.float32)
+        check_eval(m, plan, prob, xo)
+    plan.close()
+
+
+@pytest.mark.parametrize("seed,n_v,n_b,density", [(1, 50, 8, 0.4), (2, 1000, 37, 0.3), (3, 4099, 130, 0.5), (4, 30000, 300, 0.2),
+                                                   (5, 3, 1, 1.0), (6, 2500, 2000, 0.02)])
+def test_eval_parity_random_shapes(m, seed, n_v, n_b, density):
+    # ragged shapes: nnz not a multiple of 4, empty / single-entry / full rows, short D^T rows, one-column matrices
+    prob = synth_inputs.make_random(seed, n_v=n_v, n_b=n_b, density=density, empty_row_frac=0.15, full_rows=min(2, n_v))
+    plan = m.Plan(prob, max_iters=4)
+    x = np.random.default_rng(seed).uniform(0, 80, prob.n_b).astype(np.float32)
+    check_eval(m, plan, prob, x)
+    check_eval(m, plan, prob, np.zeros(prob.n_b, np.float32))
+    plan.close()
+
+
+def test_eval_all_rows_empty_and_leading_trailing_empty(m):
+    rng = np.random.default_rng(0)
+    base = synth_inputs.make_random(11, n_v=600, n_b=20, density=0.3)
+    # 500 empty rows in front and behind
+    rp = np.concatenate([np.zeros(500, np.int32), base.row_ptr, np.full(500, base.row_ptr[-1], np.int32)])
+    sid = np.concatenate([rng.integers(0, 3, 500).astype(np.uint8), base.sid, rng.integers(0, 3, 500).astype(np.uint8)])
+    prob = synth_inputs.Problem("padded", 1600, 20, rp, base.col, base.val, sid, base.t_under, base.t_over, base.w_under,
+                                base.w_over, base.x0, lambda0=base.lambda0)
+    plan = m.Plan(prob, max_iters=4)
+    check_eval(m, plan, prob, prob.x0)   # zero-dose PTV rows contribute w- T^2 each and a constant residual
+    plan.close()
+    empty = synth_inputs.Problem("empty", 100, 5, np.zeros(101, np.int32), np.zeros(0, np.int32), np.zeros(0, np.float32),
+                                 sid[:100], base.t_under, base.t_over, base.w_under, base.w_over, np.ones(5, np.float32))
+    plan = m.Plan(empty, max_iters=4)
+    d, r, g, G = plan.eval(empty.x0)
+    d_o, r_o, G_o = oracle.eval_objective(empty, empty.x0.astype(np.float64))
+    assert G == G_o and not d.cpu().numpy().any() and not g.cpu().numpy().any()
+    np.testing.assert_array_equal(r.cpu().numpy(), r_o.astype(np.float32))
+    plan.set_x(empty.x0)
+    plan.run_iters(3)
+    tr = plan.trace()
+    assert tr.n_iters == 0 and tr.stop_reason == oracle.STOP_STATIONARY   # zero gradient: first trial equals x_k
+    plan.close()
+
+
+# ---------------------------------------------------------------------------------------------- the loop
+def run_gpu(m, prob, n_iters, driver, delta=0.0):
+    plan = m.Plan(prob, max_iters=max(n_iters, 1), driver=driver)
+    plan.set_x(prob.x0)
+    if delta > 0:
+        plan.run_to_tol(delta, n_iters)
+    else:
+        plan.run_iters(n_iters)
+    tr = plan.trace()
+    x = plan.get_x().cpu().numpy()
+    d = plan.get_dose().cpu().numpy()
+    cnt = plan.counters()
+    return plan, tr, x, d, cnt
+
+
+def test_three_drivers_are_bit_identical(m):
+    prob = phantom(0)
+    res = [run_gpu(m, prob, 25, drv) for drv in (m.DRIVER_HOST, m.DRIVER_GRAPH, m.DRIVER_PERSISTENT)]
+    _, tr0, x0, d0, c0 = res[0]
+    assert tr0.n_iters == 25 and tr0.n_trials.max() > 1
+    for _, tr, x, d, c in res[1:]:
+        assert tr.n_iters == tr0.n_iters and tr.stop_reason == tr0.stop_reason
+        np.testing.assert_array_equal(tr.obj, tr0.obj)
+        np.testing.assert_array_equal(tr.n_trials, tr0.n_trials)
+        np.testing.assert_array_equal(tr.lam, tr0.lam)
+        np.testing.assert_array_equal(tr.step_sq, tr0.step_sq)
+        np.testing.assert_array_equal(x, x0)
+        np.testing.assert_array_equal(d, d0)
+        assert c == c0
+    for r in res:
+        r[0].close()
+
+
+def test_runs_are_reproducible_and_resumable(m):
+    prob = phantom(0)
+    p1, tr1, x1, _, _ = run_gpu(m, prob, 20, m.DRIVER_PERSISTENT)
+    plan = m.Plan(prob, max_iters=20, driver=m.DRIVER_PERSISTENT)
+    plan.set_x(prob.x0)
+    plan.run_iters(7)
+    plan.run_iters(13)   # 7 + 13 accepted iterations in two launches == 20 in one
+    tr2 = plan.trace()
+    np.testing.assert_array_equal(tr2.obj, tr1.obj)
+    np.testing.assert_array_equal(plan.get_x().cpu().numpy(), x1)
+    plan.run_iters(5)    # trace capacity reached: nothing more happens
+    assert plan.trace().n_iters == 20
+    p1.close()
+    plan.close()
+
+
+@pytest.mark.parametrize("cfg,driver", [(0, 2), (0, 0), (1, 2)])
+def test_trajectory_parity_follow_mode(m, cfg, driver):
+    prob = phantom(cfg)
+    n = prob.n_iters
+    plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, n, driver)
+    assert tr.n_iters == n and tr.stop_reason == oracle.STOP_MAX_ITERS
+    assert fwd == 1 + tr.n_trials.sum() and trp == n
+    assert (np.diff(tr.obj) < 0).all() and (x >= 0).all()
+    fol = oracle.run(prob, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert fol.n_follow_violations == 0, "GPU accepted/rejected a trial the oracle would not (first at iteration %d)" % fol.first_violation
+    np.testing.assert_array_equal(tr.lam, fol.lam)
+    assert abs(tr.obj[-1] - fol.obj[-1]) <= TOL_G_FINAL * fol.obj[-1]
+    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    # DVH points of the final plans
+    d_o, _, _ = oracle.eval_objective(prob, fol.x)
+    dp_o, mean_o = oracle.dvh_points(prob.sid, d_o, prob.n_structures)
+    dp_g, mean_g = oracle.dvh_points(prob.sid, d.astype(np.float64), prob.n_structures)
+    assert np.nanmax(np.abs(dp_g - dp_o)) <= TOL_DVH_GY and np.nanmax(np.abs(mean_g - mean_o)) <= TOL_DVH_GY
+    # and the library's own DVH kernel gives exactly the order statistics of its own dose
+    dp_k, mean_k = plan.dvh(oracle.DVH_PCTS)
+    np.testing.assert_array_equal(dp_k, dp_g)
+    np.testing.assert_allclose(mean_k, mean_g, rtol=1e-6)
+    # free-running oracle: report where (if anywhere) the trial counts first part ways
+    free = oracle.run(prob, n_iters=n)
+    same = free.n_trials[:n] == tr.n_trials
+    if not same.all():
+        k = int(np.argmin(same))
+        print("cfg%d: free-running oracle and GPU first differ in trial count at iteration %d (margin %.3e)" % (cfg, k, free.margin[k]))
+    plan.close()
+
+
+def test_run_to_tolerance_matches_oracle_stop(m):
+    prob = phantom(0)
+    plan, tr, x, d, _ = run_gpu(m, prob, 400, m.DRIVER_PERSISTENT, delta=1e-3)
+    ref = oracle.run(prob, n_iters=400, delta=1e-3)
+    assert tr.stop_reason == oracle.STOP_TOLERANCE
+    rel = np.abs(np.diff(tr.obj)) / tr.obj[1:]
+    assert rel[-1] < 1e-3 and (rel[:-1] >= 1e-3).all()
+    assert abs(tr.n_iters - ref.n_iters) <= 1
+    plan.close()
+
+
+def test_identity_two_trials_then_stationary(m):
+    # tests/golden/hand_cases.json "identity_two_trials", now through the CUDA path
+    T = np.array([10.0, 20.0, 30.0], np.float32)
+    prob = synth_inputs.Problem("ident", 3, 3, np.array([0, 1, 2, 3], np.int32), np.array([0, 1, 2], np.int32),
+                                np.ones(3, np.float32), np.array([0, 1, 2], np.uint8), T, T, np.ones(3, np.float32),
+                                np.ones(3, np.float32), np.array([12.0, 16.0, 30.0], np.float32), eps=0.2, alpha=2.0, lambda0=1.0)
+    for drv in (0, 1, 2):
+        plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, 5, drv)
+        assert tr.n_iters == 1 and tr.stop_reason == oracle.STOP_STATIONARY
+        assert list(tr.obj) == [20.0, 0.0] and list(tr.n_trials) == [2] and list(tr.lam) == [0.5] and list(tr.step_sq) == [20.0]
+        assert list(x) == [10.0, 20.0, 30.0] and fwd == 3 and trp == 2
+        plan.close()
+
+
+def test_linesearch_stall_and_bad_inputs(m):
+    import torch
+    T = np.array([5.0], np.float32)
+    prob = synth_inputs.Problem("stall", 2, 2, np.array([0, 1, 2], np.int32), np.array([0, 1], np.int32), np.ones(2, np.float32),
+                                np.zeros(2, np.uint8), T, T, np.ones(1, np.float32), np.ones(1, np.float32),
+                                np.array([1.0, 9.0], np.float32), lambda0=1024.0, max_ls=2)
+    plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, 3, m.DRIVER_PERSISTENT)
+    assert tr.n_iters == 0 and tr.stop_reason == oracle.STOP_LS_STALLED and fwd == 1 + 3
+    np.testing.assert_array_equal(x, prob.x0)
+    with pytest.raises(m.ImrtError) as e:
+        plan.set_x(np.array([1.0, -1.0], np.float32))
+    assert e.value.status_name == "BAD_X"
+    plan.close()
+    bad = synth_inputs.Problem(**{**prob.__dict__})
+    bad.col = np.array([0, 2], np.int32)
+    with pytest.raises(m.ImrtError) as e:
+        m.Plan(bad)
+    assert e.value.status_name == "BAD_CSR"
+    bad = synth_inputs.Problem(**{**prob.__dict__})
+    bad.row_ptr = np.array([0, 2, 1], np.int32)
+    with pytest.raises(m.ImrtError) as e:
+        m.Plan(bad)
+    assert e.value.status_name == "BAD_CSR"
+    bad = synth_inputs.Problem(**{**prob.__dict__})
+    bad.sid = np.array([0, 3], np.uint8)
+    with pytest.raises(m.ImrtError) as e:
+        m.Plan(bad)
+    assert e.value.status_name == "BAD_STRUCTURE"
+    bad = synth_inputs.Problem(**{**prob.__dict__})
+    bad.val = np.array([1.0, np.inf], np.float32)
+    with pytest.raises(m.ImrtError) as e:
+        m.Plan(bad)
+    assert e.value.status_name == "BAD_CSR"
+    assert torch.cuda.is_available()
