@@ -275,6 +275,7 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         ++n_skipped;
     };
     int j = 0;
+    uint32_t q_prefix = 0;
     while (j < n_v) {
         if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
         const int r0 = j, p0a = rp[j] & ~3;
@@ -282,7 +283,6 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
             return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
                         rp[j + 1] - rp[j], CHUNK_F - 3);
         int last = j, empties = 0, jj = j + 1;
-        long long len_sum = rp[j + 1] - rp[j];
         int n_full = 1;
         while (jj < n_v && jj - r0 < MAXROWS_F) {
             const int len = rp[jj + 1] - rp[jj];
@@ -294,18 +294,16 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
             if (rp[jj + 1] - p0a > CHUNK_F) break;
             empties = 0;
             last = jj;
-            len_sum += len;
             ++n_full;
             ++jj;
         }
         const int r1 = last + 1, nrows = r1 - r0;
         n_nonempty += n_full;
-        const double mean = (double)len_sum / n_full;
-        const uint32_t lv = mean >= 96.0 ? 5u : mean >= 32.0 ? 4u : mean >= 12.0 ? 3u : 2u;
         const int mo = (int)meta.size();
         meta.push_back((uint32_t)nrows);
         meta.push_back((uint32_t)r0);
-        meta.push_back(lv);
+        meta.push_back(q_prefix & (uint32_t)(W_CONS - 1));   // warp batches dealt so far: round-robin continues across blocks
+        q_prefix += (uint32_t)((nrows + RB - 1) / RB);
         meta.push_back(0u);
         for (int row = r0; row < r1; ++row) meta.push_back((uint32_t)(rp[row] - p0a) | ((uint32_t)sid[row] << 16));
         meta.push_back((uint32_t)(rp[r1] - p0a));
@@ -549,7 +547,12 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     std::vector<int> cta_blk(grid_f + 1, 0);
     {
         std::vector<double> pre(blk.size() + 1, 0.0);
-        for (size_t b = 0; b < blk.size(); ++b) pre[b + 1] = pre[b] + 8.0 * blk[b].y + 4.0 * blk[b].w + 64.0;
+        // cost of a block in SM cycles: the slower of streaming its bytes at a 1/n_sm share of HBM bandwidth and of
+        // issuing its instructions (per-row work dominates where rows are short, e.g. at the field edges)
+        for (size_t b = 0; b < blk.size(); ++b) {
+            const double nz = blk[b].y, rows = blk[b].w - META_HDR - 1;
+            pre[b + 1] = pre[b] + std::max(0.36 * nz, 17.0 * rows + 0.125 * nz) + 20.0;
+        }
         size_t b = 0;
         for (int c = 0; c < grid_f; ++c) {
             const double want = pre[blk.size()] * c / grid_f;

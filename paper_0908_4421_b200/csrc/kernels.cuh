@@ -188,41 +188,64 @@ __device__ __forceinline__ double compute_trial(const float* x, const float* g, 
 }
 
 // ------------------------------------------------------------------------------------------------ dose pass
-// One row group of V lanes per row: gathers x+ from shared memory, fp32 FMA, shuffle reduction, then the voxel's
-// penalty and residual (Eq. (1) generalised: F = w- u^2 + w+ o^2, r = 2 (w+ o - w- u)).
-template <int V>
-__device__ __forceinline__ void fwd_rows(const int* __restrict__ col_s, const float* __restrict__ val_s,
-                                         const uint32_t* __restrict__ meta, const float* __restrict__ x_s,
-                                         const float4* __restrict__ table_s, float* __restrict__ r_out,
-                                         float* __restrict__ d_out, int ctid, double& Gacc) {
-    constexpr int NVEC = N_CONS / V;
+// One warp per row, RB rows per warp batch.  The RB per-lane partial sums are reduced together by a transposing
+// butterfly (RB-1 + log2(32/RB) shuffles per batch instead of 5 per row); the lanes that end up holding the row
+// totals then do the penalty / residual of RB voxels at once (Eq. (1) generalised: F = w- u^2 + w+ o^2,
+// r = 2 (w+ o - w- u)).  Batches are numbered across the CTA's blocks and dealt round-robin to the consumer warps,
+// which never synchronise with each other: a warp with nothing to do in this stage moves on to the next one.
+constexpr int RB = 4;
+
+__device__ __forceinline__ float row_dot(const int* __restrict__ col_s, const float* __restrict__ val_s,
+                                         const float* __restrict__ x_s, int s, int e, int lane) {
+    float a0 = 0.0f, a1 = 0.0f;
+    for (int kb = s; kb < e; kb += 64) {      // warp-uniform trip count; the ragged end is predicated
+        const int k0 = kb + lane, k1 = k0 + 32;
+        const bool p0 = k0 < e, p1 = k1 < e;
+        const int c0 = p0 ? col_s[k0] : 0;
+        const int c1 = p1 ? col_s[k1] : 0;
+        const float v0 = p0 ? val_s[k0] : 0.0f;
+        const float v1 = p1 ? val_s[k1] : 0.0f;
+        a0 = fmaf(v0, x_s[c0], a0);
+        a1 = fmaf(v1, x_s[c1], a1);
+    }
+    return a0 + a1;
+}
+
+__device__ __forceinline__ void dose_block(const int* __restrict__ col_s, const float* __restrict__ val_s,
+                                           const uint32_t* __restrict__ meta, const float* __restrict__ x_s,
+                                           const float4* __restrict__ table_s, float* __restrict__ r_out,
+                                           float* __restrict__ d_out, int warp, int lane, double& Gacc) {
     const int nrows = (int)meta[0];
     const int r0 = (int)meta[1];
-    const int vec = ctid / V, sub = ctid % V;
-    for (int row0 = 0; row0 < nrows; row0 += NVEC) {   // trip count uniform over the CTA: shuffles stay converged
-        const int row = row0 + vec;
-        const bool valid = row < nrows;
-        uint32_t m0 = 0, m1 = 0;
-        if (valid) { m0 = meta[META_HDR + row]; m1 = meta[META_HDR + row + 1]; }
-        const int e = (int)(m1 & 0xFFFFu);
-        int k = (int)(m0 & 0xFFFFu) + sub;
-        float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
-        for (; k + 3 * V < e; k += 4 * V) {
-            const int c0 = col_s[k], c1 = col_s[k + V], c2 = col_s[k + 2 * V], c3 = col_s[k + 3 * V];
-            const float v0 = val_s[k], v1 = val_s[k + V], v2 = val_s[k + 2 * V], v3 = val_s[k + 3 * V];
-            a0 = fmaf(v0, x_s[c0], a0);
-            a1 = fmaf(v1, x_s[c1], a1);
-            a2 = fmaf(v2, x_s[c2], a2);
-            a3 = fmaf(v3, x_s[c3], a3);
+    const int q0 = (int)meta[2];              // batches dealt before this block (mod W_CONS)
+    const int nbatch = (nrows + RB - 1) / RB;
+    for (int q = (warp - q0) & (W_CONS - 1); q < nbatch; q += W_CONS) {
+        const int row0 = q * RB;
+        const int nr = min(RB, nrows - row0);
+        const uint32_t m = (lane <= nr) ? meta[META_HDR + row0 + lane] : 0u;   // offsets (low 16 bits) and structure ids
+        float a[RB];
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            const int s = (int)(__shfl_sync(0xffffffffu, m, i) & 0xFFFFu);
+            const int e = (int)(__shfl_sync(0xffffffffu, m, i + 1) & 0xFFFFu);   // rows past nr: e = 0 <= s, no work
+            a[i] = row_dot(col_s, val_s, x_s, s, e, lane);
         }
-        for (; k < e; k += V) a0 = fmaf(val_s[k], x_s[col_s[k]], a0);
-        const float d = vec_sum<V>((a0 + a1) + (a2 + a3));
-        if (valid && sub == 0) {
-            const float4 t = table_s[(m0 >> 16) & 0xFFu];
+        // transposing butterfly: after the xor-16 and xor-8 steps lane l holds (part of) row 2*bit4(l) + bit3(l)
+        const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
+        float b0 = (up16 ? a[2] : a[0]) + __shfl_xor_sync(0xffffffffu, up16 ? a[0] : a[2], 16);
+        float b1 = (up16 ? a[3] : a[1]) + __shfl_xor_sync(0xffffffffu, up16 ? a[1] : a[3], 16);
+        float d = (up8 ? b1 : b0) + __shfl_xor_sync(0xffffffffu, up8 ? b0 : b1, 8);
+        d += __shfl_xor_sync(0xffffffffu, d, 4);
+        d += __shfl_xor_sync(0xffffffffu, d, 2);
+        d += __shfl_xor_sync(0xffffffffu, d, 1);
+        const int my = lane >> 3;
+        const uint32_t mm = __shfl_sync(0xffffffffu, m, my);
+        if ((lane & 7) == 0 && my < nr) {
+            const float4 t = table_s[(mm >> 16) & 0xFFu];
             const float u = fmaxf(0.0f, t.x - d);
             const float o = fmaxf(0.0f, d - t.y);
-            r_out[r0 + row] = 2.0f * (t.w * o - t.z * u);
-            if (d_out) d_out[r0 + row] = d;
+            r_out[r0 + row0 + my] = 2.0f * (t.w * o - t.z * u);
+            if (d_out) d_out[r0 + row0 + my] = d;
             Gacc += (double)t.z * ((double)u * (double)u) + (double)t.w * ((double)o * (double)o);
         }
     }
@@ -237,61 +260,63 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
     unsigned char* stages = smem + P.stage_off;
     const int b0 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x] : 0;
     const int b1 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x + 1] : 0;
-    unsigned int it = pipe.it_f;
+    int s = (int)(pipe.it_f % (unsigned int)S);
+    unsigned int ph = (pipe.it_f / (unsigned int)S) & 1u;
     double Gacc = 0.0;
 
     if (warp == W_CONS) {
-        // ---------------- producer warp: lane 0 drives the TMA unit
-        const uint64_t pol = policy_evict_first();   // the matrix is streamed once per pass: do not let it push r / x out of L2
+        // ---------------- producer warp: lane 0 drives the TMA unit; descriptors are fetched 32 at a time
+        const uint64_t pol = policy_evict_first();   // the matrix is streamed once per pass: keep it from pushing r / x out of L2
         const int aligned_end = (int)(P.nnz & ~3LL);
-        for (int b = b0; b < b1; ++b, ++it) {
-            const int s = it % S;
-            const unsigned int ph = (it / S) & 1u;
-            if (lane == 0) mbar_wait(&h->empty_f[s], ph ^ 1u);
-            __syncwarp();
-            const int4 d = P.blk[b];
-            int* col_s = reinterpret_cast<int*>(stages + (size_t)s * STAGE_F_BYTES);
-            float* val_s = reinterpret_cast<float*>(col_s + CHUNK_F);
-            uint32_t* meta_s = reinterpret_cast<uint32_t*>(val_s + CHUNK_F);
-            const int n4 = (d.y + 3) & ~3;
-            int nb = aligned_end - d.x;   // elements the bulk copy may touch without leaving the caller's arrays
-            nb = nb < 0 ? 0 : (nb > n4 ? n4 : nb);
-            // the (at most 3) entries of an unaligned matrix end are copied by hand
-            for (int k = nb + lane; k < d.y; k += 32) {
-                col_s[k] = P.col[d.x + k];
-                val_s[k] = P.val[d.x + k];
-            }
-            __syncwarp();
-            if (lane == 0) {
-                mbar_expect_tx(&h->full_f[s], (uint32_t)(nb * 8 + d.w * 4));
-                if (nb > 0) {
-                    bulk_g2s(col_s, P.col + d.x, (uint32_t)nb * 4u, &h->full_f[s], pol);
-                    bulk_g2s(val_s, P.val + d.x, (uint32_t)nb * 4u, &h->full_f[s], pol);
+        for (int bb = b0; bb < b1; bb += 32) {
+            const int4 mine = (bb + lane < b1) ? __ldg(P.blk + bb + lane) : make_int4(0, 0, 0, 0);
+            const int nb_here = min(32, b1 - bb);
+            for (int j = 0; j < nb_here; ++j) {
+                int4 d;
+                d.x = __shfl_sync(0xffffffffu, mine.x, j);
+                d.y = __shfl_sync(0xffffffffu, mine.y, j);
+                d.z = __shfl_sync(0xffffffffu, mine.z, j);
+                d.w = __shfl_sync(0xffffffffu, mine.w, j);
+                if (lane == 0) mbar_wait(&h->empty_f[s], ph ^ 1u);
+                __syncwarp();
+                int* col_s = reinterpret_cast<int*>(stages + (size_t)s * STAGE_F_BYTES);
+                float* val_s = reinterpret_cast<float*>(col_s + CHUNK_F);
+                uint32_t* meta_s = reinterpret_cast<uint32_t*>(val_s + CHUNK_F);
+                const int n4 = (d.y + 3) & ~3;
+                int nb = aligned_end - d.x;   // elements the bulk copy may touch without leaving the caller's arrays
+                nb = nb < 0 ? 0 : (nb > n4 ? n4 : nb);
+                if (nb < d.y) {               // the (at most 3) entries of an unaligned matrix end are copied by hand
+                    for (int k = nb + lane; k < d.y; k += 32) {
+                        col_s[k] = P.col[d.x + k];
+                        val_s[k] = P.val[d.x + k];
+                    }
+                    __syncwarp();
                 }
-                bulk_g2s(meta_s, P.rowmeta + d.z, (uint32_t)d.w * 4u, &h->full_f[s], pol);
+                if (lane == 0) {
+                    mbar_expect_tx(&h->full_f[s], (uint32_t)(nb * 8 + d.w * 4));
+                    if (nb > 0) {
+                        bulk_g2s(col_s, P.col + d.x, (uint32_t)nb * 4u, &h->full_f[s], pol);
+                        bulk_g2s(val_s, P.val + d.x, (uint32_t)nb * 4u, &h->full_f[s], pol);
+                    }
+                    bulk_g2s(meta_s, P.rowmeta + d.z, (uint32_t)d.w * 4u, &h->full_f[s], pol);
+                }
+                if (++s == S) { s = 0; ph ^= 1u; }
             }
         }
     } else {
         // ---------------- consumer warps
-        const int ctid = threadIdx.x;
-        for (int b = b0; b < b1; ++b, ++it) {
-            const int s = it % S;
-            const unsigned int ph = (it / S) & 1u;
+        for (int b = b0; b < b1; ++b) {
             mbar_wait(&h->full_f[s], ph);
             const int* col_s = reinterpret_cast<const int*>(stages + (size_t)s * STAGE_F_BYTES);
             const float* val_s = reinterpret_cast<const float*>(col_s + CHUNK_F);
             const uint32_t* meta_s = reinterpret_cast<const uint32_t*>(val_s + CHUNK_F);
-            switch (meta_s[2]) {
-                case 5: fwd_rows<32>(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, ctid, Gacc); break;
-                case 4: fwd_rows<16>(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, ctid, Gacc); break;
-                case 3: fwd_rows<8>(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, ctid, Gacc); break;
-                default: fwd_rows<4>(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, ctid, Gacc); break;
-            }
+            dose_block(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, warp, lane, Gacc);
             __syncwarp();
             if (lane == 0) mbar_arrive(&h->empty_f[s]);
+            if (++s == S) { s = 0; ph ^= 1u; }
         }
     }
-    pipe.it_f = it;
+    pipe.it_f += (unsigned int)(b1 - b0);
     const double Gcta = block_sum(Gacc, h);   // producer lanes contribute 0
     if (threadIdx.x == 0 && blockIdx.x < P.grid_f) Gpart[blockIdx.x] = Gcta;
     __syncthreads();
@@ -315,6 +340,8 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
     const int S = P.n_stages_t;
     unsigned char* stages = smem + P.stage_off;
     unsigned int it = pipe.it_t;
+    int s = (int)(it % (unsigned int)S);
+    unsigned int ph = (it / (unsigned int)S) & 1u;
 
     if (warp == W_CONS) {
         const uint64_t pol = policy_evict_first();
@@ -322,8 +349,6 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
             for (int rg = blockIdx.x; rg < P.n_ranges; rg += gridDim.x) {
                 const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
                 for (int cs = e0; cs < e1; cs += CHUNK_T, ++it) {
-                    const int s = it % S;
-                    const unsigned int ph = (it / S) & 1u;
                     mbar_wait(&h->empty_t[s], ph ^ 1u);
                     int n = e1 - cs;
                     n = n > CHUNK_T ? CHUNK_T : n;
@@ -334,6 +359,7 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
                     mbar_expect_tx(&h->full_t[s], 2u * bytes);
                     bulk_g2s(col_s, P.colT + (cs - shift), bytes, &h->full_t[s], pol);
                     bulk_g2s(val_s, P.valT + (cs - shift), bytes, &h->full_t[s], pol);
+                    if (++s == S) { s = 0; ph ^= 1u; }
                 }
             }
         } else {
@@ -353,8 +379,6 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
             double dacc = 0.0;
             bool touched = false;
             for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
-                const int s = it % S;
-                const unsigned int ph = (it / S) & 1u;
                 mbar_wait(&h->full_t[s], ph);
                 const int* col_s = reinterpret_cast<const int*>(stages + (size_t)s * STAGE_T_BYTES) + (R.e_begin & 3);
                 const float* val_s = reinterpret_cast<const float*>(stages + (size_t)s * STAGE_T_BYTES) + CHUNK_T_PAD + (R.e_begin & 3);
@@ -394,6 +418,7 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&h->empty_t[s]);
+                if (++s == S) { s = 0; ph ^= 1u; }
             }
             if (touched) {
                 const double sum = warp_sum(dacc);
