@@ -551,7 +551,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         // issuing its instructions (per-row work dominates where rows are short, e.g. at the field edges)
         for (size_t b = 0; b < blk.size(); ++b) {
             const double nz = blk[b].y, rows = blk[b].w - META_HDR - 1;
-            pre[b + 1] = pre[b] + std::max(0.36 * nz, 17.0 * rows + 0.125 * nz) + 20.0;
+            pre[b + 1] = pre[b] + std::max(0.36 * nz, 130.0 + 9.0 * rows + 0.15 * nz);
         }
         size_t b = 0;
         for (int c = 0; c < grid_f; ++c) {
@@ -598,12 +598,12 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
 
     // ---- shared-memory layout (one layout for the three kernels)
     const int nb_pad = (int)((n_b + 31) & ~31LL);
-    int off = SMEM_HEADER + SMEM_TABLE + SMEM_WPART;
+    int off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
     DevPlan& P = pl->P;
     memset(&P, 0, sizeof P);
+    P.wpart_off = off; off += SMEM_WPART;
     P.x_off = off; off += nb_pad * 4;
     P.g_off = off; off += nb_pad * 4;
-    P.xt_off = off; off += nb_pad * 4;
     off = (off + 127) & ~127;
     P.stage_off = off;
     const int avail = smem_optin - off;

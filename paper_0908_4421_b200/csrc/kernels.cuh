@@ -39,10 +39,9 @@ constexpr int SLICE_T = CHUNK_T / W_CONS;     // contiguous nnz per consumer war
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
 constexpr int RL_MAX = 32;                    // rows of D^T one transpose range may span
-constexpr int MAX_STAGES = 8;
+constexpr int MAX_STAGES = 12;
 constexpr int MAX_STRUCTURES = 256;
 constexpr int SMEM_HEADER = 1024;             // barriers, flags, reduction scratch
-constexpr int SMEM_TABLE = MAX_STRUCTURES * 16;
 constexpr int SMEM_WPART = RL_MAX * W_CONS * 8;
 
 enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2 };
@@ -114,7 +113,8 @@ struct DevPlan {
     double* tr_lambda;         // [cap]
     double* tr_step_sq;        // [cap]
     int* tr_trials;            // [cap]
-    int x_off, g_off, xt_off;  // byte offsets of the shared-memory vectors
+    int wpart_off;             // byte offsets into dynamic shared memory: transpose per-(row, warp) partials,
+    int x_off, g_off;          // the trial point x+ (gathered by the dose pass) and the gradient (persistent kernel)
     int stage_off;             // byte offset of the stage ring
 };
 
@@ -131,7 +131,7 @@ struct PassArgs {
 
 // ------------------------------------------------------------------------------------------------ shared memory
 struct SmemHeader {
-    uint64_t full_f[MAX_STAGES], empty_f[MAX_STAGES], full_t[MAX_STAGES], empty_t[MAX_STAGES];   // 256 B
+    uint64_t full_f[MAX_STAGES], empty_f[MAX_STAGES], full_t[MAX_STAGES], empty_t[MAX_STAGES];
     double red[32];            // block-reduction scratch
     double bcast[4];
     int flag;
@@ -172,13 +172,14 @@ __device__ __forceinline__ double block_sum(double v, SmemHeader* h) {
 
 // ------------------------------------------------------------------------------------------------ trial point
 // x+ = max(0, x - lambda g), Delta = sum (x+ - x)^2      PAPER.md:90 (projection), :109/:111 (steps 2, 4), Eq. (5).
-// fp32 elementwise, fp64 sum.  All NTHREADS threads call it; x, g, x_new may be shared or global memory.
+// fp32 elementwise, fp64 sum.  All NTHREADS threads call it; x is global (read through L2: another CTA may have
+// written it), g and x_new may be shared or global memory.
 __device__ __forceinline__ double compute_trial(const float* x, const float* g, double lambda, float* x_new, int n_b,
                                                 SmemHeader* h) {
     const float lam = (float)lambda;
     double acc = 0.0;
     for (int i = threadIdx.x; i < n_b; i += NTHREADS) {
-        const float xi = x[i];
+        const float xi = __ldcg(x + i);
         const float xn = fmaxf(0.0f, fmaf(-lam, g[i], xi));
         const float dx = xn - xi;
         acc += (double)dx * (double)dx;
@@ -188,64 +189,48 @@ __device__ __forceinline__ double compute_trial(const float* x, const float* g, 
 }
 
 // ------------------------------------------------------------------------------------------------ dose pass
-// One warp per row, RB rows per warp batch.  The RB per-lane partial sums are reduced together by a transposing
-// butterfly (RB-1 + log2(32/RB) shuffles per batch instead of 5 per row); the lanes that end up holding the row
-// totals then do the penalty / residual of RB voxels at once (Eq. (1) generalised: F = w- u^2 + w+ o^2,
-// r = 2 (w+ o - w- u)).  Batches are numbered across the CTA's blocks and dealt round-robin to the consumer warps,
-// which never synchronise with each other: a warp with nothing to do in this stage moves on to the next one.
-constexpr int RB = 4;
-
-__device__ __forceinline__ float row_dot(const int* __restrict__ col_s, const float* __restrict__ val_s,
-                                         const float* __restrict__ x_s, int s, int e, int lane) {
-    float a0 = 0.0f, a1 = 0.0f;
-    for (int kb = s; kb < e; kb += 64) {      // warp-uniform trip count; the ragged end is predicated
-        const int k0 = kb + lane, k1 = k0 + 32;
-        const bool p0 = k0 < e, p1 = k1 < e;
-        const int c0 = p0 ? col_s[k0] : 0;
-        const int c1 = p1 ? col_s[k1] : 0;
-        const float v0 = p0 ? val_s[k0] : 0.0f;
-        const float v1 = p1 ? val_s[k1] : 0.0f;
-        a0 = fmaf(v0, x_s[c0], a0);
-        a1 = fmaf(v1, x_s[c1], a1);
-    }
-    return a0 + a1;
-}
+// VW lanes per row, RB = 32 / VW rows per warp batch: the four row groups of a warp run the same trip count (the
+// longest of their rows; neighbouring voxels have rows of similar length), gather x+ from shared memory, multiply-add
+// in fp32 and reduce with log2(VW) shuffles; lane 0 of each group then does its voxel's penalty and residual
+// (Eq. (1) generalised: F = w- u^2 + w+ o^2, r = 2 (w+ o - w- u)).  Batches are numbered across the CTA's blocks and
+// dealt round-robin to the consumer warps, which never synchronise with each other: a warp with nothing to do in
+// this stage moves on to the next one.
+constexpr int VW = 8;
+constexpr int RB = 32 / VW;
 
 __device__ __forceinline__ void dose_block(const int* __restrict__ col_s, const float* __restrict__ val_s,
                                            const uint32_t* __restrict__ meta, const float* __restrict__ x_s,
                                            const float4* __restrict__ table_s, float* __restrict__ r_out,
                                            float* __restrict__ d_out, int warp, int lane, double& Gacc) {
-    const int nrows = (int)meta[0];
-    const int r0 = (int)meta[1];
-    const int q0 = (int)meta[2];              // batches dealt before this block (mod W_CONS)
+    const uint4 hdr = *reinterpret_cast<const uint4*>(meta);   // {rows, first row, batches dealt before (mod W_CONS), -}
+    const int nrows = (int)hdr.x;
     const int nbatch = (nrows + RB - 1) / RB;
-    for (int q = (warp - q0) & (W_CONS - 1); q < nbatch; q += W_CONS) {
-        const int row0 = q * RB;
-        const int nr = min(RB, nrows - row0);
-        const uint32_t m = (lane <= nr) ? meta[META_HDR + row0 + lane] : 0u;   // offsets (low 16 bits) and structure ids
-        float a[RB];
-#pragma unroll
-        for (int i = 0; i < RB; ++i) {
-            const int s = (int)(__shfl_sync(0xffffffffu, m, i) & 0xFFFFu);
-            const int e = (int)(__shfl_sync(0xffffffffu, m, i + 1) & 0xFFFFu);   // rows past nr: e = 0 <= s, no work
-            a[i] = row_dot(col_s, val_s, x_s, s, e, lane);
+    const int grp = lane / VW, sub = lane % VW;
+    for (int q = (warp - (int)hdr.z) & (W_CONS - 1); q < nbatch; q += W_CONS) {
+        const int row = q * RB + grp;
+        const bool valid = row < nrows;
+        uint32_t m0 = 0u, m1 = 0u;
+        if (valid) { m0 = meta[META_HDR + row]; m1 = meta[META_HDR + row + 1]; }
+        const int s = (int)(m0 & 0xFFFFu), e = (int)(m1 & 0xFFFFu);
+        const int len_max = __reduce_max_sync(0xffffffffu, e - s);   // warp-uniform trip count
+        float a0 = 0.0f, a1 = 0.0f;
+        int k = s + sub;
+        for (int kb = 0; kb < len_max; kb += 2 * VW, k += 2 * VW) {
+            const bool p0 = k < e, p1 = k + VW < e;
+            const int c0 = p0 ? col_s[k] : 0;
+            const int c1 = p1 ? col_s[k + VW] : 0;
+            const float v0 = p0 ? val_s[k] : 0.0f;
+            const float v1 = p1 ? val_s[k + VW] : 0.0f;
+            a0 = fmaf(v0, x_s[c0], a0);
+            a1 = fmaf(v1, x_s[c1], a1);
         }
-        // transposing butterfly: after the xor-16 and xor-8 steps lane l holds (part of) row 2*bit4(l) + bit3(l)
-        const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
-        float b0 = (up16 ? a[2] : a[0]) + __shfl_xor_sync(0xffffffffu, up16 ? a[0] : a[2], 16);
-        float b1 = (up16 ? a[3] : a[1]) + __shfl_xor_sync(0xffffffffu, up16 ? a[1] : a[3], 16);
-        float d = (up8 ? b1 : b0) + __shfl_xor_sync(0xffffffffu, up8 ? b0 : b1, 8);
-        d += __shfl_xor_sync(0xffffffffu, d, 4);
-        d += __shfl_xor_sync(0xffffffffu, d, 2);
-        d += __shfl_xor_sync(0xffffffffu, d, 1);
-        const int my = lane >> 3;
-        const uint32_t mm = __shfl_sync(0xffffffffu, m, my);
-        if ((lane & 7) == 0 && my < nr) {
-            const float4 t = table_s[(mm >> 16) & 0xFFu];
+        const float d = vec_sum<VW>(a0 + a1);
+        if (valid && sub == 0) {
+            const float4 t = table_s[(m0 >> 16) & 0xFFu];
             const float u = fmaxf(0.0f, t.x - d);
             const float o = fmaxf(0.0f, d - t.y);
-            r_out[r0 + row0 + my] = 2.0f * (t.w * o - t.z * u);
-            if (d_out) d_out[r0 + row0 + my] = d;
+            r_out[hdr.y + row] = 2.0f * (t.w * o - t.z * u);
+            if (d_out) d_out[hdr.y + row] = d;
             Gacc += (double)t.z * ((double)u * (double)u) + (double)t.w * ((double)o * (double)o);
         }
     }
@@ -263,6 +248,7 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
     int s = (int)(pipe.it_f % (unsigned int)S);
     unsigned int ph = (pipe.it_f / (unsigned int)S) & 1u;
     double Gacc = 0.0;
+    const uint32_t full_a = smem_u32(&h->full_f[0]), empty_a = smem_u32(&h->empty_f[0]), stages_a = smem_u32(stages);
 
     if (warp == W_CONS) {
         // ---------------- producer warp: lane 0 drives the TMA unit; descriptors are fetched 32 at a time
@@ -277,15 +263,14 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
                 d.y = __shfl_sync(0xffffffffu, mine.y, j);
                 d.z = __shfl_sync(0xffffffffu, mine.z, j);
                 d.w = __shfl_sync(0xffffffffu, mine.w, j);
-                if (lane == 0) mbar_wait(&h->empty_f[s], ph ^ 1u);
+                if (lane == 0) mbar_wait_a(empty_a + 8u * s, ph ^ 1u);
                 __syncwarp();
-                int* col_s = reinterpret_cast<int*>(stages + (size_t)s * STAGE_F_BYTES);
-                float* val_s = reinterpret_cast<float*>(col_s + CHUNK_F);
-                uint32_t* meta_s = reinterpret_cast<uint32_t*>(val_s + CHUNK_F);
                 const int n4 = (d.y + 3) & ~3;
                 int nb = aligned_end - d.x;   // elements the bulk copy may touch without leaving the caller's arrays
                 nb = nb < 0 ? 0 : (nb > n4 ? n4 : nb);
                 if (nb < d.y) {               // the (at most 3) entries of an unaligned matrix end are copied by hand
+                    int* col_s = reinterpret_cast<int*>(stages + (size_t)s * STAGE_F_BYTES);
+                    float* val_s = reinterpret_cast<float*>(col_s + CHUNK_F);
                     for (int k = nb + lane; k < d.y; k += 32) {
                         col_s[k] = P.col[d.x + k];
                         val_s[k] = P.val[d.x + k];
@@ -293,27 +278,32 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
                     __syncwarp();
                 }
                 if (lane == 0) {
-                    mbar_expect_tx(&h->full_f[s], (uint32_t)(nb * 8 + d.w * 4));
+                    const uint32_t st_a = stages_a + (uint32_t)s * STAGE_F_BYTES, bar = full_a + 8u * s;
+                    mbar_expect_tx_a(bar, (uint32_t)(nb * 8 + d.w * 4));
                     if (nb > 0) {
-                        bulk_g2s(col_s, P.col + d.x, (uint32_t)nb * 4u, &h->full_f[s], pol);
-                        bulk_g2s(val_s, P.val + d.x, (uint32_t)nb * 4u, &h->full_f[s], pol);
+                        bulk_g2s_a(st_a, P.col + d.x, (uint32_t)nb * 4u, bar, pol);
+                        bulk_g2s_a(st_a + CHUNK_F * 4, P.val + d.x, (uint32_t)nb * 4u, bar, pol);
                     }
-                    bulk_g2s(meta_s, P.rowmeta + d.z, (uint32_t)d.w * 4u, &h->full_f[s], pol);
+                    bulk_g2s_a(st_a + CHUNK_F * 8, P.rowmeta + d.z, (uint32_t)d.w * 4u, bar, pol);
                 }
                 if (++s == S) { s = 0; ph ^= 1u; }
             }
         }
     } else {
         // ---------------- consumer warps
+        const unsigned char* st_p = stages + (size_t)s * STAGE_F_BYTES;
+        const unsigned char* st_end = stages + (size_t)S * STAGE_F_BYTES;
+        uint32_t fb = full_a + 8u * s, eb = empty_a + 8u * s;
         for (int b = b0; b < b1; ++b) {
-            mbar_wait(&h->full_f[s], ph);
-            const int* col_s = reinterpret_cast<const int*>(stages + (size_t)s * STAGE_F_BYTES);
-            const float* val_s = reinterpret_cast<const float*>(col_s + CHUNK_F);
-            const uint32_t* meta_s = reinterpret_cast<const uint32_t*>(val_s + CHUNK_F);
+            mbar_wait_a(fb, ph);
+            const int* col_s = reinterpret_cast<const int*>(st_p);
+            const float* val_s = reinterpret_cast<const float*>(st_p + CHUNK_F * 4);
+            const uint32_t* meta_s = reinterpret_cast<const uint32_t*>(st_p + CHUNK_F * 8);
             dose_block(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, warp, lane, Gacc);
             __syncwarp();
-            if (lane == 0) mbar_arrive(&h->empty_f[s]);
-            if (++s == S) { s = 0; ph ^= 1u; }
+            if (lane == 0) mbar_arrive_a(eb);
+            st_p += STAGE_F_BYTES; fb += 8u; eb += 8u;
+            if (st_p == st_end) { st_p = stages; fb = full_a; eb = empty_a; ph ^= 1u; }
         }
     }
     pipe.it_f += (unsigned int)(b1 - b0);
@@ -583,7 +573,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dose(const __grid_constant__ De
 __global__ void __launch_bounds__(NTHREADS, 1) k_transpose(const __grid_constant__ DevPlan P, const PassArgs A) {
     SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
     float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
-    double* wpart = reinterpret_cast<double*>(imrt_smem + SMEM_HEADER + SMEM_TABLE);
+    double* wpart = reinterpret_cast<double*>(imrt_smem + P.wpart_off);
     State* st = P.st;
     cta_init(h, P, table_s);
     const int xi = st->xi, ri = st->ri;
@@ -637,18 +627,14 @@ __global__ void k_set_target(State* st, int n_more, double delta_tol) {
 __global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constant__ DevPlan P) {
     SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
     float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
-    double* wpart = reinterpret_cast<double*>(imrt_smem + SMEM_HEADER + SMEM_TABLE);
-    float* xa = reinterpret_cast<float*>(imrt_smem + P.x_off);     // x_k   (swapped with xb on accept)
+    double* wpart = reinterpret_cast<double*>(imrt_smem + P.wpart_off);
+    float* xb = reinterpret_cast<float*>(imrt_smem + P.x_off);     // x+ (the dose pass gathers from it)
     float* g_s = reinterpret_cast<float*>(imrt_smem + P.g_off);
-    float* xb = reinterpret_cast<float*>(imrt_smem + P.xt_off);    // x+
     State* st = P.st;
     cta_init(h, P, table_s);
     Loop L;
     loop_load(st, L);
     const int iter_target = st->iter_target;
-    const int xi0 = L.xi;
-    for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) xa[i] = P.xbuf[xi0][i];
-    __syncthreads();
     L.stop_reason = STOP_MAX_ITERS;
     Pipe pipe = {0u, 0u};
     unsigned int epoch = 0;
@@ -660,7 +646,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constan
         grid_barrier(&st->gridbar, epoch);
         reduce_gradient(P, P.gslot[tpar], g_s);
         __syncthreads();
-        if (!begin_line_search(st, L, xa, g_s, xb, P.n_b, h)) break;
+        if (!begin_line_search(st, L, P.xbuf[L.xi], g_s, xb, P.n_b, h)) break;   // x_k lives in global memory
         int dec;
         for (;;) {
             const int fpar = (int)(L.fwd & 1);
@@ -669,16 +655,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constan
             const double G_new = reduce_objective(P, P.Gpart[fpar], h);
             dec = armijo_decide(P, st, L, G_new, rec);
             if (dec != DEC_REJECT_RETRY) break;
-            L.step_sq = compute_trial(xa, g_s, L.lambda, xb, P.n_b, h);
+            L.step_sq = compute_trial(P.xbuf[L.xi], g_s, L.lambda, xb, P.n_b, h);
         }
-        if (dec == DEC_ACCEPT_CONTINUE || dec == DEC_ACCEPT_STOP) { float* t = xa; xa = xb; xb = t; }
+        if ((dec == DEC_ACCEPT_CONTINUE || dec == DEC_ACCEPT_STOP) && blockIdx.x == 0) {
+            // x_{k+1} = x+: publish it (L.xi already points at the new buffer); the other CTAs read it only after the
+            // next grid barrier
+            float* xg = P.xbuf[L.xi];
+            for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) xg[i] = xb[i];
+        }
         if (dec != DEC_ACCEPT_CONTINUE) break;
     }
     // every CTA has passed the last grid barrier before CTA 0 gets here with a changed state
     grid_barrier(&st->gridbar, epoch);
     if (blockIdx.x == 0) {
-        float* xg = P.xbuf[L.xi];
-        for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) xg[i] = xa[i];
         for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) P.g[i] = g_s[i];
         if (threadIdx.x == 0) {
             loop_store(st, L);
