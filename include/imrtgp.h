@@ -182,6 +182,15 @@ imrt_status imrt_plan_get_info(imrt_plan* plan, int64_t* host_info, int32_t n_in
  */
 imrt_status imrt_plan_launch_pass(imrt_plan* plan, int32_t kind, int32_t n_repeat);
 
+/*
+ * Per-CTA timing of the most recent dose (kind 0) or transpose (kind 1) pass: the global-timer nanoseconds at
+ * which each persistent CTA started and finished streaming its share of the matrix.  Shows how well the static
+ * partition is balanced.  host_start_ns / host_end_ns hold `capacity` entries; *host_n_ctas receives the grid size.
+ * Synchronises.
+ */
+imrt_status imrt_plan_get_pass_timing(imrt_plan* plan, int32_t kind, int64_t* host_start_ns, int64_t* host_end_ns,
+                                      int32_t capacity, int32_t* host_n_ctas);
+
 /* Message of the last error on this plan (or of the last failed imrt_plan_create when plan is NULL).
  * Owned by the library, valid until the next call on the same plan / thread. */
 const char* imrt_last_error(const imrt_plan* plan);

@@ -28,7 +28,7 @@ DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
 # every symbol include/imrtgp.h declares
 EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
            "imrt_plan_eval", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
-           "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_last_error", "imrt_plan_destroy",
+           "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_last_error", "imrt_plan_destroy",
            "imrt_version")
 
 
@@ -77,6 +77,7 @@ def lib() -> ctypes.CDLL:
         L.imrt_plan_get_counters.argtypes = [_P, ctypes.POINTER(i64), ctypes.POINTER(i64)]
         L.imrt_plan_get_info.argtypes = [_P, _P, i32, _P, _P, _P]
         L.imrt_plan_launch_pass.argtypes = [_P, i32, i32]
+        L.imrt_plan_get_pass_timing.argtypes = [_P, i32, _P, _P, i32, ctypes.POINTER(i32)]
         L.imrt_plan_destroy.argtypes = [_P]
         L.imrt_last_error.argtypes = [_P]
         L.imrt_last_error.restype = ctypes.c_char_p
@@ -222,6 +223,15 @@ def imrt_plan_launch_pass(plan, kind: int, n_repeat: int):
     _check(lib().imrt_plan_launch_pass(plan, kind, n_repeat), plan)
 
 
+def imrt_plan_get_pass_timing(plan, kind: int):
+    """(start_ns, end_ns) int64 arrays, one entry per CTA of the last dose (0) / transpose (1) pass."""
+    s = np.zeros(1024, np.int64)
+    e = np.zeros(1024, np.int64)
+    n = ctypes.c_int32(0)
+    _check(lib().imrt_plan_get_pass_timing(plan, kind, _hptr(s), _hptr(e), 1024, ctypes.byref(n)), plan)
+    return s[:n.value].copy(), e[:n.value].copy()
+
+
 def imrt_plan_destroy(plan):
     _check(lib().imrt_plan_destroy(plan))
 
@@ -322,6 +332,9 @@ class Plan:
         v = torch.empty(max(self.nnz, 1), dtype=torch.float32, device=self.device)
         imrt_plan_get_info(self.handle, rp, c, v)
         return rp, c[:self.nnz], v[:self.nnz]
+
+    def pass_timing(self, kind: int):
+        return imrt_plan_get_pass_timing(self.handle, int(kind))
 
     def launch_pass(self, kind: int, n_repeat: int = 1):
         imrt_plan_launch_pass(self.handle, int(kind), int(n_repeat))

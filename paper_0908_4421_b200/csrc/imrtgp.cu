@@ -121,6 +121,7 @@ struct Layout {
     float* g_scratch;
     float* d_scratch;
     int* flags;
+    unsigned long long* cta_ns;
     DvhWork dvh;
     // build scratch
     unsigned int* keysA;
@@ -159,6 +160,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.g_scratch = w.take<float>(n_b + 4);
     L.d_scratch = w.take<float>(n_v + 4);
     L.flags = w.take<int>(16);
+    L.cta_ns = w.take<unsigned long long>(4096);
     L.dvh.hist = w.take<unsigned int>((size_t)n_s * DVH_MAX_PCTS * DVH_BINS);
     L.dvh.cnt = w.take<unsigned int>((size_t)MAX_STRUCTURES);
     L.dvh.sum = w.take<double>((size_t)MAX_STRUCTURES);
@@ -621,6 +623,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.table = L.table; P.n_structures = n_structures; P.G_skip = G_skip;
     P.xbuf[0] = L.xbuf[0]; P.xbuf[1] = L.xbuf[1]; P.g = L.g; P.rbuf[0] = L.rbuf[0]; P.rbuf[1] = L.rbuf[1];
     P.Gpart[0] = L.Gpart[0]; P.Gpart[1] = L.Gpart[1]; P.gslot[0] = L.gslot[0]; P.gslot[1] = L.gslot[1];
+    P.cta_ns = L.cta_ns;
     P.st = L.st; P.tr_obj = L.tr_obj; P.tr_lambda = L.tr_lambda; P.tr_step_sq = L.tr_step_sq; P.tr_trials = L.tr_trials;
     pl->r_scratch = L.r_scratch; pl->g_scratch = L.g_scratch; pl->d_scratch = L.d_scratch;
     pl->rowT_ptr_w = L.rowT_ptr; pl->colT_w = L.colT; pl->valT_w = L.valT;
@@ -642,6 +645,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[0], 0, sizeof(double) * 1024, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[1], 0, sizeof(double) * 1024, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.g, 0, sizeof(float) * (n_b + 4), st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.cta_ns, 0, sizeof(unsigned long long) * 4096, st));
     k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, (int)n_v, L.rbuf[0], L.rbuf[1], nullptr);
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
@@ -831,6 +835,21 @@ imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info
     if (d_colT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_colT, pl->colT_w, sizeof(int) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));
     if (d_valT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_valT, pl->valT_w, sizeof(float) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(pl, cudaStreamSynchronize(st));
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_pass_timing(imrt_plan* pl, int32_t kind, int64_t* host_start_ns, int64_t* host_end_ns, int32_t capacity,
+                                      int32_t* host_n_ctas) {
+    if (!pl || kind < 0 || kind > 1 || capacity < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_pass_timing: bad argument");
+    const int n = kind == 0 ? pl->P.grid_f : (pl->prm.driver == 2 ? pl->grid_p : pl->P.grid_t);
+    std::vector<unsigned long long> t(2048);
+    CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns + 2048 * kind, sizeof(unsigned long long) * 2048, cudaMemcpyDeviceToHost, pl->stream));
+    CUDA_TRY(pl, cudaStreamSynchronize(pl->stream));
+    if (host_n_ctas) *host_n_ctas = n;
+    for (int c = 0; c < n && c < capacity; ++c) {
+        if (host_start_ns) host_start_ns[c] = (int64_t)t[2 * c];
+        if (host_end_ns) host_end_ns[c] = (int64_t)t[2 * c + 1];
+    }
     return IMRT_STATUS_OK;
 }
 

@@ -109,6 +109,7 @@ struct DevPlan {
     double* Gpart[2];          // [grid_f] objective partials, double-buffered by pass parity
     double* gslot[2];          // [n_slots] gradient partials, double-buffered
     State* st;
+    unsigned long long* cta_ns;  // [2][1024][2] per-CTA {start, end of streaming} of the last dose / transpose pass, ns
     double* tr_obj;            // trace: [cap + 1]
     double* tr_lambda;         // [cap]
     double* tr_step_sq;        // [cap]
@@ -154,6 +155,12 @@ __device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4
     }
     for (int s = threadIdx.x; s < P.n_structures; s += NTHREADS) table_s[s] = P.table[s];
     __syncthreads();
+}
+
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
 }
 
 // ------------------------------------------------------------------------------------------------ block reduce
@@ -248,14 +255,17 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
     int s = (int)(pipe.it_f % (unsigned int)S);
     unsigned int ph = (pipe.it_f / (unsigned int)S) & 1u;
     double Gacc = 0.0;
+    const unsigned long long t_start = global_ns();
     const uint32_t full_a = smem_u32(&h->full_f[0]), empty_a = smem_u32(&h->empty_f[0]), stages_a = smem_u32(stages);
 
     if (warp == W_CONS) {
         // ---------------- producer warp: lane 0 drives the TMA unit; descriptors are fetched 32 at a time
         const uint64_t pol = policy_evict_first();   // the matrix is streamed once per pass: keep it from pushing r / x out of L2
         const int aligned_end = (int)(P.nnz & ~3LL);
+        int4 next = (b0 + lane < b1) ? __ldg(P.blk + b0 + lane) : make_int4(0, 0, 0, 0);
         for (int bb = b0; bb < b1; bb += 32) {
-            const int4 mine = (bb + lane < b1) ? __ldg(P.blk + bb + lane) : make_int4(0, 0, 0, 0);
+            const int4 mine = next;       // the following 32 descriptors are requested before these are issued
+            next = (bb + 32 + lane < b1) ? __ldg(P.blk + bb + 32 + lane) : make_int4(0, 0, 0, 0);
             const int nb_here = min(32, b1 - bb);
             for (int j = 0; j < nb_here; ++j) {
                 int4 d;
@@ -279,12 +289,22 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
                 }
                 if (lane == 0) {
                     const uint32_t st_a = stages_a + (uint32_t)s * STAGE_F_BYTES, bar = full_a + 8u * s;
+#if defined(IMRT_EXP_NO_META)
+                    mbar_expect_tx_a(bar, (uint32_t)(nb * 8));
+                    bulk_g2s_a(st_a, P.col + d.x, (uint32_t)nb * 4u, bar, pol);
+                    bulk_g2s_a(st_a + CHUNK_F * 4, P.val + d.x, (uint32_t)nb * 4u, bar, pol);
+#elif defined(IMRT_EXP_ALIGNED)
+                    mbar_expect_tx_a(bar, 16384u);
+                    bulk_g2s_a(st_a, P.col + (d.x & ~31), 8192u, bar, pol);
+                    bulk_g2s_a(st_a + CHUNK_F * 4, P.val + (d.x & ~31), 8192u, bar, pol);
+#else
                     mbar_expect_tx_a(bar, (uint32_t)(nb * 8 + d.w * 4));
                     if (nb > 0) {
                         bulk_g2s_a(st_a, P.col + d.x, (uint32_t)nb * 4u, bar, pol);
                         bulk_g2s_a(st_a + CHUNK_F * 4, P.val + d.x, (uint32_t)nb * 4u, bar, pol);
                     }
                     bulk_g2s_a(st_a + CHUNK_F * 8, P.rowmeta + d.z, (uint32_t)d.w * 4u, bar, pol);
+#endif
                 }
                 if (++s == S) { s = 0; ph ^= 1u; }
             }
@@ -299,7 +319,9 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
             const int* col_s = reinterpret_cast<const int*>(st_p);
             const float* val_s = reinterpret_cast<const float*>(st_p + CHUNK_F * 4);
             const uint32_t* meta_s = reinterpret_cast<const uint32_t*>(st_p + CHUNK_F * 8);
+#ifndef IMRT_EXP_SKIP_COMPUTE
             dose_block(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, warp, lane, Gacc);
+#endif
             __syncwarp();
             if (lane == 0) mbar_arrive_a(eb);
             st_p += STAGE_F_BYTES; fb += 8u; eb += 8u;
@@ -308,7 +330,11 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
     }
     pipe.it_f += (unsigned int)(b1 - b0);
     const double Gcta = block_sum(Gacc, h);   // producer lanes contribute 0
-    if (threadIdx.x == 0 && blockIdx.x < P.grid_f) Gpart[blockIdx.x] = Gcta;
+    if (threadIdx.x == 0 && blockIdx.x < P.grid_f) {
+        Gpart[blockIdx.x] = Gcta;
+        P.cta_ns[2 * blockIdx.x] = t_start;            // when this CTA's share of the pass began and ended: lets the
+        P.cta_ns[2 * blockIdx.x + 1] = global_ns();    // host see (and rebalance) the static partition
+    }
     __syncthreads();
 }
 
@@ -330,6 +356,7 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
     const int S = P.n_stages_t;
     unsigned char* stages = smem + P.stage_off;
     unsigned int it = pipe.it_t;
+    const unsigned long long t_start = global_ns();
     int s = (int)(it % (unsigned int)S);
     unsigned int ph = (it / (unsigned int)S) & 1u;
 
@@ -427,6 +454,10 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
     pipe.it_t = it;
     __threadfence();
     __syncthreads();
+    if (threadIdx.x == 0) {
+        P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
+        P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
+    }
 }
 
 // g_i = sum of the slots of row i, in slot order (fixed).  All NTHREADS threads; g_out shared or global.
