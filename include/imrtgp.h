@@ -168,8 +168,8 @@ imrt_status imrt_plan_get_counters(imrt_plan* plan, int64_t* host_fwd_passes, in
 /*
  * Introspection for tests and the benchmark.  Synchronises.
  *   host_info[0] nnz of D^T        [1] forward row blocks     [2] forward grid (CTAs)   [3] transpose grid (CTAs)
- *   host_info[4] forward dynamic smem bytes   [5] transpose dynamic smem bytes   [6] gradient partial slots
- *   host_info[7] non-empty rows of D          [8] SM count    [9] x staged in shared memory (1) or read via L1/L2 (0)
+ *   host_info[4] dynamic shared memory bytes per CTA   [5] bytes of the re-packed D the dose pass streams
+ *   host_info[6] gradient partial slots   [7] non-empty rows of D   [8] SM count   [9] 16-bit column indices (1/0)
  * d_rowT_ptr (int32 [n_b+1]), d_colT (int32 [nnz]), d_valT (fp32 [nnz]): if non-NULL receive a copy of D^T (device).
  */
 imrt_status imrt_plan_get_info(imrt_plan* plan, int64_t* host_info, int32_t n_info,

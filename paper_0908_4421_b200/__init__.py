@@ -208,7 +208,7 @@ def imrt_plan_get_counters(plan):
     return f.value, t.value
 
 
-INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "fwd_smem", "tr_smem", "g_slots", "nonempty_rows", "n_sm", "x_in_smem")
+INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "smem_bytes", "pack_bytes", "g_slots", "nonempty_rows", "n_sm", "col16")
 
 
 def imrt_plan_get_info(plan, rowT_ptr=None, colT=None, valT=None) -> dict:

@@ -30,7 +30,7 @@ struct imrt_plan {
     size_t smem_bytes;
     int grid_p;                       // persistent kernel grid
     bool has_x;
-    int64_t n_blk, n_nonempty, n_skipped;
+    int64_t n_blk, n_nonempty, n_skipped, pack_bytes;
     // borrowed inputs
     const int32_t* row_ptr;
     const uint8_t* sid;
@@ -83,13 +83,15 @@ struct Bump {                           // the same walk sizes the workspace and
 
 struct Bounds {
     int64_t max_blk, max_meta, max_ranges, max_slots, nnz_pad;
-    size_t sort_temp;
+    size_t sort_temp, max_pack;
 };
 
 Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     Bounds b;
-    b.max_blk = 2 * (nnz / (CHUNK_F - 3) + 1) + 2 * (n_v / MAXROWS_F + 1) + n_v / 32 + 4;
+    const int64_t slots = nnz + 3 * n_v;    // every row padded to a multiple of 4 slots
+    b.max_blk = 2 * (slots / MIN_CHUNK_SLOTS + 1) + 2 * (n_v / MAXROWS_F + 1) + n_v / 32 + 4;
     b.max_meta = n_v + b.max_blk * (META_HDR + 1 + 3) + 8;
+    b.max_pack = (size_t)b.max_meta * 4 + (size_t)slots * 8 + (size_t)b.max_blk * 128 + 256;
     b.max_ranges = 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
     b.max_slots = n_b + b.max_ranges + 4;
     b.nnz_pad = ((nnz + 3) & ~(int64_t)3) + 8;
@@ -100,8 +102,10 @@ Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
 struct Layout {
     State* st;
     float4* table;
-    int4* blk;
+    int2* blk;
+    int4* pk;
     uint32_t* rowmeta;
+    unsigned char* pack;
     int* cta_blk;
     int* rowT_ptr;
     int* colT;
@@ -138,8 +142,10 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     Layout L;
     L.st = w.take<State>(1);
     L.table = w.take<float4>(MAX_STRUCTURES);
-    L.blk = w.take<int4>(B.max_blk);
+    L.blk = w.take<int2>(B.max_blk);
+    L.pk = w.take<int4>(B.max_blk);
     L.rowmeta = w.take<uint32_t>(B.max_meta);
+    L.pack = w.take<unsigned char>(B.max_pack);
     L.cta_blk = w.take<int>(1024 + 1);
     L.rowT_ptr = w.take<int>(n_b + 1);
     L.colT = w.take<int>(B.nnz_pad);
@@ -220,6 +226,33 @@ __global__ void k_fill_transpose(const unsigned int* __restrict__ perm, const in
     }
 }
 
+// Re-pack D into the dose pass's block records: one CTA per block copies the header and row table, then one warp per
+// row copies values and columns (16- or 32-bit) to the row's 16-byte aligned slot range and zero-fills the padding.
+template <bool COL16>
+__global__ void k_pack_blocks(const int4* __restrict__ pk, const uint32_t* __restrict__ meta, const int* __restrict__ row_ptr,
+                              const int* __restrict__ col, const float* __restrict__ val, unsigned char* pack) {
+    const int4 d = pk[blockIdx.x];
+    const uint32_t* m = meta + d.x;
+    unsigned char* rec = pack + (size_t)(unsigned int)d.z * 128u;
+    uint32_t* rec_w = reinterpret_cast<uint32_t*>(rec);
+    for (int i = threadIdx.x; i < d.y; i += blockDim.x) rec_w[i] = m[i];
+    const int nrows = (int)m[0], r0 = (int)m[1], slots = (int)m[3];
+    float* val_o = reinterpret_cast<float*>(rec + (size_t)d.y * 4);
+    unsigned char* col_o = reinterpret_cast<unsigned char*>(val_o + slots);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+    for (int row = warp; row < nrows; row += nwarp) {
+        const int so = (int)(m[META_HDR + row] & 0xFFFFu), se = (int)(m[META_HDR + row + 1] & 0xFFFFu);
+        const int p0 = row_ptr[r0 + row], len = row_ptr[r0 + row + 1] - p0;
+        for (int k = lane; k < se - so; k += 32) {
+            const float v = k < len ? val[p0 + k] : 0.0f;
+            const int c = k < len ? col[p0 + k] : 0;
+            val_o[so + k] = v;
+            if (COL16) reinterpret_cast<unsigned short*>(col_o)[so + k] = (unsigned short)c;
+            else reinterpret_cast<int*>(col_o)[so + k] = c;
+        }
+    }
+}
+
 // d = 0 and the matching constant residual on every row; the dose pass then overwrites the rows its blocks cover.
 __global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, int n_v, float* r0,
                                       float* r1, float* d) {
@@ -262,10 +295,19 @@ inline int grid_for(long long n, int block) {
 }
 
 // ------------------------------------------------------------------------------------------------ host builders
-// Row-aligned blocks of D for the dose pass (each fits one pipeline stage) and their packed row metadata.
+// Row-aligned blocks of D for the dose pass.  Each block becomes one self-contained record of the packed stream
+// (layout: kernels.cuh, DevPlan::pack); this lays the records out and writes their headers and row tables.
+struct BlockPlan {
+    std::vector<int2> blk;        // {record offset / 128, record bytes}                       -> device, dose pass
+    std::vector<int4> pk;         // {meta word offset, meta words, record offset / 128, 0}    -> device, pack kernel
+    std::vector<uint32_t> meta;   // headers + row tables, block after block
+    std::vector<int> rows, slots; // per block, for the cost model
+    size_t pack_bytes = 0;
+    int max_rec_bytes = 0;
+};
+
 imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::vector<uint8_t>& sid, const float4* table_h,
-                         std::vector<int4>& blk, std::vector<uint32_t>& meta, double& G_skip, int64_t& n_skipped,
-                         int64_t& n_nonempty) {
+                         int chunk_slots, int col_bytes, BlockPlan& B, double& G_skip, int64_t& n_skipped, int64_t& n_nonempty) {
     const int n_v = (int)sid.size();
     G_skip = 0.0;
     n_skipped = 0;
@@ -276,16 +318,18 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         G_skip += (double)t.z * u * u + (double)t.w * o * o;
         ++n_skipped;
     };
+    auto pad4 = [](int n) { return (n + 3) & ~3; };
     int j = 0;
     uint32_t q_prefix = 0;
+    size_t off = 0;
     while (j < n_v) {
         if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
-        const int r0 = j, p0a = rp[j] & ~3;
-        if (rp[j + 1] - p0a > CHUNK_F)
+        const int r0 = j;
+        int slots = pad4(rp[j + 1] - rp[j]);
+        if (slots > chunk_slots)
             return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
-                        rp[j + 1] - rp[j], CHUNK_F - 3);
-        int last = j, empties = 0, jj = j + 1;
-        int n_full = 1;
+                        rp[j + 1] - rp[j], chunk_slots);
+        int last = j, empties = 0, jj = j + 1, n_full = 1;
         while (jj < n_v && jj - r0 < MAXROWS_F) {
             const int len = rp[jj + 1] - rp[jj];
             if (len == 0) {
@@ -293,7 +337,8 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
                 ++jj;
                 continue;
             }
-            if (rp[jj + 1] - p0a > CHUNK_F) break;
+            if (slots + pad4(len) > chunk_slots) break;
+            slots += pad4(len);
             empties = 0;
             last = jj;
             ++n_full;
@@ -301,18 +346,30 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         }
         const int r1 = last + 1, nrows = r1 - r0;
         n_nonempty += n_full;
-        const int mo = (int)meta.size();
-        meta.push_back((uint32_t)nrows);
-        meta.push_back((uint32_t)r0);
-        meta.push_back(q_prefix & (uint32_t)(W_CONS - 1));   // warp batches dealt so far: round-robin continues across blocks
+        const int mo = (int)B.meta.size();
+        B.meta.push_back((uint32_t)nrows);
+        B.meta.push_back((uint32_t)r0);
+        B.meta.push_back(q_prefix & (uint32_t)(W_CONS - 1));   // warp batches dealt so far: round-robin continues across blocks
         q_prefix += (uint32_t)((nrows + RB - 1) / RB);
-        meta.push_back(0u);
-        for (int row = r0; row < r1; ++row) meta.push_back((uint32_t)(rp[row] - p0a) | ((uint32_t)sid[row] << 16));
-        meta.push_back((uint32_t)(rp[r1] - p0a));
-        while (meta.size() & 3) meta.push_back(0u);
-        blk.push_back(make_int4(p0a, rp[r1] - p0a, mo, (int)meta.size() - mo));
+        B.meta.push_back((uint32_t)slots);
+        int so = 0;
+        for (int row = r0; row < r1; ++row) {
+            B.meta.push_back((uint32_t)so | ((uint32_t)sid[row] << 16));
+            so += pad4(rp[row + 1] - rp[row]);
+        }
+        B.meta.push_back((uint32_t)so);
+        while ((B.meta.size() - mo - META_HDR) & 3) B.meta.push_back(0u);
+        const int mw = (int)B.meta.size() - mo;
+        const int rec = (mw * 4 + slots * (4 + col_bytes) + 127) & ~127;
+        B.blk.push_back(make_int2((int)(off / 128), rec));
+        B.pk.push_back(make_int4(mo, mw, (int)(off / 128), 0));
+        B.rows.push_back(nrows);
+        B.slots.push_back(slots);
+        B.max_rec_bytes = std::max(B.max_rec_bytes, rec);
+        off += (size_t)rec;
         j = r1;
     }
+    B.pack_bytes = off;
     return IMRT_STATUS_OK;
 }
 
@@ -535,36 +592,56 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     for (int s = 0; s < n_structures; ++s) table_h[s] = make_float4(host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]);
     CUDA_TRY(pl, cudaMemcpyAsync(L.table, table_h.data(), sizeof(float4) * MAX_STRUCTURES, cudaMemcpyHostToDevice, st));
 
-    // ---- dose-pass blocks
-    std::vector<int4> blk;
-    std::vector<uint32_t> meta;
+    // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, x+, g, stages
+    const int nb_pad = (int)((n_b + 31) & ~31LL);
+    int off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
+    DevPlan& P = pl->P;
+    memset(&P, 0, sizeof P);
+    P.wpart_off = off; off += SMEM_WPART;
+    P.x_off = off; off += nb_pad * 4;
+    P.g_off = off; off += nb_pad * 4;
+    off = (off + 127) & ~127;
+    P.stage_off = off;
+    const int avail = smem_optin - off;
+
+    // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero)
+    const bool col16 = n_b <= 65536 && !getenv("IMRTGP_COL32");
+    const int chunk_slots = col16 ? 4096 : 3072;
+    BlockPlan BP;
     double G_skip = 0.0;
-    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), blk, meta, G_skip, pl->n_skipped, pl->n_nonempty);
+    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, BP, G_skip, pl->n_skipped, pl->n_nonempty);
     if (s != IMRT_STATUS_OK) return s;
     const Bounds B = bounds_for(n_v, n_b, nnz);
-    if ((int64_t)blk.size() > B.max_blk || (int64_t)meta.size() > B.max_meta)
-        return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %zu words)", blk.size(), meta.size());
-    pl->n_blk = (int64_t)blk.size();
-    const int grid_f = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, blk.size()));
+    const size_t n_blk = BP.blk.size();
+    if ((int64_t)n_blk > B.max_blk || (int64_t)BP.meta.size() > B.max_meta || BP.pack_bytes > B.max_pack)
+        return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %zu words, %zu bytes)",
+                    n_blk, BP.meta.size(), BP.pack_bytes);
+    pl->n_blk = (int64_t)n_blk;
+    pl->pack_bytes = (int64_t)BP.pack_bytes;
+    const int grid_f = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, n_blk));
     std::vector<int> cta_blk(grid_f + 1, 0);
     {
-        std::vector<double> pre(blk.size() + 1, 0.0);
+        std::vector<double> pre(n_blk + 1, 0.0);
         // cost of a block in SM cycles: the slower of streaming its bytes at a 1/n_sm share of HBM bandwidth and of
         // issuing its instructions (per-row work dominates where rows are short, e.g. at the field edges)
-        for (size_t b = 0; b < blk.size(); ++b) {
-            const double nz = blk[b].y, rows = blk[b].w - META_HDR - 1;
-            pre[b + 1] = pre[b] + std::max(0.36 * nz, 130.0 + 9.0 * rows + 0.15 * nz);
-        }
+        for (size_t b = 0; b < n_blk; ++b)
+            pre[b + 1] = pre[b] + std::max(BP.blk[b].y / 22.4, 130.0 + 9.0 * BP.rows[b] + 0.08 * BP.slots[b]);
         size_t b = 0;
         for (int c = 0; c < grid_f; ++c) {
-            const double want = pre[blk.size()] * c / grid_f;
-            while (b < blk.size() && pre[b] < want) ++b;
+            const double want = pre[n_blk] * c / grid_f;
+            while (b < n_blk && pre[b] < want) ++b;
             cta_blk[c] = (int)b;
         }
-        cta_blk[grid_f] = (int)blk.size();
+        cta_blk[grid_f] = (int)n_blk;
     }
-    if (!blk.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.blk, blk.data(), sizeof(int4) * blk.size(), cudaMemcpyHostToDevice, st));
-    if (!meta.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.rowmeta, meta.data(), sizeof(uint32_t) * meta.size(), cudaMemcpyHostToDevice, st));
+    if (n_blk) {
+        CUDA_TRY(pl, cudaMemcpyAsync(L.blk, BP.blk.data(), sizeof(int2) * n_blk, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaMemcpyAsync(L.pk, BP.pk.data(), sizeof(int4) * n_blk, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaMemcpyAsync(L.rowmeta, BP.meta.data(), sizeof(uint32_t) * BP.meta.size(), cudaMemcpyHostToDevice, st));
+        if (col16) k_pack_blocks<true><<<(unsigned int)n_blk, 256, 0, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, L.pack);
+        else k_pack_blocks<false><<<(unsigned int)n_blk, 256, 0, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, L.pack);
+        CUDA_TRY(pl, cudaGetLastError());
+    }
     CUDA_TRY(pl, cudaMemcpyAsync(L.cta_blk, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
 
     // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1)
@@ -598,24 +675,15 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     if (!ranges.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.tr_range, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
     CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
 
-    // ---- shared-memory layout (one layout for the three kernels)
-    const int nb_pad = (int)((n_b + 31) & ~31LL);
-    int off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
-    DevPlan& P = pl->P;
-    memset(&P, 0, sizeof P);
-    P.wpart_off = off; off += SMEM_WPART;
-    P.x_off = off; off += nb_pad * 4;
-    P.g_off = off; off += nb_pad * 4;
-    off = (off + 127) & ~127;
-    P.stage_off = off;
-    const int avail = smem_optin - off;
-    const int sf = std::min(MAX_STAGES, avail / STAGE_F_BYTES), stt = std::min(MAX_STAGES, avail / STAGE_T_BYTES);
+    const int stage_f = std::max(BP.max_rec_bytes, 128);
+    const int sf = std::min(MAX_STAGES, avail / stage_f), stt = std::min(MAX_STAGES, avail / STAGE_T_BYTES);
     if (avail < 0 || sf < 2 || stt < 2)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets do not fit in shared memory next to the pipeline stages", (long long)n_b);
-    pl->smem_bytes = (size_t)off + (size_t)std::max(sf * STAGE_F_BYTES, stt * STAGE_T_BYTES);
+    pl->smem_bytes = (size_t)off + (size_t)std::max(sf * stage_f, stt * STAGE_T_BYTES);
 
-    P.col = col_idx; P.val = val; P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
-    P.blk = L.blk; P.rowmeta = L.rowmeta; P.cta_blk = L.cta_blk; P.grid_f = grid_f; P.n_stages_f = sf;
+    P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
+    P.pack = L.pack; P.blk = L.blk; P.cta_blk = L.cta_blk; P.grid_f = grid_f; P.n_stages_f = sf;
+    P.stage_f_bytes = stage_f; P.col16 = col16 ? 1 : 0;
     P.rowT_ptr = L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
     P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr;
     P.n_ranges = (int)ranges.size(); P.grid_t = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, ranges.size()));
@@ -827,8 +895,8 @@ imrt_status imrt_plan_get_counters(imrt_plan* pl, int64_t* host_fwd_passes, int6
 
 imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info, int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT) {
     if (!pl) return IMRT_STATUS_INVALID_ARG;
-    const int64_t info[10] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, (int64_t)pl->smem_bytes,
-                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, 1};
+    const int64_t info[10] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
+                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16};
     for (int i = 0; i < n_info && i < 10 && host_info; ++i) host_info[i] = info[i];
     cudaStream_t st = pl->stream;
     if (d_rowT_ptr) CUDA_TRY(pl, cudaMemcpyAsync(d_rowT_ptr, pl->rowT_ptr_w, sizeof(int) * (pl->P.n_b + 1), cudaMemcpyDeviceToDevice, st));

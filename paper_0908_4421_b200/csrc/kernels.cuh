@@ -29,11 +29,11 @@ namespace imrt {
 constexpr int W_CONS = 16;                    // consumer warps per CTA
 constexpr int N_CONS = W_CONS * 32;           // consumer threads
 constexpr int NTHREADS = N_CONS + 32;         // + one producer warp
-constexpr int CHUNK_F = 2048;                 // nnz capacity of a dose-pass stage (row-aligned blocks)
-constexpr int META_F = 256;                   // uint32 words of row metadata per dose-pass stage
-constexpr int META_HDR = 4;                   // {nrows, first row, log2 V, reserved}
-constexpr int MAXROWS_F = META_F - META_HDR - 1;
-constexpr int STAGE_F_BYTES = CHUNK_F * 8 + META_F * 4;
+// dose pass: D is re-packed once into self-contained block records (one bulk copy each, see DosePack below)
+constexpr int META_HDR = 4;                   // header words {rows, first row, batches dealt before | flags, slots}
+constexpr int MIN_CHUNK_SLOTS = 2048;           // smallest slot capacity of a dose-pass stage the host will choose
+constexpr int MAXROWS_F = 507;                // rows per block: header + row table fit 2 KB
+constexpr int META_F_BYTES = (META_HDR + MAXROWS_F + 1) * 4;
 constexpr int CHUNK_T = 4096;                 // nnz per transpose-pass stage (pure streaming)
 constexpr int SLICE_T = CHUNK_T / W_CONS;     // contiguous nnz per consumer warp per stage
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
@@ -84,11 +84,18 @@ struct DevPlan {
     const float* val;
     long long nnz;
     int n_v, n_b;
-    // dose pass: row-aligned blocks
-    const int4* blk;           // {p0a, n_elems, meta word offset, meta words}
-    const uint32_t* rowmeta;
+    // dose pass: D re-packed into block records (owned).  A record is 128-byte aligned and holds, in this order,
+    //   header  uint32[4]  {rows, first row, warp batches dealt before this block (mod W_CONS), slots}
+    //   rows    uint32[rows + 1]  slot offset of the row (low 16 bits, a multiple of 4) | structure id << 16;
+    //                             padded to a multiple of 4 words
+    //   val     fp32[slots]       every row padded with zeros to a multiple of 4 slots
+    //   col     uint16[slots] (n_b <= 65536) or int32[slots]
+    const unsigned char* pack;
+    const int2* blk;           // {record offset / 128, record bytes}
     const int* cta_blk;        // [grid_f + 1] block range per CTA
     int grid_f, n_stages_f;
+    int stage_f_bytes;         // bytes of one dose-pass stage (largest record, 128-byte multiple)
+    int col16;                 // 1: 16-bit column indices in the records
     // D^T (owned): CSR, rows = beamlets, padded with zeros to a multiple of 4 entries
     const int* rowT_ptr;
     const int* colT;
@@ -196,42 +203,55 @@ __device__ __forceinline__ double compute_trial(const float* x, const float* g, 
 }
 
 // ------------------------------------------------------------------------------------------------ dose pass
-// VW lanes per row, RB = 32 / VW rows per warp batch: the four row groups of a warp run the same trip count (the
-// longest of their rows; neighbouring voxels have rows of similar length), gather x+ from shared memory, multiply-add
-// in fp32 and reduce with log2(VW) shuffles; lane 0 of each group then does its voxel's penalty and residual
-// (Eq. (1) generalised: F = w- u^2 + w+ o^2, r = 2 (w+ o - w- u)).  Batches are numbered across the CTA's blocks and
-// dealt round-robin to the consumer warps, which never synchronise with each other: a warp with nothing to do in
-// this stage moves on to the next one.
+// VW lanes per row, RB = 32 / VW rows per warp batch, 4 consecutive slots per lane and trip: rows start on 16-byte
+// boundaries inside a record and are zero-padded to a multiple of 4 slots, so values and columns come in with one
+// 128-bit (64-bit for 16-bit columns) shared-memory load each and nothing has to be masked inside a row.  The row
+// groups of a warp run the trip count of their longest row (neighbouring voxels have rows of similar length),
+// gather x+ from shared memory, multiply-add in fp32 and reduce with log2(VW) shuffles; lane 0 of each group then
+// does its voxel's penalty and residual (Eq. (1) generalised: F = w- u^2 + w+ o^2, r = 2 (w+ o - w- u)).
+// Batches are numbered across the CTA's blocks and dealt round-robin to the consumer warps, which never
+// synchronise with each other: a warp with nothing to do in this stage moves on to the next one.
 constexpr int VW = 8;
 constexpr int RB = 32 / VW;
 
-__device__ __forceinline__ void dose_block(const int* __restrict__ col_s, const float* __restrict__ val_s,
-                                           const uint32_t* __restrict__ meta, const float* __restrict__ x_s,
+template <bool COL16>
+__device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec, const float* __restrict__ x_s,
                                            const float4* __restrict__ table_s, float* __restrict__ r_out,
                                            float* __restrict__ d_out, int warp, int lane, double& Gacc) {
-    const uint4 hdr = *reinterpret_cast<const uint4*>(meta);   // {rows, first row, batches dealt before (mod W_CONS), -}
+    const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nrows = (int)hdr.x;
     const int nbatch = (nrows + RB - 1) / RB;
+    const uint32_t* rows = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
+    const float* val_s = reinterpret_cast<const float*>(rows + ((nrows + 1 + 3) & ~3));
+    const unsigned char* col_s = reinterpret_cast<const unsigned char*>(val_s + hdr.w);
     const int grp = lane / VW, sub = lane % VW;
     for (int q = (warp - (int)hdr.z) & (W_CONS - 1); q < nbatch; q += W_CONS) {
         const int row = q * RB + grp;
         const bool valid = row < nrows;
         uint32_t m0 = 0u, m1 = 0u;
-        if (valid) { m0 = meta[META_HDR + row]; m1 = meta[META_HDR + row + 1]; }
+        if (valid) { m0 = rows[row]; m1 = rows[row + 1]; }
         const int s = (int)(m0 & 0xFFFFu), e = (int)(m1 & 0xFFFFu);
         const int len_max = __reduce_max_sync(0xffffffffu, e - s);   // warp-uniform trip count
-        float a0 = 0.0f, a1 = 0.0f;
-        int k = s + sub;
-        for (int kb = 0; kb < len_max; kb += 2 * VW, k += 2 * VW) {
-            const bool p0 = k < e, p1 = k + VW < e;
-            const int c0 = p0 ? col_s[k] : 0;
-            const int c1 = p1 ? col_s[k + VW] : 0;
-            const float v0 = p0 ? val_s[k] : 0.0f;
-            const float v1 = p1 ? val_s[k + VW] : 0.0f;
-            a0 = fmaf(v0, x_s[c0], a0);
-            a1 = fmaf(v1, x_s[c1], a1);
+        float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+        int k = s + 4 * sub;
+        for (int kb = 0; kb < len_max; kb += 4 * VW, k += 4 * VW) {
+            if (k < e) {
+                const float4 v = *reinterpret_cast<const float4*>(val_s + k);
+                int c0, c1, c2, c3;
+                if (COL16) {
+                    const uint2 c = *reinterpret_cast<const uint2*>(col_s + 2 * k);
+                    c0 = (int)(c.x & 0xFFFFu); c1 = (int)(c.x >> 16); c2 = (int)(c.y & 0xFFFFu); c3 = (int)(c.y >> 16);
+                } else {
+                    const int4 c = *reinterpret_cast<const int4*>(col_s + 4 * k);
+                    c0 = c.x; c1 = c.y; c2 = c.z; c3 = c.w;
+                }
+                a0 = fmaf(v.x, x_s[c0], a0);
+                a1 = fmaf(v.y, x_s[c1], a1);
+                a2 = fmaf(v.z, x_s[c2], a2);
+                a3 = fmaf(v.w, x_s[c3], a3);
+            }
         }
-        const float d = vec_sum<VW>(a0 + a1);
+        const float d = vec_sum<VW>((a0 + a1) + (a2 + a3));
         if (valid && sub == 0) {
             const float4 t = table_s[(m0 >> 16) & 0xFFu];
             const float u = fmaxf(0.0f, t.x - d);
@@ -245,10 +265,12 @@ __device__ __forceinline__ void dose_block(const int* __restrict__ col_s, const 
 
 // All NTHREADS threads of the CTA call this.  x_s: the trial point in shared memory.  Writes the CTA's objective
 // partial to Gpart[blockIdx.x] (thread 0).  Ends with a CTA-wide barrier.
-__device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
-                                          const float* x_s, float* r_out, float* d_out, double* Gpart, Pipe& pipe) {
+template <bool COL16>
+__device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
+                                            const float* x_s, float* r_out, float* d_out, double* Gpart, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = P.n_stages_f;
+    const uint32_t SB = (uint32_t)P.stage_f_bytes;
     unsigned char* stages = smem + P.stage_off;
     const int b0 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x] : 0;
     const int b1 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x + 1] : 0;
@@ -259,72 +281,39 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
     const uint32_t full_a = smem_u32(&h->full_f[0]), empty_a = smem_u32(&h->empty_f[0]), stages_a = smem_u32(stages);
 
     if (warp == W_CONS) {
-        // ---------------- producer warp: lane 0 drives the TMA unit; descriptors are fetched 32 at a time
-        const uint64_t pol = policy_evict_first();   // the matrix is streamed once per pass: keep it from pushing r / x out of L2
-        const int aligned_end = (int)(P.nnz & ~3LL);
-        int4 next = (b0 + lane < b1) ? __ldg(P.blk + b0 + lane) : make_int4(0, 0, 0, 0);
+        // ---------------- producer warp: lane 0 drives the TMA unit, one bulk copy per block record; the
+        // descriptors of the next 32 blocks are requested before the current 32 are issued
+        const uint64_t pol = policy_evict_first();   // streamed once per pass: keep it from pushing r / x out of L2
+        int2 next = (b0 + lane < b1) ? __ldg(P.blk + b0 + lane) : make_int2(0, 0);
         for (int bb = b0; bb < b1; bb += 32) {
-            const int4 mine = next;       // the following 32 descriptors are requested before these are issued
-            next = (bb + 32 + lane < b1) ? __ldg(P.blk + bb + 32 + lane) : make_int4(0, 0, 0, 0);
+            const int2 mine = next;
+            next = (bb + 32 + lane < b1) ? __ldg(P.blk + bb + 32 + lane) : make_int2(0, 0);
             const int nb_here = min(32, b1 - bb);
             for (int j = 0; j < nb_here; ++j) {
-                int4 d;
-                d.x = __shfl_sync(0xffffffffu, mine.x, j);
-                d.y = __shfl_sync(0xffffffffu, mine.y, j);
-                d.z = __shfl_sync(0xffffffffu, mine.z, j);
-                d.w = __shfl_sync(0xffffffffu, mine.w, j);
-                if (lane == 0) mbar_wait_a(empty_a + 8u * s, ph ^ 1u);
-                __syncwarp();
-                const int n4 = (d.y + 3) & ~3;
-                int nb = aligned_end - d.x;   // elements the bulk copy may touch without leaving the caller's arrays
-                nb = nb < 0 ? 0 : (nb > n4 ? n4 : nb);
-                if (nb < d.y) {               // the (at most 3) entries of an unaligned matrix end are copied by hand
-                    int* col_s = reinterpret_cast<int*>(stages + (size_t)s * STAGE_F_BYTES);
-                    float* val_s = reinterpret_cast<float*>(col_s + CHUNK_F);
-                    for (int k = nb + lane; k < d.y; k += 32) {
-                        col_s[k] = P.col[d.x + k];
-                        val_s[k] = P.val[d.x + k];
-                    }
-                    __syncwarp();
-                }
+                const int off128 = __shfl_sync(0xffffffffu, mine.x, j);
+                const int bytes = __shfl_sync(0xffffffffu, mine.y, j);
                 if (lane == 0) {
-                    const uint32_t st_a = stages_a + (uint32_t)s * STAGE_F_BYTES, bar = full_a + 8u * s;
-#if defined(IMRT_EXP_NO_META)
-                    mbar_expect_tx_a(bar, (uint32_t)(nb * 8));
-                    bulk_g2s_a(st_a, P.col + d.x, (uint32_t)nb * 4u, bar, pol);
-                    bulk_g2s_a(st_a + CHUNK_F * 4, P.val + d.x, (uint32_t)nb * 4u, bar, pol);
-#elif defined(IMRT_EXP_ALIGNED)
-                    mbar_expect_tx_a(bar, 16384u);
-                    bulk_g2s_a(st_a, P.col + (d.x & ~31), 8192u, bar, pol);
-                    bulk_g2s_a(st_a + CHUNK_F * 4, P.val + (d.x & ~31), 8192u, bar, pol);
-#else
-                    mbar_expect_tx_a(bar, (uint32_t)(nb * 8 + d.w * 4));
-                    if (nb > 0) {
-                        bulk_g2s_a(st_a, P.col + d.x, (uint32_t)nb * 4u, bar, pol);
-                        bulk_g2s_a(st_a + CHUNK_F * 4, P.val + d.x, (uint32_t)nb * 4u, bar, pol);
-                    }
-                    bulk_g2s_a(st_a + CHUNK_F * 8, P.rowmeta + d.z, (uint32_t)d.w * 4u, bar, pol);
-#endif
+                    mbar_wait_a(empty_a + 8u * s, ph ^ 1u);
+                    const uint32_t bar = full_a + 8u * s;
+                    mbar_expect_tx_a(bar, (uint32_t)bytes);
+                    bulk_g2s_a(stages_a + (uint32_t)s * SB, P.pack + (size_t)(unsigned int)off128 * 128u, (uint32_t)bytes, bar, pol);
                 }
                 if (++s == S) { s = 0; ph ^= 1u; }
             }
         }
     } else {
         // ---------------- consumer warps
-        const unsigned char* st_p = stages + (size_t)s * STAGE_F_BYTES;
-        const unsigned char* st_end = stages + (size_t)S * STAGE_F_BYTES;
+        const unsigned char* st_p = stages + (size_t)s * SB;
+        const unsigned char* st_end = stages + (size_t)S * SB;
         uint32_t fb = full_a + 8u * s, eb = empty_a + 8u * s;
         for (int b = b0; b < b1; ++b) {
             mbar_wait_a(fb, ph);
-            const int* col_s = reinterpret_cast<const int*>(st_p);
-            const float* val_s = reinterpret_cast<const float*>(st_p + CHUNK_F * 4);
-            const uint32_t* meta_s = reinterpret_cast<const uint32_t*>(st_p + CHUNK_F * 8);
 #ifndef IMRT_EXP_SKIP_COMPUTE
-            dose_block(col_s, val_s, meta_s, x_s, table_s, r_out, d_out, warp, lane, Gacc);
+            dose_block<COL16>(st_p, x_s, table_s, r_out, d_out, warp, lane, Gacc);
 #endif
             __syncwarp();
             if (lane == 0) mbar_arrive_a(eb);
-            st_p += STAGE_F_BYTES; fb += 8u; eb += 8u;
+            st_p += SB; fb += 8u; eb += 8u;
             if (st_p == st_end) { st_p = stages; fb = full_a; eb = empty_a; ph ^= 1u; }
         }
     }
@@ -336,6 +325,12 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
         P.cta_ns[2 * blockIdx.x + 1] = global_ns();    // host see (and rebalance) the static partition
     }
     __syncthreads();
+}
+
+__device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
+                                          const float* x_s, float* r_out, float* d_out, double* Gpart, Pipe& pipe) {
+    if (P.col16) dose_pass_t<true>(P, h, smem, table_s, x_s, r_out, d_out, Gpart, pipe);
+    else dose_pass_t<false>(P, h, smem, table_s, x_s, r_out, d_out, Gpart, pipe);
 }
 
 // Objective of a finished dose pass: fixed-order sum of the CTA partials + the constant of the skipped rows.
