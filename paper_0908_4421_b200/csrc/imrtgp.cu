@@ -31,6 +31,9 @@ struct imrt_plan {
     int grid_p;                       // persistent kernel grid
     bool has_x;
     int64_t n_blk, n_nonempty, n_skipped, pack_bytes;
+    std::vector<double> blk_cost;     // modelled, then measured, cost of every dose-pass block (host)
+    int* cta_blk_w;
+    double tune_spread[2];            // slowest / mean CTA time of the dose pass before and after tuning
     // borrowed inputs
     const int32_t* row_ptr;
     const uint8_t* sid;
@@ -373,6 +376,21 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
     return IMRT_STATUS_OK;
 }
 
+// Contiguous block ranges of (nearly) equal total cost, one per CTA.
+void partition_blocks(const std::vector<double>& cost, int grid, std::vector<int>& cta_blk) {
+    const size_t n = cost.size();
+    std::vector<double> pre(n + 1, 0.0);
+    for (size_t b = 0; b < n; ++b) pre[b + 1] = pre[b] + cost[b];
+    cta_blk.assign(grid + 1, 0);
+    size_t b = 0;
+    for (int c = 0; c < grid; ++c) {
+        const double want = pre[n] * c / grid;
+        while (b < n && pre[b] < want) ++b;
+        cta_blk[c] = (int)b;
+    }
+    cta_blk[grid] = (int)n;
+}
+
 // Equal-nnz ranges of the D^T stream, each spanning at most RL_MAX rows, and the gradient partial slots.
 void build_ranges(const std::vector<int>& rpT, int n_b, int n_sm, std::vector<TrRange>& ranges, std::vector<int>& rowslot_ptr) {
     const long long nnz = rpT[n_b];
@@ -429,6 +447,54 @@ static cudaError_t launch_persistent(imrt_plan* pl) {
     cfg.attrs = at;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k_persistent, pl->P);
+}
+
+// The static partition of the dose pass is only as good as its cost model, and the model cannot know how the
+// instruction-bound blocks (short rows at the field edges) trade against the bandwidth-bound ones on this device.
+// So measure: run the pass, read every CTA's streaming time, rescale the cost of each CTA's blocks by its measured
+// time per unit of modelled cost, re-partition, and repeat a few times.
+static imrt_status tune_partition(imrt_plan* pl) {
+    pl->tune_spread[0] = pl->tune_spread[1] = 0.0;
+    const int grid = pl->P.grid_f;
+    const size_t n_blk = pl->blk_cost.size();
+    if (getenv("IMRTGP_NO_TUNE") || n_blk < (size_t)grid * 8) return IMRT_STATUS_OK;
+    cudaStream_t st = pl->stream;
+    CUDA_TRY(pl, cudaMemsetAsync(pl->P.xbuf[0], 0, sizeof(float) * pl->P.n_b, st));
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_EVAL;
+    A.x_in = pl->P.xbuf[0];
+    A.r_out = pl->r_scratch;
+    std::vector<int> cta_blk;
+    partition_blocks(pl->blk_cost, grid, cta_blk);
+    std::vector<unsigned long long> t(2 * (size_t)grid);
+    std::vector<double> dur(grid);
+    const int rounds = 5;
+    for (int it = 0; it <= rounds; ++it) {
+        for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_dose(pl, A));   // the first warms up, the second is read
+        CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        double mean = 0.0, worst = 0.0;
+        for (int c = 0; c < grid; ++c) {
+            dur[c] = (double)(t[2 * c + 1] - t[2 * c]);
+            mean += dur[c] / grid;
+            worst = std::max(worst, dur[c]);
+        }
+        if (it == 0) pl->tune_spread[0] = worst / mean;
+        pl->tune_spread[1] = worst / mean;
+        if (it == rounds) break;
+        for (int c = 0; c < grid; ++c) {
+            double sum = 0.0;
+            for (int b = cta_blk[c]; b < cta_blk[c + 1]; ++b) sum += pl->blk_cost[b];
+            if (sum <= 0.0 || dur[c] <= 0.0) continue;
+            const double f = dur[c] / sum;
+            for (int b = cta_blk[c]; b < cta_blk[c + 1]; ++b) pl->blk_cost[b] *= f;
+        }
+        partition_blocks(pl->blk_cost, grid, cta_blk);
+        CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_blk_w, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+    }
+    return IMRT_STATUS_OK;
 }
 
 // graph:  k_begin -> WHILE(outer){ k_transpose -> WHILE(inner){ k_dose } }
@@ -619,21 +685,14 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     pl->n_blk = (int64_t)n_blk;
     pl->pack_bytes = (int64_t)BP.pack_bytes;
     const int grid_f = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, n_blk));
-    std::vector<int> cta_blk(grid_f + 1, 0);
-    {
-        std::vector<double> pre(n_blk + 1, 0.0);
-        // cost of a block in SM cycles: the slower of streaming its bytes at a 1/n_sm share of HBM bandwidth and of
-        // issuing its instructions (per-row work dominates where rows are short, e.g. at the field edges)
-        for (size_t b = 0; b < n_blk; ++b)
-            pre[b + 1] = pre[b] + std::max(BP.blk[b].y / 22.4, 130.0 + 9.0 * BP.rows[b] + 0.08 * BP.slots[b]);
-        size_t b = 0;
-        for (int c = 0; c < grid_f; ++c) {
-            const double want = pre[n_blk] * c / grid_f;
-            while (b < n_blk && pre[b] < want) ++b;
-            cta_blk[c] = (int)b;
-        }
-        cta_blk[grid_f] = (int)n_blk;
-    }
+    // cost of a block in SM cycles: the slower of streaming its bytes at a 1/n_sm share of HBM bandwidth and of
+    // issuing its instructions (per-row work dominates where rows are short, e.g. at the field edges); refined from
+    // measured per-CTA times by tune_partition() below
+    pl->blk_cost.resize(n_blk);
+    for (size_t b = 0; b < n_blk; ++b)
+        pl->blk_cost[b] = std::max(BP.blk[b].y / 22.4, 130.0 + 9.0 * BP.rows[b] + 0.08 * BP.slots[b]);
+    std::vector<int> cta_blk;
+    partition_blocks(pl->blk_cost, grid_f, cta_blk);
     if (n_blk) {
         CUDA_TRY(pl, cudaMemcpyAsync(L.blk, BP.blk.data(), sizeof(int2) * n_blk, cudaMemcpyHostToDevice, st));
         CUDA_TRY(pl, cudaMemcpyAsync(L.pk, BP.pk.data(), sizeof(int4) * n_blk, cudaMemcpyHostToDevice, st));
@@ -694,6 +753,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.cta_ns = L.cta_ns;
     P.st = L.st; P.tr_obj = L.tr_obj; P.tr_lambda = L.tr_lambda; P.tr_step_sq = L.tr_step_sq; P.tr_trials = L.tr_trials;
     pl->r_scratch = L.r_scratch; pl->g_scratch = L.g_scratch; pl->d_scratch = L.d_scratch;
+    pl->cta_blk_w = L.cta_blk;
     pl->rowT_ptr_w = L.rowT_ptr; pl->colT_w = L.colT; pl->valT_w = L.valT;
     pl->dvh = L.dvh;
     pl->grid_p = n_sm;
@@ -718,6 +778,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
 
+    s = tune_partition(pl);
+    if (s != IMRT_STATUS_OK) return s;
     if (prm->driver == 0) {
         s = build_graph(pl);
         if (s != IMRT_STATUS_OK) return s;
