@@ -58,12 +58,16 @@ def measured_peak():
 
 
 def recorded_traffic(kernel):
-    """DRAM bytes per launch from the committed ncu --set full capture (profiles/traffic.json), else None."""
+    """DRAM bytes per launch (read + write) from the committed ncu --set full capture (profiles/traffic.csv), else None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(kernel)
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == kernel:
+                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
