@@ -40,10 +40,11 @@ def workload_name(cfg_id):
     return synth_inputs.CONFIGS[cfg_id].name
 
 
-def algorithmic_bytes(prob):
-    """int32/fp32 CSR bytes one pass has to move (independent of how the library lays things out)."""
+def algorithmic_bytes(prob, R=1):
+    """int32/fp32 CSR bytes one pass has to move (independent of how the library lays things out).
+    A dose pass that evaluates R line-search trial points streams D once and writes R residual vectors."""
     nnz, n_v, n_b = prob.nnz, prob.n_v, prob.n_b
-    fwd = 8 * nnz + 4 * (n_v + 1) + 1 * n_v + 4 * n_v + 8 * n_b     # D, row_ptr, sid, r out, x and g in
+    fwd = 8 * nnz + 4 * (n_v + 1) + 1 * n_v + R * 4 * n_v + 8 * n_b   # D, row_ptr, sid, r out (per trial), x and g in
     tr = 8 * nnz + 4 * (n_b + 1) + 4 * n_v + 4 * n_b                 # D^T, rowT_ptr, r in once, g out
     return fwd, tr
 
@@ -179,15 +180,16 @@ def run_ours(args):
 
     K, W = args.steps, max(args.warmup, 3)
     prob = synth_inputs.make_phantom(args.config)
-    fwd_bytes, tr_bytes = algorithmic_bytes(prob)
     driver = DRIVERS[args.driver]
     stream = torch.cuda.current_stream(dev)
 
     t0 = time.perf_counter()
-    plan = imrt.Plan(prob, max_iters=W + K, driver=driver, device=dev)
+    plan = imrt.Plan(prob, max_iters=W + K, driver=driver, device=dev, ls_batch=args.ls_batch)
     torch.cuda.synchronize()
     plan_create_s = time.perf_counter() - t0
     info = plan.info()
+    R = info["ls_batch"]
+    fwd_bytes, tr_bytes = algorithmic_bytes(prob, R)
 
     # ---------------- timed region: W warm-up iterations, then exactly K iterations in one device-resident run
     plan.set_x(prob.x0)
@@ -224,7 +226,8 @@ def run_ours(args):
         raise SystemExit("bench.py: the run did %d of %d iterations (stop reason %s); the timing is not K steps"
                          % (tr.n_iters, W + K, imrt.STOP_NAMES[tr.stop_reason]))
     trials_timed = int(tr.n_trials[W:].sum())
-    loop_bytes = trials_timed * fwd_bytes + K * tr_bytes
+    passes_timed = int(np.ceil(tr.n_trials[W:] / R).sum())     # one dose pass evaluates up to R trial points
+    loop_bytes = passes_timed * fwd_bytes + K * tr_bytes
 
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
@@ -240,7 +243,7 @@ def run_ours(args):
             if 8 * prob.nnz > 2 * l2_bytes else "matrices are L2-resident: GB/s figures are L2, not HBM, bandwidth"
         dose_gbs = fwd_bytes / (dose_ms * 1e-3) / 1e9
         tr_gbs = tr_bytes / (tr_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "k_dose (dose SpMV + penalty + residual + objective partials)",
+        roofline = {"bound": "hbm", "kernel": "k_dose (dose SpMV for %d trial point(s) + penalty + residual + objective partials)" % R,
                     "achieved": dose_gbs, "peak": peak, "unit": "GB/s", "frac": dose_gbs / peak, "peak_source": peak_src,
                     "traffic": recorded_traffic("k_dose"), "algorithmic_bytes": fwd_bytes, "ms_per_launch": dose_ms,
                     "frac_of_nominal_8TBs": dose_gbs / 8000.0}
@@ -250,7 +253,7 @@ def run_ours(args):
 
         # ---------------- time-to-plan: the config's own stopping rule from x0 (device-resident, inputs in HBM)
         cfg = synth_inputs.CONFIGS[args.config]
-        plan2 = imrt.Plan(prob, max_iters=cfg.n_iters, driver=driver, device=dev)
+        plan2 = imrt.Plan(prob, max_iters=cfg.n_iters, driver=driver, device=dev, ls_batch=args.ls_batch)
         plan2.set_x(prob.x0)
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -281,7 +284,7 @@ def run_ours(args):
         d_x0 = torch.empty(prob.n_b, dtype=torch.float32, device=dev)
         d_x = torch.empty(prob.n_b, dtype=torch.float32, device=dev)
         d_d = torch.empty(prob.n_v, dtype=torch.float32, device=dev)
-        prm = imrt.Params(prob.eps, prob.alpha, prob.lambda0, prob.max_ls, K, driver, 0)
+        prm = imrt.Params(prob.eps, prob.alpha, prob.lambda0, prob.max_ls, K, driver, args.ls_batch)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         for dst, src in ((d_rp, h_rp), (d_col, h_col), (d_val, h_val), (d_sid, h_sid), (d_x0, h_x0)):
@@ -319,17 +322,17 @@ def run_ours(args):
                  "flush": flush}
 
     if rank == 0:
-        n_launch = {0: 2, 1: 2 + K + trials_timed, 2: 2}[driver]   # k_set_target + graph/persistent launch (+ passes)
+        n_launch = {0: 2, 1: 2 + K + passes_timed, 2: 2}[driver]   # k_set_target + graph/persistent launch (+ passes)
         if driver == 0:
-            n_launch = 1 + 1 + K + trials_timed                    # k_set_target, k_begin, K transposes, one k_dose per trial
+            n_launch = 1 + 1 + K + passes_timed                    # k_set_target, k_begin, K transposes, the dose passes
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                 "data": "synthetic",
                 "config": {"workload": prob.name, "n_v": prob.n_v, "n_b": prob.n_b, "nnz": prob.nnz,
                            "nonempty_rows": info["nonempty_rows"], "lambda0": prob.lambda0, "eps": prob.eps, "alpha": prob.alpha,
                            "driver": args.driver, "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
-                           "l2": extra.get("flush"), "trials_per_iter": trials_timed / K,
-                           "fwd_passes_timed": trials_timed, "tr_passes_timed": K},
+                           "l2": extra.get("flush"), "trials_per_iter": trials_timed / K, "ls_batch": R,
+                           "fwd_passes_timed": passes_timed, "tr_passes_timed": K},
                 "clocks": clocks, "gpu_launches": n_launch, "plan_create_s": plan_create_s,
                 "objective": {"first": float(tr.obj[0]), "after_warmup": float(tr.obj[W]), "last": float(tr.obj[-1])}}
         line.update({k: v for k, v in extra.items() if k != "flush"})
@@ -349,6 +352,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=sorted(synth_inputs.CONFIGS))
     ap.add_argument("--driver", default="persistent", choices=sorted(DRIVERS))
+    ap.add_argument("--ls-batch", type=int, default=0, choices=[0, 1, 2, 4],
+                    help="line-search trial points per dose pass (0 = library default, 4)")
     ap.add_argument("--cpu-iters", type=int, default=25, help="oracle iterations timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

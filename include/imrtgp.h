@@ -25,6 +25,10 @@
  *   - All device work is enqueued on the stream given at creation.  Calls documented "asynchronous" return
  *     without waiting for the device; calls that fill a host_ output synchronise that stream.
  *   - The plan handle is opaque and owned by the caller between imrt_plan_create and imrt_plan_destroy.
+ *   - Results of one plan are bit-reproducible from run to run (fixed-order reductions, no floating-point atomics).
+ *     Two plans of the same problem may differ in the last bits of the objective: plan creation balances the dose
+ *     pass over the SMs from MEASURED pass times, and the partition fixes the order in which objective partials are
+ *     summed.  Set the environment variable IMRTGP_NO_TUNE to keep the modelled partition (same bits every time).
  *   - There is no CPU fallback: on a machine without an sm_100 device imrt_plan_create fails with
  *     IMRT_STATUS_UNSUPPORTED_DEVICE / IMRT_STATUS_CUDA_ERROR.
  */
@@ -70,7 +74,12 @@ typedef struct imrt_params {
     int32_t max_iters;   /* trace capacity: the total number of accepted iterations between two imrt_plan_set_x  */
     int32_t driver;      /* 0: device-resident loop (CUDA graph with nested conditional WHILE nodes, no host sync
                                per step);  1: host-driven loop (one sync per trial; same kernels; for debugging)  */
-    int32_t reserved;    /* must be 0                                                                            */
+    int32_t ls_batch;    /* line-search trial points evaluated per pass over D: 1, 2 or 4 (0 = default, 4).  The
+                            trials lambda, lambda/alpha, ... are the ones steps 2-4 visit one at a time; a batch
+                            evaluates the next ls_batch of them in ONE dose pass (D is streamed once, each trial point
+                            gets its own D x+ and objective) and step 3 is then applied to them in order, so the
+                            iterates, step sizes and trial counts are bit-identical for every ls_batch.  The library
+                            lowers it when the trial vectors would not fit in shared memory (imrt_plan_get_info).  */
 } imrt_params;
 
 typedef struct imrt_plan imrt_plan;
@@ -162,7 +171,8 @@ imrt_status imrt_plan_get_trace(imrt_plan* plan, int32_t* host_n_iters_done, int
                                 double* host_obj, double* host_lambda, int32_t* host_n_trials, double* host_step_sq,
                                 int32_t capacity);
 
-/* Dose passes (D x + penalty) and transpose passes (D^T r) launched since the last imrt_plan_set_x.  Synchronises. */
+/* Dose passes (D x + penalty; one pass evaluates up to ls_batch trial points) and transpose passes (D^T r) launched
+ * since the last imrt_plan_set_x, including the pass that evaluated x_1.  Synchronises. */
 imrt_status imrt_plan_get_counters(imrt_plan* plan, int64_t* host_fwd_passes, int64_t* host_tr_passes);
 
 /*
@@ -170,15 +180,17 @@ imrt_status imrt_plan_get_counters(imrt_plan* plan, int64_t* host_fwd_passes, in
  *   host_info[0] nnz of D^T        [1] forward row blocks     [2] forward grid (CTAs)   [3] transpose grid (CTAs)
  *   host_info[4] dynamic shared memory bytes per CTA   [5] bytes of the re-packed D the dose pass streams
  *   host_info[6] gradient partial slots   [7] non-empty rows of D   [8] SM count   [9] 16-bit column indices (1/0)
+ *   host_info[10] trial points per dose pass actually used (ls_batch)   [11] dose-pass stages   [12] transpose stages
  * d_rowT_ptr (int32 [n_b+1]), d_colT (int32 [nnz]), d_valT (fp32 [nnz]): if non-NULL receive a copy of D^T (device).
  */
 imrt_status imrt_plan_get_info(imrt_plan* plan, int64_t* host_info, int32_t n_info,
                                int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT);
 
 /*
- * Launch ONE dose pass (kind 0: trial-point read, D x, penalty, residual, objective partials, reduction) or ONE
- * transpose pass (kind 1: D^T r, partial-slot reduction) on the plan's stream, n_repeat times back to back, on
- * scratch outputs, without touching the optimiser state.  For per-kernel timing / profiling only.  Asynchronous.
+ * Launch ONE dose pass of the line search (kind 0: ls_batch trial points -- here copies of the current iterate --,
+ * D x, penalty, residual, objective partials) or ONE transpose pass (kind 1: D^T r, partial-slot reduction) on the
+ * plan's stream, n_repeat times back to back, on scratch outputs, without touching the optimiser state.  For
+ * per-kernel timing / profiling only.  Asynchronous.
  */
 imrt_status imrt_plan_launch_pass(imrt_plan* plan, int32_t kind, int32_t n_repeat);
 

@@ -43,7 +43,7 @@ class Params(ctypes.Structure):
     """imrt_params (PAPER.md:92, :103, :114)."""
     _fields_ = [("eps", ctypes.c_double), ("alpha", ctypes.c_double), ("lambda0", ctypes.c_double),
                 ("max_ls", ctypes.c_int32), ("max_iters", ctypes.c_int32), ("driver", ctypes.c_int32),
-                ("reserved", ctypes.c_int32)]
+                ("ls_batch", ctypes.c_int32)]
 
 
 _lib = None
@@ -208,13 +208,14 @@ def imrt_plan_get_counters(plan):
     return f.value, t.value
 
 
-INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "smem_bytes", "pack_bytes", "g_slots", "nonempty_rows", "n_sm", "col16")
+INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "smem_bytes", "pack_bytes", "g_slots", "nonempty_rows", "n_sm", "col16",
+             "ls_batch", "fwd_stages", "tr_stages")
 
 
 def imrt_plan_get_info(plan, rowT_ptr=None, colT=None, valT=None) -> dict:
     import torch
-    info = np.zeros(10, np.int64)
-    _check(lib().imrt_plan_get_info(plan, _hptr(info), 10, _dptr(rowT_ptr, torch.int32), _dptr(colT, torch.int32),
+    info = np.zeros(len(INFO_KEYS), np.int64)
+    _check(lib().imrt_plan_get_info(plan, _hptr(info), len(INFO_KEYS), _dptr(rowT_ptr, torch.int32), _dptr(colT, torch.int32),
                                     _dptr(valT, torch.float32)), plan)
     return dict(zip(INFO_KEYS, (int(v) for v in info)))
 
@@ -244,7 +245,8 @@ class Plan:
     eps, alpha, lambda0, max_ls (numpy arrays / scalars); arrays may also already be torch CUDA tensors.
     """
 
-    def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None):
+    def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None,
+                 ls_batch: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_0908_4421_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -267,7 +269,7 @@ class Plan:
         self.n_structures = int(len(prob.t_under))
         self.max_iters = int(max_iters)
         self.params = Params(float(prob.eps), float(prob.alpha), float(prob.lambda0), int(prob.max_ls), self.max_iters,
-                             int(driver), 0)
+                             int(driver), int(ls_batch))
         nbytes = imrt_workspace_bytes(self.n_v, self.n_b, self.nnz, self.n_structures, self.max_iters)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         self.handle = imrt_plan_create(self.n_v, self.n_b, self.nnz, self.row_ptr, self.col, self.val, self.sid,

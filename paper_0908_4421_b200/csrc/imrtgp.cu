@@ -94,7 +94,7 @@ Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     const int64_t slots = nnz + 3 * n_v;    // every row padded to a multiple of 4 slots
     b.max_blk = 2 * (slots / MIN_CHUNK_SLOTS + 1) + 2 * (n_v / MAXROWS_F + 1) + n_v / 32 + 4;
     b.max_meta = n_v + b.max_blk * (META_HDR + 1 + 3) + 8;
-    b.max_pack = (size_t)b.max_meta * 4 + (size_t)slots * 8 + (size_t)b.max_blk * 128 + 256;
+    b.max_pack = (size_t)b.max_meta * 4 + ((size_t)slots + (size_t)ZPAD * b.max_blk) * 8 + (size_t)b.max_blk * 128 + 256;
     b.max_ranges = 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
     b.max_slots = n_b + b.max_ranges + 4;
     b.nnz_pad = ((nnz + 3) & ~(int64_t)3) + 8;
@@ -117,7 +117,7 @@ struct Layout {
     int* rowslot_ptr;
     float* xbuf[2];
     float* g;
-    float* rbuf[2];
+    float* rbuf[R_MAX + 1];
     double* Gpart[2];
     double* gslot[2];
     double* tr_obj;
@@ -157,9 +157,8 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.rowslot_ptr = w.take<int>(n_b + 1);
     for (int i = 0; i < 2; ++i) L.xbuf[i] = w.take<float>(n_b + 4);
     L.g = w.take<float>(n_b + 4);
-    L.rbuf[0] = w.take<float>(2 * (n_v + 4));   // the two residual buffers are contiguous (one L2 window)
-    L.rbuf[1] = L.rbuf[0] ? L.rbuf[0] + (n_v + 4) : nullptr;
-    for (int i = 0; i < 2; ++i) L.Gpart[i] = w.take<double>(1024);
+    for (int i = 0; i <= R_MAX; ++i) L.rbuf[i] = w.take<float>(n_v + 4);
+    for (int i = 0; i < 2; ++i) L.Gpart[i] = w.take<double>(1024 * R_MAX);
     for (int i = 0; i < 2; ++i) L.gslot[i] = w.take<double>(B.max_slots);
     L.tr_obj = w.take<double>((size_t)max_iters + 1);
     L.tr_lambda = w.take<double>((size_t)max_iters + 1);
@@ -241,31 +240,38 @@ __global__ void k_pack_blocks(const int4* __restrict__ pk, const uint32_t* __res
     for (int i = threadIdx.x; i < d.y; i += blockDim.x) rec_w[i] = m[i];
     const int nrows = (int)m[0], r0 = (int)m[1], slots = (int)m[3];
     float* val_o = reinterpret_cast<float*>(rec + (size_t)d.y * 4);
-    unsigned char* col_o = reinterpret_cast<unsigned char*>(val_o + slots);
+    unsigned char* col_o = reinterpret_cast<unsigned char*>(val_o + slots + ZPAD);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
     for (int row = warp; row < nrows; row += nwarp) {
         const int so = (int)(m[META_HDR + row] & 0xFFFFu), se = (int)(m[META_HDR + row + 1] & 0xFFFFu);
         const int p0 = row_ptr[r0 + row], len = row_ptr[r0 + row + 1] - p0;
         for (int k = lane; k < se - so; k += 32) {
             const float v = k < len ? val[p0 + k] : 0.0f;
-            const int c = k < len ? col[p0 + k] : 0;
+            const int c = xperm(k < len ? col[p0 + k] : 0);   // position in the shared-memory gather array
             val_o[so + k] = v;
             if (COL16) reinterpret_cast<unsigned short*>(col_o)[so + k] = (unsigned short)c;
             else reinterpret_cast<int*>(col_o)[so + k] = c;
         }
     }
+    if (threadIdx.x < ZPAD) {   // the zero slots lanes past a row's end read
+        val_o[slots + threadIdx.x] = 0.0f;
+        if (COL16) reinterpret_cast<unsigned short*>(col_o)[slots + threadIdx.x] = 0;
+        else reinterpret_cast<int*>(col_o)[slots + threadIdx.x] = 0;
+    }
 }
 
 // d = 0 and the matching constant residual on every row; the dose pass then overwrites the rows its blocks cover.
-__global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, int n_v, float* r0,
-                                      float* r1, float* d) {
+struct RPtrs { float* p[R_MAX + 1]; };
+__global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, int n_v, const RPtrs R,
+                                      float* d) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_v) return;
     const float4 t = table[sid[j]];
     const float u = fmaxf(0.0f, t.x), o = fmaxf(0.0f, -t.y);
     const float r = 2.0f * (t.w * o - t.z * u);
-    if (r0) r0[j] = r;
-    if (r1) r1[j] = r;
+#pragma unroll
+    for (int i = 0; i <= R_MAX; ++i)
+        if (R.p[i]) R.p[i][j] = r;
     if (d) d[j] = 0.0f;
 }
 
@@ -279,10 +285,10 @@ __global__ void k_check_x(const float* __restrict__ x, int n_b, State* st) {
 }
 
 __global__ void k_reset_state(State* st) {
-    st->G_k = 0.0; st->lambda = st->lambda0; st->step_sq = 0.0;
+    st->G_k = 0.0; st->lambda = st->lambda0;
     st->fwd_passes = 0; st->tr_passes = 0;
     st->iter = 0; st->iter_target = 0; st->m = 0; st->stop_reason = STOP_MAX_ITERS;
-    st->xi = 1; st->ri = 1;   // the MODE_INIT dose pass reads xbuf[0], writes rbuf[0] and flips both
+    st->xi = 0; st->ri = 0;   // the MODE_INIT dose pass reads xbuf[0], writes rbuf[1] and makes it current
     st->cont_outer = 0; st->cont_inner = 0; st->bad_x = 0;
     st->ticket_f = 0u; st->ticket_t = 0u; st->gridbar = 0u;
 }
@@ -323,7 +329,6 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
     };
     auto pad4 = [](int n) { return (n + 3) & ~3; };
     int j = 0;
-    uint32_t q_prefix = 0;
     size_t off = 0;
     while (j < n_v) {
         if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
@@ -352,8 +357,7 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         const int mo = (int)B.meta.size();
         B.meta.push_back((uint32_t)nrows);
         B.meta.push_back((uint32_t)r0);
-        B.meta.push_back(q_prefix & (uint32_t)(W_CONS - 1));   // warp batches dealt so far: round-robin continues across blocks
-        q_prefix += (uint32_t)((nrows + RB - 1) / RB);
+        B.meta.push_back(0u);
         B.meta.push_back((uint32_t)slots);
         int so = 0;
         for (int row = r0; row < r1; ++row) {
@@ -363,7 +367,7 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         B.meta.push_back((uint32_t)so);
         while ((B.meta.size() - mo - META_HDR) & 3) B.meta.push_back(0u);
         const int mw = (int)B.meta.size() - mo;
-        const int rec = (mw * 4 + slots * (4 + col_bytes) + 127) & ~127;
+        const int rec = (mw * 4 + (slots + ZPAD) * (4 + col_bytes) + 127) & ~127;
         B.blk.push_back(make_int2((int)(off / 128), rec));
         B.pk.push_back(make_int4(mo, mw, (int)(off / 128), 0));
         B.rows.push_back(nrows);
@@ -459,12 +463,9 @@ static imrt_status tune_partition(imrt_plan* pl) {
     const size_t n_blk = pl->blk_cost.size();
     if (getenv("IMRTGP_NO_TUNE") || n_blk < (size_t)grid * 8) return IMRT_STATUS_OK;
     cudaStream_t st = pl->stream;
-    CUDA_TRY(pl, cudaMemsetAsync(pl->P.xbuf[0], 0, sizeof(float) * pl->P.n_b, st));
-    PassArgs A;
+    PassArgs A;              // the loop's own dose pass (R trial points) on x = 0
     memset(&A, 0, sizeof A);
-    A.mode = MODE_EVAL;
-    A.x_in = pl->P.xbuf[0];
-    A.r_out = pl->r_scratch;
+    A.mode = MODE_TIMING;
     std::vector<int> cta_blk;
     partition_blocks(pl->blk_cost, grid, cta_blk);
     std::vector<unsigned long long> t(2 * (size_t)grid);
@@ -599,7 +600,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     if (nnz >= (1LL << 31) - 16 || n_v >= (1LL << 31) - 16 || n_b >= (1LL << 31) - 16)
         return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "sizes must fit int32");
     if (!(prm->eps > 0.0 && prm->eps < 1.0) || !(prm->alpha > 1.0) || !(prm->lambda0 > 0.0) || !std::isfinite(prm->lambda0) ||
-        prm->max_ls < 0 || prm->max_iters < 0 || prm->driver < 0 || prm->driver > 2 || prm->reserved != 0)
+        prm->max_ls < 0 || prm->max_iters < 0 || prm->driver < 0 || prm->driver > 2 || prm->ls_batch < 0 || prm->ls_batch > R_MAX)
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad imrt_params (need 0<eps<1, alpha>1, lambda0>0, driver in 0..2)");
     if (((uintptr_t)row_ptr | (uintptr_t)col_idx | (uintptr_t)val | (uintptr_t)workspace) & 15)
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: device arrays must be 16-byte aligned");
@@ -658,21 +659,17 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     for (int s = 0; s < n_structures; ++s) table_h[s] = make_float4(host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]);
     CUDA_TRY(pl, cudaMemcpyAsync(L.table, table_h.data(), sizeof(float4) * MAX_STRUCTURES, cudaMemcpyHostToDevice, st));
 
-    // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, x+, g, stages
-    const int nb_pad = (int)((n_b + 31) & ~31LL);
-    int off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
     DevPlan& P = pl->P;
     memset(&P, 0, sizeof P);
-    P.wpart_off = off; off += SMEM_WPART;
-    P.x_off = off; off += nb_pad * 4;
-    P.g_off = off; off += nb_pad * 4;
-    off = (off + 127) & ~127;
-    P.stage_off = off;
-    const int avail = smem_optin - off;
 
-    // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero)
+    // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero); a block holds
+    // MIN_CHUNK_SLOTS slots unless a longer row forces more
     const bool col16 = n_b <= 65536 && !getenv("IMRTGP_COL32");
-    const int chunk_slots = col16 ? 4096 : 3072;
+    int max_row = 0;
+    for (int64_t j = 0; j < n_v; ++j) max_row = std::max(max_row, rp[j + 1] - rp[j]);
+    const int chunk_slots = std::max(MIN_CHUNK_SLOTS, (max_row + 3) & ~3);
+    if (chunk_slots > MAX_CHUNK_SLOTS)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row of D has %d entries; this build handles rows up to %d", max_row, MAX_CHUNK_SLOTS);
     BlockPlan BP;
     double G_skip = 0.0;
     imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, BP, G_skip, pl->n_skipped, pl->n_nonempty);
@@ -734,11 +731,32 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     if (!ranges.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.tr_range, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
     CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
 
+    // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, dose
+    // scratch, the R trial points, g, stages.  R = the largest of 4, 2, 1 not above the request that leaves room for
+    // a useful ring.
     const int stage_f = std::max(BP.max_rec_bytes, 128);
-    const int sf = std::min(MAX_STAGES, avail / stage_f), stt = std::min(MAX_STAGES, avail / STAGE_T_BYTES);
+    const int nb_pad = (int)((n_b + 31) & ~31LL);
+    int R = prm->ls_batch == 0 ? R_MAX : prm->ls_batch;
+    if (getenv("IMRTGP_LS_BATCH")) R = atoi(getenv("IMRTGP_LS_BATCH"));
+    if (R != 1 && R != 2 && R != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_params.ls_batch must be 0, 1, 2 or 4");
+    int off = 0, avail = 0, sf = 0, stt = 0;
+    for (;; R /= 2) {
+        off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
+        P.wpart_off = off; off += SMEM_WPART;
+        P.dsc_off = off; off += SMEM_DSC;
+        P.x_off = off; off += nb_pad * 4 * R;
+        P.g_off = off; off += nb_pad * 4;
+        off = (off + 127) & ~127;
+        P.stage_off = off;
+        avail = smem_optin - off;
+        sf = avail > 0 ? std::min(MAX_STAGES_F, avail / stage_f) : 0;
+        stt = avail > 0 ? std::min(MAX_STAGES_T, avail / STAGE_T_BYTES) : 0;
+        if (R == 1 || (sf >= W_CONS / 2 && stt >= 3)) break;
+    }
     if (avail < 0 || sf < 2 || stt < 2)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets do not fit in shared memory next to the pipeline stages", (long long)n_b);
     pl->smem_bytes = (size_t)off + (size_t)std::max(sf * stage_f, stt * STAGE_T_BYTES);
+    P.R = R;
 
     P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
     P.pack = L.pack; P.blk = L.blk; P.cta_blk = L.cta_blk; P.grid_f = grid_f; P.n_stages_f = sf;
@@ -748,7 +766,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.n_ranges = (int)ranges.size(); P.grid_t = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, ranges.size()));
     P.n_stages_t = stt; P.n_slots = n_slots;
     P.table = L.table; P.n_structures = n_structures; P.G_skip = G_skip;
-    P.xbuf[0] = L.xbuf[0]; P.xbuf[1] = L.xbuf[1]; P.g = L.g; P.rbuf[0] = L.rbuf[0]; P.rbuf[1] = L.rbuf[1];
+    P.xbuf[0] = L.xbuf[0]; P.xbuf[1] = L.xbuf[1]; P.g = L.g;
+    for (int i = 0; i <= R_MAX; ++i) P.rbuf[i] = L.rbuf[i];
     P.Gpart[0] = L.Gpart[0]; P.Gpart[1] = L.Gpart[1]; P.gslot[0] = L.gslot[0]; P.gslot[1] = L.gslot[1];
     P.cta_ns = L.cta_ns;
     P.st = L.st; P.tr_obj = L.tr_obj; P.tr_lambda = L.tr_lambda; P.tr_step_sq = L.tr_step_sq; P.tr_trials = L.tr_trials;
@@ -766,15 +785,21 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     State st_h;
     memset(&st_h, 0, sizeof st_h);
     st_h.eps = prm->eps; st_h.alpha = prm->alpha; st_h.lambda0 = prm->lambda0; st_h.lambda = prm->lambda0;
-    st_h.max_ls = prm->max_ls; st_h.trace_cap = prm->max_iters; st_h.xi = 1; st_h.ri = 1;
+    st_h.max_ls = prm->max_ls; st_h.trace_cap = prm->max_iters; st_h.xi = 0; st_h.ri = 0;
     CUDA_TRY(pl, cudaMemcpyAsync(L.st, &st_h, sizeof st_h, cudaMemcpyHostToDevice, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.gslot[0], 0, sizeof(double) * B.max_slots, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.gslot[1], 0, sizeof(double) * B.max_slots, st));
-    CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[0], 0, sizeof(double) * 1024, st));
-    CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[1], 0, sizeof(double) * 1024, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[0], 0, sizeof(double) * 1024 * R_MAX, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[1], 0, sizeof(double) * 1024 * R_MAX, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.xbuf[0], 0, sizeof(float) * (n_b + 4), st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.xbuf[1], 0, sizeof(float) * (n_b + 4), st));
     CUDA_TRY(pl, cudaMemsetAsync(L.g, 0, sizeof(float) * (n_b + 4), st));
     CUDA_TRY(pl, cudaMemsetAsync(L.cta_ns, 0, sizeof(unsigned long long) * 4096, st));
-    k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, (int)n_v, L.rbuf[0], L.rbuf[1], nullptr);
+    {
+        RPtrs rp_all;
+        for (int i = 0; i <= R_MAX; ++i) rp_all.p[i] = L.rbuf[i];
+        k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, (int)n_v, rp_all, nullptr);
+    }
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
 
@@ -864,7 +889,10 @@ imrt_status imrt_plan_eval(imrt_plan* pl, const float* x, float* d, float* r, fl
     cudaStream_t st = pl->stream;
     float* r_used = r ? r : pl->r_scratch;
     const int n_v = pl->P.n_v;
-    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, st>>>(pl->sid, pl->P.table, n_v, r_used, nullptr, d);
+    RPtrs rp1;
+    memset(&rp1, 0, sizeof rp1);
+    rp1.p[0] = r_used;
+    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, st>>>(pl->sid, pl->P.table, n_v, rp1, d);
     PassArgs A;
     memset(&A, 0, sizeof A);
     A.mode = MODE_EVAL;
@@ -897,7 +925,9 @@ imrt_status imrt_plan_get_x(imrt_plan* pl, float* x) {
 
 static imrt_status dose_of_current_x(imrt_plan* pl, float* d) {
     const int n_v = pl->P.n_v;
-    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, pl->stream>>>(pl->sid, pl->P.table, n_v, nullptr, nullptr, d);
+    RPtrs rp0;
+    memset(&rp0, 0, sizeof rp0);
+    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, pl->stream>>>(pl->sid, pl->P.table, n_v, rp0, d);
     PassArgs A;
     memset(&A, 0, sizeof A);
     A.mode = MODE_EVAL;   // x_in NULL: the current iterate
@@ -957,9 +987,9 @@ imrt_status imrt_plan_get_counters(imrt_plan* pl, int64_t* host_fwd_passes, int6
 
 imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info, int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT) {
     if (!pl) return IMRT_STATUS_INVALID_ARG;
-    const int64_t info[10] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
-                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16};
-    for (int i = 0; i < n_info && i < 10 && host_info; ++i) host_info[i] = info[i];
+    const int64_t info[13] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
+                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.n_stages_f, pl->P.n_stages_t};
+    for (int i = 0; i < n_info && i < 13 && host_info; ++i) host_info[i] = info[i];
     cudaStream_t st = pl->stream;
     if (d_rowT_ptr) CUDA_TRY(pl, cudaMemcpyAsync(d_rowT_ptr, pl->rowT_ptr_w, sizeof(int) * (pl->P.n_b + 1), cudaMemcpyDeviceToDevice, st));
     if (d_colT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_colT, pl->colT_w, sizeof(int) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));
@@ -988,9 +1018,8 @@ imrt_status imrt_plan_launch_pass(imrt_plan* pl, int32_t kind, int32_t n_repeat)
     if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
     PassArgs A;
     memset(&A, 0, sizeof A);
-    A.mode = MODE_EVAL;
-    A.r_out = pl->r_scratch;    // dose pass: at the current iterate, outputs to scratch
-    A.g_out = pl->g_scratch;    // transpose pass: on r(x_k), output to scratch
+    A.mode = kind == 0 ? MODE_TIMING : MODE_EVAL;   // dose pass: the line search's pass, residuals to the trial buffers
+    A.g_out = pl->g_scratch;                        // transpose pass: on r(x_k), output to scratch
     for (int i = 0; i < n_repeat; ++i) CUDA_TRY(pl, kind == 0 ? launch_dose(pl, A) : launch_transpose(pl, A));
     return IMRT_STATUS_OK;
 }

@@ -29,29 +29,38 @@ namespace imrt {
 constexpr int W_CONS = 16;                    // consumer warps per CTA
 constexpr int N_CONS = W_CONS * 32;           // consumer threads
 constexpr int NTHREADS = N_CONS + 32;         // + one producer warp
-// dose pass: D is re-packed once into self-contained block records (one bulk copy each, see DosePack below)
-constexpr int META_HDR = 4;                   // header words {rows, first row, batches dealt before | flags, slots}
-constexpr int MIN_CHUNK_SLOTS = 2048;           // smallest slot capacity of a dose-pass stage the host will choose
-constexpr int MAXROWS_F = 507;                // rows per block: header + row table fit 2 KB
-constexpr int META_F_BYTES = (META_HDR + MAXROWS_F + 1) * 4;
+// dose pass: D is re-packed once into self-contained block records (one bulk copy each, see DevPlan::pack)
+constexpr int META_HDR = 4;                   // header words {rows, first row, 0, slots}
+constexpr int MIN_CHUNK_SLOTS = 1024;         // slot capacity of a block unless a longer row forces more
+constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
+constexpr int MAXROWS_F = 256;                // rows per block
+constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
+constexpr int R_MAX = 4;                      // line-search trial points evaluated per dose pass (1, 2 or 4)
 constexpr int CHUNK_T = 4096;                 // nnz per transpose-pass stage (pure streaming)
 constexpr int SLICE_T = CHUNK_T / W_CONS;     // contiguous nnz per consumer warp per stage
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
 constexpr int RL_MAX = 32;                    // rows of D^T one transpose range may span
-constexpr int MAX_STAGES = 12;
+constexpr int MAX_STAGES_F = 40;
+constexpr int MAX_STAGES_T = 12;
 constexpr int MAX_STRUCTURES = 256;
-constexpr int SMEM_HEADER = 1024;             // barriers, flags, reduction scratch
+constexpr int SMEM_HEADER = 2048;             // barriers, flags, reduction scratch
 constexpr int SMEM_WPART = RL_MAX * W_CONS * 8;
+constexpr int SMEM_DSC = W_CONS * 32 * R_MAX * 4;   // per-warp scratch: dose of 32 rows x R trial points
 
-enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2 };
+enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2, MODE_TIMING = 3 };
 enum { STOP_MAX_ITERS = 0, STOP_TOLERANCE = 1, STOP_STATIONARY = 2, STOP_LS_STALLED = 3 };
+
+// Beamlet i lives at position xperm(i) of the shared-memory copy of x+: bits [4:2] of i move to the bottom.  A row
+// group's 8 lanes read 4 consecutive slots each, i.e. columns ~4 apart in a run of neighbouring beamlets; with this
+// permutation they fall into 8 different banks (R = 1) / 8 different 16-byte bank groups (R = 4).  The packed
+// records store xperm(col) so the kernels never compute it.
+__host__ __device__ __forceinline__ int xperm(int i) { return (i & ~31) | ((i & 3) << 3) | ((i >> 2) & 7); }
 
 // ------------------------------------------------------------------------------------------------ device data
 struct State {                 // lives in the workspace; the single source of truth between launches
     double G_k;                // objective at the current iterate
-    double lambda;             // step size of the pending trial
-    double step_sq;            // Delta of the pending trial
+    double lambda;             // step size of the first trial of the pending batch
     double eps, alpha, lambda0, delta_tol;
     double eval_obj;           // output of MODE_EVAL dose passes
     long long fwd_passes, tr_passes;
@@ -59,10 +68,10 @@ struct State {                 // lives in the workspace; the single source of t
     int iter;                  // accepted iterations since set_x
     int iter_target;           // stop when iter reaches this
     int trace_cap;
-    int m;                     // backtracking steps taken in the current line search
+    int m;                     // backtracking steps taken in the current line search (= index of the batch's first trial)
     int stop_reason;
-    int xi;                    // xbuf[xi] is the current iterate, xbuf[xi^1] the trial point
-    int ri;                    // rbuf[ri] is r(x_k), rbuf[ri^1] receives r(x+)
+    int xi;                    // xbuf[xi] is the current iterate
+    int ri;                    // rbuf[ri] is r(x_k); trial j of a batch writes rbuf[(ri + 1 + j) % (R + 1)]
     int cont_outer, cont_inner;  // loop conditions (mirrors of the graph conditionals; read by the host driver)
     int bad_x;                 // set_x validation result
     unsigned int ticket_f, ticket_t;   // last-CTA tickets
@@ -79,23 +88,23 @@ struct TrRange {               // a contiguous piece of the D^T nnz stream, 32 b
 };
 
 struct DevPlan {
-    // D (borrowed): CSR, rows = voxels
-    const int* col;
-    const float* val;
     long long nnz;
     int n_v, n_b;
     // dose pass: D re-packed into block records (owned).  A record is 128-byte aligned and holds, in this order,
-    //   header  uint32[4]  {rows, first row, warp batches dealt before this block (mod W_CONS), slots}
+    //   header  uint32[4]  {rows, first row, 0, slots}
     //   rows    uint32[rows + 1]  slot offset of the row (low 16 bits, a multiple of 4) | structure id << 16;
     //                             padded to a multiple of 4 words
-    //   val     fp32[slots]       every row padded with zeros to a multiple of 4 slots
-    //   col     uint16[slots] (n_b <= 65536) or int32[slots]
+    //   val     fp32[slots + ZPAD]   every row padded with zeros to a multiple of 4 slots; ZPAD zeros at the end
+    //   col     uint16[slots + ZPAD] (n_b <= 65536) or int32[slots + ZPAD]: xperm(column)
+    // One record is consumed by ONE warp.
     const unsigned char* pack;
     const int2* blk;           // {record offset / 128, record bytes}
     const int* cta_blk;        // [grid_f + 1] block range per CTA
     int grid_f, n_stages_f;
     int stage_f_bytes;         // bytes of one dose-pass stage (largest record, 128-byte multiple)
     int col16;                 // 1: 16-bit column indices in the records
+    int R;                     // trial points per dose pass of the line search (1, 2 or 4)
+    int pad1;
     // D^T (owned): CSR, rows = beamlets, padded with zeros to a multiple of 4 entries
     const int* rowT_ptr;
     const int* colT;
@@ -112,8 +121,8 @@ struct DevPlan {
     // vectors
     float* xbuf[2];
     float* g;
-    float* rbuf[2];
-    double* Gpart[2];          // [grid_f] objective partials, double-buffered by pass parity
+    float* rbuf[R_MAX + 1];    // residual buffers: one holds r(x_k), the others receive r of the batch's trial points
+    double* Gpart[2];          // [grid_f][R] objective partials, double-buffered by pass parity
     double* gslot[2];          // [n_slots] gradient partials, double-buffered
     State* st;
     unsigned long long* cta_ns;  // [2][1024][2] per-CTA {start, end of streaming} of the last dose / transpose pass, ns
@@ -122,15 +131,16 @@ struct DevPlan {
     double* tr_step_sq;        // [cap]
     int* tr_trials;            // [cap]
     int wpart_off;             // byte offsets into dynamic shared memory: transpose per-(row, warp) partials,
-    int x_off, g_off;          // the trial point x+ (gathered by the dose pass) and the gradient (persistent kernel)
+    int dsc_off;               // dose-pass per-warp scratch,
+    int x_off, g_off;          // the trial points x+ [n_b][R] (gathered by the dose pass) and the gradient (persistent kernel)
     int stage_off;             // byte offset of the stage ring
 };
 
 struct PassArgs {
-    const float* x_in;         // dose pass: where to evaluate (NULL = the trial point xbuf[xi^1]; MODE_EVAL: x_k)
+    const float* x_in;         // dose pass, MODE_EVAL / MODE_INIT: where to evaluate (NULL = the current iterate)
     const float* r_in;         // transpose pass: residual (NULL = rbuf[ri])
-    float* r_out;              // dose pass: residual out (NULL = rbuf[ri^1])
-    float* d_out;              // dose pass: dose out or NULL
+    float* r_out;              // dose pass, MODE_EVAL: residual out
+    float* d_out;              // dose pass, MODE_EVAL: dose out or NULL
     float* g_out;              // transpose pass MODE_EVAL: gradient out
     int mode;
     int use_handles;           // 1 inside the conditional graph
@@ -139,8 +149,8 @@ struct PassArgs {
 
 // ------------------------------------------------------------------------------------------------ shared memory
 struct SmemHeader {
-    uint64_t full_f[MAX_STAGES], empty_f[MAX_STAGES], full_t[MAX_STAGES], empty_t[MAX_STAGES];
-    double red[32];            // block-reduction scratch
+    uint64_t full_f[MAX_STAGES_F], empty_f[MAX_STAGES_F], full_t[MAX_STAGES_T], empty_t[MAX_STAGES_T];
+    double red[32 * R_MAX];    // block-reduction scratch
     double bcast[4];
     int flag;
 };
@@ -152,9 +162,11 @@ struct Pipe {                  // running stage counters; identical in producer 
 
 __device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4* table_s) {
     if (threadIdx.x == 0) {
-        for (int s = 0; s < MAX_STAGES; ++s) {
+        for (int s = 0; s < MAX_STAGES_F; ++s) {
             mbar_init(&h->full_f[s], 1);
-            mbar_init(&h->empty_f[s], W_CONS);
+            mbar_init(&h->empty_f[s], 1);      // a dose-pass stage is consumed by one warp
+        }
+        for (int s = 0; s < MAX_STAGES_T; ++s) {
             mbar_init(&h->full_t[s], 1);
             mbar_init(&h->empty_t[s], W_CONS);
         }
@@ -183,100 +195,185 @@ __device__ __forceinline__ double block_sum(double v, SmemHeader* h) {
     for (int w = 0; w < NTHREADS / 32; ++w) s += h->red[w];
     return s;
 }
+// The same for R values at once; every component is summed in exactly the order block_sum uses.
+template <int R>
+__device__ __forceinline__ void block_sum_vec(double (&v)[R], SmemHeader* h) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[r] = warp_sum(v[r]);
+    __syncthreads();
+    if (lane == 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) h->red[r * 32 + warp] = v[r];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < NTHREADS / 32; ++w) s += h->red[r * 32 + w];
+        v[r] = s;
+    }
+}
 
-// ------------------------------------------------------------------------------------------------ trial point
+// ------------------------------------------------------------------------------------------------ trial points
 // x+ = max(0, x - lambda g), Delta = sum (x+ - x)^2      PAPER.md:90 (projection), :109/:111 (steps 2, 4), Eq. (5).
-// fp32 elementwise, fp64 sum.  All NTHREADS threads call it; x is global (read through L2: another CTA may have
-// written it), g and x_new may be shared or global memory.
-__device__ __forceinline__ double compute_trial(const float* x, const float* g, double lambda, float* x_new, int n_b,
-                                                SmemHeader* h) {
+// fp32 elementwise, fp64 sum.  A batch holds the next R trial points of the line search: lambda, lambda/alpha, ...
+// (the same division chain step 4 performs one trial at a time).  All NTHREADS threads call it; x is global (read
+// through L2: another CTA may have written it), g may be shared or global; xs is the shared-memory array the dose
+// pass gathers from, [n_b][R] at permuted positions (xperm).
+template <int R>
+__device__ __forceinline__ void trial_batch(const float* x, const float* g, double lambda, double alpha, float* xs, int n_b,
+                                            SmemHeader* h, double (&step_sq)[R]) {
+    float lam[R];
+    double l = lambda;
+#pragma unroll
+    for (int r = 0; r < R; ++r) { lam[r] = (float)l; l = l / alpha; step_sq[r] = 0.0; }
+    for (int i = threadIdx.x; i < n_b; i += NTHREADS) {
+        const float xi = __ldcg(x + i), gi = g[i];
+        float* o = xs + (size_t)xperm(i) * R;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float xn = fmaxf(0.0f, fmaf(-lam[r], gi, xi));
+            const float dx = xn - xi;
+            step_sq[r] = __fma_rn((double)dx, (double)dx, step_sq[r]);
+            o[r] = xn;
+        }
+    }
+    block_sum_vec<R>(step_sq, h);
+}
+
+// Only Delta of the first trial (the STATIONARY test of reading R4 at the start of a line search).
+__device__ __forceinline__ double first_step_sq(const float* x, const float* g, double lambda, int n_b, SmemHeader* h) {
     const float lam = (float)lambda;
     double acc = 0.0;
     for (int i = threadIdx.x; i < n_b; i += NTHREADS) {
         const float xi = __ldcg(x + i);
-        const float xn = fmaxf(0.0f, fmaf(-lam, g[i], xi));
-        const float dx = xn - xi;
-        acc += (double)dx * (double)dx;
-        x_new[i] = xn;
+        const float dx = fmaxf(0.0f, fmaf(-lam, g[i], xi)) - xi;
+        acc = __fma_rn((double)dx, (double)dx, acc);
     }
     return block_sum(acc, h);
 }
 
+// A single point x (MODE_EVAL / MODE_INIT): copy it to the gather array.
+__device__ __forceinline__ void stage_point(const float* x, float* xs, int n_b) {
+    for (int i = threadIdx.x; i < n_b; i += NTHREADS) xs[xperm(i)] = x[i];
+    __syncthreads();
+}
+
 // ------------------------------------------------------------------------------------------------ dose pass
-// VW lanes per row, RB = 32 / VW rows per warp batch, 4 consecutive slots per lane and trip: rows start on 16-byte
-// boundaries inside a record and are zero-padded to a multiple of 4 slots, so values and columns come in with one
-// 128-bit (64-bit for 16-bit columns) shared-memory load each and nothing has to be masked inside a row.  The row
-// groups of a warp run the trip count of their longest row (neighbouring voxels have rows of similar length),
-// gather x+ from shared memory, multiply-add in fp32 and reduce with log2(VW) shuffles; lane 0 of each group then
-// does its voxel's penalty and residual (Eq. (1) generalised: F = w- u^2 + w+ o^2, r = 2 (w+ o - w- u)).
-// Batches are numbered across the CTA's blocks and dealt round-robin to the consumer warps, which never
-// synchronise with each other: a warp with nothing to do in this stage moves on to the next one.
+// One block record is consumed by ONE warp (the CTA's blocks are dealt round-robin to its 16 consumer warps, which
+// never synchronise with each other).  Inside a record: VW = 8 lanes per row, 4 rows per warp batch, 4 consecutive
+// slots per lane and trip.  Rows start on 16-byte boundaries and are zero-padded to a multiple of 4 slots, so values
+// and columns come in with one 128-bit (64-bit for 16-bit columns) shared-memory load each; a lane past the end of
+// its row reads the record's zero slots instead, which keeps the trip loop free of divergent branches.  The row
+// groups of a batch run the trip count of their longest row (neighbouring voxels have rows of similar length).
+// Each lane gathers the R trial values of its 4 beamlets from shared memory ([n_b][R], one vector load per beamlet),
+// multiply-adds in fp32 (one accumulator per slot position and trial point, so the sum of a row does not depend on
+// R) and the group reduces with 3 shuffles.  Doses of 32 rows are parked in a per-warp scratch; then every lane
+// takes one row: penalty and residual per trial point (Eq. (1) generalised: F = w- u^2 + w+ o^2,
+// r = 2 (w+ o - w- u)), coalesced stores of r, fp64 accumulation of F.
 constexpr int VW = 8;
 constexpr int RB = 32 / VW;
 
-template <bool COL16>
-__device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec, const float* __restrict__ x_s,
-                                           const float4* __restrict__ table_s, float* __restrict__ r_out,
-                                           float* __restrict__ d_out, int warp, int lane, double& Gacc) {
+template <int R> struct XVec;
+template <> struct XVec<1> { float v[1]; __device__ __forceinline__ void load(const unsigned char* p) { v[0] = *reinterpret_cast<const float*>(p); } };
+template <> struct XVec<2> { float v[2]; __device__ __forceinline__ void load(const unsigned char* p) { const float2 t = *reinterpret_cast<const float2*>(p); v[0] = t.x; v[1] = t.y; } };
+template <> struct XVec<4> { float v[4]; __device__ __forceinline__ void load(const unsigned char* p) { const float4 t = *reinterpret_cast<const float4*>(p); v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w; } };
+
+template <bool COL16, int R>
+__device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
+                                           const float4* __restrict__ table_s, float* __restrict__ dsc,
+                                           float* const (&r_out)[R], float* __restrict__ d_out, int lane, double (&Gacc)[R]) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
-    const int nrows = (int)hdr.x;
-    const int nbatch = (nrows + RB - 1) / RB;
+    const int nrows = (int)hdr.x, slots = (int)hdr.w;
     const uint32_t* rows = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
-    const float* val_s = reinterpret_cast<const float*>(rows + ((nrows + 1 + 3) & ~3));
-    const unsigned char* col_s = reinterpret_cast<const unsigned char*>(val_s + hdr.w);
+    const unsigned char* val_b = reinterpret_cast<const unsigned char*>(rows + ((nrows + 1 + 3) & ~3));
+    const unsigned char* col_b = val_b + (size_t)(slots + ZPAD) * 4;
     const int grp = lane / VW, sub = lane % VW;
-    for (int q = (warp - (int)hdr.z) & (W_CONS - 1); q < nbatch; q += W_CONS) {
-        const int row = q * RB + grp;
-        const bool valid = row < nrows;
-        uint32_t m0 = 0u, m1 = 0u;
-        if (valid) { m0 = rows[row]; m1 = rows[row + 1]; }
-        const int s = (int)(m0 & 0xFFFFu), e = (int)(m1 & 0xFFFFu);
-        const int len_max = __reduce_max_sync(0xffffffffu, e - s);   // warp-uniform trip count
-        float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
-        int k = s + 4 * sub;
-        for (int kb = 0; kb < len_max; kb += 4 * VW, k += 4 * VW) {
-            if (k < e) {
-                const float4 v = *reinterpret_cast<const float4*>(val_s + k);
-                int c0, c1, c2, c3;
+    constexpr int XB = 4 * R;   // bytes per beamlet in the gather array
+    for (int c0 = 0; c0 < nrows; c0 += 32) {
+        const int nbatch = min(32 / RB, (nrows - c0 + RB - 1) / RB);
+        for (int q = 0; q < nbatch; ++q) {
+            const int row = c0 + q * RB + grp;
+            uint32_t m0 = 0u, m1 = 0u;
+            if (row < nrows) { m0 = rows[row]; m1 = rows[row + 1]; }
+            const int s = (int)(m0 & 0xFFFFu), e = (int)(m1 & 0xFFFFu);
+            const int len_max = __reduce_max_sync(0xffffffffu, e - s);   // warp-uniform trip count
+            float acc[4][R];
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[j][r] = 0.0f;
+            int k = s + 4 * sub;
+#pragma unroll 2
+            for (int kb = 0; kb < len_max; kb += 4 * VW, k += 4 * VW) {
+                const int kk = k < e ? k : slots;          // past the row's end: the zero slots
+                const float4 v = *reinterpret_cast<const float4*>(val_b + 4 * kk);
+                uint32_t o0, o1, o2, o3;                   // byte offsets into the gather array
                 if (COL16) {
-                    const uint2 c = *reinterpret_cast<const uint2*>(col_s + 2 * k);
-                    c0 = (int)(c.x & 0xFFFFu); c1 = (int)(c.x >> 16); c2 = (int)(c.y & 0xFFFFu); c3 = (int)(c.y >> 16);
+                    const uint2 c = *reinterpret_cast<const uint2*>(col_b + 2 * kk);
+                    o0 = (c.x & 0xFFFFu) * XB; o1 = (c.x >> 16) * XB; o2 = (c.y & 0xFFFFu) * XB; o3 = (c.y >> 16) * XB;
                 } else {
-                    const int4 c = *reinterpret_cast<const int4*>(col_s + 4 * k);
-                    c0 = c.x; c1 = c.y; c2 = c.z; c3 = c.w;
+                    const uint4 c = *reinterpret_cast<const uint4*>(col_b + 4 * kk);
+                    o0 = c.x * XB; o1 = c.y * XB; o2 = c.z * XB; o3 = c.w * XB;
                 }
-                a0 = fmaf(v.x, x_s[c0], a0);
-                a1 = fmaf(v.y, x_s[c1], a1);
-                a2 = fmaf(v.z, x_s[c2], a2);
-                a3 = fmaf(v.w, x_s[c3], a3);
+                XVec<R> x0, x1, x2, x3;
+                x0.load(xs_b + o0); x1.load(xs_b + o1); x2.load(xs_b + o2); x3.load(xs_b + o3);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    acc[0][r] = fmaf(v.x, x0.v[r], acc[0][r]);
+                    acc[1][r] = fmaf(v.y, x1.v[r], acc[1][r]);
+                    acc[2][r] = fmaf(v.z, x2.v[r], acc[2][r]);
+                    acc[3][r] = fmaf(v.w, x3.v[r], acc[3][r]);
+                }
+            }
+            float d[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) d[r] = vec_sum<VW>((acc[0][r] + acc[1][r]) + (acc[2][r] + acc[3][r]));
+            if (sub == 0) {   // rows past the end park a zero nobody reads
+                float* o = dsc + (q * RB + grp) * R;
+#pragma unroll
+                for (int r = 0; r < R; ++r) o[r] = d[r];
             }
         }
-        const float d = vec_sum<VW>((a0 + a1) + (a2 + a3));
-        if (valid && sub == 0) {
-            const float4 t = table_s[(m0 >> 16) & 0xFFu];
-            const float u = fmaxf(0.0f, t.x - d);
-            const float o = fmaxf(0.0f, d - t.y);
-            r_out[hdr.y + row] = 2.0f * (t.w * o - t.z * u);
-            if (d_out) d_out[hdr.y + row] = d;
-            Gacc += (double)t.z * ((double)u * (double)u) + (double)t.w * ((double)o * (double)o);
+        __syncwarp();
+        const int row = c0 + lane;
+        if (row < nrows) {
+            const float4 t = table_s[(rows[row] >> 16) & 0xFFu];
+            XVec<R> dv;
+            dv.load(reinterpret_cast<const unsigned char*>(dsc + lane * R));
+            const size_t j = (size_t)hdr.y + row;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const float dd = dv.v[r];
+                const float u = fmaxf(0.0f, t.x - dd);
+                const float o = fmaxf(0.0f, dd - t.y);
+                r_out[r][j] = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));      // explicit roundings: every
+                const double du = (double)u, d_o = (double)o;                         // instantiation sums alike
+                Gacc[r] = __dadd_rn(Gacc[r], __fma_rn((double)t.z, __dmul_rn(du, du), __dmul_rn((double)t.w, __dmul_rn(d_o, d_o))));
+            }
+            if (R == 1 && d_out) d_out[j] = dv.v[0];
         }
+        __syncwarp();
     }
 }
 
-// All NTHREADS threads of the CTA call this.  x_s: the trial point in shared memory.  Writes the CTA's objective
-// partial to Gpart[blockIdx.x] (thread 0).  Ends with a CTA-wide barrier.
-template <bool COL16>
+// All NTHREADS threads of the CTA call this.  xs: the R trial points in shared memory.  Writes the CTA's R objective
+// partials to Gpart[blockIdx.x * R ..] (thread 0).  Ends with a CTA-wide barrier.
+template <bool COL16, int R>
 __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
-                                            const float* x_s, float* r_out, float* d_out, double* Gpart, Pipe& pipe) {
+                                            const float* xs, float* const (&r_out)[R], float* d_out, double* Gpart, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int S = P.n_stages_f;
+    const unsigned int S = (unsigned int)P.n_stages_f;
     const uint32_t SB = (uint32_t)P.stage_f_bytes;
     unsigned char* stages = smem + P.stage_off;
     const int b0 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x] : 0;
     const int b1 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x + 1] : 0;
-    int s = (int)(pipe.it_f % (unsigned int)S);
-    unsigned int ph = (pipe.it_f / (unsigned int)S) & 1u;
-    double Gacc = 0.0;
+    const int nb = b1 - b0;
+    double Gacc[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) Gacc[r] = 0.0;
     const unsigned long long t_start = global_ns();
     const uint32_t full_a = smem_u32(&h->full_f[0]), empty_a = smem_u32(&h->empty_f[0]), stages_a = smem_u32(stages);
 
@@ -284,11 +381,12 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
         // ---------------- producer warp: lane 0 drives the TMA unit, one bulk copy per block record; the
         // descriptors of the next 32 blocks are requested before the current 32 are issued
         const uint64_t pol = policy_evict_first();   // streamed once per pass: keep it from pushing r / x out of L2
-        int2 next = (b0 + lane < b1) ? __ldg(P.blk + b0 + lane) : make_int2(0, 0);
-        for (int bb = b0; bb < b1; bb += 32) {
+        unsigned int s = pipe.it_f % S, ph = (pipe.it_f / S) & 1u;
+        int2 next = (lane < nb) ? __ldg(P.blk + b0 + lane) : make_int2(0, 0);
+        for (int bb = 0; bb < nb; bb += 32) {
             const int2 mine = next;
-            next = (bb + 32 + lane < b1) ? __ldg(P.blk + bb + 32 + lane) : make_int2(0, 0);
-            const int nb_here = min(32, b1 - bb);
+            next = (bb + 32 + lane < nb) ? __ldg(P.blk + b0 + bb + 32 + lane) : make_int2(0, 0);
+            const int nb_here = min(32, nb - bb);
             for (int j = 0; j < nb_here; ++j) {
                 const int off128 = __shfl_sync(0xffffffffu, mine.x, j);
                 const int bytes = __shfl_sync(0xffffffffu, mine.y, j);
@@ -296,49 +394,57 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
                     mbar_wait_a(empty_a + 8u * s, ph ^ 1u);
                     const uint32_t bar = full_a + 8u * s;
                     mbar_expect_tx_a(bar, (uint32_t)bytes);
-                    bulk_g2s_a(stages_a + (uint32_t)s * SB, P.pack + (size_t)(unsigned int)off128 * 128u, (uint32_t)bytes, bar, pol);
+                    bulk_g2s_a(stages_a + s * SB, P.pack + (size_t)(unsigned int)off128 * 128u, (uint32_t)bytes, bar, pol);
                 }
                 if (++s == S) { s = 0; ph ^= 1u; }
             }
         }
     } else {
-        // ---------------- consumer warps
-        const unsigned char* st_p = stages + (size_t)s * SB;
-        const unsigned char* st_end = stages + (size_t)S * SB;
-        uint32_t fb = full_a + 8u * s, eb = empty_a + 8u * s;
-        for (int b = b0; b < b1; ++b) {
-            mbar_wait_a(fb, ph);
+        // ---------------- consumer warps: warp w takes the CTA's blocks w, w + 16, ...
+        float* dsc = reinterpret_cast<float*>(smem + P.dsc_off) + warp * 32 * R_MAX;
+        const unsigned char* xs_b = reinterpret_cast<const unsigned char*>(xs);
+        for (int i = warp; i < nb; i += W_CONS) {
+            const unsigned int it = pipe.it_f + (unsigned int)i;
+            const unsigned int s = it % S, ph = (it / S) & 1u;
+            mbar_wait_a(full_a + 8u * s, ph);
 #ifndef IMRT_EXP_SKIP_COMPUTE
-            dose_block<COL16>(st_p, x_s, table_s, r_out, d_out, warp, lane, Gacc);
+            dose_block<COL16, R>(stages + (size_t)s * SB, xs_b, table_s, dsc, r_out, d_out, lane, Gacc);
 #endif
             __syncwarp();
-            if (lane == 0) mbar_arrive_a(eb);
-            st_p += SB; fb += 8u; eb += 8u;
-            if (st_p == st_end) { st_p = stages; fb = full_a; eb = empty_a; ph ^= 1u; }
+            if (lane == 0) mbar_arrive_a(empty_a + 8u * s);
         }
     }
-    pipe.it_f += (unsigned int)(b1 - b0);
-    const double Gcta = block_sum(Gacc, h);   // producer lanes contribute 0
+    pipe.it_f += (unsigned int)nb;
+    block_sum_vec<R>(Gacc, h);   // producer lanes contribute 0
     if (threadIdx.x == 0 && blockIdx.x < P.grid_f) {
-        Gpart[blockIdx.x] = Gcta;
+#pragma unroll
+        for (int r = 0; r < R; ++r) Gpart[blockIdx.x * R + r] = Gacc[r];
         P.cta_ns[2 * blockIdx.x] = t_start;            // when this CTA's share of the pass began and ended: lets the
         P.cta_ns[2 * blockIdx.x + 1] = global_ns();    // host see (and rebalance) the static partition
     }
     __syncthreads();
 }
 
+template <int R>
 __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
-                                          const float* x_s, float* r_out, float* d_out, double* Gpart, Pipe& pipe) {
-    if (P.col16) dose_pass_t<true>(P, h, smem, table_s, x_s, r_out, d_out, Gpart, pipe);
-    else dose_pass_t<false>(P, h, smem, table_s, x_s, r_out, d_out, Gpart, pipe);
+                                          const float* xs, float* const (&r_out)[R], float* d_out, double* Gpart, Pipe& pipe) {
+    if (P.col16) dose_pass_t<true, R>(P, h, smem, table_s, xs, r_out, d_out, Gpart, pipe);
+    else dose_pass_t<false, R>(P, h, smem, table_s, xs, r_out, d_out, Gpart, pipe);
 }
 
-// Objective of a finished dose pass: fixed-order sum of the CTA partials + the constant of the skipped rows.
-// Every thread of the calling CTA gets the value.
-__device__ __forceinline__ double reduce_objective(const DevPlan& P, const double* Gpart, SmemHeader* h) {
-    double v = 0.0;
-    for (int c = threadIdx.x; c < P.grid_f; c += NTHREADS) v += __ldcg(Gpart + c);
-    return block_sum(v, h) + P.G_skip;
+// Objectives of a finished dose pass: fixed-order sums of the CTA partials + the constant of the skipped rows.
+// Every thread of the calling CTA gets the values.
+template <int R>
+__device__ __forceinline__ void reduce_objective(const DevPlan& P, const double* Gpart, SmemHeader* h, double (&G)[R]) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) G[r] = 0.0;
+    for (int c = threadIdx.x; c < P.grid_f; c += NTHREADS) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) G[r] += __ldcg(Gpart + c * R + r);
+    }
+    block_sum_vec<R>(G, h);
+#pragma unroll
+    for (int r = 0; r < R; ++r) G[r] += P.G_skip;
 }
 
 // ------------------------------------------------------------------------------------------------ transpose pass
@@ -467,64 +573,73 @@ __device__ __forceinline__ void reduce_gradient(const DevPlan& P, const double* 
 
 // ------------------------------------------------------------------------------------------------ scalar logic
 struct Loop {                  // the loop's scalar state, replicated in registers by the persistent kernel
-    double G_k, lambda, step_sq;
+    double G_k, lambda;
     int iter, m, stop_reason, xi, ri;
     long long fwd, tr;
 };
 
-// After a transpose pass of the loop: start the line search (PAPER.md:109 step 2).  Returns true if a trial is pending.
-// Called by all threads with identical arguments; x, g, x_trial may be shared or global.
-__device__ __forceinline__ bool begin_line_search(const State* st, Loop& L, const float* x, const float* g, float* x_trial,
-                                                  int n_b, SmemHeader* h) {
+// After a transpose pass of the loop: start the line search (PAPER.md:109 step 2).  Returns true if trials are pending.
+// Called by all threads with identical arguments; x is global, g may be shared or global.
+__device__ __forceinline__ bool begin_line_search(const State* st, Loop& L, const float* x, const float* g, int n_b, SmemHeader* h) {
     L.tr += 1;
     if (L.G_k == 0.0) { L.stop_reason = STOP_STATIONARY; return false; }   // reading R4
     L.lambda = st->lambda0;
     L.m = 0;
-    L.step_sq = compute_trial(x, g, L.lambda, x_trial, n_b, h);
-    if (L.step_sq == 0.0) { L.stop_reason = STOP_STATIONARY; return false; }   // reading R4
+    if (first_step_sq(x, g, L.lambda, n_b, h) == 0.0) { L.stop_reason = STOP_STATIONARY; return false; }   // reading R4
     return true;
 }
 
 enum { DEC_ACCEPT_CONTINUE = 0, DEC_ACCEPT_STOP = 1, DEC_REJECT_RETRY = 2, DEC_REJECT_STOP = 3 };
 
-// After a dose pass of the loop: Armijo test (PAPER.md:110 step 3, Eq. (5)), step 4 or step 5.  Scalar work only; the
-// caller recomputes the trial point on DEC_REJECT_RETRY.  write_trace: only one CTA records.
-__device__ __forceinline__ int armijo_decide(const DevPlan& P, const State* st, Loop& L, double G_new, bool write_trace) {
+// After a dose pass of the loop that evaluated the R trial points lambda, lambda/alpha, ...: steps 3-5 of PAPER.md:110-112
+// applied to them IN ORDER, exactly as the one-trial-at-a-time loop would: Armijo test (Eq. (5)) on trial j; the first
+// trial that passes is accepted (j_acc) and the later ones are ignored; each failure is one step 4.  Scalar work only.
+// write_trace: only one CTA records.
+template <int R>
+__device__ __forceinline__ int armijo_decide(const DevPlan& P, const State* st, Loop& L, const double (&G_new)[R],
+                                             const double (&step_sq)[R], bool write_trace, int& j_acc) {
     L.fwd += 1;
-    const double C = L.G_k - (st->eps / L.lambda) * L.step_sq;   // Eq. (5)
-    if (G_new < C) {                                              // step 3, strict as printed
-        const int k = L.iter;
-        if (write_trace) {
-            P.tr_obj[k + 1] = G_new;
-            P.tr_lambda[k] = L.lambda;
-            P.tr_step_sq[k] = L.step_sq;
-            P.tr_trials[k] = L.m + 1;
+    j_acc = -1;
+    double lam = L.lambda;
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+        const double C = L.G_k - (st->eps / lam) * step_sq[j];       // Eq. (5)
+        if (G_new[j] < C) {                                           // step 3, strict as printed
+            const int k = L.iter;
+            if (write_trace) {
+                P.tr_obj[k + 1] = G_new[j];
+                P.tr_lambda[k] = lam;
+                P.tr_step_sq[k] = step_sq[j];
+                P.tr_trials[k] = L.m + 1;
+            }
+            const double G_old = L.G_k;
+            L.G_k = G_new[j];
+            L.iter = k + 1;
+            L.xi ^= 1;
+            L.ri = (L.ri + 1 + j) % (R + 1);
+            j_acc = j;
+            if (st->delta_tol > 0.0 && (G_new[j] == 0.0 || fabs(G_new[j] - G_old) / G_new[j] < st->delta_tol)) {   // step 5
+                L.stop_reason = STOP_TOLERANCE;
+                return DEC_ACCEPT_STOP;
+            }
+            if (L.iter >= st->iter_target) { L.stop_reason = STOP_MAX_ITERS; return DEC_ACCEPT_STOP; }
+            return DEC_ACCEPT_CONTINUE;
         }
-        const double G_old = L.G_k;
-        L.G_k = G_new;
-        L.iter = k + 1;
-        L.xi ^= 1;
-        L.ri ^= 1;
-        if (st->delta_tol > 0.0 && (G_new == 0.0 || fabs(G_new - G_old) / G_new < st->delta_tol)) {   // step 5
-            L.stop_reason = STOP_TOLERANCE;
-            return DEC_ACCEPT_STOP;
-        }
-        if (L.iter >= st->iter_target) { L.stop_reason = STOP_MAX_ITERS; return DEC_ACCEPT_STOP; }
-        return DEC_ACCEPT_CONTINUE;
+        L.m += 1;                                                     // step 4
+        if (L.m > st->max_ls) { L.stop_reason = STOP_LS_STALLED; return DEC_REJECT_STOP; }
+        lam = lam / st->alpha;
     }
-    L.m += 1;                                                     // step 4
-    if (L.m > st->max_ls) { L.stop_reason = STOP_LS_STALLED; return DEC_REJECT_STOP; }
-    L.lambda = L.lambda / st->alpha;
+    L.lambda = lam;            // first step size of the next batch
     return DEC_REJECT_RETRY;
 }
 
 __device__ __forceinline__ void loop_load(const State* st, Loop& L) {
-    L.G_k = st->G_k; L.lambda = st->lambda; L.step_sq = st->step_sq;
+    L.G_k = st->G_k; L.lambda = st->lambda;
     L.iter = st->iter; L.m = st->m; L.stop_reason = st->stop_reason; L.xi = st->xi; L.ri = st->ri;
     L.fwd = st->fwd_passes; L.tr = st->tr_passes;
 }
 __device__ __forceinline__ void loop_store(State* st, const Loop& L) {
-    st->G_k = L.G_k; st->lambda = L.lambda; st->step_sq = L.step_sq;
+    st->G_k = L.G_k; st->lambda = L.lambda;
     st->iter = L.iter; st->m = L.m; st->stop_reason = L.stop_reason; st->xi = L.xi; st->ri = L.ri;
     st->fwd_passes = L.fwd; st->tr_passes = L.tr;
 }
@@ -543,45 +658,64 @@ __device__ __forceinline__ bool cta_is_last(unsigned int* ticket, SmemHeader* h)
     return h->flag != 0;
 }
 
+// x_{k+1} = trial point j of the batch: copy it from the gather array to global memory.
+template <int R>
+__device__ __forceinline__ void publish_x(const float* xs, int j, float* x_out, int n_b) {
+    for (int i = threadIdx.x; i < n_b; i += NTHREADS) x_out[i] = xs[(size_t)xperm(i) * R + j];
+}
+
 // ------------------------------------------------------------------------------------------------ kernels
 extern __shared__ __align__(128) unsigned char imrt_smem[];
 
-// Dose pass as a kernel of its own (graph / host drivers, set_x, eval, get_dose).
-__global__ void __launch_bounds__(NTHREADS, 1) k_dose(const __grid_constant__ DevPlan P, const PassArgs A) {
-    SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
-    float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
-    float* x_s = reinterpret_cast<float*>(imrt_smem + P.x_off);
+// A single-point dose pass (MODE_EVAL: eval / get_dose / timing; MODE_INIT: G(x_1), r(x_1)).  Uses the R = 1 path.
+__device__ __forceinline__ void dose_single(const DevPlan& P, const PassArgs& A, SmemHeader* h, const float4* table_s, float* xs) {
     State* st = P.st;
-    cta_init(h, P, table_s);
     const int xi = st->xi, ri = st->ri;
-    const float* x_in = A.x_in ? A.x_in : (A.mode == MODE_EVAL ? P.xbuf[xi] : P.xbuf[xi ^ 1]);
-    float* r_out = A.r_out ? A.r_out : P.rbuf[ri ^ 1];
-    for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) x_s[i] = x_in[i];
-    __syncthreads();
+    const int r_next = (ri + 1) % (P.R + 1);
+    const float* x_in = A.x_in ? A.x_in : P.xbuf[xi];
+    float* const r_out[1] = {A.mode == MODE_EVAL ? A.r_out : P.rbuf[r_next]};
+    stage_point(x_in, xs, P.n_b);
     Pipe pipe = {0u, 0u};
     const int par = (int)(st->fwd_passes & 1);
-    dose_pass(P, h, imrt_smem, table_s, x_s, r_out, A.d_out, P.Gpart[par], pipe);
+    dose_pass<1>(P, h, imrt_smem, table_s, xs, r_out, A.mode == MODE_EVAL ? A.d_out : nullptr, P.Gpart[par], pipe);
+    __threadfence();
+    if (!cta_is_last(&st->ticket_f, h)) return;
+    double G[1];
+    reduce_objective<1>(P, P.Gpart[par], h, G);
+    if (threadIdx.x != 0) return;
+    if (A.mode == MODE_EVAL) {
+        st->eval_obj = G[0];            // not counted: fwd_passes / tr_passes count the loop's passes
+    } else {
+        st->G_k = G[0]; st->fwd_passes += 1; st->ri = r_next;   // xbuf[xi] already holds x_1
+        P.tr_obj[0] = G[0];
+    }
+}
+
+// One batch of R line-search trials (graph / host drivers): every CTA builds the trial points itself.
+template <int R>
+__device__ __forceinline__ void dose_trials(const DevPlan& P, const PassArgs& A, SmemHeader* h, const float4* table_s, float* xs) {
+    State* st = P.st;
+    const int xi = st->xi, ri = st->ri;
+    double step_sq[R];
+    trial_batch<R>(P.xbuf[xi], P.g, st->lambda, st->alpha, xs, P.n_b, h, step_sq);
+    __syncthreads();
+    float* r_out[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) r_out[j] = P.rbuf[(ri + 1 + j) % (R + 1)];
+    Pipe pipe = {0u, 0u};
+    const int par = (int)(st->fwd_passes & 1);
+    dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[par], pipe);
     __threadfence();
     if (!cta_is_last(&st->ticket_f, h)) return;
 
     // ---- the last CTA to finish takes the decision
-    const double G_new = reduce_objective(P, P.Gpart[par], h);
-    if (A.mode == MODE_EVAL) {
-        if (threadIdx.x == 0) st->eval_obj = G_new;   // not counted: fwd_passes / tr_passes count the loop's passes
-        return;
-    }
-    if (A.mode == MODE_INIT) {
-        if (threadIdx.x == 0) {
-            st->G_k = G_new; st->fwd_passes += 1; st->ri = ri ^ 1; st->xi = xi ^ 1;
-            P.tr_obj[0] = G_new;
-        }
-        return;
-    }
+    double G_new[R];
+    reduce_objective<R>(P, P.Gpart[par], h, G_new);
     Loop L;
     loop_load(st, L);
-    const int dec = armijo_decide(P, st, L, G_new, threadIdx.x == 0);
-    if (dec == DEC_REJECT_RETRY)   // x_k is xbuf[xi], the next trial goes to xbuf[xi^1]
-        L.step_sq = compute_trial(P.xbuf[xi], P.g, L.lambda, P.xbuf[xi ^ 1], P.n_b, h);
+    int j_acc;
+    const int dec = armijo_decide<R>(P, st, L, G_new, step_sq, threadIdx.x == 0, j_acc);
+    if (j_acc >= 0) publish_x<R>(xs, j_acc, P.xbuf[xi ^ 1], P.n_b);
     if (threadIdx.x == 0) {
         loop_store(st, L);
         const int inner = (dec == DEC_REJECT_RETRY);
@@ -593,6 +727,42 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dose(const __grid_constant__ De
             cudaGraphSetConditional(A.h_outer, outer);
         }
     }
+}
+
+// The loop's R-point dose pass on R copies of the current iterate, residuals to the trial buffers, no decision and no
+// state change: what plan creation times to balance the partition and what imrt_plan_launch_pass launches.
+template <int R>
+__device__ __forceinline__ void dose_timing(const DevPlan& P, SmemHeader* h, const float4* table_s, float* xs) {
+    State* st = P.st;
+    const float* x = P.xbuf[st->xi];
+    const int ri = st->ri;
+    for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) {
+        const float v = x[i];
+#pragma unroll
+        for (int r = 0; r < R; ++r) xs[(size_t)xperm(i) * R + r] = v;
+    }
+    __syncthreads();
+    float* r_out[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) r_out[j] = P.rbuf[(ri + 1 + j) % (R + 1)];
+    Pipe pipe = {0u, 0u};
+    dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[(int)(st->fwd_passes & 1)], pipe);
+}
+
+// Dose pass as a kernel of its own (graph / host drivers, set_x, eval, get_dose).
+__global__ void __launch_bounds__(NTHREADS, 1) k_dose(const __grid_constant__ DevPlan P, const PassArgs A) {
+    SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
+    float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
+    float* xs = reinterpret_cast<float*>(imrt_smem + P.x_off);
+    cta_init(h, P, table_s);
+    if (A.mode == MODE_TIMING) {
+        if (P.R == 4) dose_timing<4>(P, h, table_s, xs);
+        else if (P.R == 2) dose_timing<2>(P, h, table_s, xs);
+        else dose_timing<1>(P, h, table_s, xs);
+    } else if (A.mode != MODE_TRIAL) dose_single(P, A, h, table_s, xs);
+    else if (P.R == 4) dose_trials<4>(P, A, h, table_s, xs);
+    else if (P.R == 2) dose_trials<2>(P, A, h, table_s, xs);
+    else dose_trials<1>(P, A, h, table_s, xs);
 }
 
 // Transpose pass as a kernel of its own.
@@ -617,7 +787,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_transpose(const __grid_constant
     __syncthreads();
     Loop L;
     loop_load(st, L);
-    const bool pending = begin_line_search(st, L, P.xbuf[xi], P.g, P.xbuf[xi ^ 1], P.n_b, h);
+    const bool pending = begin_line_search(st, L, P.xbuf[xi], P.g, P.n_b, h);
     if (threadIdx.x == 0) {
         loop_store(st, L);
         st->cont_inner = pending;
@@ -648,19 +818,22 @@ __global__ void k_set_target(State* st, int n_more, double delta_tol) {
 }
 
 // The whole loop in one cooperative launch (driver 2): PAPER.md:99-114 with no host involvement at all.
-// Every CTA keeps x_k, g and x+ in shared memory and replays the same scalar decisions from the same fixed-order
-// reductions, so CTAs never exchange anything but the pass partials; CTA 0 records the trace.
-__global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constant__ DevPlan P) {
+// Every CTA keeps g and the trial points in shared memory and replays the same scalar decisions from the same
+// fixed-order reductions, so CTAs never exchange anything but the pass partials; CTA 0 records the trace and
+// publishes the accepted iterate.
+template <int R>
+__device__ __forceinline__ void persistent_loop(const DevPlan& P) {
     SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
     float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
     double* wpart = reinterpret_cast<double*>(imrt_smem + P.wpart_off);
-    float* xb = reinterpret_cast<float*>(imrt_smem + P.x_off);     // x+ (the dose pass gathers from it)
+    float* xs = reinterpret_cast<float*>(imrt_smem + P.x_off);     // the R trial points (the dose pass gathers from them)
     float* g_s = reinterpret_cast<float*>(imrt_smem + P.g_off);
     State* st = P.st;
     cta_init(h, P, table_s);
     Loop L;
     loop_load(st, L);
     const int iter_target = st->iter_target;
+    const double alpha = st->alpha;
     L.stop_reason = STOP_MAX_ITERS;
     Pipe pipe = {0u, 0u};
     unsigned int epoch = 0;
@@ -672,22 +845,26 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constan
         grid_barrier(&st->gridbar, epoch);
         reduce_gradient(P, P.gslot[tpar], g_s);
         __syncthreads();
-        if (!begin_line_search(st, L, P.xbuf[L.xi], g_s, xb, P.n_b, h)) break;   // x_k lives in global memory
-        int dec;
+        if (!begin_line_search(st, L, P.xbuf[L.xi], g_s, P.n_b, h)) break;   // x_k lives in global memory
+        int dec, j_acc;
         for (;;) {
+            double step_sq[R], G_new[R];
+            trial_batch<R>(P.xbuf[L.xi], g_s, L.lambda, alpha, xs, P.n_b, h, step_sq);
+            __syncthreads();
+            float* r_out[R];
+#pragma unroll
+            for (int j = 0; j < R; ++j) r_out[j] = P.rbuf[(L.ri + 1 + j) % (R + 1)];
             const int fpar = (int)(L.fwd & 1);
-            dose_pass(P, h, imrt_smem, table_s, xb, P.rbuf[L.ri ^ 1], nullptr, P.Gpart[fpar], pipe);
+            dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[fpar], pipe);
             grid_barrier(&st->gridbar, epoch);
-            const double G_new = reduce_objective(P, P.Gpart[fpar], h);
-            dec = armijo_decide(P, st, L, G_new, rec);
+            reduce_objective<R>(P, P.Gpart[fpar], h, G_new);
+            dec = armijo_decide<R>(P, st, L, G_new, step_sq, rec, j_acc);
             if (dec != DEC_REJECT_RETRY) break;
-            L.step_sq = compute_trial(P.xbuf[L.xi], g_s, L.lambda, xb, P.n_b, h);
         }
-        if ((dec == DEC_ACCEPT_CONTINUE || dec == DEC_ACCEPT_STOP) && blockIdx.x == 0) {
-            // x_{k+1} = x+: publish it (L.xi already points at the new buffer); the other CTAs read it only after the
+        if (j_acc >= 0 && blockIdx.x == 0) {
+            // x_{k+1}: publish it (L.xi already points at the new buffer); the other CTAs read it only after the
             // next grid barrier
-            float* xg = P.xbuf[L.xi];
-            for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) xg[i] = xb[i];
+            publish_x<R>(xs, j_acc, P.xbuf[L.xi], P.n_b);
         }
         if (dec != DEC_ACCEPT_CONTINUE) break;
     }
@@ -701,6 +878,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constan
             st->cont_inner = 0;
         }
     }
+}
+
+__global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constant__ DevPlan P) {
+    if (P.R == 4) persistent_loop<4>(P);
+    else if (P.R == 2) persistent_loop<2>(P);
+    else persistent_loop<1>(P);
 }
 
 }  // namespace imrt

@@ -128,8 +128,8 @@ def test_eval_all_rows_empty_and_leading_trailing_empty(m):
 
 
 # ---------------------------------------------------------------------------------------------- the loop
-def run_gpu(m, prob, n_iters, driver, delta=0.0):
-    plan = m.Plan(prob, max_iters=max(n_iters, 1), driver=driver)
+def run_gpu(m, prob, n_iters, driver, delta=0.0, ls_batch=0):
+    plan = m.Plan(prob, max_iters=max(n_iters, 1), driver=driver, ls_batch=ls_batch)
     plan.set_x(prob.x0)
     if delta > 0:
         plan.run_to_tol(delta, n_iters)
@@ -160,6 +160,31 @@ def test_three_drivers_are_bit_identical(m):
         r[0].close()
 
 
+@pytest.mark.parametrize("cfg,n", [(0, 50), (2, 40)])
+def test_batched_line_search_is_bit_identical_to_sequential(m, cfg, n, monkeypatch):
+    # Plans are compared with each other, so they must share one CTA partition: the measured rebalancing of plan
+    # creation (timing dependent; it changes the order in which objective partials are summed) is switched off.
+    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")
+    # imrt_params.ls_batch: 1 = one trial point per pass over D (steps 2-4 of PAPER.md:109-111 literally), 2 / 4 = the
+    # next 2 / 4 trial points in one pass.  Same iterates, objectives, step sizes and trial counts, bit for bit.
+    prob = phantom(cfg)
+    res = {R: run_gpu(m, prob, n, m.DRIVER_PERSISTENT, ls_batch=R) for R in (1, 2, 4)}
+    _, tr1, x1, d1, (fwd1, trp1) = res[1]
+    assert tr1.n_iters == n and fwd1 == 1 + tr1.n_trials.sum() and tr1.n_trials.max() > 1
+    for R in (2, 4):
+        plan, tr, x, d, (fwd, trp) = res[R]
+        assert plan.info()["ls_batch"] == R
+        np.testing.assert_array_equal(tr.obj, tr1.obj)
+        np.testing.assert_array_equal(tr.n_trials, tr1.n_trials)
+        np.testing.assert_array_equal(tr.lam, tr1.lam)
+        np.testing.assert_array_equal(tr.step_sq, tr1.step_sq)
+        np.testing.assert_array_equal(x, x1)
+        np.testing.assert_array_equal(d, d1)
+        assert trp == trp1 and fwd == 1 + np.ceil(tr.n_trials / R).sum()
+    for r in res.values():
+        r[0].close()
+
+
 def test_runs_are_reproducible_and_resumable(m):
     prob = phantom(0)
     p1, tr1, x1, _, _ = run_gpu(m, prob, 20, m.DRIVER_PERSISTENT)
@@ -182,7 +207,8 @@ def test_trajectory_parity_follow_mode(m, cfg, driver):
     n = prob.n_iters
     plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, n, driver)
     assert tr.n_iters == n and tr.stop_reason == oracle.STOP_MAX_ITERS
-    assert fwd == 1 + tr.n_trials.sum() and trp == n
+    R = plan.info()["ls_batch"]     # one dose pass evaluates up to R trial points
+    assert fwd == 1 + np.ceil(tr.n_trials / R).sum() and trp == n
     assert (np.diff(tr.obj) < 0).all() and (x >= 0).all()
     fol = oracle.run(prob, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert fol.n_follow_violations == 0, "GPU accepted/rejected a trial the oracle would not (first at iteration %d)" % fol.first_violation
@@ -225,11 +251,12 @@ def test_identity_two_trials_then_stationary(m):
                                 np.ones(3, np.float32), np.array([0, 1, 2], np.uint8), T, T, np.ones(3, np.float32),
                                 np.ones(3, np.float32), np.array([12.0, 16.0, 30.0], np.float32), eps=0.2, alpha=2.0, lambda0=1.0)
     for drv in (0, 1, 2):
-        plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, 5, drv)
-        assert tr.n_iters == 1 and tr.stop_reason == oracle.STOP_STATIONARY
-        assert list(tr.obj) == [20.0, 0.0] and list(tr.n_trials) == [2] and list(tr.lam) == [0.5] and list(tr.step_sq) == [20.0]
-        assert list(x) == [10.0, 20.0, 30.0] and fwd == 3 and trp == 2
-        plan.close()
+        for R in (1, 2, 4):
+            plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, 5, drv, ls_batch=R)
+            assert tr.n_iters == 1 and tr.stop_reason == oracle.STOP_STATIONARY
+            assert list(tr.obj) == [20.0, 0.0] and list(tr.n_trials) == [2] and list(tr.lam) == [0.5] and list(tr.step_sq) == [20.0]
+            assert list(x) == [10.0, 20.0, 30.0] and fwd == (3 if R == 1 else 2) and trp == 2
+            plan.close()
 
 
 def test_linesearch_stall_and_bad_inputs(m):
@@ -238,9 +265,12 @@ def test_linesearch_stall_and_bad_inputs(m):
     prob = synth_inputs.Problem("stall", 2, 2, np.array([0, 1, 2], np.int32), np.array([0, 1], np.int32), np.ones(2, np.float32),
                                 np.zeros(2, np.uint8), T, T, np.ones(1, np.float32), np.ones(1, np.float32),
                                 np.array([1.0, 9.0], np.float32), lambda0=1024.0, max_ls=2)
-    plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, 3, m.DRIVER_PERSISTENT)
-    assert tr.n_iters == 0 and tr.stop_reason == oracle.STOP_LS_STALLED and fwd == 1 + 3
-    np.testing.assert_array_equal(x, prob.x0)
+    for R in (1, 2, 4):
+        plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, 3, m.DRIVER_PERSISTENT, ls_batch=R)
+        assert tr.n_iters == 0 and tr.stop_reason == oracle.STOP_LS_STALLED and fwd == 1 + {1: 3, 2: 2, 4: 1}[R]
+        np.testing.assert_array_equal(x, prob.x0)
+        if R < 4:
+            plan.close()
     with pytest.raises(m.ImrtError) as e:
         plan.set_x(np.array([1.0, -1.0], np.float32))
     assert e.value.status_name == "BAD_X"
@@ -266,3 +296,39 @@ def test_linesearch_stall_and_bad_inputs(m):
         m.Plan(bad)
     assert e.value.status_name == "BAD_CSR"
     assert torch.cuda.is_available()
+
+
+# ---------------------------------------------------------------------------------------------- full size (bench configuration)
+# BASELINE.json configs[3] (headline) and configs[4] (stress), in the launch configuration bench.py times (persistent
+# driver, one CTA per SM, tuned partition).  The oracle's eval / gradient take well under a second per call even at
+# these sizes, so every output element is compared, not a sample.
+@pytest.mark.parametrize("cfg,n_iters", [(3, 30), (4, 10)])
+def test_full_size_parity(m, cfg, n_iters):
+    prob = phantom(cfg)
+    plan = m.Plan(prob, max_iters=n_iters, driver=m.DRIVER_PERSISTENT)
+    info = plan.info()
+    assert info["fwd_grid"] == info["n_sm"] and info["tr_grid"] == info["n_sm"]   # what bench.py launches
+    check_eval(m, plan, prob, prob.x0)
+    xo = oracle.run(prob, n_iters=3).x.astype(np.float32)
+    check_eval(m, plan, prob, xo)
+    # trajectory: n_iters accepted iterations from x0, oracle in follow mode
+    plan.set_x(prob.x0)
+    plan.run_iters(n_iters)
+    tr = plan.trace()
+    assert tr.n_iters == n_iters and tr.stop_reason == oracle.STOP_MAX_ITERS
+    assert (np.diff(tr.obj) < 0).all()
+    fol = oracle.run(prob, n_iters=n_iters, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert fol.n_follow_violations == 0, "first violation at iteration %d" % fol.first_violation
+    np.testing.assert_array_equal(tr.lam, fol.lam)
+    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    assert abs(tr.obj[-1] - fol.obj[-1]) <= TOL_G_FINAL * fol.obj[-1]
+    x = plan.get_x().cpu().numpy()
+    assert (x >= 0).all()
+    d = plan.get_dose().cpu().numpy()
+    d_o, _, _ = oracle.eval_objective(prob, fol.x)
+    dp_o, mean_o = oracle.dvh_points(prob.sid, d_o, prob.n_structures)
+    dp_g, mean_g = plan.dvh(oracle.DVH_PCTS)
+    assert np.nanmax(np.abs(dp_g - dp_o)) <= TOL_DVH_GY and np.nanmax(np.abs(mean_g - mean_o)) <= TOL_DVH_GY
+    assert relerr(d, d_o) <= 1e-4   # dose of the two final plans (same trial counts, fp32 vs fp64 trajectories)
+    plan.close()
+    _phantoms.pop(cfg, None)        # free ~1-3 GB of host memory
