@@ -180,7 +180,8 @@ imrt_status imrt_plan_get_counters(imrt_plan* plan, int64_t* host_fwd_passes, in
  *   host_info[0] nnz of D^T        [1] forward row blocks     [2] forward grid (CTAs)   [3] transpose grid (CTAs)
  *   host_info[4] dynamic shared memory bytes per CTA   [5] bytes of the re-packed D the dose pass streams
  *   host_info[6] gradient partial slots   [7] non-empty rows of D   [8] SM count   [9] 16-bit column indices (1/0)
- *   host_info[10] trial points per dose pass actually used (ls_batch)   [11] dose-pass stages   [12] transpose stages
+ *   host_info[10] trial points per dose pass actually used (ls_batch)   [11] dose-pass ring bytes   [12] transpose stages
+ *   host_info[13] rows of D stored in quad format (4 neighbouring rows sharing one column list)
  * d_rowT_ptr (int32 [n_b+1]), d_colT (int32 [nnz]), d_valT (fp32 [nnz]): if non-NULL receive a copy of D^T (device).
  */
 imrt_status imrt_plan_get_info(imrt_plan* plan, int64_t* host_info, int32_t n_info,

@@ -209,7 +209,7 @@ def imrt_plan_get_counters(plan):
 
 
 INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "smem_bytes", "pack_bytes", "g_slots", "nonempty_rows", "n_sm", "col16",
-             "ls_batch", "fwd_stages", "tr_stages")
+             "ls_batch", "fwd_ring_bytes", "tr_stages", "quad_rows")
 
 
 def imrt_plan_get_info(plan, rowT_ptr=None, colT=None, valT=None) -> dict:

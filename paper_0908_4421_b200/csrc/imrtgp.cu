@@ -30,9 +30,10 @@ struct imrt_plan {
     size_t smem_bytes;
     int grid_p;                       // persistent kernel grid
     bool has_x;
-    int64_t n_blk, n_nonempty, n_skipped, pack_bytes;
+    int64_t n_blk, n_nonempty, n_skipped, pack_bytes, n_quad_rows;
     std::vector<double> blk_cost;     // modelled, then measured, cost of every dose-pass block (host)
     int* cta_blk_w;
+    int4* blk_w;
     double tune_spread[2];            // slowest / mean CTA time of the dose pass before and after tuning
     // borrowed inputs
     const int32_t* row_ptr;
@@ -92,9 +93,9 @@ struct Bounds {
 Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     Bounds b;
     const int64_t slots = nnz + 3 * n_v;    // every row padded to a multiple of 4 slots
-    b.max_blk = 2 * (slots / MIN_CHUNK_SLOTS + 1) + 2 * (n_v / MAXROWS_F + 1) + n_v / 32 + 4;
-    b.max_meta = n_v + b.max_blk * (META_HDR + 1 + 3) + 8;
-    b.max_pack = (size_t)b.max_meta * 4 + ((size_t)slots + (size_t)ZPAD * b.max_blk) * 8 + (size_t)b.max_blk * 128 + 256;
+    b.max_blk = 4 * (slots / MIN_CHUNK_SLOTS + 1) + 4 * (n_v / SEG_ROWS + 1) + n_v / 16 + 8;
+    b.max_meta = n_v + b.max_blk * (META_HDR + 2 + 3) + 8;
+    b.max_pack = (size_t)b.max_meta * 4 + (size_t)slots * 8 + (size_t)b.max_blk * (128 + 48) + 256;
     b.max_ranges = 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
     b.max_slots = n_b + b.max_ranges + 4;
     b.nnz_pad = ((nnz + 3) & ~(int64_t)3) + 8;
@@ -105,7 +106,7 @@ Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
 struct Layout {
     State* st;
     float4* table;
-    int2* blk;
+    int4* blk;
     int4* pk;
     uint32_t* rowmeta;
     unsigned char* pack;
@@ -131,6 +132,7 @@ struct Layout {
     unsigned long long* cta_ns;
     DvhWork dvh;
     // build scratch
+    int* quadU;
     unsigned int* keysA;
     unsigned int* keysB;
     unsigned int* valsA;
@@ -145,7 +147,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     Layout L;
     L.st = w.take<State>(1);
     L.table = w.take<float4>(MAX_STRUCTURES);
-    L.blk = w.take<int2>(B.max_blk);
+    L.blk = w.take<int4>(B.max_blk);
     L.pk = w.take<int4>(B.max_blk);
     L.rowmeta = w.take<uint32_t>(B.max_meta);
     L.pack = w.take<unsigned char>(B.max_pack);
@@ -173,6 +175,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.dvh.cnt = w.take<unsigned int>((size_t)MAX_STRUCTURES);
     L.dvh.sum = w.take<double>((size_t)MAX_STRUCTURES);
     L.dvh.query = w.take<DvhQuery>((size_t)MAX_STRUCTURES * DVH_MAX_PCTS);
+    L.quadU = w.take<int>(n_v / 4 + 2);
     L.keysA = w.take<unsigned int>(nnz + 4);
     L.keysB = w.take<unsigned int>(nnz + 4);
     L.valsA = w.take<unsigned int>(nnz + 4);
@@ -228,35 +231,105 @@ __global__ void k_fill_transpose(const unsigned int* __restrict__ perm, const in
     }
 }
 
-// Re-pack D into the dose pass's block records: one CTA per block copies the header and row table, then one warp per
-// row copies values and columns (16- or 32-bit) to the row's 16-byte aligned slot range and zero-fills the padding.
+// Number of distinct columns in every quad (4 consecutive rows) of D: one warp per quad marks the columns in a
+// shared-memory bitmap.  Dynamic shared memory: warps x words x 4 bytes, words = ceil(n_b / 32).
+__global__ void k_quad_union(const int* __restrict__ row_ptr, const int* __restrict__ col, int n_v, int n_quads, int words, int* U) {
+    extern __shared__ uint32_t k_quad_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+    uint32_t* bm = k_quad_smem + (size_t)warp * words;
+    for (int q = blockIdx.x * nwarp + warp; q < n_quads; q += gridDim.x * nwarp) {
+        const int p0 = row_ptr[4 * q], p1 = row_ptr[min(4 * q + 4, n_v)];
+        if (p0 == p1) { if (lane == 0) U[q] = 0; continue; }
+        for (int w = lane; w < words; w += 32) bm[w] = 0u;
+        __syncwarp();
+        for (int p = p0 + lane; p < p1; p += 32) { const int c = col[p]; atomicOr(&bm[c >> 5], 1u << (c & 31)); }
+        __syncwarp();
+        int cnt = 0;
+        for (int w = lane; w < words; w += 32) cnt += __popc(bm[w]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        if (lane == 0) U[q] = cnt;
+        __syncwarp();
+    }
+}
+
+// Re-pack D into the dose pass's block records: one CTA per record copies the header and table, then
+//   row format:  one warp per row copies values and columns (16- or 32-bit) to the row's 16-byte aligned slot range
+//                and zero-fills the padding;
+//   quad format: one warp per quad marks its columns in a bitmap, ranks them (prefix popcount) and scatters every
+//                entry of the 4 rows to (rank of its column, row) -- explicit zeros where a row lacks a column.
+// Dynamic shared memory (quad format only): warps x 2 x words x 4 bytes.
 template <bool COL16>
 __global__ void k_pack_blocks(const int4* __restrict__ pk, const uint32_t* __restrict__ meta, const int* __restrict__ row_ptr,
-                              const int* __restrict__ col, const float* __restrict__ val, unsigned char* pack) {
+                              const int* __restrict__ col, const float* __restrict__ val, int n_v, int words, unsigned char* pack) {
+    extern __shared__ uint32_t k_pack_smem[];
     const int4 d = pk[blockIdx.x];
     const uint32_t* m = meta + d.x;
     unsigned char* rec = pack + (size_t)(unsigned int)d.z * 128u;
     uint32_t* rec_w = reinterpret_cast<uint32_t*>(rec);
     for (int i = threadIdx.x; i < d.y; i += blockDim.x) rec_w[i] = m[i];
-    const int nrows = (int)m[0], r0 = (int)m[1], slots = (int)m[3];
-    float* val_o = reinterpret_cast<float*>(rec + (size_t)d.y * 4);
-    unsigned char* col_o = reinterpret_cast<unsigned char*>(val_o + slots + ZPAD);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
-    for (int row = warp; row < nrows; row += nwarp) {
-        const int so = (int)(m[META_HDR + row] & 0xFFFFu), se = (int)(m[META_HDR + row + 1] & 0xFFFFu);
-        const int p0 = row_ptr[r0 + row], len = row_ptr[r0 + row + 1] - p0;
-        for (int k = lane; k < se - so; k += 32) {
-            const float v = k < len ? val[p0 + k] : 0.0f;
-            const int c = xperm(k < len ? col[p0 + k] : 0);   // position in the shared-memory gather array
-            val_o[so + k] = v;
-            if (COL16) reinterpret_cast<unsigned short*>(col_o)[so + k] = (unsigned short)c;
-            else reinterpret_cast<int*>(col_o)[so + k] = c;
+    if (d.w == 0) {
+        const int nrows = (int)m[0], r0 = (int)m[1], slots = (int)m[3];
+        float* val_o = reinterpret_cast<float*>(rec + (size_t)d.y * 4);
+        unsigned char* col_o = reinterpret_cast<unsigned char*>(val_o + slots + ZPAD);
+        for (int row = warp; row < nrows; row += nwarp) {
+            const int so = (int)(m[META_HDR + row] & 0xFFFFu), se = (int)(m[META_HDR + row + 1] & 0xFFFFu);
+            const int p0 = row_ptr[r0 + row], len = row_ptr[r0 + row + 1] - p0;
+            for (int k = lane; k < se - so; k += 32) {
+                const float v = k < len ? val[p0 + k] : 0.0f;
+                const int c = k < len ? col[p0 + k] : 0;
+                val_o[so + k] = v;
+                if (COL16) reinterpret_cast<unsigned short*>(col_o)[so + k] = (unsigned short)c;
+                else reinterpret_cast<int*>(col_o)[so + k] = c;
+            }
         }
-    }
-    if (threadIdx.x < ZPAD) {   // the zero slots lanes past a row's end read
-        val_o[slots + threadIdx.x] = 0.0f;
-        if (COL16) reinterpret_cast<unsigned short*>(col_o)[slots + threadIdx.x] = 0;
-        else reinterpret_cast<int*>(col_o)[slots + threadIdx.x] = 0;
+        if (threadIdx.x < ZPAD) {   // the zero slots lanes past a row's end read
+            val_o[slots + threadIdx.x] = 0.0f;
+            if (COL16) reinterpret_cast<unsigned short*>(col_o)[slots + threadIdx.x] = 0;
+            else reinterpret_cast<int*>(col_o)[slots + threadIdx.x] = 0;
+        }
+    } else {
+        const int nq = (int)m[0], r0 = (int)m[1], nbc = (int)m[3];
+        float* val_o = reinterpret_cast<float*>(rec + (size_t)d.y * 4);
+        unsigned short* col_o = reinterpret_cast<unsigned short*>(val_o + (size_t)(nbc + 1) * 4);
+        uint32_t* bm = k_pack_smem + (size_t)warp * 2 * words;
+        uint32_t* pre = bm + words;
+        for (int qi = warp; qi < nq; qi += nwarp) {
+            const int off = (int)(m[META_HDR + 2 * qi] & 0xFFFFu), off_n = (int)(m[META_HDR + 2 * qi + 2] & 0xFFFFu);
+            if (off_n == off) continue;
+            const int ra = r0 + 4 * qi, rb = min(ra + 4, n_v);
+            const int p0 = row_ptr[ra], p1 = row_ptr[rb];
+            for (int k = lane; k < (off_n - off) * 4; k += 32) val_o[(size_t)off * 4 + k] = 0.0f;
+            for (int k = lane; k < off_n - off; k += 32) col_o[off + k] = 0;
+            for (int w = lane; w < words; w += 32) bm[w] = 0u;
+            __syncwarp();
+            for (int p = p0 + lane; p < p1; p += 32) { const int c = col[p]; atomicOr(&bm[c >> 5], 1u << (c & 31)); }
+            __syncwarp();
+            int running = 0;
+            for (int base = 0; base < words; base += 32) {
+                const int w = base + lane;
+                const int cnt = w < words ? __popc(bm[w]) : 0;
+                int inc = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+                if (w < words) pre[w] = (uint32_t)(running + inc - cnt);
+                running += __shfl_sync(0xffffffffu, inc, 31);
+            }
+            __syncwarp();
+            for (int row = ra; row < rb; ++row) {
+                const int q0 = row_ptr[row], q1 = row_ptr[row + 1];
+                for (int p = q0 + lane; p < q1; p += 32) {
+                    const int c = col[p];
+                    const int pos = off + (int)pre[c >> 5] + __popc(bm[c >> 5] & ((1u << (c & 31)) - 1u));
+                    val_o[(size_t)pos * 4 + (row - ra)] = val[p];
+                    col_o[pos] = (unsigned short)c;
+                }
+            }
+            __syncwarp();
+        }
+        if (threadIdx.x < 4) val_o[(size_t)nbc * 4 + threadIdx.x] = 0.0f;   // the zero column
+        if (threadIdx.x < 8) col_o[nbc + threadIdx.x] = 0;
     }
 }
 
@@ -307,7 +380,7 @@ inline int grid_for(long long n, int block) {
 // Row-aligned blocks of D for the dose pass.  Each block becomes one self-contained record of the packed stream
 // (layout: kernels.cuh, DevPlan::pack); this lays the records out and writes their headers and row tables.
 struct BlockPlan {
-    std::vector<int2> blk;        // {record offset / 128, record bytes}                       -> device, dose pass
+    std::vector<int4> blk;        // {record offset / 128, record bytes, 0, 0}                 -> device, dose pass
     std::vector<int4> pk;         // {meta word offset, meta words, record offset / 128, 0}    -> device, pack kernel
     std::vector<uint32_t> meta;   // headers + row tables, block after block
     std::vector<int> rows, slots; // per block, for the cost model
@@ -315,12 +388,15 @@ struct BlockPlan {
     int max_rec_bytes = 0;
 };
 
+// quadU: distinct columns per quad (4 consecutive rows), or empty when the quad format is not on offer.
 imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::vector<uint8_t>& sid, const float4* table_h,
-                         int chunk_slots, int col_bytes, BlockPlan& B, double& G_skip, int64_t& n_skipped, int64_t& n_nonempty) {
+                         int chunk_slots, int col_bytes, const std::vector<int>& quadU, BlockPlan& B, double& G_skip,
+                         int64_t& n_skipped, int64_t& n_nonempty, int64_t& n_quad_rows) {
     const int n_v = (int)sid.size();
     G_skip = 0.0;
     n_skipped = 0;
     n_nonempty = 0;
+    n_quad_rows = 0;
     auto skip_row = [&](int j) {   // d = 0 on a row without entries: a constant of the objective
         const float4 t = table_h[sid[j]];
         const double u = std::max(0.0, (double)t.x), o = std::max(0.0, -(double)t.y);
@@ -328,53 +404,120 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         ++n_skipped;
     };
     auto pad4 = [](int n) { return (n + 3) & ~3; };
-    int j = 0;
+    auto pad8 = [](int n) { return (n + 7) & ~7; };
     size_t off = 0;
-    while (j < n_v) {
-        if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
-        const int r0 = j;
-        int slots = pad4(rp[j + 1] - rp[j]);
-        if (slots > chunk_slots)
-            return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
-                        rp[j + 1] - rp[j], chunk_slots);
-        int last = j, empties = 0, jj = j + 1, n_full = 1;
-        while (jj < n_v && jj - r0 < MAXROWS_F) {
-            const int len = rp[jj + 1] - rp[jj];
-            if (len == 0) {
-                if (++empties > 32) break;
-                ++jj;
-                continue;
-            }
-            if (slots + pad4(len) > chunk_slots) break;
-            slots += pad4(len);
-            empties = 0;
-            last = jj;
-            ++n_full;
-            ++jj;
-        }
-        const int r1 = last + 1, nrows = r1 - r0;
-        n_nonempty += n_full;
-        const int mo = (int)B.meta.size();
-        B.meta.push_back((uint32_t)nrows);
-        B.meta.push_back((uint32_t)r0);
-        B.meta.push_back(0u);
-        B.meta.push_back((uint32_t)slots);
-        int so = 0;
-        for (int row = r0; row < r1; ++row) {
-            B.meta.push_back((uint32_t)so | ((uint32_t)sid[row] << 16));
-            so += pad4(rp[row + 1] - rp[row]);
-        }
-        B.meta.push_back((uint32_t)so);
+    auto close_record = [&](int mo, int payload_bytes, int fmt, int rows, int slots) {
         while ((B.meta.size() - mo - META_HDR) & 3) B.meta.push_back(0u);
         const int mw = (int)B.meta.size() - mo;
-        const int rec = (mw * 4 + (slots + ZPAD) * (4 + col_bytes) + 127) & ~127;
-        B.blk.push_back(make_int2((int)(off / 128), rec));
-        B.pk.push_back(make_int4(mo, mw, (int)(off / 128), 0));
-        B.rows.push_back(nrows);
+        const int rec = (mw * 4 + payload_bytes + 127) & ~127;
+        B.blk.push_back(make_int4((int)(off / 128), rec, 0, 0));
+        B.pk.push_back(make_int4(mo, mw, (int)(off / 128), fmt));
+        B.rows.push_back(rows);
         B.slots.push_back(slots);
         B.max_rec_bytes = std::max(B.max_rec_bytes, rec);
         off += (size_t)rec;
-        j = r1;
+    };
+
+    for (int seg0 = 0; seg0 < n_v; seg0 += SEG_ROWS) {
+        const int seg1 = std::min(n_v, seg0 + SEG_ROWS);
+        // ---- which format is smaller on this segment
+        long long bytes_rows = 0, bytes_quads = 0;
+        for (int j = seg0; j < seg1; ++j) {
+            const int len = rp[j + 1] - rp[j];
+            if (len > 0) { bytes_rows += (long long)pad4(len) * (4 + col_bytes) + 4; ++n_nonempty; }
+        }
+        bool quads = !quadU.empty() && bytes_rows > 0;
+        if (quads) {
+            for (int q = seg0 / 4; q < (seg1 + 3) / 4; ++q)
+                if (quadU[q] > 0) bytes_quads += (long long)pad8(quadU[q]) * 18 + 8;
+            quads = bytes_quads < bytes_rows;
+        }
+        if (!quads) {
+            // ---- row-format records
+            int j = seg0;
+            while (j < seg1) {
+                if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
+                const int r0 = j;
+                int slots = pad4(rp[j + 1] - rp[j]);
+                if (slots > chunk_slots)
+                    return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
+                                rp[j + 1] - rp[j], chunk_slots);
+                int last = j, empties = 0, jj = j + 1;
+                while (jj < seg1 && jj - r0 < MAXROWS_F) {
+                    const int len = rp[jj + 1] - rp[jj];
+                    if (len == 0) {
+                        if (++empties > 32) break;
+                        ++jj;
+                        continue;
+                    }
+                    if (slots + pad4(len) > chunk_slots) break;
+                    slots += pad4(len);
+                    empties = 0;
+                    last = jj;
+                    ++jj;
+                }
+                const int r1 = last + 1, nrows = r1 - r0;
+                const int mo = (int)B.meta.size();
+                B.meta.push_back((uint32_t)nrows);
+                B.meta.push_back((uint32_t)r0);
+                B.meta.push_back(0u);
+                B.meta.push_back((uint32_t)slots);
+                int so = 0;
+                for (int row = r0; row < r1; ++row) {
+                    B.meta.push_back((uint32_t)so | ((uint32_t)sid[row] << 16));
+                    so += pad4(rp[row + 1] - rp[row]);
+                }
+                B.meta.push_back((uint32_t)so);
+                close_record(mo, (slots + ZPAD) * (4 + col_bytes), 0, nrows, slots);
+                j = r1;
+            }
+        } else {
+            // ---- quad-format records
+            int q = seg0 / 4;
+            const int q_end = (seg1 + 3) / 4;
+            auto skip_quad = [&](int qq) { for (int j = 4 * qq; j < std::min(n_v, 4 * qq + 4); ++j) skip_row(j); };
+            while (q < q_end) {
+                if (quadU[q] == 0) { skip_quad(q); ++q; continue; }
+                const int q0 = q;
+                int cols = pad8(quadU[q]);
+                if (cols > 65528)
+                    return fail(pl, IMRT_STATUS_UNSUPPORTED, "rows %d..%d of D touch %d distinct columns; too many for one record", 4 * q, 4 * q + 3, quadU[q]);
+                int last = q, empties = 0, qq = q + 1;
+                while (qq < q_end && qq - q0 < QUAD_MAXQ) {
+                    if (quadU[qq] == 0) {
+                        if (++empties > 8) break;
+                        ++qq;
+                        continue;
+                    }
+                    if (cols + pad8(quadU[qq]) > QUAD_CAP) break;
+                    cols += pad8(quadU[qq]);
+                    empties = 0;
+                    last = qq;
+                    ++qq;
+                }
+                const int q1 = last + 1, nq = q1 - q0;
+                const int mo = (int)B.meta.size();
+                B.meta.push_back((uint32_t)nq);
+                B.meta.push_back((uint32_t)(4 * q0));
+                B.meta.push_back(1u);
+                B.meta.push_back((uint32_t)cols);
+                int co = 0, rows_here = 0;
+                for (int t = q0; t < q1; ++t) {
+                    uint32_t mask = 0u, sids = 0u;
+                    for (int i = 0; i < 4; ++i)
+                        if (4 * t + i < n_v) { mask |= 1u << i; sids |= (uint32_t)sid[4 * t + i] << (8 * i); ++rows_here; }
+                    B.meta.push_back((uint32_t)co | (mask << 16));
+                    B.meta.push_back(sids);
+                    co += pad8(quadU[t]);
+                }
+                B.meta.push_back((uint32_t)co);
+                B.meta.push_back(0u);
+                close_record(mo, (cols + 1) * 16 + (cols + 8) * 2, 1, rows_here, 4 * cols);
+                n_quad_rows += rows_here;
+                q = q1;
+                for (; q < q_end && quadU[q] == 0; ++q) skip_quad(q);   // trailing empties of the run belong to no record
+            }
+        }
     }
     B.pack_bytes = off;
     return IMRT_STATUS_OK;
@@ -453,6 +596,16 @@ static cudaError_t launch_persistent(imrt_plan* pl) {
     return cudaLaunchKernelEx(&cfg, k_persistent, pl->P);
 }
 
+// A new partition of the dose pass: upload it and lay out every CTA's ring schedule for it.
+static imrt_status upload_partition(imrt_plan* pl, const std::vector<int>& cta_blk) {
+    cudaStream_t st = pl->stream;
+    CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_blk_w, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
+    k_ring_layout<<<(pl->P.grid_f + 127) / 128, 128, 0, st>>>(pl->blk_w, pl->cta_blk_w, pl->P.grid_f, (unsigned int)pl->P.ring_f_bytes);
+    CUDA_TRY(pl, cudaGetLastError());
+    CUDA_TRY(pl, cudaStreamSynchronize(st));   // cta_blk is a host vector the caller may drop
+    return IMRT_STATUS_OK;
+}
+
 // The static partition of the dose pass is only as good as its cost model, and the model cannot know how the
 // instruction-bound blocks (short rows at the field edges) trade against the bandwidth-bound ones on this device.
 // So measure: run the pass, read every CTA's streaming time, rescale the cost of each CTA's blocks by its measured
@@ -492,8 +645,8 @@ static imrt_status tune_partition(imrt_plan* pl) {
             for (int b = cta_blk[c]; b < cta_blk[c + 1]; ++b) pl->blk_cost[b] *= f;
         }
         partition_blocks(pl->blk_cost, grid, cta_blk);
-        CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_blk_w, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        const imrt_status us = upload_partition(pl, cta_blk);
+        if (us != IMRT_STATUS_OK) return us;
     }
     return IMRT_STATUS_OK;
 }
@@ -670,9 +823,21 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     const int chunk_slots = std::max(MIN_CHUNK_SLOTS, (max_row + 3) & ~3);
     if (chunk_slots > MAX_CHUNK_SLOTS)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row of D has %d entries; this build handles rows up to %d", max_row, MAX_CHUNK_SLOTS);
+    // quad format on offer: count the distinct columns of every 4 consecutive rows on the device
+    const int bm_words = (int)((n_b + 31) / 32);
+    std::vector<int> quadU;
+    if (col16 && n_b <= QUAD_MAX_NB && nnz > 0 && !getenv("IMRTGP_NO_QUADS")) {
+        const int n_quads = (int)((n_v + 3) / 4);
+        quadU.resize(n_quads);
+        k_quad_union<<<std::min(n_quads / 8 + 1, n_sm * 8), 256, 8 * bm_words * sizeof(uint32_t), st>>>(row_ptr, col_idx, (int)n_v, n_quads, bm_words, L.quadU);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(quadU.data(), L.quadU, sizeof(int) * n_quads, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+    }
     BlockPlan BP;
     double G_skip = 0.0;
-    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, BP, G_skip, pl->n_skipped, pl->n_nonempty);
+    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, quadU, BP, G_skip, pl->n_skipped,
+                                 pl->n_nonempty, pl->n_quad_rows);
     if (s != IMRT_STATUS_OK) return s;
     const Bounds B = bounds_for(n_v, n_b, nnz);
     const size_t n_blk = BP.blk.size();
@@ -691,14 +856,14 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     std::vector<int> cta_blk;
     partition_blocks(pl->blk_cost, grid_f, cta_blk);
     if (n_blk) {
-        CUDA_TRY(pl, cudaMemcpyAsync(L.blk, BP.blk.data(), sizeof(int2) * n_blk, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaMemcpyAsync(L.blk, BP.blk.data(), sizeof(int4) * n_blk, cudaMemcpyHostToDevice, st));
         CUDA_TRY(pl, cudaMemcpyAsync(L.pk, BP.pk.data(), sizeof(int4) * n_blk, cudaMemcpyHostToDevice, st));
         CUDA_TRY(pl, cudaMemcpyAsync(L.rowmeta, BP.meta.data(), sizeof(uint32_t) * BP.meta.size(), cudaMemcpyHostToDevice, st));
-        if (col16) k_pack_blocks<true><<<(unsigned int)n_blk, 256, 0, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, L.pack);
-        else k_pack_blocks<false><<<(unsigned int)n_blk, 256, 0, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, L.pack);
+        const size_t pk_smem = quadU.empty() ? 0 : 8 * 2 * bm_words * sizeof(uint32_t);
+        if (col16) k_pack_blocks<true><<<(unsigned int)n_blk, 256, pk_smem, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, (int)n_v, bm_words, L.pack);
+        else k_pack_blocks<false><<<(unsigned int)n_blk, 256, 0, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, (int)n_v, bm_words, L.pack);
         CUDA_TRY(pl, cudaGetLastError());
     }
-    CUDA_TRY(pl, cudaMemcpyAsync(L.cta_blk, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
 
     // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1)
     CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
@@ -732,14 +897,15 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
 
     // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, dose
-    // scratch, the R trial points, g, stages.  R = the largest of 4, 2, 1 not above the request that leaves room for
-    // a useful ring.
-    const int stage_f = std::max(BP.max_rec_bytes, 128);
+    // scratch, the R trial points, g, then the ring (dose pass) / stages (transpose pass).  R = the largest of 4, 2, 1
+    // not above the request that leaves the ring room for 16 records of average size (one per consumer warp).
+    const int max_rec = std::max(BP.max_rec_bytes, 128);
+    const long long avg_rec = n_blk ? (long long)(BP.pack_bytes / n_blk) : 128;
     const int nb_pad = (int)((n_b + 31) & ~31LL);
     int R = prm->ls_batch == 0 ? R_MAX : prm->ls_batch;
     if (getenv("IMRTGP_LS_BATCH")) R = atoi(getenv("IMRTGP_LS_BATCH"));
     if (R != 1 && R != 2 && R != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_params.ls_batch must be 0, 1, 2 or 4");
-    int off = 0, avail = 0, sf = 0, stt = 0;
+    int off = 0, avail = 0, stt = 0;
     for (;; R /= 2) {
         off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
         P.wpart_off = off; off += SMEM_WPART;
@@ -749,18 +915,20 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         off = (off + 127) & ~127;
         P.stage_off = off;
         avail = smem_optin - off;
-        sf = avail > 0 ? std::min(MAX_STAGES_F, avail / stage_f) : 0;
+        avail = (smem_optin - off) & ~127;
         stt = avail > 0 ? std::min(MAX_STAGES_T, avail / STAGE_T_BYTES) : 0;
-        if (R == 1 || (sf >= W_CONS / 2 && stt >= 3)) break;
+        if (R == 1 || (avail >= 2 * max_rec && avail >= W_CONS * avg_rec && stt >= 3)) break;
     }
-    if (avail < 0 || sf < 2 || stt < 2)
-        return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets do not fit in shared memory next to the pipeline stages", (long long)n_b);
-    pl->smem_bytes = (size_t)off + (size_t)std::max(sf * stage_f, stt * STAGE_T_BYTES);
+    if (avail < 2 * max_rec || stt < 2)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets and records of up to %d bytes do not fit in shared memory", (long long)n_b, max_rec);
+    pl->smem_bytes = (size_t)off + (size_t)avail;
     P.R = R;
+    P.ring_f_bytes = avail;
+    P.max_rec_bytes = max_rec;
 
     P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
-    P.pack = L.pack; P.blk = L.blk; P.cta_blk = L.cta_blk; P.grid_f = grid_f; P.n_stages_f = sf;
-    P.stage_f_bytes = stage_f; P.col16 = col16 ? 1 : 0;
+    P.pack = L.pack; P.blk = L.blk; P.cta_blk = L.cta_blk; P.grid_f = grid_f;
+    P.col16 = col16 ? 1 : 0;
     P.rowT_ptr = L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
     P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr;
     P.n_ranges = (int)ranges.size(); P.grid_t = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, ranges.size()));
@@ -773,6 +941,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.st = L.st; P.tr_obj = L.tr_obj; P.tr_lambda = L.tr_lambda; P.tr_step_sq = L.tr_step_sq; P.tr_trials = L.tr_trials;
     pl->r_scratch = L.r_scratch; pl->g_scratch = L.g_scratch; pl->d_scratch = L.d_scratch;
     pl->cta_blk_w = L.cta_blk;
+    pl->blk_w = L.blk;
     pl->rowT_ptr_w = L.rowT_ptr; pl->colT_w = L.colT; pl->valT_w = L.valT;
     pl->dvh = L.dvh;
     pl->grid_p = n_sm;
@@ -803,6 +972,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
 
+    s = upload_partition(pl, cta_blk);
+    if (s != IMRT_STATUS_OK) return s;
     s = tune_partition(pl);
     if (s != IMRT_STATUS_OK) return s;
     if (prm->driver == 0) {
@@ -987,9 +1158,9 @@ imrt_status imrt_plan_get_counters(imrt_plan* pl, int64_t* host_fwd_passes, int6
 
 imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info, int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT) {
     if (!pl) return IMRT_STATUS_INVALID_ARG;
-    const int64_t info[13] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
-                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.n_stages_f, pl->P.n_stages_t};
-    for (int i = 0; i < n_info && i < 13 && host_info; ++i) host_info[i] = info[i];
+    const int64_t info[14] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
+                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.ring_f_bytes, pl->P.n_stages_t, pl->n_quad_rows};
+    for (int i = 0; i < n_info && i < 14 && host_info; ++i) host_info[i] = info[i];
     cudaStream_t st = pl->stream;
     if (d_rowT_ptr) CUDA_TRY(pl, cudaMemcpyAsync(d_rowT_ptr, pl->rowT_ptr_w, sizeof(int) * (pl->P.n_b + 1), cudaMemcpyDeviceToDevice, st));
     if (d_colT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_colT, pl->colT_w, sizeof(int) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));

@@ -34,6 +34,10 @@ constexpr int META_HDR = 4;                   // header words {rows, first row, 
 constexpr int MIN_CHUNK_SLOTS = 1024;         // slot capacity of a block unless a longer row forces more
 constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
 constexpr int MAXROWS_F = 256;                // rows per block
+constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered up to this many beamlets (pack-kernel bitmap)
+constexpr int QUAD_CAP = 384;                 // union columns per quad-format record unless one quad needs more
+constexpr int QUAD_MAXQ = 64;                 // quads per record
+constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
 constexpr int R_MAX = 4;                      // line-search trial points evaluated per dose pass (1, 2 or 4)
 constexpr int CHUNK_T = 4096;                 // nnz per transpose-pass stage (pure streaming)
@@ -41,21 +45,15 @@ constexpr int SLICE_T = CHUNK_T / W_CONS;     // contiguous nnz per consumer war
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
 constexpr int RL_MAX = 32;                    // rows of D^T one transpose range may span
-constexpr int MAX_STAGES_F = 40;
+constexpr int RING_ENTRIES = 64;              // dose-pass records in flight per CTA (a multiple of W_CONS)
 constexpr int MAX_STAGES_T = 12;
 constexpr int MAX_STRUCTURES = 256;
-constexpr int SMEM_HEADER = 2048;             // barriers, flags, reduction scratch
+constexpr int SMEM_HEADER = 3072;             // barriers, flags, reduction scratch
 constexpr int SMEM_WPART = RL_MAX * W_CONS * 8;
 constexpr int SMEM_DSC = W_CONS * 32 * R_MAX * 4;   // per-warp scratch: dose of 32 rows x R trial points
 
 enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2, MODE_TIMING = 3 };
 enum { STOP_MAX_ITERS = 0, STOP_TOLERANCE = 1, STOP_STATIONARY = 2, STOP_LS_STALLED = 3 };
-
-// Beamlet i lives at position xperm(i) of the shared-memory copy of x+: bits [4:2] of i move to the bottom.  A row
-// group's 8 lanes read 4 consecutive slots each, i.e. columns ~4 apart in a run of neighbouring beamlets; with this
-// permutation they fall into 8 different banks (R = 1) / 8 different 16-byte bank groups (R = 4).  The packed
-// records store xperm(col) so the kernels never compute it.
-__host__ __device__ __forceinline__ int xperm(int i) { return (i & ~31) | ((i & 3) << 3) | ((i >> 2) & 7); }
 
 // ------------------------------------------------------------------------------------------------ device data
 struct State {                 // lives in the workspace; the single source of truth between launches
@@ -91,17 +89,27 @@ struct DevPlan {
     long long nnz;
     int n_v, n_b;
     // dose pass: D re-packed into block records (owned).  A record is 128-byte aligned and holds, in this order,
+    // ROW format (any matrix):
     //   header  uint32[4]  {rows, first row, 0, slots}
     //   rows    uint32[rows + 1]  slot offset of the row (low 16 bits, a multiple of 4) | structure id << 16;
     //                             padded to a multiple of 4 words
     //   val     fp32[slots + ZPAD]   every row padded with zeros to a multiple of 4 slots; ZPAD zeros at the end
-    //   col     uint16[slots + ZPAD] (n_b <= 65536) or int32[slots + ZPAD]: xperm(column)
+    //   col     uint16[slots + ZPAD] (n_b <= 65536) or int32[slots + ZPAD]
+    // QUAD format (chosen per 256-row segment where it is smaller; n_b <= QUAD_MAX_NB):
+    //   header  uint32[4]  {quads, first row (a multiple of 4), 1, union columns incl. padding}
+    //   quads   uint32[2 (quads + 1)]  {column offset of the quad (low 16 bits, a multiple of 8) | row-exists mask << 16,
+    //                                   the 4 structure ids}; the last pair holds the total; padded to 4 words
+    //   val     fp32[columns + 1][4]   per union column the 4 rows' values; unions padded to a multiple of 8 columns
+    //                                  with zeros; one zero column at the end
+    //   col     uint16[columns + 8]
     // One record is consumed by ONE warp.
     const unsigned char* pack;
-    const int2* blk;           // {record offset / 128, record bytes}
+    const int4* blk;           // {record offset / 128, record bytes, ring offset, blocks of the CTA to reclaim first}:
+                               // the last two are the ring schedule of the current partition (k_ring_layout)
     const int* cta_blk;        // [grid_f + 1] block range per CTA
-    int grid_f, n_stages_f;
-    int stage_f_bytes;         // bytes of one dose-pass stage (largest record, 128-byte multiple)
+    int grid_f;
+    int ring_f_bytes;          // bytes of the dose pass's shared-memory ring (records are placed at their own size)
+    int max_rec_bytes;         // largest record
     int col16;                 // 1: 16-bit column indices in the records
     int R;                     // trial points per dose pass of the line search (1, 2 or 4)
     int pad1;
@@ -149,7 +157,8 @@ struct PassArgs {
 
 // ------------------------------------------------------------------------------------------------ shared memory
 struct SmemHeader {
-    uint64_t full_f[MAX_STAGES_F], empty_f[MAX_STAGES_F], full_t[MAX_STAGES_T], empty_t[MAX_STAGES_T];
+    uint64_t full_f[RING_ENTRIES], full_t[MAX_STAGES_T], empty_t[MAX_STAGES_T];
+    uint32_t next_blk[W_CONS];        // dose pass: number (over the CTA's life) of the next block each consumer warp will finish
     double red[32 * R_MAX];    // block-reduction scratch
     double bcast[4];
     int flag;
@@ -162,10 +171,7 @@ struct Pipe {                  // running stage counters; identical in producer 
 
 __device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4* table_s) {
     if (threadIdx.x == 0) {
-        for (int s = 0; s < MAX_STAGES_F; ++s) {
-            mbar_init(&h->full_f[s], 1);
-            mbar_init(&h->empty_f[s], 1);      // a dose-pass stage is consumed by one warp
-        }
+        for (int s = 0; s < RING_ENTRIES; ++s) mbar_init(&h->full_f[s], 1);
         for (int s = 0; s < MAX_STAGES_T; ++s) {
             mbar_init(&h->full_t[s], 1);
             mbar_init(&h->empty_t[s], W_CONS);
@@ -221,7 +227,7 @@ __device__ __forceinline__ void block_sum_vec(double (&v)[R], SmemHeader* h) {
 // fp32 elementwise, fp64 sum.  A batch holds the next R trial points of the line search: lambda, lambda/alpha, ...
 // (the same division chain step 4 performs one trial at a time).  All NTHREADS threads call it; x is global (read
 // through L2: another CTA may have written it), g may be shared or global; xs is the shared-memory array the dose
-// pass gathers from, [n_b][R] at permuted positions (xperm).
+// pass gathers from, [n_b][R].
 template <int R>
 __device__ __forceinline__ void trial_batch(const float* x, const float* g, double lambda, double alpha, float* xs, int n_b,
                                             SmemHeader* h, double (&step_sq)[R]) {
@@ -231,7 +237,7 @@ __device__ __forceinline__ void trial_batch(const float* x, const float* g, doub
     for (int r = 0; r < R; ++r) { lam[r] = (float)l; l = l / alpha; step_sq[r] = 0.0; }
     for (int i = threadIdx.x; i < n_b; i += NTHREADS) {
         const float xi = __ldcg(x + i), gi = g[i];
-        float* o = xs + (size_t)xperm(i) * R;
+        float* o = xs + (size_t)i * R;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float xn = fmaxf(0.0f, fmaf(-lam[r], gi, xi));
@@ -257,7 +263,7 @@ __device__ __forceinline__ double first_step_sq(const float* x, const float* g, 
 
 // A single point x (MODE_EVAL / MODE_INIT): copy it to the gather array.
 __device__ __forceinline__ void stage_point(const float* x, float* xs, int n_b) {
-    for (int i = threadIdx.x; i < n_b; i += NTHREADS) xs[xperm(i)] = x[i];
+    for (int i = threadIdx.x; i < n_b; i += NTHREADS) xs[i] = x[i];
     __syncthreads();
 }
 
@@ -359,15 +365,92 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
     }
 }
 
+// The same for a record in QUAD format: 4 consecutive rows of D (neighbouring voxels, which see nearly the same
+// beamlets) share one sorted list of columns, the union of theirs; per union column the record holds the 4 rows'
+// values as one 16-byte vector (explicit zeros where a row has no entry) and one 16-bit column.  8 lanes per quad,
+// 4 quads per warp batch; per trip a lane takes union columns k, k+8, k+16, k+24: one vector load of 4 values, one
+// column, ONE gather of the R trial values, 4 R multiply-adds.  Against the row format this needs a quarter of the
+// gathers and of the column bytes and -- where the rows of a quad overlap well -- fewer bytes of HBM traffic per
+// non-zero (18 bytes per union column).  The 4 x R row sums of a quad are reduced over its 8 lanes by a transposing
+// butterfly (4 R shuffles), after which lanes 0, 2, 4, 6 each hold one row: penalty, residual, objective as above.
+template <int R>
+__device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
+                                                 const float4* __restrict__ table_s, float* const (&r_out)[R],
+                                                 float* __restrict__ d_out, int lane, double (&Gacc)[R]) {
+    const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
+    const int nq = (int)hdr.x, nbc = (int)hdr.w;
+    const uint32_t* qt = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
+    const unsigned char* val_b = reinterpret_cast<const unsigned char*>(qt + ((2 * (nq + 1) + 3) & ~3));
+    const unsigned char* col_b = val_b + (size_t)(nbc + 1) * 16;
+    const int grp = lane >> 3, sub = lane & 7;
+    constexpr int XB = 4 * R;
+    for (int b = 0; b < nq; b += 4) {
+        const int qi = b + grp;
+        uint32_t w0 = 0u, w1 = 0u, wn = 0u;
+        if (qi < nq) {
+            const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qi);
+            w0 = w.x; w1 = w.y; wn = qt[2 * qi + 2];
+        }
+        const int s = (int)(w0 & 0xFFFFu), e = (int)(wn & 0xFFFFu);
+        const int len_max = __reduce_max_sync(0xffffffffu, e - s);   // warp-uniform trip count
+        float acc[4][R];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int r = 0; r < R; ++r) acc[i][r] = 0.0f;
+        int k = s + sub;
+        for (int kb = 0; kb < len_max; kb += 32, k += 32) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int kj = k + 8 * j;
+                const int kk = kj < e ? kj : nbc;          // past the quad's end: the zero column
+                const float4 v = *reinterpret_cast<const float4*>(val_b + 16 * kk);
+                const uint32_t c = *reinterpret_cast<const unsigned short*>(col_b + 2 * kk);
+                XVec<R> x;
+                x.load(xs_b + c * XB);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    acc[0][r] = fmaf(v.x, x.v[r], acc[0][r]);
+                    acc[1][r] = fmaf(v.y, x.v[r], acc[1][r]);
+                    acc[2][r] = fmaf(v.z, x.v[r], acc[2][r]);
+                    acc[3][r] = fmaf(v.w, x.v[r], acc[3][r]);
+                }
+            }
+        }
+        // transposing butterfly: after xor 4 a lane keeps rows {0,1} or {2,3}, after xor 2 one row, xor 1 completes it
+        const bool hi4 = (sub & 4) != 0, hi2 = (sub & 2) != 0;
+        float d[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float a0 = (hi4 ? acc[2][r] : acc[0][r]) + __shfl_xor_sync(0xffffffffu, hi4 ? acc[0][r] : acc[2][r], 4);
+            const float a1 = (hi4 ? acc[3][r] : acc[1][r]) + __shfl_xor_sync(0xffffffffu, hi4 ? acc[1][r] : acc[3][r], 4);
+            const float h = (hi2 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi2 ? a0 : a1, 2);
+            d[r] = h + __shfl_xor_sync(0xffffffffu, h, 1);
+        }
+        const int rr = (hi4 ? 2 : 0) + (hi2 ? 1 : 0);
+        if (!(sub & 1) && ((w0 >> (16 + rr)) & 1u)) {      // the row exists (w0 = 0 for a quad past the end)
+            const float4 t = table_s[(w1 >> (8 * rr)) & 0xFFu];
+            const size_t jrow = (size_t)hdr.y + 4 * qi + rr;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const float u = fmaxf(0.0f, t.x - d[r]);
+                const float o = fmaxf(0.0f, d[r] - t.y);
+                r_out[r][jrow] = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));
+                const double du = (double)u, d_o = (double)o;
+                Gacc[r] = __dadd_rn(Gacc[r], __fma_rn((double)t.z, __dmul_rn(du, du), __dmul_rn((double)t.w, __dmul_rn(d_o, d_o))));
+            }
+            if (R == 1 && d_out) d_out[jrow] = d[0];
+        }
+    }
+}
+
 // All NTHREADS threads of the CTA call this.  xs: the R trial points in shared memory.  Writes the CTA's R objective
 // partials to Gpart[blockIdx.x * R ..] (thread 0).  Ends with a CTA-wide barrier.
 template <bool COL16, int R>
 __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
                                             const float* xs, float* const (&r_out)[R], float* d_out, double* Gpart, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const unsigned int S = (unsigned int)P.n_stages_f;
-    const uint32_t SB = (uint32_t)P.stage_f_bytes;
-    unsigned char* stages = smem + P.stage_off;
+    unsigned char* ring = smem + P.stage_off;
     const int b0 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x] : 0;
     const int b1 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x + 1] : 0;
     const int nb = b1 - b0;
@@ -375,44 +458,71 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
 #pragma unroll
     for (int r = 0; r < R; ++r) Gacc[r] = 0.0;
     const unsigned long long t_start = global_ns();
-    const uint32_t full_a = smem_u32(&h->full_f[0]), empty_a = smem_u32(&h->empty_f[0]), stages_a = smem_u32(stages);
+    const uint32_t full_a = smem_u32(&h->full_f[0]), ring_a = smem_u32(ring);
+    volatile uint32_t* next_blk = h->next_blk;
+    const unsigned int it0 = pipe.it_f;        // blocks are numbered over the CTA's life: this pass has it0 .. it0 + nb - 1
+    if (warp < W_CONS && lane == 0) next_blk[warp] = it0 + (unsigned int)warp;
+    __syncthreads();
 
+    // The ring: records keep their own size (128-byte multiples) and are laid end to end in a circular byte buffer;
+    // a record that does not fit before the end starts over at 0.  Where each record goes, and how many of the CTA's
+    // earlier blocks must have left the ring before its copy may be issued, depends only on the record sizes, so it is
+    // computed once per partition (k_ring_layout) and travels with the block descriptors.  Block number `it` uses
+    // full barrier it % 64 in phase it / 64; a warp's consecutive blocks are 16 apart, so the previous user of a
+    // barrier is always a block the same warp has already finished.  Space is reclaimed in issue order: every
+    // consumer warp publishes the number of the next block it will finish, and the minimum over the warps bounds
+    // the blocks that are gone.
     if (warp == W_CONS) {
         // ---------------- producer warp: lane 0 drives the TMA unit, one bulk copy per block record; the
         // descriptors of the next 32 blocks are requested before the current 32 are issued
         const uint64_t pol = policy_evict_first();   // streamed once per pass: keep it from pushing r / x out of L2
-        unsigned int s = pipe.it_f % S, ph = (pipe.it_f / S) & 1u;
-        int2 next = (lane < nb) ? __ldg(P.blk + b0 + lane) : make_int2(0, 0);
+        unsigned int gone = it0;                       // every block numbered below this has been consumed
+        int4 next = (lane < nb) ? __ldg(P.blk + b0 + lane) : make_int4(0, 0, 0, 0);
         for (int bb = 0; bb < nb; bb += 32) {
-            const int2 mine = next;
-            next = (bb + 32 + lane < nb) ? __ldg(P.blk + b0 + bb + 32 + lane) : make_int2(0, 0);
+            const int4 mine = next;
+            next = (bb + 32 + lane < nb) ? __ldg(P.blk + b0 + bb + 32 + lane) : make_int4(0, 0, 0, 0);
             const int nb_here = min(32, nb - bb);
             for (int j = 0; j < nb_here; ++j) {
                 const int off128 = __shfl_sync(0xffffffffu, mine.x, j);
-                const int bytes = __shfl_sync(0xffffffffu, mine.y, j);
-                if (lane == 0) {
-                    mbar_wait_a(empty_a + 8u * s, ph ^ 1u);
-                    const uint32_t bar = full_a + 8u * s;
-                    mbar_expect_tx_a(bar, (uint32_t)bytes);
-                    bulk_g2s_a(stages_a + s * SB, P.pack + (size_t)(unsigned int)off128 * 128u, (uint32_t)bytes, bar, pol);
+                const uint32_t bytes = (uint32_t)__shfl_sync(0xffffffffu, mine.y, j);
+                const uint32_t at = (uint32_t)__shfl_sync(0xffffffffu, mine.z, j);
+                const unsigned int need = it0 + (unsigned int)__shfl_sync(0xffffffffu, mine.w, j);
+                while ((int)(need - gone) > 0) {
+                    const unsigned int v = next_blk[lane & (W_CONS - 1)];
+                    gone = __reduce_min_sync(0xffffffffu, v - it0) + it0;     // numbers wrap: compare relative to it0
                 }
-                if (++s == S) { s = 0; ph ^= 1u; }
+                if (lane == 0) {
+                    __threadfence_block();   // the consumers' reads of the space (seen through next_blk) come first
+                    const uint32_t bar = full_a + 8u * ((it0 + (unsigned int)(bb + j)) & (RING_ENTRIES - 1));
+                    mbar_expect_tx_a(bar, bytes);
+                    bulk_g2s_a(ring_a + at, P.pack + (size_t)(unsigned int)off128 * 128u, bytes, bar, pol);
+                }
             }
         }
     } else {
         // ---------------- consumer warps: warp w takes the CTA's blocks w, w + 16, ...
         float* dsc = reinterpret_cast<float*>(smem + P.dsc_off) + warp * 32 * R_MAX;
         const unsigned char* xs_b = reinterpret_cast<const unsigned char*>(xs);
+        int at_next = (warp < nb) ? __ldg(&P.blk[b0 + warp].z) : 0;
         for (int i = warp; i < nb; i += W_CONS) {
-            const unsigned int it = pipe.it_f + (unsigned int)i;
-            const unsigned int s = it % S, ph = (it / S) & 1u;
-            mbar_wait_a(full_a + 8u * s, ph);
+            const int at = at_next;
+            if (i + W_CONS < nb) at_next = __ldg(&P.blk[b0 + i + W_CONS].z);
+            const unsigned int it = it0 + (unsigned int)i;
+            mbar_wait_a(full_a + 8u * (it & (RING_ENTRIES - 1)), (it / RING_ENTRIES) & 1u);
 #ifndef IMRT_EXP_SKIP_COMPUTE
-            dose_block<COL16, R>(stages + (size_t)s * SB, xs_b, table_s, dsc, r_out, d_out, lane, Gacc);
+            const unsigned char* rec = ring + at;
+            if (COL16 && reinterpret_cast<const uint32_t*>(rec)[2] != 0u)      // header word 2: record format
+                dose_block_quads<R>(rec, xs_b, table_s, r_out, d_out, lane, Gacc);
+            else
+                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, lane, Gacc);
 #endif
             __syncwarp();
-            if (lane == 0) mbar_arrive_a(empty_a + 8u * s);
+            if (lane == 0) {
+                __threadfence_block();
+                next_blk[warp] = it + (unsigned int)W_CONS;
+            }
         }
+        if (lane == 0) next_blk[warp] = it0 + (unsigned int)nb + (unsigned int)W_CONS;   // nothing left: never the minimum
     }
     pipe.it_f += (unsigned int)nb;
     block_sum_vec<R>(Gacc, h);   // producer lanes contribute 0
@@ -661,11 +771,42 @@ __device__ __forceinline__ bool cta_is_last(unsigned int* ticket, SmemHeader* h)
 // x_{k+1} = trial point j of the batch: copy it from the gather array to global memory.
 template <int R>
 __device__ __forceinline__ void publish_x(const float* xs, int j, float* x_out, int n_b) {
-    for (int i = threadIdx.x; i < n_b; i += NTHREADS) x_out[i] = xs[(size_t)xperm(i) * R + j];
+    for (int i = threadIdx.x; i < n_b; i += NTHREADS) x_out[i] = xs[(size_t)i * R + j];
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
 extern __shared__ __align__(128) unsigned char imrt_smem[];
+
+// The dose pass's ring schedule for the current partition: thread c walks CTA c's blocks in order, places every
+// record in a circular buffer of ring_bytes (end to end; a record that does not fit before the end starts over at
+// 0) and notes how many earlier blocks must have left the ring first (at most RING_ENTRIES in flight).
+__global__ void k_ring_layout(int4* blk, const int* __restrict__ cta_blk, int grid_f, unsigned int ring_bytes) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= grid_f) return;
+    const int b0 = cta_blk[c], b1 = cta_blk[c + 1];
+    unsigned int head = 0u;
+    int tail = b0;
+    for (int b = b0; b < b1; ++b) {
+        const unsigned int bytes = (unsigned int)blk[b].y;
+        unsigned int at;
+        for (;;) {
+            bool fits;
+            if (tail == b) { at = 0u; fits = true; }                 // nothing in flight
+            else {
+                const unsigned int t = (unsigned int)blk[tail].z;    // the oldest record in flight
+                if (head > t) {
+                    if (head + bytes <= ring_bytes) { at = head; fits = true; }
+                    else { at = 0u; fits = bytes <= t; }
+                } else { at = head; fits = head + bytes <= t; }
+            }
+            if (fits && b - tail < RING_ENTRIES) break;
+            ++tail;
+        }
+        head = at + bytes;
+        blk[b].z = (int)at;
+        blk[b].w = tail - b0;
+    }
+}
 
 // A single-point dose pass (MODE_EVAL: eval / get_dose / timing; MODE_INIT: G(x_1), r(x_1)).  Uses the R = 1 path.
 __device__ __forceinline__ void dose_single(const DevPlan& P, const PassArgs& A, SmemHeader* h, const float4* table_s, float* xs) {
@@ -739,7 +880,7 @@ __device__ __forceinline__ void dose_timing(const DevPlan& P, SmemHeader* h, con
     for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) {
         const float v = x[i];
 #pragma unroll
-        for (int r = 0; r < R; ++r) xs[(size_t)xperm(i) * R + r] = v;
+        for (int r = 0; r < R; ++r) xs[(size_t)i * R + r] = v;
     }
     __syncthreads();
     float* r_out[R];
