@@ -495,7 +495,12 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
                     last = qq;
                     ++qq;
                 }
-                const int q1 = last + 1, nq = q1 - q0;
+                int q1 = last + 1, nq = q1 - q0;
+                if (nq > TEAM && nq % TEAM) {      // a team of TEAM warps takes one quad each per round: keep rounds full
+                    for (int t = q1 - nq % TEAM; t < q1; ++t) cols -= pad8(quadU[t]);
+                    q1 -= nq % TEAM;
+                    nq = q1 - q0;
+                }
                 const int mo = (int)B.meta.size();
                 B.meta.push_back((uint32_t)nq);
                 B.meta.push_back((uint32_t)(4 * q0));
@@ -917,7 +922,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         avail = smem_optin - off;
         avail = (smem_optin - off) & ~127;
         stt = avail > 0 ? std::min(MAX_STAGES_T, avail / STAGE_T_BYTES) : 0;
-        if (R == 1 || (avail >= 2 * max_rec && avail >= W_CONS * avg_rec && stt >= 3)) break;
+        if (R == 1 || (avail >= 2 * max_rec && avail >= (W_CONS / 2) * avg_rec && stt >= 3)) break;
     }
     if (avail < 2 * max_rec || stt < 2)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets and records of up to %d bytes do not fit in shared memory", (long long)n_b, max_rec);

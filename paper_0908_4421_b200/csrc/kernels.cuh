@@ -27,6 +27,14 @@ namespace imrt {
 
 // ------------------------------------------------------------------------------------------------ constants
 constexpr int W_CONS = 16;                    // consumer warps per CTA
+#ifndef IMRT_TEAM
+#define IMRT_TEAM 1
+#endif
+#ifndef IMRT_QUAD_CAP
+#define IMRT_QUAD_CAP 512
+#endif
+constexpr int TEAM = IMRT_TEAM;               // consumer warps that work on one dose-pass record together
+constexpr int N_TEAMS = W_CONS / TEAM;
 constexpr int N_CONS = W_CONS * 32;           // consumer threads
 constexpr int NTHREADS = N_CONS + 32;         // + one producer warp
 // dose pass: D is re-packed once into self-contained block records (one bulk copy each, see DevPlan::pack)
@@ -35,7 +43,7 @@ constexpr int MIN_CHUNK_SLOTS = 1024;         // slot capacity of a block unless
 constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
 constexpr int MAXROWS_F = 256;                // rows per block
 constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered up to this many beamlets (pack-kernel bitmap)
-constexpr int QUAD_CAP = 384;                 // union columns per quad-format record unless one quad needs more
+constexpr int QUAD_CAP = IMRT_QUAD_CAP;                 // union columns per quad-format record unless one quad needs more
 constexpr int QUAD_MAXQ = 64;                 // quads per record
 constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
@@ -45,7 +53,7 @@ constexpr int SLICE_T = CHUNK_T / W_CONS;     // contiguous nnz per consumer war
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
 constexpr int RL_MAX = 32;                    // rows of D^T one transpose range may span
-constexpr int RING_ENTRIES = 64;              // dose-pass records in flight per CTA (a multiple of W_CONS)
+constexpr int RING_ENTRIES = 64;              // dose-pass records in flight per CTA (a multiple of the team count)
 constexpr int MAX_STAGES_T = 12;
 constexpr int MAX_STRUCTURES = 256;
 constexpr int SMEM_HEADER = 3072;             // barriers, flags, reduction scratch
@@ -290,7 +298,7 @@ template <> struct XVec<4> { float v[4]; __device__ __forceinline__ void load(co
 template <bool COL16, int R>
 __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
                                            const float4* __restrict__ table_s, float* __restrict__ dsc,
-                                           float* const (&r_out)[R], float* __restrict__ d_out, int lane, double (&Gacc)[R]) {
+                                           float* const (&r_out)[R], float* __restrict__ d_out, int tw, int lane, double (&Gacc)[R]) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nrows = (int)hdr.x, slots = (int)hdr.w;
     const uint32_t* rows = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
@@ -298,10 +306,14 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
     const unsigned char* col_b = val_b + (size_t)(slots + ZPAD) * 4;
     const int grp = lane / VW, sub = lane % VW;
     constexpr int XB = 4 * R;   // bytes per beamlet in the gather array
-    for (int c0 = 0; c0 < nrows; c0 += 32) {
-        const int nbatch = min(32 / RB, (nrows - c0 + RB - 1) / RB);
-        for (int q = 0; q < nbatch; ++q) {
-            const int row = c0 + q * RB + grp;
+    const int nbatch = (nrows + RB - 1) / RB;
+    // warp tw of the team takes the batches tw, tw + TEAM, ...; 8 of its batches (32 rows) make one penalty step
+    for (int q0 = tw; q0 < nbatch; q0 += 8 * TEAM) {
+#pragma unroll 1
+        for (int kq = 0; kq < 8; ++kq) {
+            const int q = q0 + kq * TEAM;
+            if (q >= nbatch) break;
+            const int row = q * RB + grp;
             uint32_t m0 = 0u, m1 = 0u;
             if (row < nrows) { m0 = rows[row]; m1 = rows[row + 1]; }
             const int s = (int)(m0 & 0xFFFFu), e = (int)(m1 & 0xFFFFu);
@@ -338,13 +350,13 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
 #pragma unroll
             for (int r = 0; r < R; ++r) d[r] = vec_sum<VW>((acc[0][r] + acc[1][r]) + (acc[2][r] + acc[3][r]));
             if (sub == 0) {   // rows past the end park a zero nobody reads
-                float* o = dsc + (q * RB + grp) * R;
+                float* o = dsc + (kq * RB + grp) * R;
 #pragma unroll
                 for (int r = 0; r < R; ++r) o[r] = d[r];
             }
         }
         __syncwarp();
-        const int row = c0 + lane;
+        const int row = (q0 + (lane / RB) * TEAM) * RB + (lane % RB);     // the row parked at position `lane`
         if (row < nrows) {
             const float4 t = table_s[(rows[row] >> 16) & 0xFFu];
             XVec<R> dv;
@@ -356,7 +368,7 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
                 const float u = fmaxf(0.0f, t.x - dd);
                 const float o = fmaxf(0.0f, dd - t.y);
                 r_out[r][j] = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));      // explicit roundings: every
-                const double du = (double)u, d_o = (double)o;                         // instantiation sums alike
+                const double du = (double)u, d_o = (double)o;                     // instantiation sums alike
                 Gacc[r] = __dadd_rn(Gacc[r], __fma_rn((double)t.z, __dmul_rn(du, du), __dmul_rn((double)t.w, __dmul_rn(d_o, d_o))));
             }
             if (R == 1 && d_out) d_out[j] = dv.v[0];
@@ -367,79 +379,90 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
 
 // The same for a record in QUAD format: 4 consecutive rows of D (neighbouring voxels, which see nearly the same
 // beamlets) share one sorted list of columns, the union of theirs; per union column the record holds the 4 rows'
-// values as one 16-byte vector (explicit zeros where a row has no entry) and one 16-bit column.  8 lanes per quad,
-// 4 quads per warp batch; per trip a lane takes union columns k, k+8, k+16, k+24: one vector load of 4 values, one
-// column, ONE gather of the R trial values, 4 R multiply-adds.  Against the row format this needs a quarter of the
-// gathers and of the column bytes and -- where the rows of a quad overlap well -- fewer bytes of HBM traffic per
-// non-zero (18 bytes per union column).  The 4 x R row sums of a quad are reduced over its 8 lanes by a transposing
-// butterfly (4 R shuffles), after which lanes 0, 2, 4, 6 each hold one row: penalty, residual, objective as above.
+// values as one 16-byte vector (explicit zeros where a row has no entry) and one 16-bit column.  A warp takes one
+// quad at a time: per trip every lane takes one union column -- one vector load of 4 values, one column, ONE
+// gather of the R trial values (32 neighbouring beamlets: conflict-free), 4 R multiply-adds.  Against the row format
+// this needs a quarter of the gathers and of the column bytes and -- where the rows of a quad overlap well -- fewer
+// bytes of HBM traffic per non-zero (18 bytes per union column).  The 4 x R row sums are reduced over the warp by a
+// butterfly whose first two steps split the rows (xor 16: rows {0,1} | {2,3}; xor 8: one row), so lanes 0, 8, 16, 24
+// end up with one row each: penalty, residual, objective as above.
+// Which trial point of a batch a lane ends up with after the quad reduction, and whether it ends up with a sum at all.
+template <int R> __device__ __forceinline__ int quad_trial(int lane) { return R == 4 ? ((lane >> 1) & 3) : R == 2 ? ((lane >> 2) & 1) : 0; }
+template <int R> __device__ __forceinline__ bool quad_owner(int lane) { return (lane & (R == 4 ? 1 : R == 2 ? 3 : 7)) == 0; }
+
+// The reduction is one xor butterfly over the 32 lanes for every (row, trial) sum -- the same tree of additions
+// whatever R is -- but at each step a lane keeps only half of what it holds: xor 16 splits the rows {0,1} | {2,3},
+// xor 8 leaves one row, xor 4 / xor 2 split the trial points (R = 4; xor 4 only for R = 2).  4 R shuffles instead of
+// 5 x 4 R, and lane (b4 b3 b2 b1 0) ends with row 2 b4 + b3 of trial 2 b2 + b1: one penalty evaluation per lane.
+// my_r: the residual buffer of this lane's trial.  Gq: this lane's objective partial (of its own trial).
 template <int R>
 __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
-                                                 const float4* __restrict__ table_s, float* const (&r_out)[R],
-                                                 float* __restrict__ d_out, int lane, double (&Gacc)[R]) {
+                                                 const float4* __restrict__ table_s, float* __restrict__ my_r,
+                                                 float* __restrict__ d_out, int tw, int lane, double& Gq) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nq = (int)hdr.x, nbc = (int)hdr.w;
     const uint32_t* qt = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
     const unsigned char* val_b = reinterpret_cast<const unsigned char*>(qt + ((2 * (nq + 1) + 3) & ~3));
     const unsigned char* col_b = val_b + (size_t)(nbc + 1) * 16;
-    const int grp = lane >> 3, sub = lane & 7;
     constexpr int XB = 4 * R;
-    for (int b = 0; b < nq; b += 4) {
-        const int qi = b + grp;
-        uint32_t w0 = 0u, w1 = 0u, wn = 0u;
-        if (qi < nq) {
-            const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qi);
-            w0 = w.x; w1 = w.y; wn = qt[2 * qi + 2];
-        }
-        const int s = (int)(w0 & 0xFFFFu), e = (int)(wn & 0xFFFFu);
-        const int len_max = __reduce_max_sync(0xffffffffu, e - s);   // warp-uniform trip count
+    const bool hi16 = (lane & 16) != 0, hi8 = (lane & 8) != 0, hi4 = (lane & 4) != 0, hi2 = (lane & 2) != 0;
+    const int rr = (hi16 ? 2 : 0) + (hi8 ? 1 : 0);         // the row this lane ends up with
+    const bool owner = quad_owner<R>(lane);
+    for (int qi = tw; qi < nq; qi += TEAM) {               // warp tw of the team takes the quads tw, tw + TEAM, ...
+        const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qi);
+        const int s = (int)(w.x & 0xFFFFu), e = (int)(qt[2 * qi + 2] & 0xFFFFu);
         float acc[4][R];
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int r = 0; r < R; ++r) acc[i][r] = 0.0f;
-        int k = s + sub;
-        for (int kb = 0; kb < len_max; kb += 32, k += 32) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int kj = k + 8 * j;
-                const int kk = kj < e ? kj : nbc;          // past the quad's end: the zero column
-                const float4 v = *reinterpret_cast<const float4*>(val_b + 16 * kk);
-                const uint32_t c = *reinterpret_cast<const unsigned short*>(col_b + 2 * kk);
-                XVec<R> x;
-                x.load(xs_b + c * XB);
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    acc[0][r] = fmaf(v.x, x.v[r], acc[0][r]);
-                    acc[1][r] = fmaf(v.y, x.v[r], acc[1][r]);
-                    acc[2][r] = fmaf(v.z, x.v[r], acc[2][r]);
-                    acc[3][r] = fmaf(v.w, x.v[r], acc[3][r]);
-                }
-            }
-        }
-        // transposing butterfly: after xor 4 a lane keeps rows {0,1} or {2,3}, after xor 2 one row, xor 1 completes it
-        const bool hi4 = (sub & 4) != 0, hi2 = (sub & 2) != 0;
-        float d[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float a0 = (hi4 ? acc[2][r] : acc[0][r]) + __shfl_xor_sync(0xffffffffu, hi4 ? acc[0][r] : acc[2][r], 4);
-            const float a1 = (hi4 ? acc[3][r] : acc[1][r]) + __shfl_xor_sync(0xffffffffu, hi4 ? acc[1][r] : acc[3][r], 4);
-            const float h = (hi2 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi2 ? a0 : a1, 2);
-            d[r] = h + __shfl_xor_sync(0xffffffffu, h, 1);
-        }
-        const int rr = (hi4 ? 2 : 0) + (hi2 ? 1 : 0);
-        if (!(sub & 1) && ((w0 >> (16 + rr)) & 1u)) {      // the row exists (w0 = 0 for a quad past the end)
-            const float4 t = table_s[(w1 >> (8 * rr)) & 0xFFu];
-            const size_t jrow = (size_t)hdr.y + 4 * qi + rr;
+#pragma unroll 2
+        for (int k0 = s; k0 < e; k0 += 32) {
+            const int k = k0 + lane;
+            const int kk = k < e ? k : nbc;                // past the quad's end: the zero column
+            const float4 v = *reinterpret_cast<const float4*>(val_b + 16 * kk);
+            const uint32_t c = *reinterpret_cast<const unsigned short*>(col_b + 2 * kk);
+            XVec<R> x;
+            x.load(xs_b + c * XB);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const float u = fmaxf(0.0f, t.x - d[r]);
-                const float o = fmaxf(0.0f, d[r] - t.y);
-                r_out[r][jrow] = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));
-                const double du = (double)u, d_o = (double)o;
-                Gacc[r] = __dadd_rn(Gacc[r], __fma_rn((double)t.z, __dmul_rn(du, du), __dmul_rn((double)t.w, __dmul_rn(d_o, d_o))));
+                acc[0][r] = fmaf(v.x, x.v[r], acc[0][r]);
+                acc[1][r] = fmaf(v.y, x.v[r], acc[1][r]);
+                acc[2][r] = fmaf(v.z, x.v[r], acc[2][r]);
+                acc[3][r] = fmaf(v.w, x.v[r], acc[3][r]);
             }
-            if (R == 1 && d_out) d_out[jrow] = d[0];
+        }
+        float h[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float a0 = (hi16 ? acc[2][r] : acc[0][r]) + __shfl_xor_sync(0xffffffffu, hi16 ? acc[0][r] : acc[2][r], 16);
+            const float a1 = (hi16 ? acc[3][r] : acc[1][r]) + __shfl_xor_sync(0xffffffffu, hi16 ? acc[1][r] : acc[3][r], 16);
+            h[r] = (hi8 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi8 ? a0 : a1, 8);
+        }
+        float d;
+        if (R == 4) {
+            const float g0 = (hi4 ? h[R > 2 ? 2 : 0] : h[0]) + __shfl_xor_sync(0xffffffffu, hi4 ? h[0] : h[R > 2 ? 2 : 0], 4);
+            const float g1 = (hi4 ? h[R > 3 ? 3 : 0] : h[R > 1 ? 1 : 0]) + __shfl_xor_sync(0xffffffffu, hi4 ? h[R > 1 ? 1 : 0] : h[R > 3 ? 3 : 0], 4);
+            const float f = (hi2 ? g1 : g0) + __shfl_xor_sync(0xffffffffu, hi2 ? g0 : g1, 2);
+            d = f + __shfl_xor_sync(0xffffffffu, f, 1);
+        } else if (R == 2) {
+            float g = (hi4 ? h[R > 1 ? 1 : 0] : h[0]) + __shfl_xor_sync(0xffffffffu, hi4 ? h[0] : h[R > 1 ? 1 : 0], 4);
+            g += __shfl_xor_sync(0xffffffffu, g, 2);
+            d = g + __shfl_xor_sync(0xffffffffu, g, 1);
+        } else {
+            float g = h[0] + __shfl_xor_sync(0xffffffffu, h[0], 4);
+            g += __shfl_xor_sync(0xffffffffu, g, 2);
+            d = g + __shfl_xor_sync(0xffffffffu, g, 1);
+        }
+        if (owner && ((w.x >> (16 + rr)) & 1u)) {          // the row exists
+            const float4 t = table_s[(w.y >> (8 * rr)) & 0xFFu];
+            const size_t jrow = (size_t)hdr.y + 4 * qi + rr;
+            const float u = fmaxf(0.0f, t.x - d);
+            const float o = fmaxf(0.0f, d - t.y);
+            my_r[jrow] = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));
+            const double du = (double)u, d_o = (double)o;
+            Gq = __dadd_rn(Gq, __fma_rn((double)t.z, __dmul_rn(du, du), __dmul_rn((double)t.w, __dmul_rn(d_o, d_o))));
+            if (R == 1 && d_out) d_out[jrow] = d;
         }
     }
 }
@@ -454,22 +477,24 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
     const int b0 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x] : 0;
     const int b1 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x + 1] : 0;
     const int nb = b1 - b0;
-    double Gacc[R];
+    double Gacc[R];              // objective partials of the row-format records (every lane, every trial) ...
 #pragma unroll
     for (int r = 0; r < R; ++r) Gacc[r] = 0.0;
+    double Gq = 0.0;             // ... and of the quad-format records (this lane's trial only)
     const unsigned long long t_start = global_ns();
     const uint32_t full_a = smem_u32(&h->full_f[0]), ring_a = smem_u32(ring);
     volatile uint32_t* next_blk = h->next_blk;
     const unsigned int it0 = pipe.it_f;        // blocks are numbered over the CTA's life: this pass has it0 .. it0 + nb - 1
-    if (warp < W_CONS && lane == 0) next_blk[warp] = it0 + (unsigned int)warp;
+    const int team = warp / TEAM, tw = warp % TEAM;
+    if (warp < W_CONS && lane == 0) next_blk[warp] = it0 + (unsigned int)team;
     __syncthreads();
 
     // The ring: records keep their own size (128-byte multiples) and are laid end to end in a circular byte buffer;
     // a record that does not fit before the end starts over at 0.  Where each record goes, and how many of the CTA's
     // earlier blocks must have left the ring before its copy may be issued, depends only on the record sizes, so it is
     // computed once per partition (k_ring_layout) and travels with the block descriptors.  Block number `it` uses
-    // full barrier it % 64 in phase it / 64; a warp's consecutive blocks are 16 apart, so the previous user of a
-    // barrier is always a block the same warp has already finished.  Space is reclaimed in issue order: every
+    // full barrier it % 64 in phase it / 64; a team's consecutive blocks are 4 apart, so the previous user of a
+    // barrier is always a block the same warps have already finished.  Space is reclaimed in issue order: every
     // consumer warp publishes the number of the next block it will finish, and the minimum over the warps bounds
     // the blocks that are gone.
     if (warp == W_CONS) {
@@ -500,32 +525,43 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
             }
         }
     } else {
-        // ---------------- consumer warps: warp w takes the CTA's blocks w, w + 16, ...
+        // ---------------- consumer warps: team t (4 warps) takes the CTA's blocks t, t + 4, ...; inside a record the
+        // team's warps split the quads / row batches
         float* dsc = reinterpret_cast<float*>(smem + P.dsc_off) + warp * 32 * R_MAX;
         const unsigned char* xs_b = reinterpret_cast<const unsigned char*>(xs);
-        int at_next = (warp < nb) ? __ldg(&P.blk[b0 + warp].z) : 0;
-        for (int i = warp; i < nb; i += W_CONS) {
+        float* my_r = r_out[0];
+#pragma unroll
+        for (int r = 1; r < R; ++r) my_r = quad_trial<R>(lane) == r ? r_out[r] : my_r;
+        int at_next = (team < nb) ? __ldg(&P.blk[b0 + team].z) : 0;
+        for (int i = team; i < nb; i += N_TEAMS) {
             const int at = at_next;
-            if (i + W_CONS < nb) at_next = __ldg(&P.blk[b0 + i + W_CONS].z);
+            if (i + N_TEAMS < nb) at_next = __ldg(&P.blk[b0 + i + N_TEAMS].z);
             const unsigned int it = it0 + (unsigned int)i;
             mbar_wait_a(full_a + 8u * (it & (RING_ENTRIES - 1)), (it / RING_ENTRIES) & 1u);
 #ifndef IMRT_EXP_SKIP_COMPUTE
             const unsigned char* rec = ring + at;
             if (COL16 && reinterpret_cast<const uint32_t*>(rec)[2] != 0u)      // header word 2: record format
-                dose_block_quads<R>(rec, xs_b, table_s, r_out, d_out, lane, Gacc);
+                dose_block_quads<R>(rec, xs_b, table_s, my_r, d_out, tw, lane, Gq);
             else
-                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, lane, Gacc);
+                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, tw, lane, Gacc);
 #endif
             __syncwarp();
             if (lane == 0) {
                 __threadfence_block();
-                next_blk[warp] = it + (unsigned int)W_CONS;
+                next_blk[warp] = it + (unsigned int)N_TEAMS;
             }
         }
-        if (lane == 0) next_blk[warp] = it0 + (unsigned int)nb + (unsigned int)W_CONS;   // nothing left: never the minimum
+        if (lane == 0) next_blk[warp] = it0 + (unsigned int)nb + (unsigned int)N_TEAMS;   // nothing left: never the minimum
     }
     pipe.it_f += (unsigned int)nb;
+    // the two kinds of partials are summed separately (each in an order that does not depend on R) and then added
+    double Gqv[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) Gqv[r] = (warp < W_CONS && quad_trial<R>(lane) == r) ? Gq : 0.0;
     block_sum_vec<R>(Gacc, h);   // producer lanes contribute 0
+    block_sum_vec<R>(Gqv, h);
+#pragma unroll
+    for (int r = 0; r < R; ++r) Gacc[r] += Gqv[r];
     if (threadIdx.x == 0 && blockIdx.x < P.grid_f) {
 #pragma unroll
         for (int r = 0; r < R; ++r) Gpart[blockIdx.x * R + r] = Gacc[r];
