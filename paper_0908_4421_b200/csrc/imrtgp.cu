@@ -86,7 +86,7 @@ struct Bump {                           // the same walk sizes the workspace and
 };
 
 struct Bounds {
-    int64_t max_blk, max_meta, max_ranges, max_slots, nnz_pad;
+    int64_t max_blk, max_meta, max_ranges, max_slots, nnz_pad, nnz_pack;
     size_t sort_temp, max_pack;
 };
 
@@ -99,6 +99,7 @@ Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     b.max_ranges = 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
     b.max_slots = n_b + b.max_ranges + 4;
     b.nnz_pad = ((nnz + 3) & ~(int64_t)3) + 8;
+    b.nnz_pack = nnz + 128 * n_b + 128;         // packed D^T: every row padded to a multiple of 128 entries
     b.sort_temp = (size_t)(16 << 20) + (size_t)nnz;
     return b;
 }
@@ -114,6 +115,10 @@ struct Layout {
     int* rowT_ptr;
     int* colT;
     float* valT;
+    float* valP;
+    unsigned short* idP;
+    unsigned int* baseP;
+    int* rowP_ptr;
     TrRange* tr_range;
     int* rowslot_ptr;
     float* xbuf[2];
@@ -155,6 +160,10 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.rowT_ptr = w.take<int>(n_b + 1);
     L.colT = w.take<int>(B.nnz_pad);
     L.valT = w.take<float>(B.nnz_pad);
+    L.valP = w.take<float>(B.nnz_pack);
+    L.idP = w.take<unsigned short>(B.nnz_pack);
+    L.baseP = w.take<unsigned int>(B.nnz_pack / 32 + 4);
+    L.rowP_ptr = w.take<int>(n_b + 1);
     L.tr_range = w.take<TrRange>(B.max_ranges);
     L.rowslot_ptr = w.take<int>(n_b + 1);
     for (int i = 0; i < 2; ++i) L.xbuf[i] = w.take<float>(n_b + 4);
@@ -330,6 +339,31 @@ __global__ void k_pack_blocks(const int4* __restrict__ pk, const uint32_t* __res
         }
         if (threadIdx.x < 4) val_o[(size_t)nbc * 4 + threadIdx.x] = 0.0f;   // the zero column
         if (threadIdx.x < 8) col_o[nbc + threadIdx.x] = 0;
+    }
+}
+
+// The packed D^T stream: one warp per aligned group of 32 entries of the padded stream.  Entries past the end of a row
+// repeat its last voxel with value 0.  flags[2] is raised when a group spans more than 65535 voxels (no 16-bit form).
+__global__ void k_pack_transpose(const int* __restrict__ rowT_ptr, const int* __restrict__ rowP_ptr, const int* __restrict__ colT,
+                                 const float* __restrict__ valT, int n_b, long long n_groups, float* valP, unsigned short* idP,
+                                 unsigned int* baseP, int* flags) {
+    const int lane = threadIdx.x & 31;
+    for (long long t = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; t < n_groups; t += ((long long)gridDim.x * blockDim.x) >> 5) {
+        const int e = (int)(t * 32);
+        int lo = 0, hi = n_b;          // the row holding packed position e: largest i with rowP_ptr[i] <= e
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (rowP_ptr[mid] <= e) lo = mid; else hi = mid - 1;
+        }
+        const int k = e - rowP_ptr[lo] + lane, len = rowT_ptr[lo + 1] - rowT_ptr[lo];
+        const int src = rowT_ptr[lo] + min(k, len - 1);
+        const int id = len > 0 ? colT[src] : 0;
+        const float v = k < len ? valT[src] : 0.0f;
+        const int base = __shfl_sync(0xffffffffu, id, 0);
+        if (id - base > 65535) flags[2] = 1;
+        valP[e + lane] = v;
+        idP[e + lane] = (unsigned short)(id - base);
+        if (lane == 0) baseP[t] = (unsigned int)base;
     }
 }
 
@@ -544,13 +578,13 @@ void partition_blocks(const std::vector<double>& cost, int grid, std::vector<int
 }
 
 // Equal-nnz ranges of the D^T stream, each spanning at most RL_MAX rows, and the gradient partial slots.
-void build_ranges(const std::vector<int>& rpT, int n_b, int n_sm, std::vector<TrRange>& ranges, std::vector<int>& rowslot_ptr) {
+void build_ranges(const std::vector<int>& rpT, int n_b, int n_sm, int align, std::vector<TrRange>& ranges, std::vector<int>& rowslot_ptr) {
     const long long nnz = rpT[n_b];
     ranges.clear();
     rowslot_ptr.assign(n_b + 1, 0);
     if (nnz == 0) return;
     long long per = (nnz + n_sm - 1) / n_sm;
-    per = (per + 3) & ~3LL;
+    per = (per + align - 1) / align * align;
     std::vector<int> cnt(n_b, 0);
     long long e = 0;
     int row = 0, slot = 0;
@@ -895,7 +929,20 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     // ---- transpose-pass ranges and gradient slots
     std::vector<TrRange> ranges;
     std::vector<int> rowslot;
-    build_ranges(rpT, (int)n_b, n_sm, ranges, rowslot);
+    // ---- the packed stream the transpose pass reads (16-bit voxel offsets), unless a group of 32 entries is too wide
+    bool id16 = nnz > 0 && !getenv("IMRTGP_NO_ID16") && nnz + 128 * n_b + 128 < (1LL << 31);
+    std::vector<int> rpP((size_t)n_b + 1, 0);
+    if (id16) {
+        for (int64_t i = 0; i < n_b; ++i) rpP[i + 1] = rpP[i] + ((rpT[i + 1] - rpT[i] + 127) & ~127);
+        const long long n_groups = rpP[n_b] / 32;
+        CUDA_TRY(pl, cudaMemcpyAsync(L.rowP_ptr, rpP.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
+        if (n_groups > 0) k_pack_transpose<<<grid_for(n_groups * 32, 256), 256, 0, st>>>(L.rowT_ptr, L.rowP_ptr, L.colT, L.valT, (int)n_b, n_groups, L.valP, L.idP, L.baseP, L.flags);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        if (flags_h[2]) id16 = false;
+    }
+    build_ranges(id16 ? rpP : rpT, (int)n_b, n_sm, id16 ? 128 : 4, ranges, rowslot);
     if ((int64_t)ranges.size() > B.max_ranges) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: %zu transpose ranges exceed the bound", ranges.size());
     const int n_slots = rowslot[n_b];
     if (!ranges.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.tr_range, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
@@ -910,6 +957,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     int R = prm->ls_batch == 0 ? R_MAX : prm->ls_batch;
     if (getenv("IMRTGP_LS_BATCH")) R = atoi(getenv("IMRTGP_LS_BATCH"));
     if (R != 1 && R != 2 && R != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_params.ls_batch must be 0, 1, 2 or 4");
+    const int stage_t = id16 ? CHUNK_T * 6 + CHUNK_T / 8 : STAGE_T_BYTES;
     int off = 0, avail = 0, stt = 0;
     for (;; R /= 2) {
         off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
@@ -921,7 +969,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         P.stage_off = off;
         avail = smem_optin - off;
         avail = (smem_optin - off) & ~127;
-        stt = avail > 0 ? std::min(MAX_STAGES_T, avail / STAGE_T_BYTES) : 0;
+        stt = avail > 0 ? std::min(MAX_STAGES_T, avail / stage_t) : 0;
         if (R == 1 || (avail >= 2 * max_rec && avail >= (W_CONS / 2) * avg_rec && stt >= 3)) break;
     }
     if (avail < 2 * max_rec || stt < 2)
@@ -934,7 +982,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
     P.pack = L.pack; P.blk = L.blk; P.cta_blk = L.cta_blk; P.grid_f = grid_f;
     P.col16 = col16 ? 1 : 0;
-    P.rowT_ptr = L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
+    P.rowT_ptr = id16 ? L.rowP_ptr : L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
+    P.valP = L.valP; P.idP = L.idP; P.baseP = L.baseP; P.id16 = id16 ? 1 : 0; P.stage_t_bytes = stage_t;
     P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr;
     P.n_ranges = (int)ranges.size(); P.grid_t = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, ranges.size()));
     P.n_stages_t = stt; P.n_slots = n_slots;

@@ -121,10 +121,18 @@ struct DevPlan {
     int col16;                 // 1: 16-bit column indices in the records
     int R;                     // trial points per dose pass of the line search (1, 2 or 4)
     int pad1;
-    // D^T (owned): CSR, rows = beamlets, padded with zeros to a multiple of 4 entries
-    const int* rowT_ptr;
+    // D^T (owned): CSR, rows = beamlets, padded with zeros to a multiple of 4 entries ...
+    const int* rowT_ptr;       // row pointers of the stream the transpose pass reads (the packed one when id16)
     const int* colT;
     const float* valT;
+    // ... and, unless a row has neighbouring entries more than 65535 voxels apart, the packed stream the transpose
+    // pass reads instead (id16 = 1): every row padded to a multiple of 128 entries (zero values), voxel ids as
+    // 16-bit offsets from one 32-bit base per aligned group of 32 entries: 6.1 instead of 8 bytes per non-zero
+    const float* valP;
+    const unsigned short* idP;
+    const unsigned int* baseP;
+    int id16;
+    int stage_t_bytes;         // bytes of one transpose-pass stage
     // transpose pass: equal-nnz ranges
     const TrRange* tr_range;
     const int* rowslot_ptr;    // [n_b + 1] slots of row i are [rowslot_ptr[i], rowslot_ptr[i+1])
@@ -597,7 +605,8 @@ __device__ __forceinline__ void reduce_objective(const DevPlan& P, const double*
 // Streams equal-nnz ranges of D^T; every consumer warp owns a contiguous slice of each stage, gathers r, and keeps
 // an fp64 running sum per row of D^T; per (warp,row) sums meet in shared memory and leave as one fp64 partial
 // per (range,row) slot.  All NTHREADS threads call this.  Ends with a CTA-wide barrier.
-__device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
+template <bool ID16>
+__device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
                                                const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = P.n_stages_t;
@@ -616,13 +625,23 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
                     mbar_wait(&h->empty_t[s], ph ^ 1u);
                     int n = e1 - cs;
                     n = n > CHUNK_T ? CHUNK_T : n;
-                    const int shift = e0 & 3;   // 16-byte source alignment: start the copy up to 3 entries early
-                    const uint32_t bytes = (uint32_t)((n + shift + 3) & ~3) * 4u;   // D^T is padded: always in bounds
-                    int* col_s = reinterpret_cast<int*>(stages + (size_t)s * STAGE_T_BYTES);
-                    float* val_s = reinterpret_cast<float*>(col_s + CHUNK_T_PAD);
-                    mbar_expect_tx(&h->full_t[s], 2u * bytes);
-                    bulk_g2s(col_s, P.colT + (cs - shift), bytes, &h->full_t[s], pol);
-                    bulk_g2s(val_s, P.valT + (cs - shift), bytes, &h->full_t[s], pol);
+                    unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
+                    if (ID16) {
+                        // packed stream: rows padded to 128 entries, so n is a multiple of 128 and everything is aligned;
+                        // stage = values | 16-bit voxel offsets | one 32-bit base per 32 entries
+                        mbar_expect_tx(&h->full_t[s], (uint32_t)n * 6u + (uint32_t)n / 8u);
+                        bulk_g2s(st, P.valP + cs, (uint32_t)n * 4u, &h->full_t[s], pol);
+                        bulk_g2s(st + CHUNK_T * 4, P.idP + cs, (uint32_t)n * 2u, &h->full_t[s], pol);
+                        bulk_g2s(st + CHUNK_T * 6, P.baseP + cs / 32, (uint32_t)n / 8u, &h->full_t[s], pol);
+                    } else {
+                        const int shift = e0 & 3;   // 16-byte source alignment: start the copy up to 3 entries early
+                        const uint32_t bytes = (uint32_t)((n + shift + 3) & ~3) * 4u;   // D^T is padded: always in bounds
+                        int* col_s = reinterpret_cast<int*>(st);
+                        float* val_s = reinterpret_cast<float*>(col_s + CHUNK_T_PAD);
+                        mbar_expect_tx(&h->full_t[s], 2u * bytes);
+                        bulk_g2s(col_s, P.colT + (cs - shift), bytes, &h->full_t[s], pol);
+                        bulk_g2s(val_s, P.valT + (cs - shift), bytes, &h->full_t[s], pol);
+                    }
                     if (++s == S) { s = 0; ph ^= 1u; }
                 }
             }
@@ -644,8 +663,12 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
             bool touched = false;
             for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
                 mbar_wait(&h->full_t[s], ph);
-                const int* col_s = reinterpret_cast<const int*>(stages + (size_t)s * STAGE_T_BYTES) + (R.e_begin & 3);
-                const float* val_s = reinterpret_cast<const float*>(stages + (size_t)s * STAGE_T_BYTES) + CHUNK_T_PAD + (R.e_begin & 3);
+                const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
+                const int* col_s = reinterpret_cast<const int*>(st) + (R.e_begin & 3);
+                const float* val_s = ID16 ? reinterpret_cast<const float*>(st)
+                                          : reinterpret_cast<const float*>(st) + CHUNK_T_PAD + (R.e_begin & 3);
+                const unsigned short* id_s = reinterpret_cast<const unsigned short*>(st + CHUNK_T * 4);
+                const unsigned int* base_s = reinterpret_cast<const unsigned int*>(st + CHUNK_T * 6);
                 const int ce = min(cs + CHUNK_T, R.e_end);
                 int pos = cs + warp * SLICE_T;
                 const int b = min(pos + SLICE_T, ce);
@@ -664,7 +687,24 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
                     const int* cp = col_s + (pos - cs);
                     const float* vp = val_s + (pos - cs);
                     float acc = 0.0f;
-                    if (seg_end - pos == SLICE_T) {
+                    if (ID16) {
+                        // pos and seg_end are multiples of 32 (rows are padded): whole 32-entry tiles, one base each
+                        const unsigned short* ip = id_s + (pos - cs);
+                        const unsigned int* bp = base_s + (pos - cs) / 32;
+                        const int nt = (seg_end - pos) / 32;
+                        if (nt == SLICE_T / 32) {
+                            unsigned int c[SLICE_T / 32];
+                            float rr[SLICE_T / 32];
+#pragma unroll
+                            for (int u = 0; u < SLICE_T / 32; ++u) c[u] = bp[u] + ip[lane + 32 * u];
+#pragma unroll
+                            for (int u = 0; u < SLICE_T / 32; ++u) rr[u] = ld_keep(r_in + c[u], keep);
+#pragma unroll
+                            for (int u = 0; u < SLICE_T / 32; ++u) acc = fmaf(vp[lane + 32 * u], rr[u], acc);
+                        } else {
+                            for (int u = 0; u < nt; ++u) acc = fmaf(vp[lane + 32 * u], ld_keep(r_in + (bp[u] + ip[lane + 32 * u]), keep), acc);
+                        }
+                    } else if (seg_end - pos == SLICE_T) {
                         int c[SLICE_T / 32];
                         float rr[SLICE_T / 32];
 #pragma unroll
@@ -705,6 +745,12 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
         P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
         P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
     }
+}
+
+__device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
+                                               const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
+    if (P.id16) transpose_pass_t<true>(P, h, smem, wpart, r_in, gslot, pipe);
+    else transpose_pass_t<false>(P, h, smem, wpart, r_in, gslot, pipe);
 }
 
 // g_i = sum of the slots of row i, in slot order (fixed).  All NTHREADS threads; g_out shared or global.
