@@ -970,7 +970,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         avail = smem_optin - off;
         avail = (smem_optin - off) & ~127;
         stt = avail > 0 ? std::min(MAX_STAGES_T, avail / stage_t) : 0;
-        if (R == 1 || (avail >= 2 * max_rec && avail >= (W_CONS / 2) * avg_rec && stt >= 3)) break;
+        if (R == 1 || (avail >= 2 * max_rec && avail >= (W_CONS / 2) * avg_rec && stt >= 2)) break;
     }
     if (avail < 2 * max_rec || stt < 2)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "n_b = %lld beamlets and records of up to %d bytes do not fit in shared memory", (long long)n_b, max_rec);

@@ -49,7 +49,8 @@ constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
 constexpr int R_MAX = 4;                      // line-search trial points evaluated per dose pass (1, 2 or 4)
 constexpr int CHUNK_T = 4096;                 // nnz per transpose-pass stage (pure streaming)
-constexpr int SLICE_T = CHUNK_T / W_CONS;     // contiguous nnz per consumer warp per stage
+constexpr int TGROUPS = 2;                    // the consumer warps take the stages in turns, in this many groups:
+constexpr int SLICE_T = CHUNK_T / (W_CONS / TGROUPS);   // contiguous nnz per warp of a stage's group (gathers in flight)
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
 constexpr int RL_MAX = 32;                    // rows of D^T one transpose range may span
@@ -190,7 +191,7 @@ __device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4
         for (int s = 0; s < RING_ENTRIES; ++s) mbar_init(&h->full_f[s], 1);
         for (int s = 0; s < MAX_STAGES_T; ++s) {
             mbar_init(&h->full_t[s], 1);
-            mbar_init(&h->empty_t[s], W_CONS);
+            mbar_init(&h->empty_t[s], W_CONS / TGROUPS);
         }
         mbar_fence_init();
     }
@@ -662,6 +663,10 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
             double dacc = 0.0;
             bool touched = false;
             for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
+                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage
+                    if (++s == S) { s = 0; ph ^= 1u; }
+                    continue;
+                }
                 mbar_wait(&h->full_t[s], ph);
                 const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
                 const int* col_s = reinterpret_cast<const int*>(st) + (R.e_begin & 3);
@@ -670,7 +675,7 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
                 const unsigned short* id_s = reinterpret_cast<const unsigned short*>(st + CHUNK_T * 4);
                 const unsigned int* base_s = reinterpret_cast<const unsigned int*>(st + CHUNK_T * 6);
                 const int ce = min(cs + CHUNK_T, R.e_end);
-                int pos = cs + warp * SLICE_T;
+                int pos = cs + (warp % (W_CONS / TGROUPS)) * SLICE_T;
                 const int b = min(pos + SLICE_T, ce);
                 while (pos < b) {
                     while (cur_end <= pos) {   // the slice moved past the end of the current row (warp-uniform)
