@@ -34,6 +34,13 @@ struct imrt_plan {
     std::vector<double> blk_cost;     // modelled, then measured, cost of every dose-pass block (host)
     int* cta_blk_w;
     int4* blk_w;
+    std::vector<int> rp_tr;           // row pointers of the stream the transpose pass reads (host copy)
+    std::vector<double> tr_share;     // share of that stream per CTA
+    int tr_align;
+    int64_t max_ranges, max_slots;
+    TrRange* tr_range_w;
+    int* rowslot_w;
+    int* cta_rng_w;
     double tune_spread[2];            // slowest / mean CTA time of the dose pass before and after tuning
     // borrowed inputs
     const int32_t* row_ptr;
@@ -96,7 +103,7 @@ Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     b.max_blk = 4 * (slots / MIN_CHUNK_SLOTS + 1) + 4 * (n_v / SEG_ROWS + 1) + n_v / 16 + 8;
     b.max_meta = n_v + b.max_blk * (META_HDR + 2 + 3) + 8;
     b.max_pack = (size_t)b.max_meta * 4 + (size_t)slots * 8 + (size_t)b.max_blk * (128 + 48) + 256;
-    b.max_ranges = 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
+    b.max_ranges = 2 * 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
     b.max_slots = n_b + b.max_ranges + 4;
     b.nnz_pad = ((nnz + 3) & ~(int64_t)3) + 8;
     b.nnz_pack = nnz + 128 * n_b + 128;         // packed D^T: every row padded to a multiple of 128 entries
@@ -121,6 +128,7 @@ struct Layout {
     int* rowP_ptr;
     TrRange* tr_range;
     int* rowslot_ptr;
+    int* cta_rng;
     float* xbuf[2];
     float* g;
     float* rbuf[R_MAX + 1];
@@ -166,6 +174,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.rowP_ptr = w.take<int>(n_b + 1);
     L.tr_range = w.take<TrRange>(B.max_ranges);
     L.rowslot_ptr = w.take<int>(n_b + 1);
+    L.cta_rng = w.take<int>(1024 + 1);
     for (int i = 0; i < 2; ++i) L.xbuf[i] = w.take<float>(n_b + 4);
     L.g = w.take<float>(n_b + 4);
     for (int i = 0; i <= R_MAX; ++i) L.rbuf[i] = w.take<float>(n_v + 4);
@@ -578,34 +587,43 @@ void partition_blocks(const std::vector<double>& cost, int grid, std::vector<int
 }
 
 // Equal-nnz ranges of the D^T stream, each spanning at most RL_MAX rows, and the gradient partial slots.
-void build_ranges(const std::vector<int>& rpT, int n_b, int n_sm, int align, std::vector<TrRange>& ranges, std::vector<int>& rowslot_ptr) {
+// One contiguous, `align`-aligned share of the D^T stream per CTA -- share[c] of the total, equal shares unless plan
+// creation has measured otherwise -- cut into ranges of at most RL_MAX rows, and the gradient partial slots.
+void build_ranges(const std::vector<int>& rpT, int n_b, const std::vector<double>& share, int align, std::vector<TrRange>& ranges,
+                  std::vector<int>& rowslot_ptr, std::vector<int>& cta_rng) {
     const long long nnz = rpT[n_b];
+    const int grid = (int)share.size();
     ranges.clear();
     rowslot_ptr.assign(n_b + 1, 0);
+    cta_rng.assign(grid + 1, 0);
     if (nnz == 0) return;
-    long long per = (nnz + n_sm - 1) / n_sm;
-    per = (per + align - 1) / align * align;
     std::vector<int> cnt(n_b, 0);
     long long e = 0;
     int row = 0, slot = 0;
-    while (e < nnz) {
-        while (rpT[row + 1] <= e) ++row;
-        TrRange R;
-        memset(&R, 0, sizeof R);
-        R.e_begin = (int)e;
-        R.first_row = row;
-        long long e_end = std::min(nnz, e + per);
-        e_end = std::min<long long>(e_end, rpT[std::min(n_b, row + RL_MAX)]);
-        R.e_end = (int)e_end;
-        int last = row;
-        while (rpT[last + 1] < e_end) ++last;
-        R.n_rows = last - row + 1;
-        R.slot_base = slot;
-        for (int i = row; i <= last; ++i) ++cnt[i];
-        slot += R.n_rows;
-        ranges.push_back(R);
-        e = e_end;
+    double cum = 0.0;
+    for (int c = 0; c < grid; ++c) {
+        cta_rng[c] = (int)ranges.size();
+        cum += share[c];
+        long long stop = c == grid - 1 ? nnz : std::min<long long>(nnz, (long long)(cum * (double)nnz / align + 0.5) * align);
+        while (e < stop) {
+            while (rpT[row + 1] <= e) ++row;
+            TrRange R;
+            memset(&R, 0, sizeof R);
+            R.e_begin = (int)e;
+            R.first_row = row;
+            const long long e_end = std::min<long long>(stop, rpT[std::min(n_b, row + RL_MAX)]);
+            R.e_end = (int)e_end;
+            int last = row;
+            while (rpT[last + 1] < e_end) ++last;
+            R.n_rows = last - row + 1;
+            R.slot_base = slot;
+            for (int i = row; i <= last; ++i) ++cnt[i];
+            slot += R.n_rows;
+            ranges.push_back(R);
+            e = e_end;
+        }
     }
+    cta_rng[grid] = (int)ranges.size();
     for (int i = 0; i < n_b; ++i) rowslot_ptr[i + 1] = rowslot_ptr[i] + cnt[i];
 }
 
@@ -642,6 +660,45 @@ static imrt_status upload_partition(imrt_plan* pl, const std::vector<int>& cta_b
     k_ring_layout<<<(pl->P.grid_f + 127) / 128, 128, 0, st>>>(pl->blk_w, pl->cta_blk_w, pl->P.grid_f, (unsigned int)pl->P.ring_f_bytes);
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));   // cta_blk is a host vector the caller may drop
+    return IMRT_STATUS_OK;
+}
+
+// The same for the transpose pass: equal shares of the D^T stream do not take equal time (the gathers of r hit the L2
+// differently from SM to SM), so measure every CTA's pass time and hand out shares in proportion to measured speed.
+static imrt_status tune_transpose(imrt_plan* pl) {
+    const int grid = pl->P.grid_t, n_b = pl->P.n_b;
+    if (getenv("IMRTGP_NO_TUNE") || grid < 2 || pl->rp_tr[n_b] < (long long)grid * 8 * CHUNK_T) return IMRT_STATUS_OK;
+    cudaStream_t st = pl->stream;
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_EVAL;
+    A.r_in = pl->P.rbuf[0];
+    A.g_out = pl->g_scratch;
+    std::vector<unsigned long long> t(2 * (size_t)grid);
+    std::vector<TrRange> ranges;
+    std::vector<int> rowslot, cta_rng;
+    for (int it = 0; it < 4; ++it) {
+        for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_transpose(pl, A));   // the first warms up, the second is read
+        CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns + 2048, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        double sum = 0.0;
+        std::vector<double> share(grid);
+        for (int c = 0; c < grid; ++c) {
+            const double dur = (double)(t[2 * c + 1] - t[2 * c]);
+            share[c] = dur > 0.0 ? pl->tr_share[c] / dur : pl->tr_share[c];     // share per unit time = speed
+            sum += share[c];
+        }
+        for (int c = 0; c < grid; ++c) share[c] /= sum;
+        build_ranges(pl->rp_tr, n_b, share, pl->tr_align, ranges, rowslot, cta_rng);
+        if ((int64_t)ranges.size() > pl->max_ranges || rowslot[n_b] + 4 > pl->max_slots) break;   // keep the last good schedule
+        pl->tr_share = share;
+        CUDA_TRY(pl, cudaMemcpyAsync(pl->tr_range_w, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaMemcpyAsync(pl->rowslot_w, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_rng_w, cta_rng.data(), sizeof(int) * cta_rng.size(), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        pl->P.n_ranges = (int)ranges.size();
+        pl->P.n_slots = rowslot[n_b];
+    }
     return IMRT_STATUS_OK;
 }
 
@@ -928,7 +985,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
 
     // ---- transpose-pass ranges and gradient slots
     std::vector<TrRange> ranges;
-    std::vector<int> rowslot;
+    std::vector<int> rowslot, cta_rng_h;
     // ---- the packed stream the transpose pass reads (16-bit voxel offsets), unless a group of 32 entries is too wide
     bool id16 = nnz > 0 && !getenv("IMRTGP_NO_ID16") && nnz + 128 * n_b + 128 < (1LL << 31);
     std::vector<int> rpP((size_t)n_b + 1, 0);
@@ -942,11 +999,18 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaStreamSynchronize(st));
         if (flags_h[2]) id16 = false;
     }
-    build_ranges(id16 ? rpP : rpT, (int)n_b, n_sm, id16 ? 128 : 4, ranges, rowslot);
+    pl->rp_tr = id16 ? rpP : rpT;
+    pl->tr_align = id16 ? 128 : 4;
+    const int grid_t = (int)std::max<long long>(1, std::min<long long>(n_sm, (long long)pl->rp_tr[n_b] / (4 * CHUNK_T) + 1));
+    pl->tr_share.assign(grid_t, 1.0 / grid_t);
+    build_ranges(pl->rp_tr, (int)n_b, pl->tr_share, pl->tr_align, ranges, rowslot, cta_rng_h);
     if ((int64_t)ranges.size() > B.max_ranges) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: %zu transpose ranges exceed the bound", ranges.size());
     const int n_slots = rowslot[n_b];
     if (!ranges.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.tr_range, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
     CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(L.cta_rng, cta_rng_h.data(), sizeof(int) * cta_rng_h.size(), cudaMemcpyHostToDevice, st));
+    pl->max_ranges = B.max_ranges; pl->max_slots = B.max_slots;
+    pl->tr_range_w = L.tr_range; pl->rowslot_w = L.rowslot_ptr; pl->cta_rng_w = L.cta_rng;
 
     // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, dose
     // scratch, the R trial points, g, then the ring (dose pass) / stages (transpose pass).  R = the largest of 4, 2, 1
@@ -984,8 +1048,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.col16 = col16 ? 1 : 0;
     P.rowT_ptr = id16 ? L.rowP_ptr : L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
     P.valP = L.valP; P.idP = L.idP; P.baseP = L.baseP; P.id16 = id16 ? 1 : 0; P.stage_t_bytes = stage_t;
-    P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr;
-    P.n_ranges = (int)ranges.size(); P.grid_t = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, ranges.size()));
+    P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr; P.cta_rng = L.cta_rng;
+    P.n_ranges = (int)ranges.size(); P.grid_t = grid_t;
     P.n_stages_t = stt; P.n_slots = n_slots;
     P.table = L.table; P.n_structures = n_structures; P.G_skip = G_skip;
     P.xbuf[0] = L.xbuf[0]; P.xbuf[1] = L.xbuf[1]; P.g = L.g;
@@ -1029,6 +1093,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     s = upload_partition(pl, cta_blk);
     if (s != IMRT_STATUS_OK) return s;
     s = tune_partition(pl);
+    if (s != IMRT_STATUS_OK) return s;
+    s = tune_transpose(pl);
     if (s != IMRT_STATUS_OK) return s;
     if (prm->driver == 0) {
         s = build_graph(pl);

@@ -137,6 +137,7 @@ struct DevPlan {
     // transpose pass: equal-nnz ranges
     const TrRange* tr_range;
     const int* rowslot_ptr;    // [n_b + 1] slots of row i are [rowslot_ptr[i], rowslot_ptr[i+1])
+    const int* cta_rng;        // [grid_t + 1] ranges of CTA c are [cta_rng[c], cta_rng[c+1])
     int n_ranges, grid_t, n_stages_t, n_slots;
     // penalty table and skipped (matrix-free) rows
     const float4* table;       // (t_under, t_over, w_under, w_over)
@@ -613,6 +614,8 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
     const int S = P.n_stages_t;
     unsigned char* stages = smem + P.stage_off;
     unsigned int it = pipe.it_t;
+    const int rg0 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x] : 0;       // this CTA's ranges
+    const int rg1 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x + 1] : 0;
     const unsigned long long t_start = global_ns();
     int s = (int)(it % (unsigned int)S);
     unsigned int ph = (it / (unsigned int)S) & 1u;
@@ -620,7 +623,7 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
     if (warp == W_CONS) {
         const uint64_t pol = policy_evict_first();
         if (lane == 0) {
-            for (int rg = blockIdx.x; rg < P.n_ranges; rg += gridDim.x) {
+            for (int rg = rg0; rg < rg1; ++rg) {
                 const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
                 for (int cs = e0; cs < e1; cs += CHUNK_T, ++it) {
                     mbar_wait(&h->empty_t[s], ph ^ 1u);
@@ -647,14 +650,14 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
                 }
             }
         } else {
-            for (int rg = blockIdx.x; rg < P.n_ranges; rg += gridDim.x) {
+            for (int rg = rg0; rg < rg1; ++rg) {
                 const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
                 it += (unsigned int)((e1 - e0 + CHUNK_T - 1) / CHUNK_T);
             }
         }
     } else {
         const uint64_t keep = policy_evict_last();
-        for (int rg = blockIdx.x; rg < P.n_ranges; rg += gridDim.x) {
+        for (int rg = rg0; rg < rg1; ++rg) {
             const TrRange R = P.tr_range[rg];
             for (int i = threadIdx.x; i < RL_MAX * W_CONS; i += N_CONS) wpart[i] = 0.0;
             named_bar_sync(1, N_CONS);
