@@ -677,7 +677,7 @@ static imrt_status tune_transpose(imrt_plan* pl) {
     std::vector<unsigned long long> t(2 * (size_t)grid);
     std::vector<TrRange> ranges;
     std::vector<int> rowslot, cta_rng;
-    for (int it = 0; it < 4; ++it) {
+    for (int it = 0; it < 6; ++it) {
         for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_transpose(pl, A));   // the first warms up, the second is read
         CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns + 2048, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(pl, cudaStreamSynchronize(st));

@@ -31,12 +31,13 @@ constexpr int W_CONS = 16;                    // consumer warps per CTA
 #define IMRT_TEAM 1
 #endif
 #ifndef IMRT_QUAD_CAP
-#define IMRT_QUAD_CAP 512
+#define IMRT_QUAD_CAP 384
 #endif
 constexpr int TEAM = IMRT_TEAM;               // consumer warps that work on one dose-pass record together
 constexpr int N_TEAMS = W_CONS / TEAM;
 constexpr int N_CONS = W_CONS * 32;           // consumer threads
-constexpr int NTHREADS = N_CONS + 32;         // + one producer warp
+constexpr int N_PROD = 2;                     // producer warps of the dose pass (the transpose pass uses the first only)
+constexpr int NTHREADS = N_CONS + 32 * N_PROD;
 // dose pass: D is re-packed once into self-contained block records (one bulk copy each, see DevPlan::pack)
 constexpr int META_HDR = 4;                   // header words {rows, first row, 0, slots}
 constexpr int MIN_CHUNK_SLOTS = 1024;         // slot capacity of a block unless a longer row forces more
@@ -253,15 +254,28 @@ __device__ __forceinline__ void trial_batch(const float* x, const float* g, doub
     double l = lambda;
 #pragma unroll
     for (int r = 0; r < R; ++r) { lam[r] = (float)l; l = l / alpha; step_sq[r] = 0.0; }
-    for (int i = threadIdx.x; i < n_b; i += NTHREADS) {
-        const float xi = __ldcg(x + i), gi = g[i];
-        float* o = xs + (size_t)i * R;
+    constexpr int U = 4;         // rows per thread whose loads are issued together (x comes from L2)
+    for (int base = threadIdx.x; base < n_b; base += NTHREADS * U) {
+        float xv[U], gv[U];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float xn = fmaxf(0.0f, fmaf(-lam[r], gi, xi));
-            const float dx = xn - xi;
-            step_sq[r] = __fma_rn((double)dx, (double)dx, step_sq[r]);
-            o[r] = xn;
+        for (int u = 0; u < U; ++u) {
+            const int i = base + u * NTHREADS;
+            xv[u] = i < n_b ? __ldcg(x + i) : 0.0f;
+            gv[u] = i < n_b ? g[i] : 0.0f;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int i = base + u * NTHREADS;
+            if (i < n_b) {
+                float* o = xs + (size_t)i * R;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float xn = fmaxf(0.0f, fmaf(-lam[r], gv[u], xv[u]));
+                    const float dx = xn - xv[u];
+                    step_sq[r] = __fma_rn((double)dx, (double)dx, step_sq[r]);
+                    o[r] = xn;
+                }
+            }
         }
     }
     block_sum_vec<R>(step_sq, h);
@@ -507,28 +521,32 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
     // barrier is always a block the same warps have already finished.  Space is reclaimed in issue order: every
     // consumer warp publishes the number of the next block it will finish, and the minimum over the warps bounds
     // the blocks that are gone.
-    if (warp == W_CONS) {
-        // ---------------- producer warp: lane 0 drives the TMA unit, one bulk copy per block record; the
-        // descriptors of the next 32 blocks are requested before the current 32 are issued
+    if (warp >= W_CONS) {
+        // ---------------- producer warps: producer p issues the CTA's blocks p, p + N_PROD, ... (lane 0 drives the TMA
+        // unit, one bulk copy per block record); the descriptors of its next 32 blocks are requested before the current
+        // 32 are issued
+        const int pw = warp - W_CONS;
         const uint64_t pol = policy_evict_first();   // streamed once per pass: keep it from pushing r / x out of L2
         unsigned int gone = it0;                       // every block numbered below this has been consumed
-        int4 next = (lane < nb) ? __ldg(P.blk + b0 + lane) : make_int4(0, 0, 0, 0);
-        for (int bb = 0; bb < nb; bb += 32) {
+        int4 next = (pw + N_PROD * lane < nb) ? __ldg(P.blk + b0 + pw + N_PROD * lane) : make_int4(0, 0, 0, 0);
+        for (int bb = pw; bb < nb; bb += 32 * N_PROD) {
             const int4 mine = next;
-            next = (bb + 32 + lane < nb) ? __ldg(P.blk + b0 + bb + 32 + lane) : make_int4(0, 0, 0, 0);
-            const int nb_here = min(32, nb - bb);
+            next = (bb + N_PROD * (32 + lane) < nb) ? __ldg(P.blk + b0 + bb + N_PROD * (32 + lane)) : make_int4(0, 0, 0, 0);
+            const int nb_here = min(32, (nb - bb + N_PROD - 1) / N_PROD);
             for (int j = 0; j < nb_here; ++j) {
                 const int off128 = __shfl_sync(0xffffffffu, mine.x, j);
                 const uint32_t bytes = (uint32_t)__shfl_sync(0xffffffffu, mine.y, j);
                 const uint32_t at = (uint32_t)__shfl_sync(0xffffffffu, mine.z, j);
                 const unsigned int need = it0 + (unsigned int)__shfl_sync(0xffffffffu, mine.w, j);
-                while ((int)(need - gone) > 0) {
-                    const unsigned int v = next_blk[lane & (W_CONS - 1)];
-                    gone = __reduce_min_sync(0xffffffffu, v - it0) + it0;     // numbers wrap: compare relative to it0
+                if ((int)(need - gone) > 0) {
+                    do {
+                        const unsigned int v = next_blk[lane & (W_CONS - 1)];
+                        gone = __reduce_min_sync(0xffffffffu, v - it0) + it0;     // numbers wrap: compare relative to it0
+                    } while ((int)(need - gone) > 0);
+                    __threadfence_block();   // the consumers' reads of the space (seen through next_blk) come first
                 }
                 if (lane == 0) {
-                    __threadfence_block();   // the consumers' reads of the space (seen through next_blk) come first
-                    const uint32_t bar = full_a + 8u * ((it0 + (unsigned int)(bb + j)) & (RING_ENTRIES - 1));
+                    const uint32_t bar = full_a + 8u * ((it0 + (unsigned int)(bb + N_PROD * j)) & (RING_ENTRIES - 1));
                     mbar_expect_tx_a(bar, bytes);
                     bulk_g2s_a(ring_a + at, P.pack + (size_t)(unsigned int)off128 * 128u, bytes, bar, pol);
                 }
@@ -620,9 +638,9 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
     int s = (int)(it % (unsigned int)S);
     unsigned int ph = (it / (unsigned int)S) & 1u;
 
-    if (warp == W_CONS) {
+    if (warp >= W_CONS) {
         const uint64_t pol = policy_evict_first();
-        if (lane == 0) {
+        if (warp == W_CONS && lane == 0) {
             for (int rg = rg0; rg < rg1; ++rg) {
                 const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
                 for (int cs = e0; cs < e1; cs += CHUNK_T, ++it) {
@@ -763,11 +781,24 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
 
 // g_i = sum of the slots of row i, in slot order (fixed).  All NTHREADS threads; g_out shared or global.
 __device__ __forceinline__ void reduce_gradient(const DevPlan& P, const double* gslot, float* g_out) {
-    for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) {
-        const int s0 = __ldg(P.rowslot_ptr + i), s1 = __ldg(P.rowslot_ptr + i + 1);
-        double sum = 0.0;
-        for (int s = s0; s < s1; ++s) sum += __ldcg(gslot + s);
-        g_out[i] = (float)sum;
+    constexpr int U = 4;         // rows per thread whose loads are issued together (the slots come from L2)
+    for (int base = threadIdx.x; base < P.n_b; base += NTHREADS * U) {
+        int s0[U], s1[U];
+        double sum[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int i = base + u * NTHREADS;
+            s0[u] = i < P.n_b ? __ldg(P.rowslot_ptr + i) : 0;
+            s1[u] = i < P.n_b ? __ldg(P.rowslot_ptr + i + 1) : 0;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) sum[u] = s0[u] < s1[u] ? __ldcg(gslot + s0[u]) : 0.0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            for (int s = s0[u] + 1; s < s1[u]; ++s) sum[u] += __ldcg(gslot + s);     // same order as one plain loop
+            const int i = base + u * NTHREADS;
+            if (i < P.n_b) g_out[i] = (float)sum[u];
+        }
     }
 }
 
@@ -1076,11 +1107,17 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P) {
         grid_barrier(&st->gridbar, epoch);
         reduce_gradient(P, P.gslot[tpar], g_s);
         __syncthreads();
-        if (!begin_line_search(st, L, P.xbuf[L.xi], g_s, P.n_b, h)) break;   // x_k lives in global memory
-        int dec, j_acc;
+        // start of the line search (PAPER.md:109 step 2; the same decisions begin_line_search takes, with the first
+        // trial's Delta taken from the batch that is built anyway).  x_k lives in global memory.
+        L.tr += 1;
+        if (L.G_k == 0.0) { L.stop_reason = STOP_STATIONARY; break; }          // reading R4
+        L.lambda = st->lambda0;
+        L.m = 0;
+        int dec, j_acc = -1;
         for (;;) {
             double step_sq[R], G_new[R];
             trial_batch<R>(P.xbuf[L.xi], g_s, L.lambda, alpha, xs, P.n_b, h, step_sq);
+            if (L.m == 0 && step_sq[0] == 0.0) { L.stop_reason = STOP_STATIONARY; dec = DEC_REJECT_STOP; break; }   // reading R4
             __syncthreads();
             float* r_out[R];
 #pragma unroll
