@@ -663,8 +663,45 @@ static imrt_status upload_partition(imrt_plan* pl, const std::vector<int>& cta_b
     return IMRT_STATUS_OK;
 }
 
+// A short run of the device-resident loop from x = whatever xbuf[0] holds (zeros at plan creation), for its per-CTA
+// pass timers: inside the loop the passes follow each other without launch gaps and the SMs do not behave quite as
+// they do for an isolated launch, so the final rounds of both rebalancings are measured here.
+static imrt_status timing_loop_run(imrt_plan* pl) {
+    cudaStream_t st = pl->stream;
+    k_reset_state<<<1, 1, 0, st>>>(pl->P.st);
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_INIT;
+    CUDA_TRY(pl, launch_dose(pl, A));
+    k_set_target<<<1, 1, 0, st>>>(pl->P.st, 3, 0.0);
+    CUDA_TRY(pl, launch_persistent(pl));
+    k_reset_state<<<1, 1, 0, st>>>(pl->P.st);
+    CUDA_TRY(pl, cudaGetLastError());
+    return IMRT_STATUS_OK;
+}
+static bool can_time_in_loop(const imrt_plan* pl) { return pl->prm.max_iters >= 3 && !getenv("IMRTGP_NO_LOOP_TUNE"); }
+
 // The same for the transpose pass: equal shares of the D^T stream do not take equal time (the gathers of r hit the L2
 // differently from SM to SM), so measure every CTA's pass time and hand out shares in proportion to measured speed.
+// Cut the D^T stream into the given per-CTA shares and upload the schedule.  false: the tables would not fit.
+static imrt_status upload_shares(imrt_plan* pl, const std::vector<double>& share, bool& fits) {
+    const int n_b = pl->P.n_b;
+    cudaStream_t st = pl->stream;
+    std::vector<TrRange> ranges;
+    std::vector<int> rowslot, cta_rng;
+    build_ranges(pl->rp_tr, n_b, share, pl->tr_align, ranges, rowslot, cta_rng);
+    fits = (int64_t)ranges.size() <= pl->max_ranges && rowslot[n_b] + 4 <= pl->max_slots;
+    if (!fits) return IMRT_STATUS_OK;
+    pl->tr_share = share;
+    CUDA_TRY(pl, cudaMemcpyAsync(pl->tr_range_w, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(pl->rowslot_w, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_rng_w, cta_rng.data(), sizeof(int) * cta_rng.size(), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    pl->P.n_ranges = (int)ranges.size();
+    pl->P.n_slots = rowslot[n_b];
+    return IMRT_STATUS_OK;
+}
+
 static imrt_status tune_transpose(imrt_plan* pl) {
     const int grid = pl->P.grid_t, n_b = pl->P.n_b;
     if (getenv("IMRTGP_NO_TUNE") || grid < 2 || pl->rp_tr[n_b] < (long long)grid * 8 * CHUNK_T) return IMRT_STATUS_OK;
@@ -675,29 +712,38 @@ static imrt_status tune_transpose(imrt_plan* pl) {
     A.r_in = pl->P.rbuf[0];
     A.g_out = pl->g_scratch;
     std::vector<unsigned long long> t(2 * (size_t)grid);
-    std::vector<TrRange> ranges;
-    std::vector<int> rowslot, cta_rng;
-    for (int it = 0; it < 6; ++it) {
-        for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_transpose(pl, A));   // the first warms up, the second is read
+    const int iso_rounds = 3, rounds = iso_rounds + (can_time_in_loop(pl) ? 5 : 0);
+    double best_worst = 1e300;
+    std::vector<double> best_share;
+    for (int it = 0; it <= rounds; ++it) {
+        if (it < iso_rounds) {
+            for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_transpose(pl, A));   // the first warms up, the second is read
+        } else {
+            const imrt_status ls = timing_loop_run(pl);
+            if (ls != IMRT_STATUS_OK) return ls;
+        }
         CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns + 2048, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(pl, cudaStreamSynchronize(st));
-        double sum = 0.0;
+        double sum = 0.0, worst = 0.0;
         std::vector<double> share(grid);
         for (int c = 0; c < grid; ++c) {
             const double dur = (double)(t[2 * c + 1] - t[2 * c]);
+            worst = std::max(worst, dur);
             share[c] = dur > 0.0 ? pl->tr_share[c] / dur : pl->tr_share[c];     // share per unit time = speed
             sum += share[c];
         }
+        // keep the best schedule seen in the final kind of measurement (in the loop if possible, else isolated)
+        if (it >= (rounds > iso_rounds ? iso_rounds : 0) && worst < best_worst) { best_worst = worst; best_share = pl->tr_share; }
+        if (it == rounds) break;
         for (int c = 0; c < grid; ++c) share[c] /= sum;
-        build_ranges(pl->rp_tr, n_b, share, pl->tr_align, ranges, rowslot, cta_rng);
-        if ((int64_t)ranges.size() > pl->max_ranges || rowslot[n_b] + 4 > pl->max_slots) break;   // keep the last good schedule
-        pl->tr_share = share;
-        CUDA_TRY(pl, cudaMemcpyAsync(pl->tr_range_w, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(pl, cudaMemcpyAsync(pl->rowslot_w, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_rng_w, cta_rng.data(), sizeof(int) * cta_rng.size(), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
-        pl->P.n_ranges = (int)ranges.size();
-        pl->P.n_slots = rowslot[n_b];
+        bool fits = true;
+        const imrt_status us = upload_shares(pl, share, fits);
+        if (us != IMRT_STATUS_OK) return us;
+        if (!fits) break;      // keep the last good schedule
+    }
+    if (!best_share.empty() && best_share != pl->tr_share) {
+        bool fits = true;
+        return upload_shares(pl, best_share, fits);
     }
     return IMRT_STATUS_OK;
 }
@@ -719,9 +765,17 @@ static imrt_status tune_partition(imrt_plan* pl) {
     partition_blocks(pl->blk_cost, grid, cta_blk);
     std::vector<unsigned long long> t(2 * (size_t)grid);
     std::vector<double> dur(grid);
-    const int rounds = 5;
+    const int iso_rounds = 3;
+    const int rounds = iso_rounds + (can_time_in_loop(pl) ? 5 : 0);
+    double best_worst = 1e300;
+    std::vector<int> best_blk;
     for (int it = 0; it <= rounds; ++it) {
-        for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_dose(pl, A));   // the first warms up, the second is read
+        if (it < iso_rounds) {
+            for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_dose(pl, A));   // the first warms up, the second is read
+        } else {
+            const imrt_status ls = timing_loop_run(pl);
+            if (ls != IMRT_STATUS_OK) return ls;
+        }
         CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(pl, cudaStreamSynchronize(st));
         double mean = 0.0, worst = 0.0;
@@ -731,7 +785,8 @@ static imrt_status tune_partition(imrt_plan* pl) {
             worst = std::max(worst, dur[c]);
         }
         if (it == 0) pl->tune_spread[0] = worst / mean;
-        pl->tune_spread[1] = worst / mean;
+        // keep the best partition seen in the final kind of measurement (in the loop if possible, else isolated)
+        if (it >= (rounds > iso_rounds ? iso_rounds : 0) && worst < best_worst) { best_worst = worst; best_blk = cta_blk; pl->tune_spread[1] = worst / mean; }
         if (it == rounds) break;
         for (int c = 0; c < grid; ++c) {
             double sum = 0.0;
@@ -744,6 +799,7 @@ static imrt_status tune_partition(imrt_plan* pl) {
         const imrt_status us = upload_partition(pl, cta_blk);
         if (us != IMRT_STATUS_OK) return us;
     }
+    if (!best_blk.empty() && best_blk != cta_blk) return upload_partition(pl, best_blk);
     return IMRT_STATUS_OK;
 }
 
