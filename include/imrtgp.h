@@ -123,6 +123,16 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
 imrt_status imrt_plan_set_x(imrt_plan* plan, const float* x0);
 
 /*
+ * Optional per-voxel limits -- the paper's own model, in which T_j is the dose of the original plan in voxel j
+ * or the desired cumulative dose minus the dose already delivered:
+ *   u_j = max(0, t_under_v[j] - d_j),  o_j = max(0, d_j - t_over_v[j]);   the weights stay those of the voxel's structure.
+ * t_under_v, t_over_v: fp32 [n_v] (device, borrowed until the next call or imrt_plan_destroy); either may be NULL
+ * (= keep the structure's limit); both NULL returns to per-structure limits.  Invalidates the current iterate:
+ * call imrt_plan_set_x afterwards.  Asynchronous.
+ */
+imrt_status imrt_plan_set_voxel_limits(imrt_plan* plan, const float* t_under_v, const float* t_over_v);
+
+/*
  * Run n_iters more ACCEPTED gradient-projection iterations (steps 1-4 of PAPER.md:105-111, each with its own Armijo
  * line search) unless a STATIONARY / LINESEARCH_STALLED exit happens first.  No stop test (fixed-count mode).
  * Asynchronous: with driver = 0 this is one cudaGraphLaunch.  The trace must have room (max_iters).

@@ -42,6 +42,8 @@ def _load():
         lib = ctypes.CDLL(build())
         lib.oracle_eval.argtypes = [ctypes.c_int64] + [_P] * 12
         lib.oracle_eval.restype = None
+        lib.oracle_eval_v.argtypes = [ctypes.c_int64] + [_P] * 14
+        lib.oracle_eval_v.restype = None
         lib.oracle_grad.argtypes = [ctypes.c_int64, ctypes.c_int64] + [_P] * 5
         lib.oracle_grad.restype = None
         lib.oracle_trial_point.argtypes = [ctypes.c_int64, _P, _P, ctypes.c_double, _P, _P]
@@ -50,6 +52,10 @@ def _load():
                                    [ctypes.c_double] * 4 + [ctypes.c_int, ctypes.c_int] +
                                    [_P, ctypes.c_double] + [_P] * 11)
         lib.oracle_run.restype = ctypes.c_int
+        lib.oracle_run_v.argtypes = ([ctypes.c_int64, ctypes.c_int64] + [_P] * 10 +
+                                     [ctypes.c_double] * 4 + [ctypes.c_int, ctypes.c_int] +
+                                     [_P, ctypes.c_double] + [_P] * 11)
+        lib.oracle_run_v.restype = ctypes.c_int
         lib.oracle_dvh.argtypes = [ctypes.c_int64, _P, _P, ctypes.c_int, _P, ctypes.c_int, _P, _P]
         lib.oracle_dvh.restype = None
         _lib = lib
@@ -71,6 +77,12 @@ def _csr(prob):
             _c(prob.w_over, np.float32))
 
 
+def _voxel_limits(prob):
+    """Optional per-voxel limits of a problem (attributes tv_under / tv_over, float32 [n_v]) or (None, None)."""
+    tvu, tvo = getattr(prob, "tv_under", None), getattr(prob, "tv_over", None)
+    return (None if tvu is None else _c(tvu, np.float32)), (None if tvo is None else _c(tvo, np.float32))
+
+
 def eval_objective(prob, x):
     """(d, r, G) at x.  imrt_oracle.c: oracle_eval."""
     lib = _load()
@@ -79,8 +91,9 @@ def eval_objective(prob, x):
     d = np.empty(prob.n_v, np.float64)
     r = np.empty(prob.n_v, np.float64)
     G = ctypes.c_double(0.0)
-    lib.oracle_eval(prob.n_v, _p(rp), _p(col), _p(val), _p(sid), _p(tu), _p(to), _p(wu), _p(wo),
-                    _p(x), _p(d), _p(r), ctypes.addressof(G))
+    tvu, tvo = _voxel_limits(prob)
+    lib.oracle_eval_v(prob.n_v, _p(rp), _p(col), _p(val), _p(sid), _p(tu), _p(to), _p(wu), _p(wo), _p(tvu), _p(tvo),
+                      _p(x), _p(d), _p(r), ctypes.addressof(G))
     return d, r, G.value
 
 
@@ -143,7 +156,8 @@ def run(prob, x0=None, n_iters=None, delta=None, follow_trials=None, tau_rel=1e-
     first = ctypes.c_int(-1)
     fwd = ctypes.c_int64(0)
     tr = ctypes.c_int64(0)
-    k = lib.oracle_run(prob.n_v, prob.n_b, _p(rp), _p(col), _p(val), _p(sid), _p(tu), _p(to), _p(wu), _p(wo),
+    tvu, tvo = _voxel_limits(prob)
+    k = lib.oracle_run_v(prob.n_v, prob.n_b, _p(rp), _p(col), _p(val), _p(sid), _p(tu), _p(to), _p(wu), _p(wo), _p(tvu), _p(tvo),
                        float(prob.eps if eps is None else eps), float(prob.alpha if alpha is None else alpha),
                        float(prob.lambda0 if lambda0 is None else lambda0), dl,
                        int(prob.max_ls if max_ls is None else max_ls), n,

@@ -26,6 +26,7 @@
  *   R5  Step 5 (operator lost in the text): |G_new - G_old| / G_new < delta with the newest pair.
  *   R6  lambda restarts at the fixed lambda0 every outer iteration.
  *   R7  "Run N iterations" = N accepted outer iterations.
+ *   R16 Optional per-voxel limits T-_j / T+_j (the paper's own T_j) override the per-structure ones.
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force dense D x; closed forms on hand cases; central
  * finite differences of G for the gradient; zero penalty when every voxel is at its bound; the hand-derived
@@ -51,22 +52,36 @@ enum { ORACLE_STOP_MAX_ITERS = 0, ORACLE_STOP_TOLERANCE = 1, ORACLE_STOP_STATION
  *   G  += w-_s u_j^2 + w+_s o_j^2                  (plain left-to-right sum)
  *   r_j = 2 (w+_s o_j - w-_s u_j)
  * d and r may be NULL.
+ *
+ * Per-voxel limits (reading R16; "T_j for all j in V represents the dose distribution in the original
+ * treatment plan", :195 cumulative-dose re-optimisation): when tv_under / tv_over are not NULL, voxel j uses
+ * T-_j = tv_under[j] / T+_j = tv_over[j] instead of its structure's limits; the weights stay per structure.  The
+ * paper's literal model is tv_under = tv_over = T_j with w- = 1 on targets, 0 elsewhere, and w+ = 1.
  */
-void oracle_eval(int64_t n_v, const int32_t *row_ptr, const int32_t *col, const float *val, const uint8_t *sid,
-                 const float *t_under, const float *t_over, const float *w_under, const float *w_over,
-                 const double *x, double *d, double *r, double *G_out) {
+void oracle_eval_v(int64_t n_v, const int32_t *row_ptr, const int32_t *col, const float *val, const uint8_t *sid,
+                   const float *t_under, const float *t_over, const float *w_under, const float *w_over,
+                   const float *tv_under, const float *tv_over,
+                   const double *x, double *d, double *r, double *G_out) {
     double G = 0.0;
     for (int64_t j = 0; j < n_v; ++j) {
         double dj = 0.0;
         for (int64_t p = row_ptr[j]; p < row_ptr[j + 1]; ++p) dj += (double)val[p] * x[col[p]];
         const int s = sid[j];
-        const double u = fmax(0.0, (double)t_under[s] - dj);
-        const double o = fmax(0.0, dj - (double)t_over[s]);
+        const double tu = tv_under ? (double)tv_under[j] : (double)t_under[s];
+        const double to = tv_over ? (double)tv_over[j] : (double)t_over[s];
+        const double u = fmax(0.0, tu - dj);
+        const double o = fmax(0.0, dj - to);
         G += (double)w_under[s] * u * u + (double)w_over[s] * o * o;
         if (d) d[j] = dj;
         if (r) r[j] = 2.0 * ((double)w_over[s] * o - (double)w_under[s] * u);
     }
     *G_out = G;
+}
+
+void oracle_eval(int64_t n_v, const int32_t *row_ptr, const int32_t *col, const float *val, const uint8_t *sid,
+                 const float *t_under, const float *t_over, const float *w_under, const float *w_over,
+                 const double *x, double *d, double *r, double *G_out) {
+    oracle_eval_v(n_v, row_ptr, col, val, sid, t_under, t_over, w_under, w_over, NULL, NULL, x, d, r, G_out);
 }
 
 /* grad(r): g = D^T r by scatter over the rows of D (the oracle never forms D^T).   Reading R3. */
@@ -105,8 +120,9 @@ void oracle_trial_point(int64_t n_b, const double *x, const double *g, double la
  *          step_sq[k] (Delta of the accepted trial), margin[k] = (C - G+) / G_k of the accepted trial.
  * Returns the number of accepted iterations n.
  */
-int oracle_run(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *col, const float *val,
+int oracle_run_v(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *col, const float *val,
                const uint8_t *sid, const float *t_under, const float *t_over, const float *w_under, const float *w_over,
+               const float *tv_under, const float *tv_over,
                double eps, double alpha, double lambda0, double delta_tol, int max_ls, int max_iters,
                const int32_t *follow_trials, double tau_rel,
                double *x, double *obj, double *lambda_out, int32_t *n_trials, double *step_sq, double *margin,
@@ -121,7 +137,7 @@ int oracle_run(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *
     int reason = ORACLE_STOP_MAX_ITERS;
     double G_k;
 
-    oracle_eval(n_v, row_ptr, col, val, sid, t_under, t_over, w_under, w_over, x, NULL, r, &G_k);
+    oracle_eval_v(n_v, row_ptr, col, val, sid, t_under, t_over, w_under, w_over, tv_under, tv_over, x, NULL, r, &G_k);
     ++fwd;
     obj[0] = G_k;
     int k = 0; /* number of accepted iterations so far */
@@ -136,7 +152,7 @@ int oracle_run(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *
         for (;;) {
             oracle_trial_point(n_b, x, g, lambda, x_new, &delta);
             if (m == 0 && delta == 0.0) { reason = ORACLE_STOP_STATIONARY; stop = 1; break; }
-            oracle_eval(n_v, row_ptr, col, val, sid, t_under, t_over, w_under, w_over, x_new, NULL, r_new, &G_new);
+            oracle_eval_v(n_v, row_ptr, col, val, sid, t_under, t_over, w_under, w_over, tv_under, tv_over, x_new, NULL, r_new, &G_new);
             ++fwd;
             C = G_k - (eps / lambda) * delta; /* Eq. (5) */
             int accept;
@@ -176,6 +192,18 @@ int oracle_run(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *
     if (n_tr_passes) *n_tr_passes = tr;
     free(g); free(x_new); free(r); free(r_new);
     return k;
+}
+
+int oracle_run(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *col, const float *val,
+               const uint8_t *sid, const float *t_under, const float *t_over, const float *w_under, const float *w_over,
+               double eps, double alpha, double lambda0, double delta_tol, int max_ls, int max_iters,
+               const int32_t *follow_trials, double tau_rel,
+               double *x, double *obj, double *lambda_out, int32_t *n_trials, double *step_sq, double *margin,
+               int *stop_reason, int *n_follow_violations, int *first_violation,
+               int64_t *n_fwd_passes, int64_t *n_tr_passes) {
+    return oracle_run_v(n_v, n_b, row_ptr, col, val, sid, t_under, t_over, w_under, w_over, NULL, NULL, eps, alpha, lambda0,
+                        delta_tol, max_ls, max_iters, follow_trials, tau_rel, x, obj, lambda_out, n_trials, step_sq, margin,
+                        stop_reason, n_follow_violations, first_violation, n_fwd_passes, n_tr_passes);
 }
 
 /*

@@ -26,7 +26,7 @@ STOP_NAMES = ("MAX_ITERS", "TOLERANCE", "STATIONARY", "LINESEARCH_STALLED")
 DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
 
 # every symbol include/imrtgp.h declares
-EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
+EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_set_voxel_limits", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
            "imrt_plan_eval", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
            "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_last_error", "imrt_plan_destroy",
            "imrt_version")
@@ -67,6 +67,7 @@ def lib() -> ctypes.CDLL:
         L.imrt_plan_create.argtypes = [ctypes.POINTER(_P), i64, i64, i64, _P, _P, _P, _P, i32, _P, _P, _P, _P,
                                        ctypes.POINTER(Params), _P, ctypes.c_size_t, _P]
         L.imrt_plan_set_x.argtypes = [_P, _P]
+        L.imrt_plan_set_voxel_limits.argtypes = [_P, _P, _P]
         L.imrt_plan_run_iters.argtypes = [_P, i32]
         L.imrt_plan_run_to_tol.argtypes = [_P, dbl, i32]
         L.imrt_plan_eval.argtypes = [_P, _P, _P, _P, _P, ctypes.POINTER(dbl)]
@@ -143,6 +144,12 @@ def imrt_plan_create(n_v, n_b, nnz, row_ptr, col_idx, val, structure_id, t_under
 def imrt_plan_set_x(plan, x0):
     import torch
     _check(lib().imrt_plan_set_x(plan, _dptr(x0, torch.float32)), plan)
+
+
+def imrt_plan_set_voxel_limits(plan, t_under_v=None, t_over_v=None):
+    """Per-voxel limits (fp32 CUDA tensors [n_v], borrowed: keep them alive) or None for the structure's limit."""
+    import torch
+    _check(lib().imrt_plan_set_voxel_limits(plan, _dptr(t_under_v, torch.float32), _dptr(t_over_v, torch.float32)), plan)
 
 
 def imrt_plan_run_iters(plan, n_iters: int):
@@ -275,6 +282,9 @@ class Plan:
         self.handle = imrt_plan_create(self.n_v, self.n_b, self.nnz, self.row_ptr, self.col, self.val, self.sid,
                                        prob.t_under, prob.t_over, prob.w_under, prob.w_over, self.params, self.workspace,
                                        self.stream.cuda_stream)
+        self._tvu = self._tvo = None
+        if getattr(prob, "tv_under", None) is not None or getattr(prob, "tv_over", None) is not None:
+            self.set_voxel_limits(getattr(prob, "tv_under", None), getattr(prob, "tv_over", None))
 
     # -- the calls of the C-ABI
     def set_x(self, x0):
@@ -283,6 +293,19 @@ class Plan:
             x0 = torch.from_numpy(np.ascontiguousarray(x0, dtype=np.float32))
         self._x0 = x0.to(device=self.device, dtype=torch.float32).contiguous()
         imrt_plan_set_x(self.handle, self._x0)
+
+    def set_voxel_limits(self, t_under_v=None, t_over_v=None):
+        import torch
+
+        def dev(a):
+            if a is None:
+                return None
+            if not isinstance(a, torch.Tensor):
+                a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+            return a.to(device=self.device, dtype=torch.float32).contiguous()
+
+        self._tvu, self._tvo = dev(t_under_v), dev(t_over_v)      # borrowed by the plan: keep them alive
+        imrt_plan_set_voxel_limits(self.handle, self._tvu, self._tvo)
 
     def run_iters(self, n: int):
         imrt_plan_run_iters(self.handle, int(n))

@@ -5,6 +5,7 @@
 #include "../../include/imrtgp.h"
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -146,6 +147,7 @@ struct Layout {
     DvhWork dvh;
     // build scratch
     int* quadU;
+    unsigned char* covered;
     unsigned int* keysA;
     unsigned int* keysB;
     unsigned int* valsA;
@@ -194,6 +196,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.dvh.sum = w.take<double>((size_t)MAX_STRUCTURES);
     L.dvh.query = w.take<DvhQuery>((size_t)MAX_STRUCTURES * DVH_MAX_PCTS);
     L.quadU = w.take<int>(n_v / 4 + 2);
+    L.covered = w.take<unsigned char>(n_v + 4);
     L.keysA = w.take<unsigned int>(nnz + 4);
     L.keysB = w.take<unsigned int>(nnz + 4);
     L.valsA = w.take<unsigned int>(nnz + 4);
@@ -376,19 +379,51 @@ __global__ void k_pack_transpose(const int* __restrict__ rowT_ptr, const int* __
     }
 }
 
-// d = 0 and the matching constant residual on every row; the dose pass then overwrites the rows its blocks cover.
 struct RPtrs { float* p[R_MAX + 1]; };
-__global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, int n_v, const RPtrs R,
-                                      float* d) {
+// d = 0 and the matching constant residual on every row; the dose pass then overwrites the rows its blocks cover.
+__global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, const State* st, int n_v,
+                                      const RPtrs R, float* d) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_v) return;
-    const float4 t = table[sid[j]];
+    float4 t = table[sid[j]];
+    if (st->tvu) t.x = st->tvu[j];
+    if (st->tvo) t.y = st->tvo[j];
     const float u = fmaxf(0.0f, t.x), o = fmaxf(0.0f, -t.y);
-    const float r = 2.0f * (t.w * o - t.z * u);
+    const float r = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));
 #pragma unroll
     for (int i = 0; i <= R_MAX; ++i)
         if (R.p[i]) R.p[i][j] = r;
     if (d) d[j] = 0.0f;
+}
+
+// The constants of the rows no record covers (dose 0 whatever x is): their objective, State::G_skip, summed in a fixed
+// order by ONE block, and their residual in every residual buffer of the loop.  Runs at plan creation and whenever
+// the per-voxel limits change.
+__global__ void k_skip_constants(const uint8_t* __restrict__ sid, const unsigned char* __restrict__ covered,
+                                 const float4* __restrict__ table, State* st, int n_v, const RPtrs R) {
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (int j = threadIdx.x; j < n_v; j += blockDim.x) {
+        if (covered[j]) continue;
+        float4 t = table[sid[j]];
+        if (st->tvu) t.x = st->tvu[j];
+        if (st->tvo) t.y = st->tvo[j];
+        const float u = fmaxf(0.0f, t.x), o = fmaxf(0.0f, -t.y);
+        const float r = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));
+#pragma unroll
+        for (int i = 0; i <= R_MAX; ++i)
+            if (R.p[i]) R.p[i][j] = r;
+        const double du = (double)u, d_o = (double)o;
+        acc = __dadd_rn(acc, __fma_rn((double)t.z, __dmul_rn(du, du), __dmul_rn((double)t.w, __dmul_rn(d_o, d_o))));
+    }
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += red[w];
+        st->G_skip = s;
+    }
 }
 
 __global__ void k_check_x(const float* __restrict__ x, int n_b, State* st) {
@@ -433,17 +468,15 @@ struct BlockPlan {
 
 // quadU: distinct columns per quad (4 consecutive rows), or empty when the quad format is not on offer.
 imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::vector<uint8_t>& sid, const float4* table_h,
-                         int chunk_slots, int col_bytes, const std::vector<int>& quadU, BlockPlan& B, double& G_skip,
-                         int64_t& n_skipped, int64_t& n_nonempty, int64_t& n_quad_rows) {
+                         int chunk_slots, int col_bytes, const std::vector<int>& quadU, BlockPlan& B,
+                         std::vector<unsigned char>& covered, int64_t& n_skipped, int64_t& n_nonempty, int64_t& n_quad_rows) {
     const int n_v = (int)sid.size();
-    G_skip = 0.0;
+    covered.assign((size_t)n_v, 1);
     n_skipped = 0;
     n_nonempty = 0;
     n_quad_rows = 0;
-    auto skip_row = [&](int j) {   // d = 0 on a row without entries: a constant of the objective
-        const float4 t = table_h[sid[j]];
-        const double u = std::max(0.0, (double)t.x), o = std::max(0.0, -(double)t.y);
-        G_skip += (double)t.z * u * u + (double)t.w * o * o;
+    auto skip_row = [&](int j) {   // d = 0 on a row without entries: a constant of the objective (k_skip_constants)
+        covered[j] = 0;
         ++n_skipped;
     };
     auto pad4 = [](int n) { return (n + 3) & ~3; };
@@ -874,6 +907,21 @@ static imrt_status build_graph(imrt_plan* pl) {
     return IMRT_STATUS_OK;
 }
 
+// Phase timer of plan creation (IMRTGP_PROFILE_CREATE=1 prints the phases to stderr).
+struct PhaseTimer {
+    bool on;
+    cudaStream_t st;
+    std::chrono::steady_clock::time_point t0;
+    PhaseTimer(cudaStream_t s) : on(getenv("IMRTGP_PROFILE_CREATE") != nullptr), st(s), t0(std::chrono::steady_clock::now()) {}
+    void mark(const char* what) {
+        if (!on) return;
+        cudaStreamSynchronize(st);
+        const auto t1 = std::chrono::steady_clock::now();
+        fprintf(stderr, "imrt_plan_create: %-28s %8.3f ms\n", what, std::chrono::duration<double, std::milli>(t1 - t0).count());
+        t0 = t1;
+    }
+};
+
 // ------------------------------------------------------------------------------------------------ C-ABI
 extern "C" {
 
@@ -941,6 +989,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     // every early return below releases the handle
     struct Guard { imrt_plan* p; ~Guard() { if (p) { g_create_error = p->err; delete p; } } } guard{pl};
 
+    PhaseTimer phase(st);
     // ---- validate what the host can see: row_ptr and structure ids
     std::vector<int> rp((size_t)n_v + 1);
     std::vector<uint8_t> sid((size_t)n_v);
@@ -959,6 +1008,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     for (int64_t j = 0; j < n_v; ++j)
         if (sid[j] >= n_structures) return fail(pl, IMRT_STATUS_BAD_STRUCTURE, "structure_id[%lld] = %d >= n_structures", (long long)j, sid[j]);
 
+    phase.mark("validate");
     // ---- penalty table
     std::vector<float4> table_h(MAX_STRUCTURES, make_float4(0, 0, 0, 0));
     for (int s = 0; s < n_structures; ++s) table_h[s] = make_float4(host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]);
@@ -986,11 +1036,14 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaMemcpyAsync(quadU.data(), L.quadU, sizeof(int) * n_quads, cudaMemcpyDeviceToHost, st));
         CUDA_TRY(pl, cudaStreamSynchronize(st));
     }
+    phase.mark("quad union counts");
     BlockPlan BP;
-    double G_skip = 0.0;
-    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, quadU, BP, G_skip, pl->n_skipped,
+    std::vector<unsigned char> covered;
+    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, quadU, BP, covered, pl->n_skipped,
                                  pl->n_nonempty, pl->n_quad_rows);
     if (s != IMRT_STATUS_OK) return s;
+    CUDA_TRY(pl, cudaMemcpyAsync(L.covered, covered.data(), (size_t)n_v, cudaMemcpyHostToDevice, st));
+    phase.mark("build_blocks (host)");
     const Bounds B = bounds_for(n_v, n_b, nnz);
     const size_t n_blk = BP.blk.size();
     if ((int64_t)n_blk > B.max_blk || (int64_t)BP.meta.size() > B.max_meta || BP.pack_bytes > B.max_pack)
@@ -1017,6 +1070,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaGetLastError());
     }
 
+    phase.mark("pack records");
     // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1)
     CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.valT, 0, sizeof(float) * B.nnz_pad, st));
@@ -1042,6 +1096,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     // ---- transpose-pass ranges and gradient slots
     std::vector<TrRange> ranges;
     std::vector<int> rowslot, cta_rng_h;
+    phase.mark("transpose (sort + gather)");
     // ---- the packed stream the transpose pass reads (16-bit voxel offsets), unless a group of 32 entries is too wide
     bool id16 = nnz > 0 && !getenv("IMRTGP_NO_ID16") && nnz + 128 * n_b + 128 < (1LL << 31);
     std::vector<int> rpP((size_t)n_b + 1, 0);
@@ -1068,6 +1123,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     pl->max_ranges = B.max_ranges; pl->max_slots = B.max_slots;
     pl->tr_range_w = L.tr_range; pl->rowslot_w = L.rowslot_ptr; pl->cta_rng_w = L.cta_rng;
 
+    phase.mark("pack D^T, ranges");
     // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, dose
     // scratch, the R trial points, g, then the ring (dose pass) / stages (transpose pass).  R = the largest of 4, 2, 1
     // not above the request that leaves the ring room for 16 records of average size (one per consumer warp).
@@ -1107,7 +1163,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr; P.cta_rng = L.cta_rng;
     P.n_ranges = (int)ranges.size(); P.grid_t = grid_t;
     P.n_stages_t = stt; P.n_slots = n_slots;
-    P.table = L.table; P.n_structures = n_structures; P.G_skip = G_skip;
+    P.table = L.table; P.n_structures = n_structures; P.covered = L.covered;
     P.xbuf[0] = L.xbuf[0]; P.xbuf[1] = L.xbuf[1]; P.g = L.g;
     for (int i = 0; i <= R_MAX; ++i) P.rbuf[i] = L.rbuf[i];
     P.Gpart[0] = L.Gpart[0]; P.Gpart[1] = L.Gpart[1]; P.gslot[0] = L.gslot[0]; P.gslot[1] = L.gslot[1];
@@ -1141,17 +1197,21 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     {
         RPtrs rp_all;
         for (int i = 0; i <= R_MAX; ++i) rp_all.p[i] = L.rbuf[i];
-        k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, (int)n_v, rp_all, nullptr);
+        k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, L.st, (int)n_v, rp_all, nullptr);
+        k_skip_constants<<<1, 1024, 0, st>>>(structure_id, L.covered, L.table, L.st, (int)n_v, rp_all);
     }
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
 
     s = upload_partition(pl, cta_blk);
     if (s != IMRT_STATUS_OK) return s;
+    phase.mark("state, first schedule");
     s = tune_partition(pl);
     if (s != IMRT_STATUS_OK) return s;
+    phase.mark("rebalance dose pass");
     s = tune_transpose(pl);
     if (s != IMRT_STATUS_OK) return s;
+    phase.mark("rebalance transpose pass");
     if (prm->driver == 0) {
         s = build_graph(pl);
         if (s != IMRT_STATUS_OK) return s;
@@ -1185,6 +1245,21 @@ imrt_status imrt_plan_set_x(imrt_plan* pl, const float* x0) {
     A.mode = MODE_INIT;   // G(x_1), r(x_1): reads xbuf[0], writes rbuf[0], flips xi / ri to 0
     CUDA_TRY(pl, launch_dose(pl, A));
     pl->has_x = true;
+    return IMRT_STATUS_OK;
+}
+
+__global__ void k_set_limits(State* st, const float* tvu, const float* tvo) { st->tvu = tvu; st->tvo = tvo; }
+
+imrt_status imrt_plan_set_voxel_limits(imrt_plan* pl, const float* t_under_v, const float* t_over_v) {
+    if (!pl) return IMRT_STATUS_INVALID_ARG;
+    if (((uintptr_t)t_under_v | (uintptr_t)t_over_v) & 3) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_voxel_limits: misaligned array");
+    cudaStream_t st = pl->stream;
+    k_set_limits<<<1, 1, 0, st>>>(pl->P.st, t_under_v, t_over_v);
+    RPtrs rp_all;
+    for (int i = 0; i <= R_MAX; ++i) rp_all.p[i] = pl->P.rbuf[i];
+    k_skip_constants<<<1, 1024, 0, st>>>(pl->sid, pl->P.covered, pl->P.table, pl->P.st, pl->P.n_v, rp_all);
+    CUDA_TRY(pl, cudaGetLastError());
+    pl->has_x = false;     // G(x_1), r(x_1) belong to the old limits
     return IMRT_STATUS_OK;
 }
 
@@ -1239,7 +1314,7 @@ imrt_status imrt_plan_eval(imrt_plan* pl, const float* x, float* d, float* r, fl
     RPtrs rp1;
     memset(&rp1, 0, sizeof rp1);
     rp1.p[0] = r_used;
-    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, st>>>(pl->sid, pl->P.table, n_v, rp1, d);
+    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, st>>>(pl->sid, pl->P.table, pl->P.st, n_v, rp1, d);
     PassArgs A;
     memset(&A, 0, sizeof A);
     A.mode = MODE_EVAL;
@@ -1274,7 +1349,7 @@ static imrt_status dose_of_current_x(imrt_plan* pl, float* d) {
     const int n_v = pl->P.n_v;
     RPtrs rp0;
     memset(&rp0, 0, sizeof rp0);
-    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, pl->stream>>>(pl->sid, pl->P.table, n_v, rp0, d);
+    k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, pl->stream>>>(pl->sid, pl->P.table, pl->P.st, n_v, rp0, d);
     PassArgs A;
     memset(&A, 0, sizeof A);
     A.mode = MODE_EVAL;   // x_in NULL: the current iterate

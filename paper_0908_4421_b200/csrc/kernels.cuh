@@ -71,6 +71,9 @@ struct State {                 // lives in the workspace; the single source of t
     double lambda;             // step size of the first trial of the pending batch
     double eps, alpha, lambda0, delta_tol;
     double eval_obj;           // output of MODE_EVAL dose passes
+    double G_skip;             // objective of the rows no block covers (their dose is 0: a constant)
+    const float* tvu;          // optional per-voxel limits T-_j / T+_j [n_v] (NULL: the structure's, reading R16)
+    const float* tvo;
     long long fwd_passes, tr_passes;
     int max_ls;
     int iter;                  // accepted iterations since set_x
@@ -144,7 +147,7 @@ struct DevPlan {
     const float4* table;       // (t_under, t_over, w_under, w_over)
     int n_structures;
     int pad0;
-    double G_skip;             // objective of the rows no block covers (d = 0 there, constant)
+    const unsigned char* covered;   // [n_v] 1: the row belongs to a record; 0: dose 0, constant penalty (State::G_skip)
     // vectors
     float* xbuf[2];
     float* g;
@@ -314,6 +317,15 @@ __device__ __forceinline__ void stage_point(const float* x, float* xs, int n_b) 
 constexpr int VW = 8;
 constexpr int RB = 32 / VW;
 
+struct VoxelLimits {           // optional per-voxel limits (State::tvu / tvo), loaded once per pass
+    const float* tu;
+    const float* to;
+    __device__ __forceinline__ void apply(float4& t, size_t j) const {
+        if (tu) t.x = __ldg(tu + j);
+        if (to) t.y = __ldg(to + j);
+    }
+};
+
 template <int R> struct XVec;
 template <> struct XVec<1> { float v[1]; __device__ __forceinline__ void load(const unsigned char* p) { v[0] = *reinterpret_cast<const float*>(p); } };
 template <> struct XVec<2> { float v[2]; __device__ __forceinline__ void load(const unsigned char* p) { const float2 t = *reinterpret_cast<const float2*>(p); v[0] = t.x; v[1] = t.y; } };
@@ -322,7 +334,8 @@ template <> struct XVec<4> { float v[4]; __device__ __forceinline__ void load(co
 template <bool COL16, int R>
 __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
                                            const float4* __restrict__ table_s, float* __restrict__ dsc,
-                                           float* const (&r_out)[R], float* __restrict__ d_out, int tw, int lane, double (&Gacc)[R]) {
+                                           float* const (&r_out)[R], float* __restrict__ d_out, const VoxelLimits vl, int tw, int lane,
+                                           double (&Gacc)[R]) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nrows = (int)hdr.x, slots = (int)hdr.w;
     const uint32_t* rows = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
@@ -382,10 +395,11 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
         __syncwarp();
         const int row = (q0 + (lane / RB) * TEAM) * RB + (lane % RB);     // the row parked at position `lane`
         if (row < nrows) {
-            const float4 t = table_s[(rows[row] >> 16) & 0xFFu];
+            float4 t = table_s[(rows[row] >> 16) & 0xFFu];
             XVec<R> dv;
             dv.load(reinterpret_cast<const unsigned char*>(dsc + lane * R));
             const size_t j = (size_t)hdr.y + row;
+            vl.apply(t, j);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const float dd = dv.v[r];
@@ -422,7 +436,7 @@ template <int R> __device__ __forceinline__ bool quad_owner(int lane) { return (
 template <int R>
 __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
                                                  const float4* __restrict__ table_s, float* __restrict__ my_r,
-                                                 float* __restrict__ d_out, int tw, int lane, double& Gq) {
+                                                 float* __restrict__ d_out, const VoxelLimits vl, int tw, int lane, double& Gq) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nq = (int)hdr.x, nbc = (int)hdr.w;
     const uint32_t* qt = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
@@ -479,8 +493,9 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
             d = g + __shfl_xor_sync(0xffffffffu, g, 1);
         }
         if (owner && ((w.x >> (16 + rr)) & 1u)) {          // the row exists
-            const float4 t = table_s[(w.y >> (8 * rr)) & 0xFFu];
+            float4 t = table_s[(w.y >> (8 * rr)) & 0xFFu];
             const size_t jrow = (size_t)hdr.y + 4 * qi + rr;
+            vl.apply(t, jrow);
             const float u = fmaxf(0.0f, t.x - d);
             const float o = fmaxf(0.0f, d - t.y);
             my_r[jrow] = 2.0f * __fmaf_rn(t.w, o, -__fmul_rn(t.z, u));
@@ -560,6 +575,7 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
         float* my_r = r_out[0];
 #pragma unroll
         for (int r = 1; r < R; ++r) my_r = quad_trial<R>(lane) == r ? r_out[r] : my_r;
+        const VoxelLimits vl = {P.st->tvu, P.st->tvo};
         int at_next = (team < nb) ? __ldg(&P.blk[b0 + team].z) : 0;
         for (int i = team; i < nb; i += N_TEAMS) {
             const int at = at_next;
@@ -569,9 +585,9 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
 #ifndef IMRT_EXP_SKIP_COMPUTE
             const unsigned char* rec = ring + at;
             if (COL16 && reinterpret_cast<const uint32_t*>(rec)[2] != 0u)      // header word 2: record format
-                dose_block_quads<R>(rec, xs_b, table_s, my_r, d_out, tw, lane, Gq);
+                dose_block_quads<R>(rec, xs_b, table_s, my_r, d_out, vl, tw, lane, Gq);
             else
-                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, tw, lane, Gacc);
+                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, vl, tw, lane, Gacc);
 #endif
             __syncwarp();
             if (lane == 0) {
@@ -618,7 +634,9 @@ __device__ __forceinline__ void reduce_objective(const DevPlan& P, const double*
     }
     block_sum_vec<R>(G, h);
 #pragma unroll
-    for (int r = 0; r < R; ++r) G[r] += P.G_skip;
+    const double G_skip = P.st->G_skip;
+#pragma unroll
+    for (int r = 0; r < R; ++r) G[r] += G_skip;
 }
 
 // ------------------------------------------------------------------------------------------------ transpose pass

@@ -135,6 +135,8 @@ class Problem:
     max_ls: int = 40
     n_iters: int = 50
     voxel_ids: np.ndarray | None = None   # row -> linear grid id (phantoms only)
+    tv_under: np.ndarray | None = None    # optional per-voxel limits, float32 [n_v] (PAPER.md:58 T_j); None = per structure
+    tv_over: np.ndarray | None = None
     meta: dict = field(default_factory=dict)
 
     @property

@@ -332,3 +332,35 @@ def test_full_size_parity(m, cfg, n_iters):
     assert relerr(d, d_o) <= 1e-4   # dose of the two final plans (same trial counts, fp32 vs fp64 trajectories)
     plan.close()
     _phantoms.pop(cfg, None)        # free ~1-3 GB of host memory
+
+
+# ---------------------------------------------------------------------------------------------- per-voxel limits
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_per_voxel_limits_parity(m, cfg):
+    # the paper's own model: every voxel has its own T_j (here the structure's limit perturbed per voxel, both sides,
+    # including voxels whose row of D is empty: their constant penalty and residual must follow the per-voxel limits)
+    import copy
+    prob = copy.copy(phantom(cfg))
+    rng = np.random.default_rng(100 + cfg)
+    prob.tv_under = (prob.t_under[prob.sid] * rng.uniform(0.9, 1.1, prob.n_v)).astype(np.float32)
+    prob.tv_over = (prob.t_over[prob.sid] * rng.uniform(0.9, 1.1, prob.n_v)).astype(np.float32)
+    plan = m.Plan(prob, max_iters=20)
+    check_eval(m, plan, prob, prob.x0)
+    plan.set_x(prob.x0)
+    plan.run_iters(20)
+    tr = plan.trace()
+    fol = oracle.run(prob, n_iters=20, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert tr.n_iters == 20 and fol.n_follow_violations == 0
+    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    # back to per-structure limits: the plan behaves as if the call had never happened
+    plan.set_voxel_limits(None, None)
+    base = phantom(cfg)
+    check_eval(m, plan, base, base.x0)
+    # only the upper limits per voxel
+    half = copy.copy(base)
+    half.tv_over = prob.tv_over
+    plan.set_voxel_limits(None, half.tv_over)
+    check_eval(m, plan, half, half.x0)
+    with pytest.raises(m.ImrtError):
+        plan.run_iters(1)                 # the iterate was invalidated: set_x first
+    plan.close()

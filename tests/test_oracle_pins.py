@@ -287,3 +287,43 @@ def test_dvh_hand_case():
     assert list(dp[0]) == c["D_p"] and mean[0] == c["mean"]
     assert list(dp[1]) == [200.0, 200.0, 200.0, 100.0, 100.0] and mean[1] == 150.0
     assert np.isnan(dp[2]).all() and np.isnan(mean[2])
+
+
+# ------------------------------------------------------------------ per-voxel limits  (reading R16)
+def test_per_voxel_limits_are_the_papers_literal_model():
+    # Eq. (1) with its own T_j per voxel: F-_j = max(0, T_j - z_j)^2 on targets, F+_j = max(0, z_j - T_j)^2 on all voxels,
+    # written out here independently of the oracle; gradient 2 D^T (o - u [targets]) checked by central differences.
+    rng = np.random.default_rng(21)
+    D = rng.uniform(0, 1, (15, 5)) * (rng.random((15, 5)) < 0.6)
+    sid = [0] * 6 + [1] * 9                       # structure 0 = targets
+    T = rng.uniform(5, 60, 15).astype(np.float32)
+    prob = dense_problem(D, sid, [999, 999], [999, 999], [1, 0], [1, 1], np.ones(5))   # per-structure limits unused
+    prob.tv_under, prob.tv_over = T.copy(), T.copy()
+    x = rng.uniform(0, 40, 5)
+    z = D.astype(np.float32).astype(np.float64) @ x
+    G_paper = sum(max(0.0, T[j] - z[j]) ** 2 for j in range(6)) + sum(max(0.0, z[j] - T[j]) ** 2 for j in range(15))
+    d, r, G = oracle.eval_objective(prob, x)
+    assert abs(G - G_paper) <= 1e-12 * G_paper
+    g = oracle.gradient(prob, r)
+    for i in range(5):
+        h = 1e-5 * (1 + abs(x[i]))
+        xp, xm = x.copy(), x.copy()
+        xp[i] += h
+        xm[i] -= h
+        fd = (oracle.eval_objective(prob, xp)[2] - oracle.eval_objective(prob, xm)[2]) / (2 * h)
+        assert abs(fd - g[i]) <= 1e-6 * max(1.0, abs(g[i]))
+    # per-voxel arrays that repeat the structure's limits change nothing, bit for bit
+    base = synth_inputs.make_phantom(0)
+    ref = oracle.run(base, n_iters=8)
+    base.tv_under, base.tv_over = base.t_under[base.sid].copy(), base.t_over[base.sid].copy()
+    same = oracle.run(base, n_iters=8)
+    np.testing.assert_array_equal(ref.obj, same.obj)
+    np.testing.assert_array_equal(ref.x, same.x)
+    # only one side given: the other keeps the structure's limit
+    base.tv_under = None
+    base.tv_over = (base.t_over[base.sid] * 0.9).astype(np.float32)
+    x_hot = np.full(base.n_b, 40.0)               # hot enough for voxels to sit above their upper limits
+    G_tight = oracle.eval_objective(base, x_hot)[2]
+    base.tv_over = None
+    G_plain = oracle.eval_objective(base, x_hot)[2]
+    assert G_tight > G_plain                      # tighter upper limits, same lower limits: a larger penalty
