@@ -7,11 +7,14 @@
 //   trial point     x+ = max(0, x - lambda g), Delta = ||x+ - x||^2       PAPER.md:90, :109-111, :128 kernel 4
 //   Armijo / stop   C = G_k - (eps/lambda) Delta, accept iff G+ < C        PAPER.md:92-95 Eq. (5), :110-114
 //
-// Both passes are persistent CTAs (one per SM): a producer warp streams the matrix with 1-D bulk async copies
-// (cp.async.bulk, the TMA unit) into a ring of shared-memory stages guarded by mbarriers; 16 consumer warps
-// gather the vector (x+ from shared memory, r through L1/L2 with an evict-last hint), multiply-add in fp32 and
-// reduce with warp shuffles.  Objective and gradient partials are fp64 and are combined in a fixed order, so a run
-// is bit-reproducible and no floating-point atomics are used anywhere.
+// Both passes are persistent CTAs (one per SM): producer warps stream the matrix with 1-D bulk async copies
+// (cp.async.bulk, the TMA unit) into shared memory guarded by mbarriers; 16 consumer warps gather the vector (the
+// trial points x+ from shared memory, r through L1/L2 with an evict-last hint), multiply-add in fp32 and reduce with
+// warp shuffles.  The dose pass evaluates R = 1, 2 or 4 line-search trial points per pass over D (one record per
+// consumer warp, records travelling through a byte ring whose schedule is laid out at plan creation); the transpose
+// pass streams a packed D^T in fixed stages shared by the consumer warps.  Objective and gradient partials are fp64
+// and are combined in a fixed order, so a plan's runs are bit-reproducible and no floating-point atomics are used
+// anywhere.
 //
 // The same pass bodies are driven three ways (imrt_params.driver): by one cooperative persistent kernel that
 // holds the whole loop (grid barrier between passes, replicated scalar state), by a CUDA graph with nested
@@ -27,13 +30,8 @@ namespace imrt {
 
 // ------------------------------------------------------------------------------------------------ constants
 constexpr int W_CONS = 16;                    // consumer warps per CTA
-#ifndef IMRT_TEAM
-#define IMRT_TEAM 1
-#endif
-#ifndef IMRT_QUAD_CAP
-#define IMRT_QUAD_CAP 384
-#endif
-constexpr int TEAM = IMRT_TEAM;               // consumer warps that work on one dose-pass record together
+constexpr int TEAM = 1;                       // consumer warps that split one dose-pass record (the block functions take
+                                              // (tw, TEAM); teams of 4 measured slower: profiles/r01_notes.md)
 constexpr int N_TEAMS = W_CONS / TEAM;
 constexpr int N_CONS = W_CONS * 32;           // consumer threads
 constexpr int N_PROD = 2;                     // producer warps of the dose pass (the transpose pass uses the first only)
@@ -44,7 +42,7 @@ constexpr int MIN_CHUNK_SLOTS = 1024;         // slot capacity of a block unless
 constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
 constexpr int MAXROWS_F = 256;                // rows per block
 constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered up to this many beamlets (pack-kernel bitmap)
-constexpr int QUAD_CAP = IMRT_QUAD_CAP;                 // union columns per quad-format record unless one quad needs more
+constexpr int QUAD_CAP = 384;                 // union columns per quad-format record unless one quad needs more
 constexpr int QUAD_MAXQ = 64;                 // quads per record
 constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
