@@ -153,6 +153,29 @@ imrt_status imrt_plan_run_to_tol(imrt_plan* plan, double delta, int32_t max_iter
  */
 imrt_status imrt_plan_eval(imrt_plan* plan, const float* x, float* d, float* r, float* g, double* host_obj);
 
+/*
+ * g = D^T r for an arbitrary r (fp32 [n_v], device) -> g (fp32 [n_b], device): one transpose pass, the optimiser state is
+ * not touched.  With imrt_plan_eval (which leaves r(x)) and imrt_trial_point this is what a host-driven loop over
+ * several plans -- one per row slab of D, on one GPU each -- is made of: the partial objectives and gradients of the
+ * slabs add up (paper_0908_4421_b200/sharded.py).  Asynchronous.
+ */
+imrt_status imrt_plan_gradient(imrt_plan* plan, const float* r, float* g);
+
+/*
+ * The trial point of PAPER.md:90 / :109-111 outside a plan: x_out = max(0, x - lambda g) (fp32 [n_b], device) and
+ * *step_sq = ||x_out - x||^2 (fp64, DEVICE pointer), summed in a fixed order.  stream: a cudaStream_t as void*.
+ * Asynchronous.
+ */
+imrt_status imrt_trial_point(const float* x, const float* g, double lambda, int64_t n_b, float* x_out, double* step_sq, void* stream);
+
+/*
+ * The two scalar decisions of the loop for a HOST-driven loop (pure host arithmetic, the formulas the device loop uses):
+ *   imrt_armijo_accepts  step 3 with Eq. (5): 1 iff G_new < G_k - (eps / lambda) step_sq
+ *   imrt_stop_test       step 5 (reading R5): 1 iff delta > 0 and (G_new == 0 or |G_new - G_old| / G_new < delta)
+ */
+int32_t imrt_armijo_accepts(double G_k, double G_new, double step_sq, double eps, double lambda);
+int32_t imrt_stop_test(double G_old, double G_new, double delta);
+
 /* Copy the current iterate to x (fp32 [n_b], device).  Asynchronous. */
 imrt_status imrt_plan_get_x(imrt_plan* plan, float* x);
 

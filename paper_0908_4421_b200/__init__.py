@@ -27,7 +27,7 @@ DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
 
 # every symbol include/imrtgp.h declares
 EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_set_voxel_limits", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
-           "imrt_plan_eval", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
+           "imrt_plan_eval", "imrt_plan_gradient", "imrt_trial_point", "imrt_armijo_accepts", "imrt_stop_test", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
            "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_last_error", "imrt_plan_destroy",
            "imrt_version")
 
@@ -71,6 +71,10 @@ def lib() -> ctypes.CDLL:
         L.imrt_plan_run_iters.argtypes = [_P, i32]
         L.imrt_plan_run_to_tol.argtypes = [_P, dbl, i32]
         L.imrt_plan_eval.argtypes = [_P, _P, _P, _P, _P, ctypes.POINTER(dbl)]
+        L.imrt_plan_gradient.argtypes = [_P, _P, _P]
+        L.imrt_trial_point.argtypes = [_P, _P, dbl, i64, _P, _P, _P]
+        L.imrt_armijo_accepts.argtypes = [dbl] * 5
+        L.imrt_stop_test.argtypes = [dbl] * 3
         L.imrt_plan_get_x.argtypes = [_P, _P]
         L.imrt_plan_get_dose.argtypes = [_P, _P]
         L.imrt_plan_dvh.argtypes = [_P, _P, i32, _P, _P]
@@ -85,7 +89,9 @@ def lib() -> ctypes.CDLL:
         L.imrt_version.argtypes = []
         L.imrt_version.restype = ctypes.c_char_p
         for name in EXPORTS:
-            if name not in ("imrt_last_error", "imrt_version"):
+            if name in ("imrt_armijo_accepts", "imrt_stop_test"):
+                getattr(L, name).restype = ctypes.c_int32
+            elif name not in ("imrt_last_error", "imrt_version"):
                 getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -166,6 +172,26 @@ def imrt_plan_eval(plan, x, d=None, r=None, g=None) -> float:
     _check(lib().imrt_plan_eval(plan, _dptr(x, torch.float32), _dptr(d, torch.float32), _dptr(r, torch.float32),
                                 _dptr(g, torch.float32), ctypes.byref(obj)), plan)
     return obj.value
+
+
+def imrt_plan_gradient(plan, r, g):
+    import torch
+    _check(lib().imrt_plan_gradient(plan, _dptr(r, torch.float32), _dptr(g, torch.float32)), plan)
+
+
+def imrt_trial_point(x, g, lam: float, x_out, step_sq, stream_ptr: int = 0):
+    """x_out = max(0, x - lam g); step_sq: float64 CUDA tensor of one element receiving ||x_out - x||^2."""
+    import torch
+    _check(lib().imrt_trial_point(_dptr(x, torch.float32), _dptr(g, torch.float32), float(lam), x.numel(),
+                                  _dptr(x_out, torch.float32), _dptr(step_sq, torch.float64), ctypes.c_void_p(stream_ptr)))
+
+
+def imrt_armijo_accepts(G_k: float, G_new: float, step_sq: float, eps: float, lam: float) -> bool:
+    return bool(lib().imrt_armijo_accepts(G_k, G_new, step_sq, eps, lam))
+
+
+def imrt_stop_test(G_old: float, G_new: float, delta: float) -> bool:
+    return bool(lib().imrt_stop_test(G_old, G_new, delta))
 
 
 def imrt_plan_get_x(plan, x):

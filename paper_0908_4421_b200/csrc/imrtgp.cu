@@ -1337,6 +1337,55 @@ imrt_status imrt_plan_eval(imrt_plan* pl, const float* x, float* d, float* r, fl
     return IMRT_STATUS_OK;
 }
 
+imrt_status imrt_plan_gradient(imrt_plan* pl, const float* r, float* g) {
+    if (!pl || !r || !g) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_gradient: null argument");
+    PassArgs T;
+    memset(&T, 0, sizeof T);
+    T.mode = MODE_EVAL;
+    T.r_in = r;
+    T.g_out = g;
+    CUDA_TRY(pl, launch_transpose(pl, T));
+    return IMRT_STATUS_OK;
+}
+
+// x+ = max(0, x - lambda g), Delta = ||x+ - x||^2 by ONE block, fixed summation order (Eq. (5)).
+__global__ void k_trial_point(const float* __restrict__ x, const float* __restrict__ g, double lambda, int n_b, float* x_out, double* step_sq) {
+    __shared__ double red[32];
+    const float lam = (float)lambda;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n_b; i += blockDim.x) {
+        const float xi = x[i];
+        const float xn = fmaxf(0.0f, fmaf(-lam, g[i], xi));
+        const float dx = xn - xi;
+        acc = __fma_rn((double)dx, (double)dx, acc);
+        x_out[i] = xn;
+    }
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += red[w];
+        *step_sq = s;
+    }
+}
+
+imrt_status imrt_trial_point(const float* x, const float* g, double lambda, int64_t n_b, float* x_out, double* step_sq, void* stream) {
+    if (!x || !g || !x_out || !step_sq || n_b < 1 || n_b >= (1LL << 31) || !(lambda > 0.0))
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_trial_point: bad argument");
+    k_trial_point<<<1, 1024, 0, (cudaStream_t)stream>>>(x, g, lambda, (int)n_b, x_out, step_sq);
+    CUDA_TRY(nullptr, cudaGetLastError());
+    return IMRT_STATUS_OK;
+}
+
+int32_t imrt_armijo_accepts(double G_k, double G_new, double step_sq, double eps, double lambda) {
+    return G_new < G_k - (eps / lambda) * step_sq ? 1 : 0;        // step 3 with Eq. (5), strict as printed
+}
+
+int32_t imrt_stop_test(double G_old, double G_new, double delta) {
+    return (delta > 0.0 && (G_new == 0.0 || fabs(G_new - G_old) / G_new < delta)) ? 1 : 0;     // step 5, reading R5
+}
+
 imrt_status imrt_plan_get_x(imrt_plan* pl, float* x) {
     if (!pl || !x) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_x: null argument");
     if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");

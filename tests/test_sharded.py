@@ -1,0 +1,153 @@
+"""Row-sharded driver (paper_0908_4421_b200/sharded.py): slab selection, the loop and its two
+collectives under the gloo backend with world_size 2 on CPU (the local shards are oracle-backed stand-ins: the
+library has no CPU path), and -- on a GPU -- two slabs of the real kernels adding up to the single-plan result."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+import oracle
+import synth_inputs
+from paper_0908_4421_b200 import sharded
+
+
+class OracleShard:
+    """CPU stand-in for GpuShard: the same three operations on a row slab, computed by the fp64 oracle."""
+    device = "cpu"
+
+    def __init__(self, sub):
+        self.sub, self.r = sub, None
+
+    def vector(self, x0):
+        import torch
+        return torch.from_numpy(np.asarray(x0, np.float64).copy())
+
+    def eval_partial(self, x):
+        _, self.r, G = oracle.eval_objective(self.sub, x.numpy())
+        return G
+
+    def grad_partial(self):
+        import torch
+        return torch.from_numpy(oracle.gradient(self.sub, self.r))
+
+    def trial_point(self, x, g, lam):
+        import torch
+        xn, step = oracle.trial_point(x.numpy(), g.numpy(), lam)
+        return torch.from_numpy(xn), step
+
+
+def test_slabs_cover_the_rows_and_balance_the_nonzeros():
+    prob = synth_inputs.make_phantom(0)
+    for world in (1, 2, 3, 8):
+        b = sharded.slab_bounds(prob.row_ptr, world)
+        assert b[0] == 0 and b[-1] == prob.n_v and (np.diff(b) >= 0).all()
+        nnz = np.diff(prob.row_ptr[b].astype(np.int64))
+        assert nnz.sum() == prob.nnz and nnz.max() - nnz.min() <= 2 * np.diff(prob.row_ptr).max()
+        rows = 0
+        for q in range(world):
+            sub, (r0, r1) = sharded.shard_rows(prob, world, q)
+            assert sub.n_v == r1 - r0 and sub.row_ptr[0] == 0 and sub.row_ptr[-1] == sub.col.shape[0] == sub.val.shape[0]
+            np.testing.assert_array_equal(sub.sid, prob.sid[r0:r1])
+            rows += sub.n_v
+        assert rows == prob.n_v
+    # an empty matrix and more ranks than rows
+    empty = synth_inputs.Problem("e", 3, 2, np.zeros(4, np.int32), np.zeros(0, np.int32), np.zeros(0, np.float32), np.zeros(3, np.uint8),
+                                 prob.t_under, prob.t_over, prob.w_under, prob.w_over, np.ones(2, np.float32))
+    b = sharded.slab_bounds(empty.row_ptr, 5)
+    assert b[0] == 0 and b[-1] == 3 and (np.diff(b) >= 0).all()
+
+
+def _worker(rank, world, port, n_iters, out):
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        prob = synth_inputs.make_phantom(0)
+        sub, _ = sharded.shard_rows(prob, world, rank)
+        opt = sharded.ShardedOptimizer(prob, OracleShard(sub))
+        tr = opt.run(prob.x0, n_iters)
+        out[rank] = (tr.n_iters, tr.stop_reason, tr.obj.tolist(), tr.lam.tolist(), tr.n_trials.tolist(), opt.x.numpy().tolist())
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_gloo_reproduce_the_single_process_loop():
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    n_iters, world = 12, 2
+    out = mp.Manager().dict()
+    mp.spawn(_worker, args=(world, port, n_iters, out), nprocs=world, join=True)
+    prob = synth_inputs.make_phantom(0)
+    ref = oracle.run(prob, n_iters=n_iters)
+    assert set(out.keys()) == {0, 1}
+    for rank in (0, 1):
+        n, reason, obj, lam, trials, x = out[rank]
+        assert n == ref.n_iters == n_iters and reason == ref.stop_reason
+        assert trials == ref.n_trials.tolist() and lam == ref.lam.tolist()
+        np.testing.assert_allclose(obj, ref.obj, rtol=1e-12)          # the partial sums are added in another order
+        np.testing.assert_allclose(x, ref.x, rtol=1e-9, atol=1e-12)
+    assert out[0] == out[1]                                           # the iterates stay replicated, bit for bit
+
+
+def test_stationary_and_tolerance_exits_without_a_process_group():
+    prob = synth_inputs.make_phantom(0)
+    opt = sharded.ShardedOptimizer(prob, OracleShard(prob))
+    tr = opt.run(prob.x0, 400, delta=1e-3)
+    ref = oracle.run(prob, n_iters=400, delta=1e-3)
+    assert tr.stop_reason == sharded.STOP_TOLERANCE == ref.stop_reason and tr.n_iters == ref.n_iters
+    np.testing.assert_array_equal(tr.obj, ref.obj)                    # one slab: the very same arithmetic
+    T = np.array([10.0, 20.0, 30.0], np.float32)
+    ident = synth_inputs.Problem("ident", 3, 3, np.array([0, 1, 2, 3], np.int32), np.array([0, 1, 2], np.int32), np.ones(3, np.float32),
+                                 np.array([0, 1, 2], np.uint8), T, T, np.ones(3, np.float32), np.ones(3, np.float32),
+                                 np.array([12.0, 16.0, 30.0], np.float32), eps=0.2, alpha=2.0, lambda0=1.0)
+    tr = sharded.ShardedOptimizer(ident, OracleShard(ident)).run(ident.x0, 5)
+    assert tr.n_iters == 1 and tr.stop_reason == sharded.STOP_STATIONARY and tr.obj.tolist() == [20.0, 0.0] and tr.n_trials.tolist() == [2]
+
+
+class _TwoSlabs:
+    """Two GpuShards on one device whose partials are added here: what the all-reduce does across two GPUs."""
+
+    def __init__(self, prob, device):
+        self.a = sharded.GpuShard(sharded.shard_rows(prob, 2, 0)[0], device)
+        self.b = sharded.GpuShard(sharded.shard_rows(prob, 2, 1)[0], device)
+        self.device = self.a.device
+
+    def vector(self, x0):
+        return self.a.vector(x0)
+
+    def eval_partial(self, x):
+        return self.a.eval_partial(x) + self.b.eval_partial(x)
+
+    def grad_partial(self):
+        return self.a.grad_partial() + self.b.grad_partial()
+
+    def trial_point(self, x, g, lam):
+        return self.a.trial_point(x, g, lam)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_two_slabs_of_the_cuda_path_add_up(cfg):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_0908_4421_b200 as m
+    prob = synth_inputs.make_phantom(cfg)
+    n = 15
+    plan = m.Plan(prob, max_iters=n)
+    plan.set_x(prob.x0)
+    plan.run_iters(n)
+    tr1 = plan.trace()
+    one = sharded.ShardedOptimizer(prob, sharded.GpuShard(prob, "cuda:0")).run(prob.x0, n)
+    two = sharded.ShardedOptimizer(prob, _TwoSlabs(prob, "cuda:0")).run(prob.x0, n)
+    for tr in (one, two):
+        assert tr.n_iters == n
+        np.testing.assert_array_equal(tr.n_trials, tr1.n_trials)
+        np.testing.assert_array_equal(tr.lam, tr1.lam)
+        np.testing.assert_allclose(tr.obj, tr1.obj, rtol=2e-5)     # other slabs, other summation order in fp32: the per-kernel tolerance
+    fol = oracle.run(prob, n_iters=n, follow_trials=two.n_trials, tau_rel=1e-6)
+    assert fol.n_follow_violations == 0 and abs(two.obj[-1] - fol.obj[-1]) <= 1e-4 * fol.obj[-1]
+    plan.close()
