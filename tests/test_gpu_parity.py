@@ -364,3 +364,54 @@ def test_per_voxel_limits_parity(m, cfg):
     with pytest.raises(m.ImrtError):
         plan.run_iters(1)                 # the iterate was invalidated: set_x first
     plan.close()
+
+
+# ---------------------------------------------------------------------------------------------- the fallback layouts
+@pytest.mark.parametrize("env", ["IMRTGP_NO_QUADS", "IMRTGP_COL32", "IMRTGP_NO_ID16", "IMRTGP_NO_TUNE"])
+def test_fallback_layouts_parity(m, env, monkeypatch):
+    # the layouts a plan falls back to when the matrix does not suit the packed ones: row-format records everywhere,
+    # 32-bit column indices (n_b > 65,536), the 32-bit D^T stream (a group of 32 entries wider than 65,535 voxels), and
+    # the modelled (unmeasured) partitions -- forced here through the library's environment switches
+    monkeypatch.setenv(env, "1")
+    for prob in (phantom(0), phantom(1),
+                 synth_inputs.make_random(21, n_v=4099, n_b=130, density=0.5, empty_row_frac=0.15, full_rows=2)):
+        plan = m.Plan(prob, max_iters=12)
+        info = plan.info()
+        if env == "IMRTGP_NO_QUADS":
+            assert info["quad_rows"] == 0
+        if env == "IMRTGP_COL32":
+            assert info["col16"] == 0 and info["quad_rows"] == 0
+        x = np.random.default_rng(5).uniform(0, 60, prob.n_b).astype(np.float32)
+        check_eval(m, plan, prob, x)
+        plan.set_x(prob.x0)
+        plan.run_iters(12)
+        tr = plan.trace()
+        fol = oracle.run(prob, n_iters=12, follow_trials=tr.n_trials, tau_rel=1e-6)
+        assert tr.n_iters == fol.n_iters and fol.n_follow_violations == 0
+        assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+        plan.close()
+
+
+def test_wide_transpose_groups_use_the_32_bit_stream(m):
+    # a beamlet whose voxels lie more than 65,535 rows apart inside one group of 32 entries: no 16-bit offsets possible
+    n_v, n_b = 200000, 6
+    rows = np.arange(0, n_v, 2500)                     # 80 rows, 2,500 apart: 32 consecutive entries span 77,500 voxels
+    rp = np.zeros(n_v + 1, np.int32)
+    rp[rows + 1] = n_b
+    rp = np.cumsum(rp).astype(np.int32)
+    rng = np.random.default_rng(9)
+    col = np.tile(np.arange(n_b, dtype=np.int32), rows.shape[0])
+    val = rng.uniform(0.1, 1.0, col.shape[0]).astype(np.float32)
+    sid = (np.arange(n_v) % 3).astype(np.uint8)
+    base = synth_inputs.make_random(1, n_v=50, n_b=8)
+    prob = synth_inputs.Problem("wide", n_v, n_b, rp, col, val, sid, base.t_under, base.t_over, base.w_under, base.w_over,
+                                rng.uniform(0.5, 1.5, n_b).astype(np.float32))
+    prob.lambda0, _ = synth_inputs.pick_lambda0(rp, col, val, sid, base.w_under, base.w_over)
+    plan = m.Plan(prob, max_iters=8)
+    check_eval(m, plan, prob, prob.x0 * 30)
+    plan.set_x(prob.x0)
+    plan.run_iters(8)
+    tr = plan.trace()
+    fol = oracle.run(prob, n_iters=8, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert fol.n_follow_violations == 0 and np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    plan.close()
