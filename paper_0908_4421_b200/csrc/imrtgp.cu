@@ -218,6 +218,17 @@ __global__ void k_validate(const int* __restrict__ col, const float* __restrict_
     if (bad_val) flags[1] = 1;
 }
 
+// columns strictly ascending inside every row (one warp per row); a violation raises flags[3]
+__global__ void k_validate_rows(const int* __restrict__ row_ptr, const int* __restrict__ col, int n_v, int* flags) {
+    const int lane = threadIdx.x & 31;
+    int bad = 0;
+    for (long long j = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; j < n_v; j += ((long long)gridDim.x * blockDim.x) >> 5) {
+        const int p0 = row_ptr[j], p1 = row_ptr[j + 1];
+        for (int p = p0 + 1 + lane; p < p1; p += 32) bad |= col[p] <= col[p - 1];
+    }
+    if (bad) flags[3] = 1;
+}
+
 __global__ void k_iota_keys(const int* __restrict__ col, unsigned int* keys, unsigned int* vals, long long nnz) {
     for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < nnz; p += (long long)gridDim.x * blockDim.x) {
         keys[p] = (unsigned int)col[p];
@@ -1005,6 +1016,13 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         if (rp[j + 1] < rp[j]) return fail(pl, IMRT_STATUS_BAD_CSR, "row_ptr decreases at row %lld", (long long)j);
     if (flags_h[0]) return fail(pl, IMRT_STATUS_BAD_CSR, "a column index is outside [0, n_b)");
     if (flags_h[1]) return fail(pl, IMRT_STATUS_BAD_CSR, "a value of D is not finite");
+    if (nnz > 0) {      // row_ptr is sane: the rows can be walked
+        k_validate_rows<<<grid_for(n_v * 32, 256), 256, 0, st>>>(row_ptr, col_idx, (int)n_v, L.flags);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        if (flags_h[3]) return fail(pl, IMRT_STATUS_BAD_CSR, "column indices are not strictly ascending inside a row");
+    }
     for (int64_t j = 0; j < n_v; ++j)
         if (sid[j] >= n_structures) return fail(pl, IMRT_STATUS_BAD_STRUCTURE, "structure_id[%lld] = %d >= n_structures", (long long)j, sid[j]);
 

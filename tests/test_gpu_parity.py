@@ -285,6 +285,11 @@ def test_linesearch_stall_and_bad_inputs(m):
     with pytest.raises(m.ImrtError) as e:
         m.Plan(bad)
     assert e.value.status_name == "BAD_CSR"
+    dup = synth_inputs.Problem("dup", 2, 3, np.array([0, 2, 3], np.int32), np.array([1, 1, 0], np.int32), np.ones(3, np.float32),
+                               np.zeros(2, np.uint8), T, T, np.ones(1, np.float32), np.ones(1, np.float32), np.ones(3, np.float32))
+    with pytest.raises(m.ImrtError) as e:          # a repeated column (and, equally, descending columns)
+        m.Plan(dup)
+    assert e.value.status_name == "BAD_CSR"
     bad = synth_inputs.Problem(**{**prob.__dict__})
     bad.sid = np.array([0, 3], np.uint8)
     with pytest.raises(m.ImrtError) as e:
