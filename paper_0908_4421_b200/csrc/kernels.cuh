@@ -738,7 +738,11 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
                             unsigned int c[SLICE_T / 32];
                             float rr[SLICE_T / 32];
 #pragma unroll
+#ifdef IMRT_EXP_NOGATHER
+                            for (int u = 0; u < SLICE_T / 32; ++u) c[u] = (bp[u] + ip[lane + 32 * u]) & 1023u;
+#else
                             for (int u = 0; u < SLICE_T / 32; ++u) c[u] = bp[u] + ip[lane + 32 * u];
+#endif
 #pragma unroll
                             for (int u = 0; u < SLICE_T / 32; ++u) rr[u] = ld_keep(r_in + c[u], keep);
 #pragma unroll
