@@ -234,3 +234,35 @@ def make_random(seed: int, n_v: int, n_b: int, density: float = 0.3, n_structure
     if col.size:
         prob.lambda0, _ = pick_lambda0(row_ptr, prob.col, val, sid, w_u, w_o)
     return prob
+
+
+def mixed_resolution(prob: Problem, body_sid: int = 3) -> Problem:
+    """The paper's mixed-resolution problem: voxels of unspecified tissue (structure `body_sid`) are
+    doubled in each dimension, targets and OARs keep the full resolution.  A coarse voxel's row of D is the mean of
+    the rows of the fine body voxels it contains (its dose is their mean dose); it counts as ONE voxel in Eq. (1),
+    as every voxel does in the paper (reading R17).  Harness code: sparse row averaging with scipy, no
+    optimiser arithmetic.  Rows: the full-resolution voxels in their order, then the coarse voxels."""
+    import scipy.sparse as sp
+    nx, ny, nz = prob.meta["grid"]
+    vid = prob.voxel_ids
+    ix, iy, iz = vid % nx, (vid // nx) % ny, vid // (nx * ny)
+    body = prob.sid == body_sid
+    key = (ix // 2) + ((nx + 1) // 2) * ((iy // 2) + ((ny + 1) // 2) * (iz // 2))
+    fine_rows = np.flatnonzero(~body)
+    body_rows = np.flatnonzero(body)
+    uniq, inv = np.unique(key[body_rows], return_inverse=True)
+    counts = np.bincount(inv).astype(np.float64)
+    D = sp.csr_matrix((prob.val.astype(np.float64), prob.col, prob.row_ptr), shape=(prob.n_v, prob.n_b))
+    S = sp.csr_matrix((1.0 / counts[inv], (inv, np.arange(body_rows.shape[0]))), shape=(uniq.shape[0], body_rows.shape[0]))
+    Dm = sp.vstack([D[fine_rows], S @ D[body_rows]]).tocsr()
+    Dm.sort_indices()
+    Dm.eliminate_zeros()
+    out = Problem(prob.name + "-mixed", Dm.shape[0], prob.n_b, Dm.indptr.astype(np.int32), Dm.indices.astype(np.int32),
+                  Dm.data.astype(np.float32),
+                  np.concatenate([prob.sid[fine_rows], np.full(uniq.shape[0], body_sid, np.uint8)]),
+                  prob.t_under, prob.t_over, prob.w_under, prob.w_over, prob.x0, eps=prob.eps, alpha=prob.alpha,
+                  delta=prob.delta, max_ls=prob.max_ls, n_iters=prob.n_iters,
+                  meta={**prob.meta, "fine_rows": int(fine_rows.shape[0]), "coarse_rows": int(uniq.shape[0]),
+                        "body_rows_merged": int(body_rows.shape[0])})
+    out.lambda0, _ = pick_lambda0(out.row_ptr, out.col, out.val, out.sid, out.w_under, out.w_over)
+    return out

@@ -420,3 +420,34 @@ def test_wide_transpose_groups_use_the_32_bit_stream(m):
     fol = oracle.run(prob, n_iters=8, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert fol.n_follow_violations == 0 and np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
     plan.close()
+
+
+# ---------------------------------------------------------------------------------------------- mixed resolution
+def test_mixed_resolution_workflow(m):
+    # "For unspecified tissue we increased the voxel size in each dimension by a factor of 2 ... The full resolution was
+    # used when evaluating the treatment quality": optimise on the mixed-resolution matrix, evaluate dose and DVH with a
+    # second plan on the full-resolution matrix.  (The row merging is input preparation: synth_inputs.mixed_resolution.)
+    fine = phantom(1)
+    mixed = synth_inputs.mixed_resolution(fine)
+    assert mixed.n_v < fine.n_v // 4 and mixed.meta["fine_rows"] == int((fine.sid != 3).sum())
+    n = 40
+    plan = m.Plan(mixed, max_iters=n)
+    check_eval(m, plan, mixed, mixed.x0)
+    plan.set_x(mixed.x0)
+    plan.run_iters(n)
+    tr = plan.trace()
+    fol = oracle.run(mixed, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert tr.n_iters == n and fol.n_follow_violations == 0
+    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    x = plan.get_x()
+    # full-resolution evaluation of that plan
+    full = m.Plan(fine, max_iters=1)
+    d, r, g, G = full.eval(x)
+    d_o, r_o, G_o = oracle.eval_objective(fine, x.cpu().numpy().astype(np.float64))
+    assert relerr(d.cpu().numpy(), d_o) <= TOL_KERNEL and abs(G - G_o) <= TOL_KERNEL * G_o
+    full.set_x(x)
+    dp_g, mean_g = full.dvh(oracle.DVH_PCTS)
+    dp_o, mean_o = oracle.dvh_points(fine.sid, d_o, fine.n_structures)
+    assert np.nanmax(np.abs(dp_g - dp_o)) <= TOL_DVH_GY and np.nanmax(np.abs(mean_g - mean_o)) <= TOL_DVH_GY
+    plan.close()
+    full.close()

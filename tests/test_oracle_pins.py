@@ -327,3 +327,26 @@ def test_per_voxel_limits_are_the_papers_literal_model():
     base.tv_over = None
     G_plain = oracle.eval_objective(base, x_hot)[2]
     assert G_tight > G_plain                      # tighter upper limits, same lower limits: a larger penalty
+
+
+# ------------------------------------------------------------------ input preparation: mixed resolution
+def test_mixed_resolution_rows_are_block_means(phantom0):
+    # harness check: a coarse voxel's dose is the mean dose of the fine body voxels in its 2x2x2 block, target / OAR rows
+    # are untouched, and the beamlet side is unchanged
+    mixed = synth_inputs.mixed_resolution(phantom0)
+    x = np.random.default_rng(3).uniform(0, 30, phantom0.n_b)
+    d_fine = oracle.eval_objective(phantom0, x)[0]
+    d_mixed = oracle.eval_objective(mixed, x)[0]
+    nx, ny, nz = phantom0.meta["grid"]
+    vid = phantom0.voxel_ids
+    key = (vid % nx) // 2 + ((nx + 1) // 2) * (((vid // nx) % ny) // 2 + ((ny + 1) // 2) * ((vid // (nx * ny)) // 2))
+    body = phantom0.sid == 3
+    n_fine = int((~body).sum())
+    np.testing.assert_allclose(d_mixed[:n_fine], d_fine[~body], rtol=1e-6, atol=1e-9)
+    means = {}
+    for k, dv in zip(key[body], d_fine[body]):
+        means.setdefault(int(k), []).append(dv)
+    expect = np.array([np.mean(means[k]) for k in sorted(means)])
+    assert mixed.n_v == n_fine + expect.shape[0] and mixed.n_b == phantom0.n_b
+    np.testing.assert_allclose(d_mixed[n_fine:], expect, rtol=1e-5, atol=1e-7)     # fp32 rounding of the merged values
+    assert (mixed.sid[n_fine:] == 3).all() and (mixed.sid[:n_fine] != 3).all()
