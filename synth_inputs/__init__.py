@@ -266,3 +266,37 @@ def mixed_resolution(prob: Problem, body_sid: int = 3) -> Problem:
                         "body_rows_merged": int(body_rows.shape[0])})
     out.lambda0, _ = pick_lambda0(out.row_ptr, out.col, out.val, out.sid, out.w_under, out.w_over)
     return out
+
+
+def make_banded(seed: int, n_v: int, n_b: int, width: int, jitter: float, empty_frac: float, n_structures: int = 3) -> Problem:
+    """Rows whose column sets drift slowly from row to row (neighbouring rows overlap, as neighbouring voxels do), with
+    holes, empty rows and rows of very different lengths: the shapes that make a plan mix its record formats."""
+    rng = np.random.default_rng(seed)
+    rows, c0 = [], 0.0
+    for _ in range(n_v):
+        if rng.random() < empty_frac:
+            rows.append(np.empty(0, np.int64))
+            continue
+        c0 = (c0 + rng.uniform(0, jitter)) % max(1, n_b - width)
+        w = max(1, int(width * rng.uniform(0.5, 1.0)))
+        cols = np.arange(int(c0), min(n_b, int(c0) + w))
+        if rng.random() < 0.3 and cols.size > 3:
+            cols = np.unique(np.delete(cols, rng.integers(0, cols.size, size=max(1, cols.size // 6))))
+        rows.append(cols)
+    row_ptr = np.zeros(n_v + 1, np.int32)
+    row_ptr[1:] = np.cumsum([len(r) for r in rows])
+    col = np.concatenate(rows).astype(np.int32) if row_ptr[-1] else np.empty(0, np.int32)
+    val = rng.uniform(0.05, 1.0, col.shape[0]).astype(np.float32)
+    sid = rng.integers(0, n_structures, n_v).astype(np.uint8)
+    sid[: max(1, n_v // 3)] = 0
+    t_u = np.zeros(n_structures, np.float32)
+    t_o = rng.uniform(20.0, 60.0, n_structures).astype(np.float32)
+    w_u = np.zeros(n_structures, np.float32)
+    w_o = rng.uniform(0.5, 10.0, n_structures).astype(np.float32)
+    t_u[0] = t_o[0] = 70.0
+    w_u[0] = w_o[0] = 100.0
+    x0 = rng.uniform(0.5, 1.5, n_b).astype(np.float32)
+    prob = Problem("banded-%d" % seed, n_v, n_b, row_ptr, col, val, sid, t_u, t_o, w_u, w_o, x0, n_iters=10)
+    if col.size:
+        prob.lambda0, _ = pick_lambda0(row_ptr, col, val, sid, w_u, w_o)
+    return prob
