@@ -491,7 +491,7 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         ++n_skipped;
     };
     auto pad4 = [](int n) { return (n + 3) & ~3; };
-    auto pad8 = [](int n) { return (n + 7) & ~7; };
+    auto pad8 = [](int n) { return n; };   // unions are not padded: a lane past the end of a quad reads the zero column
     size_t off = 0;
     auto close_record = [&](int mo, int payload_bytes, int fmt, int rows, int slots) {
         while ((B.meta.size() - mo - META_HDR) & 3) B.meta.push_back(0u);

@@ -107,11 +107,10 @@ struct DevPlan {
     //   val     fp32[slots + ZPAD]   every row padded with zeros to a multiple of 4 slots; ZPAD zeros at the end
     //   col     uint16[slots + ZPAD] (n_b <= 65536) or int32[slots + ZPAD]
     // QUAD format (chosen per 256-row segment where it is smaller; n_b <= QUAD_MAX_NB):
-    //   header  uint32[4]  {quads, first row (a multiple of 4), 1, union columns incl. padding}
-    //   quads   uint32[2 (quads + 1)]  {column offset of the quad (low 16 bits, a multiple of 8) | row-exists mask << 16,
+    //   header  uint32[4]  {quads, first row (a multiple of 4), 1, union columns}
+    //   quads   uint32[2 (quads + 1)]  {column offset of the quad (low 16 bits) | row-exists mask << 16,
     //                                   the 4 structure ids}; the last pair holds the total; padded to 4 words
-    //   val     fp32[columns + 1][4]   per union column the 4 rows' values; unions padded to a multiple of 8 columns
-    //                                  with zeros; one zero column at the end
+    //   val     fp32[columns + 1][4]   per union column the 4 rows' values; one zero column at the end
     //   col     uint16[columns + 8]
     // One record is consumed by ONE warp.
     const unsigned char* pack;
