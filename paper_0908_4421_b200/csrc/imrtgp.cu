@@ -101,7 +101,7 @@ struct Bounds {
 Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     Bounds b;
     const int64_t slots = nnz + 3 * n_v;    // every row padded to a multiple of 4 slots
-    b.max_blk = 4 * (slots / MIN_CHUNK_SLOTS + 1) + 4 * (n_v / SEG_ROWS + 1) + n_v / 16 + 8;
+    b.max_blk = 4 * (slots / MIN_CHUNK_SLOTS + 1) + 4 * (n_v / SEG_ROWS + 1) + n_v / 16 + 8 + 8 * TARGET_RECORDS;
     b.max_meta = n_v + b.max_blk * (META_HDR + 2 + 3) + 8;
     b.max_pack = (size_t)b.max_meta * 4 + (size_t)slots * 8 + (size_t)b.max_blk * (128 + 48) + 256;
     b.max_ranges = 2 * 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
@@ -468,6 +468,22 @@ inline int grid_for(long long n, int block) {
 // ------------------------------------------------------------------------------------------------ host builders
 // Row-aligned blocks of D for the dose pass.  Each block becomes one self-contained record of the packed stream
 // (layout: kernels.cuh, DevPlan::pack); this lays the records out and writes their headers and row tables.
+// How much a record may hold.  Large matrices get the full sizes; a small one is cut into at least ~TARGET_RECORDS
+// records so that every consumer warp of every CTA has several (a record is consumed by one warp).
+struct RecordCaps {
+    int chunk_slots;   // row format: slots per record
+    int max_rows;      // row format: rows per record
+    int quad_cap;      // quad format: union columns per record
+};
+static RecordCaps record_caps(int64_t n_v, int64_t nnz) {
+    auto clampi = [](int64_t v, int lo, int hi) { return (int)std::max<int64_t>(lo, std::min<int64_t>(hi, v)); };
+    RecordCaps c;
+    c.chunk_slots = clampi((nnz / TARGET_RECORDS + 3) & ~(int64_t)3, 64, MIN_CHUNK_SLOTS);
+    c.max_rows = clampi(n_v / TARGET_RECORDS, 8, MAXROWS_F);
+    c.quad_cap = clampi(nnz / 3 / TARGET_RECORDS, 32, QUAD_CAP);
+    return c;
+}
+
 struct BlockPlan {
     std::vector<int4> blk;        // {record offset / 128, record bytes, 0, 0}                 -> device, dose pass
     std::vector<int4> pk;         // {meta word offset, meta words, record offset / 128, 0}    -> device, pack kernel
@@ -479,7 +495,7 @@ struct BlockPlan {
 
 // quadU: distinct columns per quad (4 consecutive rows), or empty when the quad format is not on offer.
 imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::vector<uint8_t>& sid, const float4* table_h,
-                         int chunk_slots, int col_bytes, const std::vector<int>& quadU, BlockPlan& B,
+                         const RecordCaps caps, int col_bytes, const std::vector<int>& quadU, BlockPlan& B,
                          std::vector<unsigned char>& covered, int64_t& n_skipped, int64_t& n_nonempty, int64_t& n_quad_rows) {
     const int n_v = (int)sid.size();
     covered.assign((size_t)n_v, 1);
@@ -525,19 +541,19 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
             while (j < seg1) {
                 if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
                 const int r0 = j;
-                int slots = pad4(rp[j + 1] - rp[j]);
-                if (slots > chunk_slots)
+                int slots = pad4(rp[j + 1] - rp[j]);      // a row longer than the cap gets a record of its own
+                if (slots > MAX_CHUNK_SLOTS)
                     return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
-                                rp[j + 1] - rp[j], chunk_slots);
+                                rp[j + 1] - rp[j], MAX_CHUNK_SLOTS);
                 int last = j, empties = 0, jj = j + 1;
-                while (jj < seg1 && jj - r0 < MAXROWS_F) {
+                while (jj < seg1 && jj - r0 < caps.max_rows) {
                     const int len = rp[jj + 1] - rp[jj];
                     if (len == 0) {
                         if (++empties > 32) break;
                         ++jj;
                         continue;
                     }
-                    if (slots + pad4(len) > chunk_slots) break;
+                    if (slots + pad4(len) > caps.chunk_slots) break;
                     slots += pad4(len);
                     empties = 0;
                     last = jj;
@@ -576,7 +592,7 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
                         ++qq;
                         continue;
                     }
-                    if (cols + pad8(quadU[qq]) > QUAD_CAP) break;
+                    if (cols + pad8(quadU[qq]) > caps.quad_cap) break;
                     cols += pad8(quadU[qq]);
                     empties = 0;
                     last = qq;
@@ -1040,9 +1056,9 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     const bool col16 = n_b <= 65536 && !getenv("IMRTGP_COL32");
     int max_row = 0;
     for (int64_t j = 0; j < n_v; ++j) max_row = std::max(max_row, rp[j + 1] - rp[j]);
-    const int chunk_slots = std::max(MIN_CHUNK_SLOTS, (max_row + 3) & ~3);
-    if (chunk_slots > MAX_CHUNK_SLOTS)
+    if (max_row > MAX_CHUNK_SLOTS)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row of D has %d entries; this build handles rows up to %d", max_row, MAX_CHUNK_SLOTS);
+    const RecordCaps caps = record_caps(n_v, nnz);
     // quad format on offer: count the distinct columns of every 4 consecutive rows on the device
     const int bm_words = (int)((n_b + 31) / 32);
     std::vector<int> quadU;
@@ -1057,7 +1073,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     phase.mark("quad union counts");
     BlockPlan BP;
     std::vector<unsigned char> covered;
-    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), chunk_slots, col16 ? 2 : 4, quadU, BP, covered, pl->n_skipped,
+    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), caps, col16 ? 2 : 4, quadU, BP, covered, pl->n_skipped,
                                  pl->n_nonempty, pl->n_quad_rows);
     if (s != IMRT_STATUS_OK) return s;
     CUDA_TRY(pl, cudaMemcpyAsync(L.covered, covered.data(), (size_t)n_v, cudaMemcpyHostToDevice, st));

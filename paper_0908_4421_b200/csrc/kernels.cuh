@@ -45,6 +45,7 @@ constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered
 constexpr int QUAD_CAP = 384;                 // union columns per quad-format record unless one quad needs more
 constexpr int QUAD_MAXQ = 64;                 // quads per record
 constexpr int SEG_ROWS = 256;                 // rows per format decision
+constexpr int TARGET_RECORDS = 8192;          // a small matrix is cut into at least about this many records (imrtgp.cu)
 constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
 constexpr int R_MAX = 4;                      // line-search trial points evaluated per dose pass (1, 2 or 4)
 constexpr int CHUNK_T = 4096;                 // nnz per transpose-pass stage (pure streaming)

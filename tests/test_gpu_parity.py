@@ -142,7 +142,8 @@ def run_gpu(m, prob, n_iters, driver, delta=0.0, ls_batch=0):
     return plan, tr, x, d, cnt
 
 
-def test_three_drivers_are_bit_identical(m):
+def test_three_drivers_are_bit_identical(m, monkeypatch):
+    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")     # plans are compared with each other: they must share one partition
     prob = phantom(0)
     res = [run_gpu(m, prob, 25, drv) for drv in (m.DRIVER_HOST, m.DRIVER_GRAPH, m.DRIVER_PERSISTENT)]
     _, tr0, x0, d0, c0 = res[0]
@@ -185,7 +186,8 @@ def test_batched_line_search_is_bit_identical_to_sequential(m, cfg, n, monkeypat
         r[0].close()
 
 
-def test_runs_are_reproducible_and_resumable(m):
+def test_runs_are_reproducible_and_resumable(m, monkeypatch):
+    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")     # two plans are compared: they must share one partition
     prob = phantom(0)
     p1, tr1, x1, _, _ = run_gpu(m, prob, 20, m.DRIVER_PERSISTENT)
     plan = m.Plan(prob, max_iters=20, driver=m.DRIVER_PERSISTENT)
