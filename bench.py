@@ -58,13 +58,14 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def recorded_traffic(kernel):
-    """DRAM bytes per launch (read + write) from the committed ncu --set full capture (profiles/traffic.csv), else None."""
+def recorded_traffic(kernel, workload):
+    """DRAM bytes per launch (read + write) from the committed ncu --set full capture of this workload
+    (profiles/traffic.csv), else None."""
     try:
         import csv
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for row in csv.DictReader(f):
-                if row["kernel"] == kernel:
+                if row["kernel"] == kernel and row.get("workload", workload) == workload:
                     return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
     except Exception:
         pass
@@ -245,7 +246,7 @@ def run_ours(args):
             if 8 * prob.nnz > 2 * l2_bytes else "matrices are L2-resident: GB/s figures are L2, not HBM, bandwidth"
         dose_gbs = fwd_bytes / (dose_ms * 1e-3) / 1e9
         tr_gbs = tr_bytes / (tr_ms * 1e-3) / 1e9
-        t_dose, t_tr = recorded_traffic("k_dose"), recorded_traffic("k_transpose")
+        t_dose, t_tr = recorded_traffic("k_dose", prob.name), recorded_traffic("k_transpose", prob.name)
         roofline = {"bound": "hbm", "kernel": "k_dose (dose SpMV for %d trial point(s) + penalty + residual + objective partials)" % R,
                     "achieved": dose_gbs, "peak": peak, "unit": "GB/s", "frac": dose_gbs / peak, "peak_source": peak_src,
                     "traffic": t_dose, "algorithmic_bytes": fwd_bytes, "ms_per_launch": dose_ms,
