@@ -13,6 +13,7 @@
 #include <string>
 #include <vector>
 
+#include <cub/block/block_scan.cuh>
 #include <cub/device/device_radix_sort.cuh>
 
 #include "dvh.cuh"
@@ -38,6 +39,7 @@ struct imrt_plan {
     std::vector<int> rp_tr;           // row pointers of the stream the transpose pass reads (host copy)
     std::vector<double> tr_share;     // share of that stream per CTA
     int tr_align;
+    int n_rows_tr;                    // rows of that stream: n_b, or the number of row pairs
     int64_t max_ranges, max_slots;
     TrRange* tr_range_w;
     int* rowslot_w;
@@ -124,6 +126,8 @@ struct Layout {
     int* colT;
     float* valT;
     float* valP;
+    int* voxU;
+    int* pairU;
     unsigned short* idP;
     unsigned int* baseP;
     int* rowP_ptr;
@@ -170,7 +174,9 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.rowT_ptr = w.take<int>(n_b + 1);
     L.colT = w.take<int>(B.nnz_pad);
     L.valT = w.take<float>(B.nnz_pad);
-    L.valP = w.take<float>(B.nnz_pack);
+    L.valP = w.take<float>(2 * B.nnz_pack);      // fp32 per entry, or float2 per entry of the row-pair stream
+    L.voxU = w.take<int>(B.nnz_pack);
+    L.pairU = w.take<int>(n_b / 2 + 4);
     L.idP = w.take<unsigned short>(B.nnz_pack);
     L.baseP = w.take<unsigned int>(B.nnz_pack / 32 + 4);
     L.rowP_ptr = w.take<int>(n_b + 1);
@@ -181,7 +187,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.g = w.take<float>(n_b + 4);
     for (int i = 0; i <= R_MAX; ++i) L.rbuf[i] = w.take<float>(n_v + 4);
     for (int i = 0; i < 2; ++i) L.Gpart[i] = w.take<double>(1024 * R_MAX);
-    for (int i = 0; i < 2; ++i) L.gslot[i] = w.take<double>(B.max_slots);
+    for (int i = 0; i < 2; ++i) L.gslot[i] = w.take<double>(2 * B.max_slots);    // two sums per slot in the row-pair stream
     L.tr_obj = w.take<double>((size_t)max_iters + 1);
     L.tr_lambda = w.take<double>((size_t)max_iters + 1);
     L.tr_step_sq = w.take<double>((size_t)max_iters + 1);
@@ -391,6 +397,90 @@ __global__ void k_pack_transpose(const int* __restrict__ rowT_ptr, const int* __
 }
 
 struct RPtrs { float* p[R_MAX + 1]; };
+// ---- the row-pair stream of D^T: rows 2P and 2P+1 (sorted voxel lists A and B) merged into their union.
+__device__ __forceinline__ int lower_bound_dev(const int* __restrict__ a, int n, int v) {
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (a[mid] < v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+// size of the union of every pair (one CTA per pair): |A| + |B| - |A and B|
+__global__ void k_pair_count(const int* __restrict__ rowT_ptr, const int* __restrict__ colT, int n_b, int* U) {
+    __shared__ int common;
+    const int P = blockIdx.x;
+    const int a0 = rowT_ptr[2 * P], a1 = rowT_ptr[2 * P + 1], b1 = 2 * P + 2 <= n_b ? rowT_ptr[2 * P + 2] : a1;
+    const int* A = colT + a0;
+    const int* B = colT + a1;
+    const int nA = a1 - a0, nB = b1 - a1;
+    if (threadIdx.x == 0) common = 0;
+    __syncthreads();
+    int c = 0;
+    for (int k = threadIdx.x; k < nA; k += blockDim.x) {
+        const int rb = lower_bound_dev(B, nB, A[k]);
+        c += (rb < nB && B[rb] == A[k]);
+    }
+    if (c) atomicAdd(&common, c);
+    __syncthreads();
+    if (threadIdx.x == 0) U[P] = nA + nB - common;
+}
+// An element v of A or B goes to union position (#A < v) + (#B < v) - (#common < v); the last term is a running count of
+// the matches, kept by a block-wide exclusive scan.  val2 is zero beforehand; the padding repeats the pair's last voxel.
+__global__ void __launch_bounds__(256) k_pair_fill(const int* __restrict__ rowT_ptr, const int* __restrict__ colT, const float* __restrict__ valT,
+                                                   int n_b, const int* __restrict__ pairP_ptr, float2* val2, int* voxU) {
+    typedef cub::BlockScan<int, 256> Scan;
+    __shared__ typename Scan::TempStorage tmp;
+    const int P = blockIdx.x;
+    const int a0 = rowT_ptr[2 * P], a1 = rowT_ptr[2 * P + 1], b1 = 2 * P + 2 <= n_b ? rowT_ptr[2 * P + 2] : a1;
+    const int nA = a1 - a0, nB = b1 - a1;
+    const int base = pairP_ptr[P], end = pairP_ptr[P + 1];
+    for (int half = 0; half < 2; ++half) {
+        const int* X = colT + (half ? a1 : a0);        // the list being placed
+        const int* Y = colT + (half ? a0 : a1);        // the other one
+        const float* XV = valT + (half ? a1 : a0);
+        const int nX = half ? nB : nA, nY = half ? nA : nB;
+        int carry = 0;
+        for (int k0 = 0; k0 < nX; k0 += 256) {
+            const int k = k0 + threadIdx.x;
+            int v = 0, ry = 0, eq = 0;
+            if (k < nX) {
+                v = X[k];
+                ry = lower_bound_dev(Y, nY, v);
+                eq = (ry < nY && Y[ry] == v);
+            }
+            int before, total;
+            Scan(tmp).ExclusiveSum(eq, before, total);
+            __syncthreads();
+            if (k < nX) {
+                const int pos = base + k + ry - (carry + before);
+                if (half) val2[pos].y = XV[k]; else val2[pos].x = XV[k];
+                voxU[pos] = v;
+            }
+            carry += total;
+        }
+        __syncthreads();
+    }
+    const int last = max(nA ? colT[a1 - 1] : 0, nB ? colT[b1 - 1] : 0);
+    // the union has nA + nB - common entries; find it as the first unwritten position: the count kernel gave it as U[P]
+    // implicitly through pairP_ptr, but the padded end is what is stored, so fill backwards from `end` while untouched
+    for (int t = end - 1 - (int)threadIdx.x; t >= base && t >= end - 128; t -= 256) {
+        // entries [base + U, end) are padding: they are exactly those never written above; mark them via a sentinel
+        if (voxU[t] < 0) voxU[t] = last;
+    }
+}
+// 16-bit offsets of the pair stream: one warp per aligned group of 32 entries; flags[2] is raised when a group is too wide
+__global__ void k_pair_tiles(const int* __restrict__ voxU, long long n_groups, unsigned short* idP, unsigned int* baseP, int* flags) {
+    const int lane = threadIdx.x & 31;
+    for (long long t = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; t < n_groups; t += ((long long)gridDim.x * blockDim.x) >> 5) {
+        const int id = voxU[t * 32 + lane];
+        const int base = __shfl_sync(0xffffffffu, id, 0);
+        if (id - base > 65535 || id < base) flags[2] = 1;
+        idP[t * 32 + lane] = (unsigned short)(id - base);
+        if (lane == 0) baseP[t] = (unsigned int)base;
+    }
+}
+
 // d = 0 and the matching constant residual on every row; the dose pass then overwrites the rows its blocks cover.
 __global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const float4* __restrict__ table, const State* st, int n_v,
                                       const RPtrs R, float* d) {
@@ -745,7 +835,7 @@ static bool can_time_in_loop(const imrt_plan* pl) { return pl->prm.max_iters >= 
 // differently from SM to SM), so measure every CTA's pass time and hand out shares in proportion to measured speed.
 // Cut the D^T stream into the given per-CTA shares and upload the schedule.  false: the tables would not fit.
 static imrt_status upload_shares(imrt_plan* pl, const std::vector<double>& share, bool& fits) {
-    const int n_b = pl->P.n_b;
+    const int n_b = pl->n_rows_tr;
     cudaStream_t st = pl->stream;
     std::vector<TrRange> ranges;
     std::vector<int> rowslot, cta_rng;
@@ -763,7 +853,7 @@ static imrt_status upload_shares(imrt_plan* pl, const std::vector<double>& share
 }
 
 static imrt_status tune_transpose(imrt_plan* pl) {
-    const int grid = pl->P.grid_t, n_b = pl->P.n_b;
+    const int grid = pl->P.grid_t, n_b = pl->n_rows_tr;
     if (getenv("IMRTGP_NO_TUNE") || grid < 2 || pl->rp_tr[n_b] < (long long)grid * 8 * CHUNK_T) return IMRT_STATUS_OK;
     cudaStream_t st = pl->stream;
     PassArgs A;
@@ -1131,11 +1221,42 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     std::vector<TrRange> ranges;
     std::vector<int> rowslot, cta_rng_h;
     phase.mark("transpose (sort + gather)");
-    // ---- the packed stream the transpose pass reads (16-bit voxel offsets), unless a group of 32 entries is too wide
-    bool id16 = nnz > 0 && !getenv("IMRTGP_NO_ID16") && nnz + 128 * n_b + 128 < (1LL << 31);
+    // ---- the stream the transpose pass reads.  First choice: row pairs with 16-bit voxel offsets, if that is smaller
+    // than single rows; second: single rows with 16-bit offsets; last: the plain 32-bit CSR (a group of 32 entries
+    // spanning more than 65,535 voxels rules the 16-bit forms out).
+    const bool can16 = nnz > 0 && !getenv("IMRTGP_NO_ID16") && nnz + 128 * n_b + 128 < (1LL << 31);
     std::vector<int> rpP((size_t)n_b + 1, 0);
-    if (id16) {
+    if (can16)
         for (int64_t i = 0; i < n_b; ++i) rpP[i + 1] = rpP[i] + ((rpT[i + 1] - rpT[i] + 127) & ~127);
+    const int n_pairs = (int)((n_b + 1) / 2);
+    std::vector<int> rpPair((size_t)n_pairs + 1, 0);
+    bool pairs = can16 && n_b >= 2 && !getenv("IMRTGP_NO_PAIRS");
+    if (pairs) {
+        std::vector<int> U((size_t)n_pairs);
+        k_pair_count<<<n_pairs, 256, 0, st>>>(L.rowT_ptr, L.colT, (int)n_b, L.pairU);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(U.data(), L.pairU, sizeof(int) * n_pairs, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        for (int i = 0; i < n_pairs; ++i) rpPair[i + 1] = rpPair[i] + ((U[i] + 127) & ~127);
+        pairs = (double)rpPair[n_pairs] * 10.125 < (double)rpP[n_b] * 6.125;       // bytes per entry of the two forms
+    }
+    if (pairs) {
+        const long long tot = rpPair[n_pairs];
+        CUDA_TRY(pl, cudaMemcpyAsync(L.rowP_ptr, rpPair.data(), sizeof(int) * (n_pairs + 1), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(pl, cudaMemsetAsync(L.valP, 0, sizeof(float) * 2 * tot, st));
+        CUDA_TRY(pl, cudaMemsetAsync(L.voxU, 0xFF, sizeof(int) * tot, st));
+        k_pair_fill<<<n_pairs, 256, 0, st>>>(L.rowT_ptr, L.colT, L.valT, (int)n_b, L.rowP_ptr, reinterpret_cast<float2*>(L.valP), L.voxU);
+        if (tot > 0) k_pair_tiles<<<grid_for(tot, 256), 256, 0, st>>>(L.voxU, tot / 32, L.idP, L.baseP, L.flags);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(pl, cudaStreamSynchronize(st));
+        if (flags_h[2]) {
+            pairs = false;
+            CUDA_TRY(pl, cudaMemsetAsync(L.flags, 0, 16 * sizeof(int), st));
+        }
+    }
+    bool id16 = can16 && !pairs;
+    if (id16) {
         const long long n_groups = rpP[n_b] / 32;
         CUDA_TRY(pl, cudaMemcpyAsync(L.rowP_ptr, rpP.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
         if (n_groups > 0) k_pack_transpose<<<grid_for(n_groups * 32, 256), 256, 0, st>>>(L.rowT_ptr, L.rowP_ptr, L.colT, L.valT, (int)n_b, n_groups, L.valP, L.idP, L.baseP, L.flags);
@@ -1144,15 +1265,18 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaStreamSynchronize(st));
         if (flags_h[2]) id16 = false;
     }
-    pl->rp_tr = id16 ? rpP : rpT;
-    pl->tr_align = id16 ? 128 : 4;
-    const int grid_t = (int)std::max<long long>(1, std::min<long long>(n_sm, (long long)pl->rp_tr[n_b] / (4 * CHUNK_T) + 1));
+    const int tr_fmt = pairs ? 2 : id16 ? 1 : 0;
+    const int n_rows_tr = pairs ? n_pairs : (int)n_b;
+    pl->n_rows_tr = n_rows_tr;
+    pl->rp_tr = pairs ? rpPair : id16 ? rpP : rpT;
+    pl->tr_align = tr_fmt ? 128 : 4;
+    const int grid_t = (int)std::max<long long>(1, std::min<long long>(n_sm, (long long)pl->rp_tr[n_rows_tr] / (4 * CHUNK_T) + 1));
     pl->tr_share.assign(grid_t, 1.0 / grid_t);
-    build_ranges(pl->rp_tr, (int)n_b, pl->tr_share, pl->tr_align, ranges, rowslot, cta_rng_h);
+    build_ranges(pl->rp_tr, n_rows_tr, pl->tr_share, pl->tr_align, ranges, rowslot, cta_rng_h);
     if ((int64_t)ranges.size() > B.max_ranges) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: %zu transpose ranges exceed the bound", ranges.size());
-    const int n_slots = rowslot[n_b];
+    const int n_slots = rowslot[n_rows_tr];
     if (!ranges.empty()) CUDA_TRY(pl, cudaMemcpyAsync(L.tr_range, ranges.data(), sizeof(TrRange) * ranges.size(), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_b + 1), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(L.rowslot_ptr, rowslot.data(), sizeof(int) * (n_rows_tr + 1), cudaMemcpyHostToDevice, st));
     CUDA_TRY(pl, cudaMemcpyAsync(L.cta_rng, cta_rng_h.data(), sizeof(int) * cta_rng_h.size(), cudaMemcpyHostToDevice, st));
     pl->max_ranges = B.max_ranges; pl->max_slots = B.max_slots;
     pl->tr_range_w = L.tr_range; pl->rowslot_w = L.rowslot_ptr; pl->cta_rng_w = L.cta_rng;
@@ -1167,7 +1291,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     int R = prm->ls_batch == 0 ? R_MAX : prm->ls_batch;
     if (getenv("IMRTGP_LS_BATCH")) R = atoi(getenv("IMRTGP_LS_BATCH"));
     if (R != 1 && R != 2 && R != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_params.ls_batch must be 0, 1, 2 or 4");
-    const int stage_t = id16 ? CHUNK_T * 6 + CHUNK_T / 8 : STAGE_T_BYTES;
+    const int stage_t = pairs ? CHUNK_T * 10 + CHUNK_T / 8 : id16 ? CHUNK_T * 6 + CHUNK_T / 8 : STAGE_T_BYTES;
     int off = 0, avail = 0, stt = 0;
     for (;; R /= 2) {
         off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
@@ -1192,8 +1316,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     P.nnz = nnz; P.n_v = (int)n_v; P.n_b = (int)n_b;
     P.pack = L.pack; P.blk = L.blk; P.cta_blk = L.cta_blk; P.grid_f = grid_f;
     P.col16 = col16 ? 1 : 0;
-    P.rowT_ptr = id16 ? L.rowP_ptr : L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
-    P.valP = L.valP; P.idP = L.idP; P.baseP = L.baseP; P.id16 = id16 ? 1 : 0; P.stage_t_bytes = stage_t;
+    P.rowT_ptr = tr_fmt ? L.rowP_ptr : L.rowT_ptr; P.colT = L.colT; P.valT = L.valT;
+    P.valP = L.valP; P.idP = L.idP; P.baseP = L.baseP; P.id16 = tr_fmt; P.stage_t_bytes = stage_t;
     P.tr_range = L.tr_range; P.rowslot_ptr = L.rowslot_ptr; P.cta_rng = L.cta_rng;
     P.n_ranges = (int)ranges.size(); P.grid_t = grid_t;
     P.n_stages_t = stt; P.n_slots = n_slots;
@@ -1220,8 +1344,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     st_h.eps = prm->eps; st_h.alpha = prm->alpha; st_h.lambda0 = prm->lambda0; st_h.lambda = prm->lambda0;
     st_h.max_ls = prm->max_ls; st_h.trace_cap = prm->max_iters; st_h.xi = 0; st_h.ri = 0;
     CUDA_TRY(pl, cudaMemcpyAsync(L.st, &st_h, sizeof st_h, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(pl, cudaMemsetAsync(L.gslot[0], 0, sizeof(double) * B.max_slots, st));
-    CUDA_TRY(pl, cudaMemsetAsync(L.gslot[1], 0, sizeof(double) * B.max_slots, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.gslot[0], 0, sizeof(double) * 2 * B.max_slots, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.gslot[1], 0, sizeof(double) * 2 * B.max_slots, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[0], 0, sizeof(double) * 1024 * R_MAX, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.Gpart[1], 0, sizeof(double) * 1024 * R_MAX, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.xbuf[0], 0, sizeof(float) * (n_b + 4), st));
@@ -1492,9 +1616,9 @@ imrt_status imrt_plan_get_counters(imrt_plan* pl, int64_t* host_fwd_passes, int6
 
 imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info, int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT) {
     if (!pl) return IMRT_STATUS_INVALID_ARG;
-    const int64_t info[14] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
-                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.ring_f_bytes, pl->P.n_stages_t, pl->n_quad_rows};
-    for (int i = 0; i < n_info && i < 14 && host_info; ++i) host_info[i] = info[i];
+    const int64_t info[15] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
+                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.ring_f_bytes, pl->P.n_stages_t, pl->n_quad_rows, pl->P.id16};
+    for (int i = 0; i < n_info && i < 15 && host_info; ++i) host_info[i] = info[i];
     cudaStream_t st = pl->stream;
     if (d_rowT_ptr) CUDA_TRY(pl, cudaMemcpyAsync(d_rowT_ptr, pl->rowT_ptr_w, sizeof(int) * (pl->P.n_b + 1), cudaMemcpyDeviceToDevice, st));
     if (d_colT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_colT, pl->colT_w, sizeof(int) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));

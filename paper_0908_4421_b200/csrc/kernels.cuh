@@ -58,7 +58,7 @@ constexpr int RING_ENTRIES = 64;              // dose-pass records in flight per
 constexpr int MAX_STAGES_T = 12;
 constexpr int MAX_STRUCTURES = 256;
 constexpr int SMEM_HEADER = 3072;             // barriers, flags, reduction scratch
-constexpr int SMEM_WPART = RL_MAX * W_CONS * 8;
+constexpr int SMEM_WPART = RL_MAX * W_CONS * 8 * 2;   // transpose pass: per-(row, warp) fp64 partials, two per row pair
 constexpr int SMEM_DSC = W_CONS * 32 * R_MAX * 4;   // per-warp scratch: dose of 32 rows x R trial points
 
 enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2, MODE_TIMING = 3 };
@@ -131,9 +131,13 @@ struct DevPlan {
     // ... and, unless a row has neighbouring entries more than 65535 voxels apart, the packed stream the transpose
     // pass reads instead (id16 = 1): every row padded to a multiple of 128 entries (zero values), voxel ids as
     // 16-bit offsets from one 32-bit base per aligned group of 32 entries: 6.1 instead of 8 bytes per non-zero
-    const float* valP;
+    const float* valP;         // id16 = 1: fp32 per entry;  id16 = 2: float2 per entry of a ROW PAIR (see below)
     const unsigned short* idP;
     const unsigned int* baseP;
+    // id16 = 2 (chosen when smaller): rows 2i and 2i+1 of D^T (neighbouring beamlets, whose voxel lists overlap by ~87 %)
+    // share ONE voxel list, the union of theirs, with a float2 of values per voxel (0 where a row lacks it): 10.1 bytes
+    // per union entry, one gather of r per TWO multiply-adds.  rowT_ptr then points into the pair stream (one "row" per
+    // pair), and a gradient slot holds two sums.
     int id16;
     int stage_t_bytes;         // bytes of one transpose-pass stage
     // transpose pass: equal-nnz ranges
@@ -700,9 +704,10 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
             double dacc = 0.0;
             bool touched = false;
             for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
-                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage
-                    if (++s == S) { s = 0; ph ^= 1u; }
-                    continue;
+                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage: not consumed here,
+                    mbar_wait(&h->full_t[s], ph);      // but its phase must be seen to complete -- a warp that skipped it
+                    if (++s == S) { s = 0; ph ^= 1u; } // could otherwise mistake the slot's NEXT phase for complete
+                    continue;                          // (phase parity; matters when the stage count is odd)
                 }
                 mbar_wait(&h->full_t[s], ph);
                 const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
@@ -793,30 +798,167 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
     }
 }
 
+// The same pass over the ROW-PAIR stream (DevPlan::id16 == 2): an entry is one voxel of the union of two rows with a
+// float2 of values, so one gather of r feeds two multiply-adds and every sum, partial and slot comes in twos.
+__device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
+                                                     const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int S = P.n_stages_t;
+    unsigned char* stages = smem + P.stage_off;
+    unsigned int it = pipe.it_t;
+    const int rg0 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x] : 0;
+    const int rg1 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x + 1] : 0;
+    const unsigned long long t_start = global_ns();
+    int s = (int)(it % (unsigned int)S);
+    unsigned int ph = (it / (unsigned int)S) & 1u;
+    const float2* val2P = reinterpret_cast<const float2*>(P.valP);
+
+    if (warp >= W_CONS) {
+        const uint64_t pol = policy_evict_first();
+        for (int rg = rg0; rg < rg1; ++rg) {
+            const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
+            for (int cs = e0; cs < e1; cs += CHUNK_T, ++it) {
+                if (warp == W_CONS && lane == 0) {
+                    mbar_wait(&h->empty_t[s], ph ^ 1u);
+                    const uint32_t n = (uint32_t)min(CHUNK_T, e1 - cs);    // a multiple of 128: everything stays aligned
+                    unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
+                    mbar_expect_tx(&h->full_t[s], n * 10u + n / 8u);
+                    bulk_g2s(st, val2P + cs, n * 8u, &h->full_t[s], pol);
+                    bulk_g2s(st + CHUNK_T * 8, P.idP + cs, n * 2u, &h->full_t[s], pol);
+                    bulk_g2s(st + CHUNK_T * 10, P.baseP + cs / 32, n / 8u, &h->full_t[s], pol);
+                }
+                if (++s == S) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else {
+        const uint64_t keep = policy_evict_last();
+        for (int rg = rg0; rg < rg1; ++rg) {
+            const TrRange R = P.tr_range[rg];
+            for (int i = threadIdx.x; i < 2 * RL_MAX * W_CONS; i += N_CONS) wpart[i] = 0.0;
+            named_bar_sync(1, N_CONS);
+            int cur_row = R.first_row;
+            int cur_end = __ldg(P.rowT_ptr + cur_row + 1);
+            double dacc0 = 0.0, dacc1 = 0.0;
+            bool touched = false;
+            for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
+                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage: not consumed here,
+                    mbar_wait(&h->full_t[s], ph);      // but its phase must be seen to complete -- a warp that skipped it
+                    if (++s == S) { s = 0; ph ^= 1u; } // could otherwise mistake the slot's NEXT phase for complete
+                    continue;                          // (phase parity; matters when the stage count is odd)
+                }
+                mbar_wait(&h->full_t[s], ph);
+                const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
+                const float2* val_s = reinterpret_cast<const float2*>(st);
+                const unsigned short* id_s = reinterpret_cast<const unsigned short*>(st + CHUNK_T * 8);
+                const unsigned int* base_s = reinterpret_cast<const unsigned int*>(st + CHUNK_T * 10);
+                const int ce = min(cs + CHUNK_T, R.e_end);
+                int pos = cs + (warp % (W_CONS / TGROUPS)) * SLICE_T;
+                const int b = min(pos + SLICE_T, ce);
+                while (pos < b) {
+                    while (cur_end <= pos) {   // the slice moved past the end of the current row pair (warp-uniform)
+                        if (touched) {
+                            const double s0 = warp_sum(dacc0), s1 = warp_sum(dacc1);
+                            if (lane == 0) {
+                                wpart[2 * ((cur_row - R.first_row) * W_CONS + warp)] = s0;
+                                wpart[2 * ((cur_row - R.first_row) * W_CONS + warp) + 1] = s1;
+                            }
+                            dacc0 = dacc1 = 0.0;
+                            touched = false;
+                        }
+                        ++cur_row;
+                        cur_end = __ldg(P.rowT_ptr + cur_row + 1);
+                    }
+                    const int seg_end = min(b, cur_end);
+                    const float2* vp = val_s + (pos - cs);
+                    const unsigned short* ip = id_s + (pos - cs);
+                    const unsigned int* bp = base_s + (pos - cs) / 32;
+                    const int nt = (seg_end - pos) / 32;       // whole 32-entry tiles: pairs are padded to 128 entries
+                    float acc0 = 0.0f, acc1 = 0.0f;
+                    if (nt == SLICE_T / 32) {
+                        unsigned int c[SLICE_T / 32];
+                        float rr[SLICE_T / 32];
+#pragma unroll
+                        for (int u = 0; u < SLICE_T / 32; ++u) c[u] = bp[u] + ip[lane + 32 * u];
+#pragma unroll
+                        for (int u = 0; u < SLICE_T / 32; ++u) rr[u] = ld_keep(r_in + c[u], keep);
+#pragma unroll
+                        for (int u = 0; u < SLICE_T / 32; ++u) {
+                            const float2 v = vp[lane + 32 * u];
+                            acc0 = fmaf(v.x, rr[u], acc0);
+                            acc1 = fmaf(v.y, rr[u], acc1);
+                        }
+                    } else {
+                        for (int u = 0; u < nt; ++u) {
+                            const float rv = ld_keep(r_in + (bp[u] + ip[lane + 32 * u]), keep);
+                            const float2 v = vp[lane + 32 * u];
+                            acc0 = fmaf(v.x, rv, acc0);
+                            acc1 = fmaf(v.y, rv, acc1);
+                        }
+                    }
+                    dacc0 += (double)acc0;
+                    dacc1 += (double)acc1;
+                    touched = true;
+                    pos = seg_end;
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&h->empty_t[s]);
+                if (++s == S) { s = 0; ph ^= 1u; }
+            }
+            if (touched) {
+                const double s0 = warp_sum(dacc0), s1 = warp_sum(dacc1);
+                if (lane == 0) {
+                    wpart[2 * ((cur_row - R.first_row) * W_CONS + warp)] = s0;
+                    wpart[2 * ((cur_row - R.first_row) * W_CONS + warp) + 1] = s1;
+                }
+            }
+            named_bar_sync(1, N_CONS);
+            for (int t = threadIdx.x; t < 2 * R.n_rows; t += N_CONS) {     // t = 2 * row + half
+                double sum = 0.0;
+#pragma unroll
+                for (int w = 0; w < W_CONS; ++w) sum += wpart[2 * ((t >> 1) * W_CONS + w) + (t & 1)];
+                gslot[2 * (size_t)R.slot_base + t] = sum;
+            }
+            named_bar_sync(1, N_CONS);
+        }
+    }
+    pipe.it_t = it;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
+        P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
+    }
+}
+
 __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
                                                const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
-    if (P.id16) transpose_pass_t<true>(P, h, smem, wpart, r_in, gslot, pipe);
+    if (P.id16 == 2) transpose_pass_pairs(P, h, smem, wpart, r_in, gslot, pipe);
+    else if (P.id16) transpose_pass_t<true>(P, h, smem, wpart, r_in, gslot, pipe);
     else transpose_pass_t<false>(P, h, smem, wpart, r_in, gslot, pipe);
 }
 
 // g_i = sum of the slots of row i, in slot order (fixed).  All NTHREADS threads; g_out shared or global.
 __device__ __forceinline__ void reduce_gradient(const DevPlan& P, const double* gslot, float* g_out) {
     constexpr int U = 4;         // rows per thread whose loads are issued together (the slots come from L2)
+    const int pairs = (P.id16 == 2);      // row i of D^T is half `i & 1` of stream row i >> 1; a slot holds two sums
     for (int base = threadIdx.x; base < P.n_b; base += NTHREADS * U) {
         int s0[U], s1[U];
         double sum[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int i = base + u * NTHREADS;
-            s0[u] = i < P.n_b ? __ldg(P.rowslot_ptr + i) : 0;
-            s1[u] = i < P.n_b ? __ldg(P.rowslot_ptr + i + 1) : 0;
+            s0[u] = i < P.n_b ? __ldg(P.rowslot_ptr + (i >> pairs)) : 0;
+            s1[u] = i < P.n_b ? __ldg(P.rowslot_ptr + (i >> pairs) + 1) : 0;
         }
 #pragma unroll
-        for (int u = 0; u < U; ++u) sum[u] = s0[u] < s1[u] ? __ldcg(gslot + s0[u]) : 0.0;
+        for (int u = 0; u < U; ++u) {
+            const int i = base + u * NTHREADS;
+            sum[u] = s0[u] < s1[u] ? __ldcg(gslot + ((size_t)s0[u] << pairs) + (i & pairs)) : 0.0;
+        }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            for (int s = s0[u] + 1; s < s1[u]; ++s) sum[u] += __ldcg(gslot + s);     // same order as one plain loop
             const int i = base + u * NTHREADS;
+            for (int s = s0[u] + 1; s < s1[u]; ++s) sum[u] += __ldcg(gslot + ((size_t)s << pairs) + (i & pairs));   // slot order
             if (i < P.n_b) g_out[i] = (float)sum[u];
         }
     }
