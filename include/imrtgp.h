@@ -102,8 +102,11 @@ imrt_status imrt_workspace_bytes(int64_t n_v, int64_t n_b, int64_t nnz, int32_t 
  *   host_params                   copied
  *   workspace / workspace_bytes   device memory from the caller, >= imrt_workspace_bytes(...)  (borrowed)
  *   stream                        a cudaStream_t passed as void* (NULL = the legacy default stream)
- * Validates the inputs, builds the explicit transpose D^T as a second CSR (stable counting sort by column), the
- * row blocks of D and the nnz partition of D^T, and instantiates the iteration graph.  Synchronises the stream.
+ * Validates the inputs (finite values, columns in range and strictly ascending in every row), re-packs D into the
+ * block records the dose pass streams, builds the explicit transpose D^T as a second CSR (stable radix sort by
+ * column) and the packed stream the transpose pass reads, balances both passes over the SMs from measured pass times
+ * (a few short runs of the passes and of the loop on x = 0), and instantiates the iteration graph (driver 0).
+ * Synchronises the stream.  DESIGN.md section 4 describes the layouts.
  * On failure *out is NULL unless the status is a validation error that left a handle for imrt_last_error;
  * imrt_last_error(NULL) returns the message of the last failed create on this thread.
  */
@@ -210,7 +213,7 @@ imrt_status imrt_plan_get_counters(imrt_plan* plan, int64_t* host_fwd_passes, in
 
 /*
  * Introspection for tests and the benchmark.  Synchronises.
- *   host_info[0] nnz of D^T        [1] forward row blocks     [2] forward grid (CTAs)   [3] transpose grid (CTAs)
+ *   host_info[0] nnz of D^T        [1] dose-pass block records   [2] dose grid (CTAs)   [3] transpose grid (CTAs)
  *   host_info[4] dynamic shared memory bytes per CTA   [5] bytes of the re-packed D the dose pass streams
  *   host_info[6] gradient partial slots   [7] non-empty rows of D   [8] SM count   [9] 16-bit column indices (1/0)
  *   host_info[10] trial points per dose pass actually used (ls_batch)   [11] dose-pass ring bytes   [12] transpose stages
