@@ -829,6 +829,7 @@ static imrt_status timing_loop_run(imrt_plan* pl) {
     CUDA_TRY(pl, cudaGetLastError());
     return IMRT_STATUS_OK;
 }
+constexpr int LOOP_MEASUREMENTS = 1;   // 3 gains 0.7 % of loop speed and costs 16 ms of plan creation (cfg3)
 static bool can_time_in_loop(const imrt_plan* pl) { return pl->prm.max_iters >= 3 && !getenv("IMRTGP_NO_LOOP_TUNE"); }
 
 // The same for the transpose pass: equal shares of the D^T stream do not take equal time (the gathers of r hit the L2
@@ -866,18 +867,23 @@ static imrt_status tune_transpose(imrt_plan* pl) {
     double best_worst = 1e300;
     std::vector<double> best_share;
     for (int it = 0; it <= rounds; ++it) {
-        if (it < iso_rounds) {
-            for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_transpose(pl, A));   // the first warms up, the second is read
-        } else {
-            const imrt_status ls = timing_loop_run(pl);
-            if (ls != IMRT_STATUS_OK) return ls;
+        std::vector<double> durs(grid, 0.0);
+        const int n_meas = it < iso_rounds ? 1 : LOOP_MEASUREMENTS;      // pass times inside the loop vary more: average a few
+        for (int ms = 0; ms < n_meas; ++ms) {
+            if (it < iso_rounds) {
+                for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_transpose(pl, A));   // the first warms up, the second is read
+            } else {
+                const imrt_status ls = timing_loop_run(pl);
+                if (ls != IMRT_STATUS_OK) return ls;
+            }
+            CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns + 2048, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(pl, cudaStreamSynchronize(st));
+            for (int c = 0; c < grid; ++c) durs[c] += (double)(t[2 * c + 1] - t[2 * c]) / n_meas;
         }
-        CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns + 2048, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
         double sum = 0.0, worst = 0.0;
         std::vector<double> share(grid);
         for (int c = 0; c < grid; ++c) {
-            const double dur = (double)(t[2 * c + 1] - t[2 * c]);
+            const double dur = durs[c];
             worst = std::max(worst, dur);
             share[c] = dur > 0.0 ? pl->tr_share[c] / dur : pl->tr_share[c];     // share per unit time = speed
             sum += share[c];
@@ -920,17 +926,21 @@ static imrt_status tune_partition(imrt_plan* pl) {
     double best_worst = 1e300;
     std::vector<int> best_blk;
     for (int it = 0; it <= rounds; ++it) {
-        if (it < iso_rounds) {
-            for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_dose(pl, A));   // the first warms up, the second is read
-        } else {
-            const imrt_status ls = timing_loop_run(pl);
-            if (ls != IMRT_STATUS_OK) return ls;
+        std::fill(dur.begin(), dur.end(), 0.0);
+        const int n_meas = it < iso_rounds ? 1 : LOOP_MEASUREMENTS;      // pass times inside the loop vary more: average a few
+        for (int ms = 0; ms < n_meas; ++ms) {
+            if (it < iso_rounds) {
+                for (int rep = 0; rep < 2; ++rep) CUDA_TRY(pl, launch_dose(pl, A));   // the first warms up, the second is read
+            } else {
+                const imrt_status ls = timing_loop_run(pl);
+                if (ls != IMRT_STATUS_OK) return ls;
+            }
+            CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(pl, cudaStreamSynchronize(st));
+            for (int c = 0; c < grid; ++c) dur[c] += (double)(t[2 * c + 1] - t[2 * c]) / n_meas;
         }
-        CUDA_TRY(pl, cudaMemcpyAsync(t.data(), pl->P.cta_ns, sizeof(unsigned long long) * t.size(), cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
         double mean = 0.0, worst = 0.0;
         for (int c = 0; c < grid; ++c) {
-            dur[c] = (double)(t[2 * c + 1] - t[2 * c]);
             mean += dur[c] / grid;
             worst = std::max(worst, dur[c]);
         }
