@@ -244,20 +244,26 @@ def run_ours(args):
         l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
         flush = "inputs larger than L2 (D and D^T %.0f MB each vs %.0f MB L2)" % (8 * prob.nnz / 1e6, l2_bytes / 1e6) \
             if 8 * prob.nnz > 2 * l2_bytes else "matrices are L2-resident: GB/s figures are L2, not HBM, bandwidth"
-        dose_gbs = fwd_bytes / (dose_ms * 1e-3) / 1e9
-        tr_gbs = tr_bytes / (tr_ms * 1e-3) / 1e9
+        # the library re-encodes the matrices, so the roofline fraction uses the bytes its own layouts make
+        # a pass move (packed D + residual writes + x, g; the D^T stream + one read of r + g), and the CSR-equivalent
+        # "effective" GB/s (algorithmic bytes / time) is quoted separately
+        dose_layout = info["pack_bytes"] + 16 * info["fwd_blocks"] + R * 4 * info["nonempty_rows"] + 8 * prob.n_b
+        tr_layout = info["tr_stream_bytes"] + 4 * prob.n_v + 4 * prob.n_b
+        dose_gbs = dose_layout / (dose_ms * 1e-3) / 1e9
+        tr_gbs = tr_layout / (tr_ms * 1e-3) / 1e9
+        dose_eff = fwd_bytes / (dose_ms * 1e-3) / 1e9
+        tr_eff = tr_bytes / (tr_ms * 1e-3) / 1e9
         t_dose, t_tr = recorded_traffic("k_dose", prob.name), recorded_traffic("k_transpose", prob.name)
         roofline = {"bound": "hbm", "kernel": "k_dose (dose SpMV for %d trial point(s) + penalty + residual + objective partials)" % R,
                     "achieved": dose_gbs, "peak": peak, "unit": "GB/s", "frac": dose_gbs / peak, "peak_source": peak_src,
-                    "traffic": t_dose, "algorithmic_bytes": fwd_bytes, "ms_per_launch": dose_ms,
-                    "dram_gbs": (t_dose / (dose_ms * 1e-3) / 1e9) if t_dose else None,
-                    "dram_frac": (t_dose / (dose_ms * 1e-3) / 1e9 / peak) if t_dose else None,
-                    "note": "the packed layouts move fewer bytes than the CSR-based algorithmic count: dram_* = ncu traffic / live time",
+                    "traffic": t_dose, "bytes_per_launch": dose_layout, "ms_per_launch": dose_ms,
+                    "effective_csr_gbs": dose_eff, "algorithmic_csr_bytes": fwd_bytes,
+                    "note": "achieved / frac use the bytes of the library's own layouts (quad-row records); effective_csr_gbs = "
+                            "CSR-equivalent algorithmic bytes / time; traffic = ncu dram bytes of the committed capture",
                     "frac_of_nominal_8TBs": dose_gbs / 8000.0}
         roofline_tr = {"bound": "hbm", "kernel": "k_transpose (D^T r on the explicit transpose CSR)", "achieved": tr_gbs,
-                       "peak": peak, "unit": "GB/s", "frac": tr_gbs / peak, "traffic": t_tr, "dram_gbs": (t_tr / (tr_ms * 1e-3) / 1e9) if t_tr else None,
-                       "dram_frac": (t_tr / (tr_ms * 1e-3) / 1e9 / peak) if t_tr else None,
-                       "algorithmic_bytes": tr_bytes, "ms_per_launch": tr_ms, "frac_of_nominal_8TBs": tr_gbs / 8000.0}
+                       "peak": peak, "unit": "GB/s", "frac": tr_gbs / peak, "traffic": t_tr, "bytes_per_launch": tr_layout, "ms_per_launch": tr_ms,
+                       "effective_csr_gbs": tr_eff, "algorithmic_csr_bytes": tr_bytes, "frac_of_nominal_8TBs": tr_gbs / 8000.0}
 
         # ---------------- time-to-plan: the config's own stopping rule from x0 (device-resident, inputs in HBM)
         cfg = synth_inputs.CONFIGS[args.config]
@@ -326,7 +332,9 @@ def run_ours(args):
                    "trials_per_iter": float(res.n_trials.mean())}
 
         extra = {"roofline": roofline, "roofline_transpose": roofline_tr, "time_to_plan": ttp, "e2e": e2e, "cpu_baseline": cpu,
-                 "loop_gbs": loop_bytes / (ms * 1e-3) / 1e9, "loop_frac_of_peak": loop_bytes / (ms * 1e-3) / 1e9 / peak,
+                 "loop_effective_csr_gbs": loop_bytes / (ms * 1e-3) / 1e9,
+                 "loop_gbs": (passes_timed * dose_layout + K * tr_layout) / (ms * 1e-3) / 1e9,
+                 "loop_frac_of_peak": (passes_timed * dose_layout + K * tr_layout) / (ms * 1e-3) / 1e9 / peak,
                  "flush": flush}
 
     if rank == 0:

@@ -219,6 +219,7 @@ imrt_status imrt_plan_get_counters(imrt_plan* plan, int64_t* host_fwd_passes, in
  *   host_info[10] trial points per dose pass actually used (ls_batch)   [11] dose-pass ring bytes   [12] transpose stages
  *   host_info[13] rows of D stored in quad format (4 neighbouring rows sharing one column list)
  *   host_info[14] stream the transpose pass reads: 0 plain 32-bit CSR, 1 rows with 16-bit voxel offsets, 2 row pairs
+ *   host_info[15] bytes of that stream
  * d_rowT_ptr (int32 [n_b+1]), d_colT (int32 [nnz]), d_valT (fp32 [nnz]): if non-NULL receive a copy of D^T (device).
  */
 imrt_status imrt_plan_get_info(imrt_plan* plan, int64_t* host_info, int32_t n_info,

@@ -242,7 +242,7 @@ def imrt_plan_get_counters(plan):
 
 
 INFO_KEYS = ("nnzT", "fwd_blocks", "fwd_grid", "tr_grid", "smem_bytes", "pack_bytes", "g_slots", "nonempty_rows", "n_sm", "col16",
-             "ls_batch", "fwd_ring_bytes", "tr_stages", "quad_rows", "tr_format")
+             "ls_batch", "fwd_ring_bytes", "tr_stages", "quad_rows", "tr_format", "tr_stream_bytes")
 
 
 def imrt_plan_get_info(plan, rowT_ptr=None, colT=None, valT=None) -> dict:

@@ -40,6 +40,7 @@ struct imrt_plan {
     std::vector<double> tr_share;     // share of that stream per CTA
     int tr_align;
     int n_rows_tr;                    // rows of that stream: n_b, or the number of row pairs
+    int64_t tr_stream_bytes;          // bytes of that stream (values + voxel ids / offsets + bases)
     int64_t max_ranges, max_slots;
     TrRange* tr_range_w;
     int* rowslot_w;
@@ -1278,6 +1279,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     const int tr_fmt = pairs ? 2 : id16 ? 1 : 0;
     const int n_rows_tr = pairs ? n_pairs : (int)n_b;
     pl->n_rows_tr = n_rows_tr;
+    pl->tr_stream_bytes = pairs ? (int64_t)rpPair[n_pairs] * 10 + rpPair[n_pairs] / 8
+                          : id16 ? (int64_t)rpP[n_b] * 6 + rpP[n_b] / 8 : (int64_t)nnz * 8;
     pl->rp_tr = pairs ? rpPair : id16 ? rpP : rpT;
     pl->tr_align = tr_fmt ? 128 : 4;
     const int grid_t = (int)std::max<long long>(1, std::min<long long>(n_sm, (long long)pl->rp_tr[n_rows_tr] / (4 * CHUNK_T) + 1));
@@ -1626,9 +1629,9 @@ imrt_status imrt_plan_get_counters(imrt_plan* pl, int64_t* host_fwd_passes, int6
 
 imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info, int32_t* d_rowT_ptr, int32_t* d_colT, float* d_valT) {
     if (!pl) return IMRT_STATUS_INVALID_ARG;
-    const int64_t info[15] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
-                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.ring_f_bytes, pl->P.n_stages_t, pl->n_quad_rows, pl->P.id16};
-    for (int i = 0; i < n_info && i < 15 && host_info; ++i) host_info[i] = info[i];
+    const int64_t info[16] = {(int64_t)pl->P.nnz, pl->n_blk, pl->P.grid_f, pl->P.grid_t, (int64_t)pl->smem_bytes, pl->pack_bytes,
+                              pl->P.n_slots, pl->n_nonempty, pl->n_sm, pl->P.col16, pl->P.R, pl->P.ring_f_bytes, pl->P.n_stages_t, pl->n_quad_rows, pl->P.id16, pl->tr_stream_bytes};
+    for (int i = 0; i < n_info && i < 16 && host_info; ++i) host_info[i] = info[i];
     cudaStream_t st = pl->stream;
     if (d_rowT_ptr) CUDA_TRY(pl, cudaMemcpyAsync(d_rowT_ptr, pl->rowT_ptr_w, sizeof(int) * (pl->P.n_b + 1), cudaMemcpyDeviceToDevice, st));
     if (d_colT && pl->P.nnz) CUDA_TRY(pl, cudaMemcpyAsync(d_colT, pl->colT_w, sizeof(int) * pl->P.nnz, cudaMemcpyDeviceToDevice, st));
