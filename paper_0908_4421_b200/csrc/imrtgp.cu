@@ -104,7 +104,7 @@ struct Bounds {
 Bounds bounds_for(int64_t n_v, int64_t n_b, int64_t nnz) {
     Bounds b;
     const int64_t slots = nnz + 3 * n_v;    // every row padded to a multiple of 4 slots
-    b.max_blk = 4 * (slots / MIN_CHUNK_SLOTS + 1) + 4 * (n_v / SEG_ROWS + 1) + n_v / 16 + 8 + 8 * TARGET_RECORDS;
+    b.max_blk = 4 * (slots / ROW_REC_SLOTS + 1) + 4 * (n_v / SEG_ROWS + 1) + n_v / 16 + 8 + 8 * TARGET_RECORDS;
     b.max_meta = n_v + b.max_blk * (META_HDR + 2 + 3) + 8;
     b.max_pack = (size_t)b.max_meta * 4 + (size_t)slots * 8 + (size_t)b.max_blk * (128 + 48) + 256;
     b.max_ranges = 2 * 1024 + n_b / RL_MAX + 2 * (n_b / RL_MAX + 1) + 4;
@@ -569,7 +569,7 @@ struct RecordCaps {
 static RecordCaps record_caps(int64_t n_v, int64_t nnz) {
     auto clampi = [](int64_t v, int lo, int hi) { return (int)std::max<int64_t>(lo, std::min<int64_t>(hi, v)); };
     RecordCaps c;
-    c.chunk_slots = clampi((nnz / TARGET_RECORDS + 3) & ~(int64_t)3, 64, MIN_CHUNK_SLOTS);
+    c.chunk_slots = clampi((nnz / TARGET_RECORDS + 3) & ~(int64_t)3, 64, ROW_REC_SLOTS);
     c.max_rows = clampi(n_v / TARGET_RECORDS, 8, MAXROWS_F);
     c.quad_cap = clampi(nnz / 3 / TARGET_RECORDS, 32, QUAD_CAP);
     return c;
@@ -1153,7 +1153,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     memset(&P, 0, sizeof P);
 
     // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero); a block holds
-    // MIN_CHUNK_SLOTS slots unless a longer row forces more
+    // ROW_REC_SLOTS slots unless a longer row forces more
     const bool col16 = n_b <= 65536 && !getenv("IMRTGP_COL32");
     int max_row = 0;
     for (int64_t j = 0; j < n_v; ++j) max_row = std::max(max_row, rp[j + 1] - rp[j]);

@@ -38,7 +38,7 @@ constexpr int N_PROD = 2;                     // producer warps of the dose pass
 constexpr int NTHREADS = N_CONS + 32 * N_PROD;
 // dose pass: D is re-packed once into self-contained block records (one bulk copy each, see DevPlan::pack)
 constexpr int META_HDR = 4;                   // header words {rows, first row, 0, slots}
-constexpr int MIN_CHUNK_SLOTS = 1024;         // slot capacity of a block unless a longer row forces more
+constexpr int ROW_REC_SLOTS = 1024;           // slots per row-format record (fewer for small matrices; one longer row alone)
 constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
 constexpr int MAXROWS_F = 256;                // rows per block
 constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered up to this many beamlets (pack-kernel bitmap)
