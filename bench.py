@@ -413,7 +413,7 @@ def main():
     ap.add_argument("--driver", default="persistent", choices=sorted(DRIVERS))
     ap.add_argument("--ls-batch", type=int, default=0, choices=[0, 1, 2, 4],
                     help="line-search trial points per dose pass (0 = library default, 4)")
-    ap.add_argument("--cpu-iters", type=int, default=25, help="oracle iterations timed for cpu_baseline")
+    ap.add_argument("--cpu-iters", type=int, default=60, help="oracle iterations timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sharded", action="store_true",
                     help="one problem over all ranks (row slabs of D, NCCL all-reduces) instead of one replica per rank")

@@ -1308,8 +1308,9 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     int off = 0, avail = 0, stt = 0;
     for (;; R /= 2) {
         off = SMEM_HEADER + ((n_structures * 16 + 127) & ~127);
-        P.wpart_off = off; off += SMEM_WPART;
-        P.dsc_off = off; off += SMEM_DSC;
+        P.wpart_off = off;                    // the transpose pass's partials and the dose pass's row scratch share one
+        P.dsc_off = off;                      // region: a CTA is never in both passes at once
+        off += SMEM_WPART > SMEM_DSC ? SMEM_WPART : SMEM_DSC;
         P.x_off = off; off += nb_pad * 4 * R;
         P.g_off = off; off += nb_pad * 4;
         off = (off + 127) & ~127;
