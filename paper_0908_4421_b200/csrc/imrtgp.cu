@@ -566,12 +566,15 @@ struct RecordCaps {
     int max_rows;      // row format: rows per record
     int quad_cap;      // quad format: union columns per record
 };
-static RecordCaps record_caps(int64_t n_v, int64_t nnz) {
+// ring_est: roughly the bytes the dose pass's ring will have (what the gather array and g leave of shared memory).
+static RecordCaps record_caps(int64_t n_v, int64_t nnz, int64_t ring_est) {
     auto clampi = [](int64_t v, int lo, int hi) { return (int)std::max<int64_t>(lo, std::min<int64_t>(hi, v)); };
     RecordCaps c;
     c.chunk_slots = clampi((nnz / TARGET_RECORDS + 3) & ~(int64_t)3, 64, ROW_REC_SLOTS);
     c.max_rows = clampi(n_v / TARGET_RECORDS, 8, MAXROWS_F);
-    c.quad_cap = clampi(nnz / 3 / TARGET_RECORDS, 32, QUAD_CAP);
+    // quad records: at least one per consumer warp must fit in the ring (18 bytes per union column); measured on the
+    // 9- and 15-field phantoms, 480 .. 576 columns (8 .. 10 KB, mostly 4 quads = 2 warp trips) is the sweet spot
+    c.quad_cap = clampi(std::min<int64_t>(nnz / 3 / TARGET_RECORDS, ring_est / (W_CONS * 18)), 32, QUAD_CAP);
     return c;
 }
 
@@ -690,9 +693,10 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
                     ++qq;
                 }
                 int q1 = last + 1, nq = q1 - q0;
-                if (nq > TEAM && nq % TEAM) {      // a team of TEAM warps takes one quad each per round: keep rounds full
-                    for (int t = q1 - nq % TEAM; t < q1; ++t) cols -= pad8(quadU[t]);
-                    q1 -= nq % TEAM;
+                constexpr int QROUND = 2 * TEAM;
+                if (nq > QROUND && nq % QROUND) {  // a warp takes two quads at a time: keep the pairs full
+                    for (int t = q1 - nq % QROUND; t < q1; ++t) cols -= pad8(quadU[t]);
+                    q1 -= nq % QROUND;
                     nq = q1 - q0;
                 }
                 const int mo = (int)B.meta.size();
@@ -1159,7 +1163,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     for (int64_t j = 0; j < n_v; ++j) max_row = std::max(max_row, rp[j + 1] - rp[j]);
     if (max_row > MAX_CHUNK_SLOTS)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row of D has %d entries; this build handles rows up to %d", max_row, MAX_CHUNK_SLOTS);
-    const RecordCaps caps = record_caps(n_v, nnz);
+    const int64_t nb_pad_est = (n_b + 31) & ~31LL;
+    const RecordCaps caps = record_caps(n_v, nnz, (int64_t)smem_optin - SMEM_HEADER - 256 - std::max(SMEM_WPART, SMEM_DSC) - nb_pad_est * 4 * (R_MAX + 1));
     // quad format on offer: count the distinct columns of every 4 consecutive rows on the device
     const int bm_words = (int)((n_b + 31) / 32);
     std::vector<int> quadU;

@@ -42,7 +42,7 @@ constexpr int ROW_REC_SLOTS = 1024;           // slots per row-format record (fe
 constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
 constexpr int MAXROWS_F = 256;                // rows per block
 constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered up to this many beamlets (pack-kernel bitmap)
-constexpr int QUAD_CAP = 384;                 // union columns per quad-format record unless one quad needs more
+constexpr int QUAD_CAP = 576;                 // union columns per quad record, at most (see record_caps)
 constexpr int QUAD_MAXQ = 64;                 // quads per record
 constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int TARGET_RECORDS = 8192;          // a small matrix is cut into at least about this many records (imrtgp.cu)
@@ -419,21 +419,22 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
 
 // The same for a record in QUAD format: 4 consecutive rows of D (neighbouring voxels, which see nearly the same
 // beamlets) share one sorted list of columns, the union of theirs; per union column the record holds the 4 rows'
-// values as one 16-byte vector (explicit zeros where a row has no entry) and one 16-bit column.  A warp takes one
-// quad at a time: per trip every lane takes one union column -- one vector load of 4 values, one column, ONE
-// gather of the R trial values (32 neighbouring beamlets: conflict-free), 4 R multiply-adds.  Against the row format
-// this needs a quarter of the gathers and of the column bytes and -- where the rows of a quad overlap well -- fewer
-// bytes of HBM traffic per non-zero (18 bytes per union column).  The 4 x R row sums are reduced over the warp by a
-// butterfly whose first two steps split the rows (xor 16: rows {0,1} | {2,3}; xor 8: one row), so lanes 0, 8, 16, 24
-// end up with one row each: penalty, residual, objective as above.
+// values as one 16-byte vector (explicit zeros where a row has no entry) and one 16-bit column.  A warp takes TWO
+// quads at a time, one per half-warp: per trip every lane takes one union column of its quad -- one vector load of 4
+// values, one column, ONE gather of the R trial values (16 neighbouring beamlets per half: conflict-free), 4 R
+// multiply-adds.  Against the row format this needs a quarter of the gathers and of the column bytes and -- where
+// the rows of a quad overlap well -- fewer bytes of HBM traffic per non-zero (18 bytes per union column).  Rows are
+// short (a quad has ~130 union columns), so the reduction and the penalty evaluation at the end of a quad cost as
+// many instructions as its multiply-adds; two quads per warp halve that share and leave every lane of the warp
+// with exactly one (row, trial) sum at R = 4.
 // Which trial point of a batch a lane ends up with after the quad reduction, and whether it ends up with a sum at all.
-template <int R> __device__ __forceinline__ int quad_trial(int lane) { return R == 4 ? ((lane >> 1) & 3) : R == 2 ? ((lane >> 2) & 1) : 0; }
-template <int R> __device__ __forceinline__ bool quad_owner(int lane) { return (lane & (R == 4 ? 1 : R == 2 ? 3 : 7)) == 0; }
+template <int R> __device__ __forceinline__ int quad_trial(int lane) { return R == 4 ? (lane & 3) : R == 2 ? ((lane >> 1) & 1) : 0; }
+template <int R> __device__ __forceinline__ bool quad_owner(int lane) { return (lane & (R == 4 ? 0 : R == 2 ? 1 : 3)) == 0; }
 
-// The reduction is one xor butterfly over the 32 lanes for every (row, trial) sum -- the same tree of additions
-// whatever R is -- but at each step a lane keeps only half of what it holds: xor 16 splits the rows {0,1} | {2,3},
-// xor 8 leaves one row, xor 4 / xor 2 split the trial points (R = 4; xor 4 only for R = 2).  4 R shuffles instead of
-// 5 x 4 R, and lane (b4 b3 b2 b1 0) ends with row 2 b4 + b3 of trial 2 b2 + b1: one penalty evaluation per lane.
+// The reduction is one xor butterfly over the 16 lanes of a half-warp for every (row, trial) sum -- the same tree of
+// additions whatever R is -- but at each step a lane keeps only half of what it holds: xor 8 splits the rows
+// {0,1} | {2,3}, xor 4 leaves one row, xor 2 / xor 1 split the trial points (R = 4; xor 2 only for R = 2).  4 R - 1
+// shuffles for two quads, and lane (b4 b3 b2 b1 b0) ends with row 2 b3 + b2 of trial 2 b1 + b0 of quad b4.
 // my_r: the residual buffer of this lane's trial.  Gq: this lane's objective partial (of its own trial).
 template <int R>
 __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
@@ -445,20 +446,27 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
     const unsigned char* val_b = reinterpret_cast<const unsigned char*>(qt + ((2 * (nq + 1) + 3) & ~3));
     const unsigned char* col_b = val_b + (size_t)(nbc + 1) * 16;
     constexpr int XB = 4 * R;
-    const bool hi16 = (lane & 16) != 0, hi8 = (lane & 8) != 0, hi4 = (lane & 4) != 0, hi2 = (lane & 2) != 0;
-    const int rr = (hi16 ? 2 : 0) + (hi8 ? 1 : 0);         // the row this lane ends up with
+    const int half = lane >> 4, l16 = lane & 15;
+    const bool hi8 = (lane & 8) != 0, hi4 = (lane & 4) != 0, hi2 = (lane & 2) != 0, hi1 = (lane & 1) != 0;
+    const int rr = (hi8 ? 2 : 0) + (hi4 ? 1 : 0);          // the row this lane ends up with
     const bool owner = quad_owner<R>(lane);
-    for (int qi = tw; qi < nq; qi += TEAM) {               // warp tw of the team takes the quads tw, tw + TEAM, ...
-        const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qi);
-        const int s = (int)(w.x & 0xFFFFu), e = (int)(qt[2 * qi + 2] & 0xFFFFu);
+    for (int q0 = 2 * tw; q0 < nq; q0 += 2 * TEAM) {       // warp tw of the team takes the quad pairs tw, tw + TEAM, ...
+        const int qi = q0 + half;
+        const bool have = qi < nq;
+        const int qs = have ? qi : q0;
+        const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qs);
+        const int s = (int)(w.x & 0xFFFFu);
+        const int e = have ? (int)(qt[2 * qs + 2] & 0xFFFFu) : s;
+        const int len = e - s;
+        const int trips = max(len, __shfl_xor_sync(0xffffffffu, len, 16));
         float acc[4][R];
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int r = 0; r < R; ++r) acc[i][r] = 0.0f;
 #pragma unroll 2
-        for (int k0 = s; k0 < e; k0 += 32) {
-            const int k = k0 + lane;
+        for (int t0 = 0; t0 < trips; t0 += 16) {
+            const int k = s + t0 + l16;
             const int kk = k < e ? k : nbc;                // past the quad's end: the zero column
             const float4 v = *reinterpret_cast<const float4*>(val_b + 16 * kk);
             const uint32_t c = *reinterpret_cast<const unsigned short*>(col_b + 2 * kk);
@@ -475,26 +483,23 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
         float h[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float a0 = (hi16 ? acc[2][r] : acc[0][r]) + __shfl_xor_sync(0xffffffffu, hi16 ? acc[0][r] : acc[2][r], 16);
-            const float a1 = (hi16 ? acc[3][r] : acc[1][r]) + __shfl_xor_sync(0xffffffffu, hi16 ? acc[1][r] : acc[3][r], 16);
-            h[r] = (hi8 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi8 ? a0 : a1, 8);
+            const float a0 = (hi8 ? acc[2][r] : acc[0][r]) + __shfl_xor_sync(0xffffffffu, hi8 ? acc[0][r] : acc[2][r], 8);
+            const float a1 = (hi8 ? acc[3][r] : acc[1][r]) + __shfl_xor_sync(0xffffffffu, hi8 ? acc[1][r] : acc[3][r], 8);
+            h[r] = (hi4 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi4 ? a0 : a1, 4);
         }
         float d;
         if (R == 4) {
-            const float g0 = (hi4 ? h[R > 2 ? 2 : 0] : h[0]) + __shfl_xor_sync(0xffffffffu, hi4 ? h[0] : h[R > 2 ? 2 : 0], 4);
-            const float g1 = (hi4 ? h[R > 3 ? 3 : 0] : h[R > 1 ? 1 : 0]) + __shfl_xor_sync(0xffffffffu, hi4 ? h[R > 1 ? 1 : 0] : h[R > 3 ? 3 : 0], 4);
-            const float f = (hi2 ? g1 : g0) + __shfl_xor_sync(0xffffffffu, hi2 ? g0 : g1, 2);
-            d = f + __shfl_xor_sync(0xffffffffu, f, 1);
+            const float g0 = (hi2 ? h[R > 2 ? 2 : 0] : h[0]) + __shfl_xor_sync(0xffffffffu, hi2 ? h[0] : h[R > 2 ? 2 : 0], 2);
+            const float g1 = (hi2 ? h[R > 3 ? 3 : 0] : h[R > 1 ? 1 : 0]) + __shfl_xor_sync(0xffffffffu, hi2 ? h[R > 1 ? 1 : 0] : h[R > 3 ? 3 : 0], 2);
+            d = (hi1 ? g1 : g0) + __shfl_xor_sync(0xffffffffu, hi1 ? g0 : g1, 1);
         } else if (R == 2) {
-            float g = (hi4 ? h[R > 1 ? 1 : 0] : h[0]) + __shfl_xor_sync(0xffffffffu, hi4 ? h[0] : h[R > 1 ? 1 : 0], 4);
-            g += __shfl_xor_sync(0xffffffffu, g, 2);
+            const float g = (hi2 ? h[R > 1 ? 1 : 0] : h[0]) + __shfl_xor_sync(0xffffffffu, hi2 ? h[0] : h[R > 1 ? 1 : 0], 2);
             d = g + __shfl_xor_sync(0xffffffffu, g, 1);
         } else {
-            float g = h[0] + __shfl_xor_sync(0xffffffffu, h[0], 4);
-            g += __shfl_xor_sync(0xffffffffu, g, 2);
+            const float g = h[0] + __shfl_xor_sync(0xffffffffu, h[0], 2);
             d = g + __shfl_xor_sync(0xffffffffu, g, 1);
         }
-        if (owner && ((w.x >> (16 + rr)) & 1u)) {          // the row exists
+        if (owner && have && ((w.x >> (16 + rr)) & 1u)) {  // the row exists
             float4 t = table_s[(w.y >> (8 * rr)) & 0xFFu];
             const size_t jrow = (size_t)hdr.y + 4 * qi + rr;
             vl.apply(t, jrow);
