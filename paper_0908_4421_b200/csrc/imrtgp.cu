@@ -812,7 +812,7 @@ static cudaError_t launch_persistent(imrt_plan* pl) {
 static imrt_status upload_partition(imrt_plan* pl, const std::vector<int>& cta_blk) {
     cudaStream_t st = pl->stream;
     CUDA_TRY(pl, cudaMemcpyAsync(pl->cta_blk_w, cta_blk.data(), sizeof(int) * cta_blk.size(), cudaMemcpyHostToDevice, st));
-    k_ring_layout<<<(pl->P.grid_f + 127) / 128, 128, 0, st>>>(pl->blk_w, pl->cta_blk_w, pl->P.grid_f, (unsigned int)pl->P.ring_f_bytes);
+    k_ring_layout<<<pl->P.grid_f, 32, 0, st>>>(pl->blk_w, pl->cta_blk_w, pl->P.grid_f, (unsigned int)pl->P.ring_f_bytes);
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));   // cta_blk is a host vector the caller may drop
     return IMRT_STATUS_OK;

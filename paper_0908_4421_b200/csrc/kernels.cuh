@@ -1065,34 +1065,56 @@ __device__ __forceinline__ void publish_x(const float* xs, int j, float* x_out, 
 // ------------------------------------------------------------------------------------------------ kernels
 extern __shared__ __align__(128) unsigned char imrt_smem[];
 
-// The dose pass's ring schedule for the current partition: thread c walks CTA c's blocks in order, places every
+// The dose pass's ring schedule for the current partition: CTA c's blocks are walked in order; the walk places every
 // record in a circular buffer of ring_bytes (end to end; a record that does not fit before the end starts over at
 // 0) and notes how many earlier blocks must have left the ring first (at most RING_ENTRIES in flight).
-__global__ void k_ring_layout(int4* blk, const int* __restrict__ cta_blk, int grid_f, unsigned int ring_bytes) {
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+// One warp per CTA of the dose pass: the lanes fetch the record sizes of 256 blocks at a time and write the results
+// back (coalesced); lane 0 does the walk in shared memory.  The tail trails the head by at most RING_ENTRIES blocks,
+// so a circular array of that many ring offsets is all the history the walk needs.
+constexpr int RING_LAYOUT_CHUNK = 256;
+__global__ void __launch_bounds__(32) k_ring_layout(int4* blk, const int* __restrict__ cta_blk, int grid_f, unsigned int ring_bytes) {
+    __shared__ unsigned int at_s[RING_ENTRIES];
+    __shared__ int bytes_s[RING_LAYOUT_CHUNK], w_s[RING_LAYOUT_CHUNK];
+    __shared__ unsigned int z_s[RING_LAYOUT_CHUNK];
+    const int c = blockIdx.x, lane = threadIdx.x;
     if (c >= grid_f) return;
     const int b0 = cta_blk[c], b1 = cta_blk[c + 1];
     unsigned int head = 0u;
     int tail = b0;
-    for (int b = b0; b < b1; ++b) {
-        const unsigned int bytes = (unsigned int)blk[b].y;
-        unsigned int at;
-        for (;;) {
-            bool fits;
-            if (tail == b) { at = 0u; fits = true; }                 // nothing in flight
-            else {
-                const unsigned int t = (unsigned int)blk[tail].z;    // the oldest record in flight
-                if (head > t) {
-                    if (head + bytes <= ring_bytes) { at = head; fits = true; }
-                    else { at = 0u; fits = bytes <= t; }
-                } else { at = head; fits = head + bytes <= t; }
+    for (int base = b0; base < b1; base += RING_LAYOUT_CHUNK) {
+        const int n = min(RING_LAYOUT_CHUNK, b1 - base);
+        for (int j = lane; j < n; j += 32) bytes_s[j] = blk[base + j].y;
+        __syncwarp();
+        if (lane == 0) {
+            for (int j = 0; j < n; ++j) {
+                const int b = base + j;
+                const unsigned int bytes = (unsigned int)bytes_s[j];
+                unsigned int at;
+                for (;;) {
+                    bool fits;
+                    if (tail == b) { at = 0u; fits = true; }                 // nothing in flight
+                    else {
+                        const unsigned int t = at_s[(tail - b0) & (RING_ENTRIES - 1)];   // the oldest record in flight
+                        if (head > t) {
+                            if (head + bytes <= ring_bytes) { at = head; fits = true; }
+                            else { at = 0u; fits = bytes <= t; }
+                        } else { at = head; fits = head + bytes <= t; }
+                    }
+                    if (fits && b - tail < RING_ENTRIES) break;
+                    ++tail;
+                }
+                head = at + bytes;
+                at_s[(b - b0) & (RING_ENTRIES - 1)] = at;
+                z_s[j] = at;
+                w_s[j] = tail - b0;
             }
-            if (fits && b - tail < RING_ENTRIES) break;
-            ++tail;
         }
-        head = at + bytes;
-        blk[b].z = (int)at;
-        blk[b].w = tail - b0;
+        __syncwarp();
+        for (int j = lane; j < n; j += 32) {
+            blk[base + j].z = (int)z_s[j];
+            blk[base + j].w = w_s[j];
+        }
+        __syncwarp();
     }
 }
 
