@@ -300,3 +300,43 @@ def make_banded(seed: int, n_v: int, n_b: int, width: int, jitter: float, empty_
     if col.size:
         prob.lambda0, _ = pick_lambda0(row_ptr, col, val, sid, w_u, w_o)
     return prob
+
+
+def make_quad_blocks(seed: int, n_quads: int, n_b: int, tail_rows: int, lengths=(0, 1, 3, 17, 40, 300),
+                     n_structures: int = 3) -> Problem:
+    """Groups of 4 consecutive rows that share one column window (so that a plan picks its quad-row records), the
+    window length drawn per group from `lengths` -- neighbouring groups differ wildly, some are empty, rows inside a
+    group drop a few columns -- followed by `tail_rows` (0..3) rows of a last, incomplete group.  No arithmetic of the
+    method here: only the sparsity pattern and random values."""
+    rng = np.random.default_rng(seed)
+    rows = []
+    n_groups = n_quads + (1 if tail_rows else 0)
+    for q in range(n_groups):
+        L = min(int(rng.choice(lengths)), n_b)
+        c0 = int(rng.integers(0, n_b - L + 1))
+        window = np.arange(c0, c0 + L)
+        for i in range(4 if q < n_quads else tail_rows):
+            if L == 0 or rng.random() < 0.1:
+                rows.append(np.empty(0, np.int64))            # a row without entries inside a group
+            else:
+                keep = rng.random(L) < rng.uniform(0.6, 1.0)
+                keep[rng.integers(0, L)] = True
+                rows.append(window[keep])
+    n_v = len(rows)
+    row_ptr = np.zeros(n_v + 1, np.int32)
+    row_ptr[1:] = np.cumsum([len(r) for r in rows])
+    col = np.concatenate(rows).astype(np.int32) if row_ptr[-1] else np.empty(0, np.int32)
+    val = rng.uniform(0.05, 1.0, col.shape[0]).astype(np.float32)
+    sid = rng.integers(0, n_structures, n_v).astype(np.uint8)
+    sid[: max(1, n_v // 3)] = 0
+    t_u = np.zeros(n_structures, np.float32)
+    t_o = rng.uniform(20.0, 60.0, n_structures).astype(np.float32)
+    w_u = np.zeros(n_structures, np.float32)
+    w_o = rng.uniform(0.5, 10.0, n_structures).astype(np.float32)
+    t_u[0] = t_o[0] = 70.0
+    w_u[0] = w_o[0] = 100.0
+    x0 = rng.uniform(0.5, 1.5, n_b).astype(np.float32)
+    prob = Problem("quadblocks-%d" % seed, n_v, n_b, row_ptr, col, val, sid, t_u, t_o, w_u, w_o, x0, n_iters=10)
+    if col.size:
+        prob.lambda0, _ = pick_lambda0(row_ptr, col, val, sid, w_u, w_o)
+    return prob

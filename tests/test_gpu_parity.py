@@ -405,6 +405,37 @@ def test_fallback_layouts_parity(m, env, monkeypatch):
         plan.close()
 
 
+@pytest.mark.parametrize("seed,n_quads,n_b,tail", [(1, 1, 40, 0), (2, 2, 64, 1), (3, 3, 300, 2), (4, 257, 512, 3), (5, 4001, 900, 0),
+                                                     (6, 1500, 2304, 1)])
+def test_quad_pairs_edge_cases(m, seed, n_quads, n_b, tail, monkeypatch):
+    # The dose pass takes the quads of a record two at a time (one per half-warp): single quads, odd counts, an
+    # incomplete last group, empty groups between long ones, neighbours of very different length, rows without entries.
+    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")
+    prob = synth_inputs.make_quad_blocks(seed, n_quads, n_b, tail)
+    x = np.random.default_rng(seed).uniform(0, 3, prob.n_b).astype(np.float32)
+    ref = None
+    for R in (4, 2, 1):
+        plan = m.Plan(prob, max_iters=8, ls_batch=R)
+        if n_quads >= 100:
+            assert plan.info()["quad_rows"] > 0          # the case really exercises the quad records
+        check_eval(m, plan, prob, x)
+        plan.set_x(prob.x0)
+        plan.run_iters(8)
+        tr = plan.trace()
+        x_end = plan.get_x().cpu().numpy()
+        assert (np.diff(tr.obj) < 0).all() and (x_end >= 0).all()
+        # the loop's own (batched) dose pass against the oracle at the point it ended in (trajectories themselves are
+        # compared on the phantoms: reading R15)
+        G_o = oracle.eval_objective(prob, x_end.astype(np.float64))[2]
+        assert abs(tr.obj[-1] - G_o) <= TOL_KERNEL * abs(G_o) + 1e-300
+        cur = (tr.obj.copy(), x_end)
+        if ref is not None:                               # every batch width: the same bits
+            np.testing.assert_array_equal(cur[0], ref[0])
+            np.testing.assert_array_equal(cur[1], ref[1])
+        ref = cur
+        plan.close()
+
+
 def test_wide_transpose_groups_use_the_32_bit_stream(m):
     # a beamlet whose voxels lie more than 65,535 rows apart inside one group of 32 entries: no 16-bit offsets possible
     n_v, n_b = 200000, 6
