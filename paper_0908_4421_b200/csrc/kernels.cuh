@@ -451,12 +451,16 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
     const int rr = (hi8 ? 2 : 0) + (hi4 ? 1 : 0);          // the row this lane ends up with
     const bool owner = quad_owner<R>(lane);
     for (int q0 = 2 * tw; q0 < nq; q0 += 2 * TEAM) {       // warp tw of the team takes the quad pairs tw, tw + TEAM, ...
-        const int qi = q0 + half;
-        const bool have = qi < nq;
-        const int qs = have ? qi : q0;
-        const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qs);
-        const int s = (int)(w.x & 0xFFFFu);
-        const int e = have ? (int)(qt[2 * qs + 2] & 0xFFFFu) : s;
+        // A quad without a partner (the record's only or last one: typically a long quad that fills a record by itself)
+        // is split between the halves instead, columns [s, mid) and [mid, e); their sums meet in one more xor step.
+        const bool lone = q0 + 1 >= nq;
+        const int qi = lone ? q0 : q0 + half;
+        const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qi);
+        int s = (int)(w.x & 0xFFFFu), e = (int)(qt[2 * qi + 2] & 0xFFFFu);
+        if (lone) {
+            const int mid = s + ((e - s + 1) >> 1);
+            if (half) s = mid; else e = mid;
+        }
         const int len = e - s;
         const int trips = max(len, __shfl_xor_sync(0xffffffffu, len, 16));
         float acc[4][R];
@@ -499,7 +503,8 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
             const float g = h[0] + __shfl_xor_sync(0xffffffffu, h[0], 2);
             d = g + __shfl_xor_sync(0xffffffffu, g, 1);
         }
-        if (owner && have && ((w.x >> (16 + rr)) & 1u)) {  // the row exists
+        if (lone) d += __shfl_xor_sync(0xffffffffu, d, 16);
+        if (owner && !(lone && half) && ((w.x >> (16 + rr)) & 1u)) {  // the row exists
             float4 t = table_s[(w.y >> (8 * rr)) & 0xFFu];
             const size_t jrow = (size_t)hdr.y + 4 * qi + rr;
             vl.apply(t, jrow);
