@@ -463,11 +463,11 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
         }
         const int len = e - s;
         const int trips = max(len, __shfl_xor_sync(0xffffffffu, len, 16));
-        float acc[4][R];
+        // rows {0,1} and {2,3} of a trial are kept as register pairs: one packed multiply-add (FFMA2, the trial value as
+        // its broadcast operand) does two rows -- 2 R instead of 4 R issue slots per column, each half an IEEE fma
+        float2 acc01[R], acc23[R];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int r = 0; r < R; ++r) acc[i][r] = 0.0f;
+        for (int r = 0; r < R; ++r) acc01[r] = acc23[r] = make_float2(0.0f, 0.0f);
 #pragma unroll 2
         for (int t0 = 0; t0 < trips; t0 += 16) {
             const int k = s + t0 + l16;
@@ -478,17 +478,16 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
             x.load(xs_b + c * XB);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                acc[0][r] = fmaf(v.x, x.v[r], acc[0][r]);
-                acc[1][r] = fmaf(v.y, x.v[r], acc[1][r]);
-                acc[2][r] = fmaf(v.z, x.v[r], acc[2][r]);
-                acc[3][r] = fmaf(v.w, x.v[r], acc[3][r]);
+                const float2 xr = make_float2(x.v[r], x.v[r]);
+                acc01[r] = __ffma2_rn(make_float2(v.x, v.y), xr, acc01[r]);
+                acc23[r] = __ffma2_rn(make_float2(v.z, v.w), xr, acc23[r]);
             }
         }
         float h[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float a0 = (hi8 ? acc[2][r] : acc[0][r]) + __shfl_xor_sync(0xffffffffu, hi8 ? acc[0][r] : acc[2][r], 8);
-            const float a1 = (hi8 ? acc[3][r] : acc[1][r]) + __shfl_xor_sync(0xffffffffu, hi8 ? acc[1][r] : acc[3][r], 8);
+            const float a0 = (hi8 ? acc23[r].x : acc01[r].x) + __shfl_xor_sync(0xffffffffu, hi8 ? acc01[r].x : acc23[r].x, 8);
+            const float a1 = (hi8 ? acc23[r].y : acc01[r].y) + __shfl_xor_sync(0xffffffffu, hi8 ? acc01[r].y : acc23[r].y, 8);
             h[r] = (hi4 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi4 ? a0 : a1, 4);
         }
         float d;
