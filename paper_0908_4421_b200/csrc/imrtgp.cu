@@ -1177,14 +1177,38 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaStreamSynchronize(st));
     }
     phase.mark("quad union counts");
+    // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1).
+    // Enqueued here, ahead of the record layout below: that runs on the host for a few ms and needs nothing of this, so
+    // the device sorts meanwhile (no workspace region is shared between the two).
+    const Bounds B = bounds_for(n_v, n_b, nnz);
+    CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.valT, 0, sizeof(float) * B.nnz_pad, st));
+    std::vector<int> rpT((size_t)n_b + 1, 0);
+    if (nnz > 0) {
+        k_iota_keys<<<grid_for(nnz, 256), 256, 0, st>>>(col_idx, L.keysA, L.valsA, nnz);
+        cub::DoubleBuffer<unsigned int> dk(L.keysA, L.keysB), dv(L.valsA, L.valsB);
+        int end_bit = 1;
+        while ((1LL << end_bit) < n_b) ++end_bit;
+        size_t temp = 0;
+        CUDA_TRY(pl, cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)nnz, 0, end_bit, st));
+        if (temp > B.sort_temp) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: radix sort needs %zu temp bytes, %zu reserved", temp, B.sort_temp);
+        CUDA_TRY(pl, cub::DeviceRadixSort::SortPairs(L.sort_temp, temp, dk, dv, (int)nnz, 0, end_bit, st));
+        k_rowT_ptr<<<(int)((n_b + 1 + 255) / 256), 256, 0, st>>>(dk.Current(), nnz, (int)n_b, L.rowT_ptr);
+        k_fill_transpose<<<grid_for(nnz, 256), 256, 0, st>>>(dv.Current(), row_ptr, (int)n_v, val, nnz, L.colT, L.valT);
+        CUDA_TRY(pl, cudaGetLastError());
+    } else {
+        CUDA_TRY(pl, cudaMemsetAsync(L.rowT_ptr, 0, sizeof(int) * (n_b + 1), st));
+    }
     BlockPlan BP;
     std::vector<unsigned char> covered;
     imrt_status s = build_blocks(pl, rp, sid, table_h.data(), caps, col16 ? 2 : 4, quadU, BP, covered, pl->n_skipped,
                                  pl->n_nonempty, pl->n_quad_rows);
-    if (s != IMRT_STATUS_OK) return s;
+    if (s != IMRT_STATUS_OK) {
+        cudaStreamSynchronize(st);     // the transpose kernels enqueued above still write to the caller's workspace
+        return s;
+    }
     CUDA_TRY(pl, cudaMemcpyAsync(L.covered, covered.data(), (size_t)n_v, cudaMemcpyHostToDevice, st));
     phase.mark("build_blocks (host)");
-    const Bounds B = bounds_for(n_v, n_b, nnz);
     const size_t n_blk = BP.blk.size();
     if ((int64_t)n_blk > B.max_blk || (int64_t)BP.meta.size() > B.max_meta || BP.pack_bytes > B.max_pack)
         return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %zu words, %zu bytes)",
@@ -1211,26 +1235,10 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     }
 
     phase.mark("pack records");
-    // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1)
-    CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
-    CUDA_TRY(pl, cudaMemsetAsync(L.valT, 0, sizeof(float) * B.nnz_pad, st));
-    std::vector<int> rpT((size_t)n_b + 1, 0);
+    // ---- the explicit transpose was enqueued before the record layout: fetch its row pointers
     if (nnz > 0) {
-        k_iota_keys<<<grid_for(nnz, 256), 256, 0, st>>>(col_idx, L.keysA, L.valsA, nnz);
-        cub::DoubleBuffer<unsigned int> dk(L.keysA, L.keysB), dv(L.valsA, L.valsB);
-        int end_bit = 1;
-        while ((1LL << end_bit) < n_b) ++end_bit;
-        size_t temp = 0;
-        CUDA_TRY(pl, cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)nnz, 0, end_bit, st));
-        if (temp > B.sort_temp) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: radix sort needs %zu temp bytes, %zu reserved", temp, B.sort_temp);
-        CUDA_TRY(pl, cub::DeviceRadixSort::SortPairs(L.sort_temp, temp, dk, dv, (int)nnz, 0, end_bit, st));
-        k_rowT_ptr<<<(int)((n_b + 1 + 255) / 256), 256, 0, st>>>(dk.Current(), nnz, (int)n_b, L.rowT_ptr);
-        k_fill_transpose<<<grid_for(nnz, 256), 256, 0, st>>>(dv.Current(), row_ptr, (int)n_v, val, nnz, L.colT, L.valT);
-        CUDA_TRY(pl, cudaGetLastError());
         CUDA_TRY(pl, cudaMemcpyAsync(rpT.data(), L.rowT_ptr, sizeof(int) * (n_b + 1), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(pl, cudaStreamSynchronize(st));
-    } else {
-        CUDA_TRY(pl, cudaMemsetAsync(L.rowT_ptr, 0, sizeof(int) * (n_b + 1), st));
     }
 
     // ---- transpose-pass ranges and gradient slots
