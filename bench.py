@@ -187,7 +187,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream(dev)
 
     t0 = time.perf_counter()
-    plan = imrt.Plan(prob, max_iters=W + K, driver=driver, device=dev, ls_batch=args.ls_batch)
+    plan = imrt.Plan(prob, max_iters=W + K, driver=driver, device=dev, ls_batch=args.ls_batch, tune_level=args.tune_level)
     torch.cuda.synchronize()
     plan_create_s = time.perf_counter() - t0
     info = plan.info()
@@ -221,6 +221,9 @@ def run_ours(args):
 
     dose_ms = time_pass(0)
     tr_ms = time_pass(1)
+    # read-only streaming ceilings: the same rings / stages move the same bytes, the consumers only wait and release
+    dose_stream_ms = time_pass(2)
+    tr_stream_ms = time_pass(3) if info["tr_format"] == 2 else None
     clocks = sampler.stop()
 
     tr = plan.trace()
@@ -254,20 +257,36 @@ def run_ours(args):
         dose_eff = fwd_bytes / (dose_ms * 1e-3) / 1e9
         tr_eff = tr_bytes / (tr_ms * 1e-3) / 1e9
         t_dose, t_tr = recorded_traffic("k_dose", prob.name), recorded_traffic("k_transpose", prob.name)
-        roofline = {"bound": "hbm", "kernel": "k_dose (dose SpMV for %d trial point(s) + penalty + residual + objective partials)" % R,
-                    "achieved": dose_gbs, "peak": peak, "unit": "GB/s", "frac": dose_gbs / peak, "peak_source": peak_src,
-                    "traffic": t_dose, "bytes_per_launch": dose_layout, "ms_per_launch": dose_ms,
-                    "effective_csr_gbs": dose_eff, "algorithmic_csr_bytes": fwd_bytes,
-                    "note": "achieved / frac use the bytes of the library's own layouts (quad-row records); effective_csr_gbs = "
-                            "CSR-equivalent algorithmic bytes / time; traffic = ncu dram bytes of the committed capture",
-                    "frac_of_nominal_8TBs": dose_gbs / 8000.0}
-        roofline_tr = {"bound": "hbm", "kernel": "k_transpose (D^T r on the explicit transpose CSR)", "achieved": tr_gbs,
-                       "peak": peak, "unit": "GB/s", "frac": tr_gbs / peak, "traffic": t_tr, "bytes_per_launch": tr_layout, "ms_per_launch": tr_ms,
-                       "effective_csr_gbs": tr_eff, "algorithmic_csr_bytes": tr_bytes, "frac_of_nominal_8TBs": tr_gbs / 8000.0}
+
+        def roof(kernel, what, ms, layout, csr, traffic, stream_ms, read_bytes):
+            gbs = layout / (ms * 1e-3) / 1e9
+            d = {"bound": "hbm", "kernel": what, "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "peak_source": peak_src,
+                 "traffic": traffic, "bytes_per_launch": layout, "ms_per_launch": ms,
+                 # the two fractions under their own names: DRAM bytes actually moved (ncu capture of this kernel and workload,
+                 # else the layout bytes) and the CSR-equivalent bytes of SURVEY.md 8(d), each / time / measured peak
+                 "frac_dram": (traffic if traffic else layout) / (ms * 1e-3) / 1e9 / peak,
+                 "frac_csr_equiv": csr / (ms * 1e-3) / 1e9 / peak,
+                 "effective_csr_gbs": csr / (ms * 1e-3) / 1e9, "algorithmic_csr_bytes": csr,
+                 "frac_of_nominal_8TBs": gbs / 8000.0}
+            if stream_ms:
+                d["stream_ceiling_gbs"] = read_bytes / (stream_ms * 1e-3) / 1e9     # the pass's reads with the arithmetic left out
+                d["stream_ceiling_ms"] = stream_ms
+                d["frac_of_stream_ceiling"] = stream_ms / ms
+            return d
+
+        r_dose = roof("k_dose", "k_dose (dose SpMV for %d trial point(s) + penalty + residual + objective partials)" % R,
+                      dose_ms, dose_layout, fwd_bytes, t_dose, dose_stream_ms, info["pack_bytes"] + 16 * info["fwd_blocks"])
+        r_tr = roof("k_transpose", "k_transpose (D^T r on the explicit transpose, %s)" % ("plain CSR", "16-bit offsets", "row pairs")[info["tr_format"]],
+                    tr_ms, tr_layout, tr_bytes, t_tr, tr_stream_ms, info["tr_stream_bytes"])
+        r_dose["note"] = ("achieved / frac use the bytes of the library's own layouts (they agree with the ncu DRAM traffic to 1 %); "
+                          "frac_csr_equiv counts the int32/fp32 CSR bytes the layouts avoid moving")
+        # `roofline` is the LONGER of the two kernels of a step; the other one rides along
+        roofline, roofline_other = (r_dose, r_tr) if dose_ms >= tr_ms else (r_tr, r_dose)
+        roofline_tr = roofline_other
 
         # ---------------- time-to-plan: the config's own stopping rule from x0 (device-resident, inputs in HBM)
         cfg = synth_inputs.CONFIGS[args.config]
-        plan2 = imrt.Plan(prob, max_iters=cfg.n_iters, driver=driver, device=dev, ls_batch=args.ls_batch)
+        plan2 = imrt.Plan(prob, max_iters=cfg.n_iters, driver=driver, device=dev, ls_batch=args.ls_batch, tuning=plan.tuning())
         plan2.set_x(prob.x0)
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -304,7 +323,7 @@ def run_ours(args):
         for dst, src in ((d_rp, h_rp), (d_col, h_col), (d_val, h_val), (d_sid, h_sid), (d_x0, h_x0)):
             dst.copy_(src, non_blocking=True)
         handle = imrt.imrt_plan_create(prob.n_v, prob.n_b, prob.nnz, d_rp, d_col, d_val, d_sid, prob.t_under, prob.t_over,
-                                       prob.w_under, prob.w_over, prm, d_ws, stream.cuda_stream)
+                                       prob.w_under, prob.w_over, prm, d_ws, stream.cuda_stream, imrt.Options(tune_level=args.tune_level))
         imrt.imrt_plan_set_x(handle, d_x0)
         imrt.imrt_plan_run_iters(handle, K)
         imrt.imrt_plan_get_x(handle, d_x)
@@ -327,11 +346,16 @@ def run_ours(args):
         if world == 1 and not args.no_cpu_baseline:
             n_cpu = max(2, min(K, args.cpu_iters))
             res, dt = oracle_iterations(prob, n_cpu)
-            cpu = {"value": res.n_iters / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            try:
+                with open("/proc/cpuinfo") as f:
+                    model = next((ln.split(":", 1)[1].strip() for ln in f if ln.startswith("model name")), "unknown")
+            except OSError:
+                model = "unknown"
+            cpu = {"value": res.n_iters / dt, "unit": UNIT, "cores": 1, "nproc": os.cpu_count(), "cpu_model": model, "kind": "oracle",
                    "sample": "first %d GP iterations of %s from x0 (%.1f s), serial fp64 oracle/imrt_oracle.c" % (res.n_iters, prob.name, dt),
                    "trials_per_iter": float(res.n_trials.mean())}
 
-        extra = {"roofline": roofline, "roofline_transpose": roofline_tr, "time_to_plan": ttp, "e2e": e2e, "cpu_baseline": cpu,
+        extra = {"roofline": roofline, "roofline_other_kernel": roofline_tr, "time_to_plan": ttp, "e2e": e2e, "cpu_baseline": cpu,
                  "loop_effective_csr_gbs": loop_bytes / (ms * 1e-3) / 1e9,
                  "loop_gbs": (passes_timed * dose_layout + K * tr_layout) / (ms * 1e-3) / 1e9,
                  "loop_frac_of_peak": (passes_timed * dose_layout + K * tr_layout) / (ms * 1e-3) / 1e9 / peak,
@@ -413,6 +437,8 @@ def main():
     ap.add_argument("--driver", default="persistent", choices=sorted(DRIVERS))
     ap.add_argument("--ls-batch", type=int, default=0, choices=[0, 1, 2, 4],
                     help="line-search trial points per dose pass (0 = library default, 4)")
+    ap.add_argument("--tune-level", type=int, default=2, choices=[0, 1, 2],
+                    help="imrt_options.tune_level: 0 modelled partitions, 1 + isolated measurements, 2 + measurements inside the loop")
     ap.add_argument("--cpu-iters", type=int, default=60, help="oracle iterations timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sharded", action="store_true",

@@ -25,10 +25,12 @@
  *   - All device work is enqueued on the stream given at creation.  Calls documented "asynchronous" return
  *     without waiting for the device; calls that fill a host_ output synchronise that stream.
  *   - The plan handle is opaque and owned by the caller between imrt_plan_create and imrt_plan_destroy.
- *   - Results of one plan are bit-reproducible from run to run (fixed-order reductions, no floating-point atomics).
- *     Two plans of the same problem may differ in the last bits of the objective: plan creation balances the dose
- *     pass over the SMs from MEASURED pass times, and the partition fixes the order in which objective partials are
- *     summed.  Set the environment variable IMRTGP_NO_TUNE to keep the modelled partition (same bits every time).
+ *   - Results of one plan are bit-reproducible from run to run (fixed-order reductions; the only atomics on the data
+ *     path add INTEGERS, which commute).  With imrt_options.tune_level = 0 (the default) two plans of the same problem
+ *     also agree bit for bit.  tune_level >= 1 balances the passes over the SMs from MEASURED pass times; the partition
+ *     fixes the order in which objective partials are summed, so two tuned plans may differ in the last bits of the
+ *     objective -- unless the second one is given the first one's partition (imrt_plan_get_tuning / host_tuning).
+ *   - The library reads no environment variables: every switch is a field of imrt_params / imrt_options.
  *   - There is no CPU fallback: on a machine without an sm_100 device imrt_plan_create fails with
  *     IMRT_STATUS_UNSUPPORTED_DEVICE / IMRT_STATUS_CUDA_ERROR.
  */
@@ -62,7 +64,9 @@ typedef enum imrt_stop_reason {
     IMRT_STOP_MAX_ITERS = 0,             /* the requested number of accepted iterations was done                 */
     IMRT_STOP_TOLERANCE = 1,             /* |G_new - G_old| / G_new < delta (or G_new == 0)                      */
     IMRT_STOP_STATIONARY = 2,            /* G(x_k) == 0, or the first trial point equals x_k                     */
-    IMRT_STOP_LINESEARCH_STALLED = 3     /* more than max_ls backtracking steps; x_k kept                        */
+    IMRT_STOP_LINESEARCH_STALLED = 3,    /* more than max_ls backtracking steps; x_k kept                        */
+    IMRT_STOP_TRACE_FULL = 4             /* the trace (imrt_params.max_iters accepted iterations since imrt_plan_set_x)
+                                            filled up before the requested number of iterations was done          */
 } imrt_stop_reason;
 
 /* Line-search / loop parameters (PAPER.md:92 "two parameters 0 < eps < 1 and alpha > 1", :103, :114). */
@@ -72,8 +76,13 @@ typedef struct imrt_params {
     double lambda0;      /* step size every line search starts from (step 2), > 0                                */
     int32_t max_ls;      /* cap on backtracking steps per iteration (reading R4), >= 0                           */
     int32_t max_iters;   /* trace capacity: the total number of accepted iterations between two imrt_plan_set_x  */
-    int32_t driver;      /* 0: device-resident loop (CUDA graph with nested conditional WHILE nodes, no host sync
-                               per step);  1: host-driven loop (one sync per trial; same kernels; for debugging)  */
+    int32_t driver;      /* who runs the loop (all three give bit-identical results):
+                            0  CUDA graph with nested conditional WHILE nodes (one cudaGraphLaunch per run, no host
+                               sync per step; one transpose pass and ceil(trials / ls_batch) dose passes per iteration)
+                            1  host-driven (one launch and one sync per pass; for debugging and per-kernel profiling)
+                            2  ONE cooperative persistent kernel holding the whole loop (the fast path; what the
+                               Python binding and bench.py use).  Needs all n_sm CTAs co-resident: 576 threads and up
+                               to 227 KB of shared memory each, i.e. an otherwise idle device.                        */
     int32_t ls_batch;    /* line-search trial points evaluated per pass over D: 1, 2 or 4 (0 = default, 4).  The
                             trials lambda, lambda/alpha, ... are the ones steps 2-4 visit one at a time; a batch
                             evaluates the next ls_batch of them in ONE dose pass (D is streamed once, each trial point
@@ -81,6 +90,32 @@ typedef struct imrt_params {
                             iterates, step sizes and trial counts are bit-identical for every ls_batch.  The library
                             lowers it when the trial vectors would not fit in shared memory (imrt_plan_get_info).  */
 } imrt_params;
+
+/*
+ * Layout / tuning switches of imrt_plan_create (all 0 = the defaults; pass NULL for all defaults).  None of them
+ * changes what is computed, only how the matrices are laid out and the work is split.
+ */
+typedef struct imrt_options {
+    int32_t tune_level;        /* 0: partitions from the cost model only -- plan creation is timing independent and two
+                                     plans of one problem give the same bits;
+                                  1: + rebalance both passes from measured per-CTA times of isolated launches;
+                                  2: + a few more rounds measured inside the device-resident loop (bench.py uses this) */
+    int32_t dose_format;       /* 0: quad records where smaller (4 neighbouring rows share a column list), else rows;
+                                  1: row-format records only                                                          */
+    int32_t col_bits;          /* 0: 16-bit column indices when n_b <= 65,536;  32: always 32-bit                     */
+    int32_t transpose_format;  /* 0: smallest of {row pairs, single rows} with 16-bit voxel offsets, else plain CSR;
+                                  1: single rows with 16-bit offsets (no pairs);  2: the plain 32-bit D^T CSR         */
+    int32_t quad_cap;          /* union columns per quad record at most (0 = default, 576; clamped to [32, 4096])     */
+    int32_t fused_gradient;    /* the persistent loop (driver 2) forms g = D^T r INSIDE the dose pass for the trial
+                                  point most likely to be accepted:  0 = default (on when the
+                                  accumulators fit in shared memory), 1 = off (a transpose pass per iteration)         */
+    int32_t profile_create;    /* 1: synchronise after every phase of plan creation and keep the phase times for
+                                  imrt_plan_get_create_times                                                           */
+    int32_t reserved0;
+    const void* host_tuning;   /* a blob written by imrt_plan_get_tuning for the same problem, options and device: the
+                                  plan takes its partitions from it instead of measuring (tune_level is ignored)       */
+    size_t host_tuning_bytes;
+} imrt_options;
 
 typedef struct imrt_plan imrt_plan;
 
@@ -100,13 +135,18 @@ imrt_status imrt_workspace_bytes(int64_t n_v, int64_t n_b, int64_t nnz, int32_t 
  *   host_t_under, host_t_over, host_w_under, host_w_over   fp32 [n_structures]  (host; copied). w >= 0, finite;
  *                                 w_under = 0 means no under-dose term for that structure.
  *   host_params                   copied
+ *   host_options                  copied; NULL = defaults
  *   workspace / workspace_bytes   device memory from the caller, >= imrt_workspace_bytes(...)  (borrowed)
  *   stream                        a cudaStream_t passed as void* (NULL = the legacy default stream)
  * Validates the inputs (finite values, columns in range and strictly ascending in every row), re-packs D into the
  * block records the dose pass streams, builds the explicit transpose D^T as a second CSR (stable radix sort by
- * column) and the packed stream the transpose pass reads, balances both passes over the SMs from measured pass times
- * (a few short runs of the passes and of the loop on x = 0), and instantiates the iteration graph (driver 0).
- * Synchronises the stream.  DESIGN.md section 4 describes the layouts.
+ * column) and the packed stream the transpose pass reads, splits both passes over the SMs (cost model; with
+ * imrt_options.tune_level >= 1 refined from measured pass times: a few short runs of the passes and of the loop on
+ * x = 0), and instantiates the iteration graph (driver 0).  Synchronises the stream.  DESIGN.md section 4 describes
+ * the layouts.
+ * Limits (IMRT_STATUS_UNSUPPORTED): sizes must fit int32; a row of D may hold at most 8,192 entries; the R trial
+ * vectors (4 R n_b bytes), the gradient (4 n_b) and two of the largest block records must fit in the 227 KB of shared
+ * memory of one CTA -- R is lowered from 4 to 2 to 1 first, which leaves room for about 25,000 beamlets.
  * On failure *out is NULL unless the status is a validation error that left a handle for imrt_last_error;
  * imrt_last_error(NULL) returns the message of the last failed create on this thread.
  */
@@ -115,7 +155,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
                              const uint8_t* structure_id, int32_t n_structures,
                              const float* host_t_under, const float* host_t_over,
                              const float* host_w_under, const float* host_w_over,
-                             const imrt_params* host_params,
+                             const imrt_params* host_params, const imrt_options* host_options,
                              void* workspace, size_t workspace_bytes, void* stream);
 
 /*
@@ -155,6 +195,16 @@ imrt_status imrt_plan_run_to_tol(imrt_plan* plan, double delta, int32_t max_iter
  * Runs the same dose / penalty / transpose kernels the loop runs.  Synchronises.
  */
 imrt_status imrt_plan_eval(imrt_plan* plan, const float* x, float* d, float* r, float* g, double* host_obj);
+
+/*
+ * The line search's batched dose pass as a parity hook: evaluate n_points (1, 2 or 4) given points in ONE pass over D,
+ * exactly as the loop evaluates a batch of trial points (the R = n_points instantiation of the kernels).
+ *   x         fp32 [n_points][n_b]  the points, one after the other                           (device)
+ *   r         fp32 [n_points][n_v]  weighted residual of every point, or NULL                 (device)
+ *   host_obj  fp64 [n_points]       G of every point
+ * The optimiser state is not touched.  Synchronises.
+ */
+imrt_status imrt_plan_eval_batch(imrt_plan* plan, int32_t n_points, const float* x, float* r, double* host_obj);
 
 /*
  * g = D^T r for an arbitrary r (fp32 [n_v], device) -> g (fp32 [n_b], device): one transpose pass, the optimiser state is
@@ -230,6 +280,9 @@ imrt_status imrt_plan_get_info(imrt_plan* plan, int64_t* host_info, int32_t n_in
  * D x, penalty, residual, objective partials) or ONE transpose pass (kind 1: D^T r, partial-slot reduction) on the
  * plan's stream, n_repeat times back to back, on scratch outputs, without touching the optimiser state.  For
  * per-kernel timing / profiling only.  Asynchronous.
+ * kind 2 / 3: the read-only STREAMING CEILING of the dose / transpose pass -- the same producers move every byte the
+ * pass reads through the same shared-memory ring / stages, the consumer warps only wait and release (no arithmetic, no
+ * gathers, no stores).  What the pass could reach if its consumers were free (kind 3: row-pair stream only).
  */
 imrt_status imrt_plan_launch_pass(imrt_plan* plan, int32_t kind, int32_t n_repeat);
 
@@ -241,6 +294,44 @@ imrt_status imrt_plan_launch_pass(imrt_plan* plan, int32_t kind, int32_t n_repea
  */
 imrt_status imrt_plan_get_pass_timing(imrt_plan* plan, int32_t kind, int64_t* host_start_ns, int64_t* host_end_ns,
                                       int32_t capacity, int32_t* host_n_ctas);
+
+/*
+ * The partitions of the two passes as an opaque blob, for imrt_options.host_tuning of a later plan of the same problem
+ * (same D, options and device): that plan skips the measurements and reproduces this plan's results bit for bit.
+ * *host_bytes receives the size; the blob is written if host_buf is not NULL and capacity suffices
+ * (IMRT_STATUS_INVALID_ARG otherwise).  Host only.
+ */
+imrt_status imrt_plan_get_tuning(imrt_plan* plan, void* host_buf, size_t capacity, size_t* host_bytes);
+
+/*
+ * Phase times of imrt_plan_create in milliseconds (only with imrt_options.profile_create = 1, else *host_n = 0):
+ *   [0] validation  [1] quad union counts  [2] record layout  [3] record packing  [4] transpose (sort + gather)
+ *   [5] D^T stream packing, ranges  [6] state, first schedule  [7] dose-pass tuning  [8] transpose-pass tuning  [9] graph
+ */
+imrt_status imrt_plan_get_create_times(imrt_plan* plan, double* host_ms, int32_t capacity, int32_t* host_n);
+
+/*
+ * Mixed-resolution row merging (section 3.1: "for unspecified tissue we increased the voxel size in each
+ * dimension by a factor of 2"; reading R17).  The rows of D whose group_id is equal are replaced by ONE row,
+ * their mean -- the dose of a coarse voxel is the mean dose of the fine voxels it contains.  Merged row g holds every
+ * column some row of group g stores, ascending, with value (sum over the group's rows in ascending row order, fp64) /
+ * (rows in the group), rounded to fp32; a group without rows gives an empty row.  The result is a CSR the caller owns and
+ * can hand to imrt_plan_create; the full-resolution D stays available for plan evaluation (imrt_plan_eval / _dvh).
+ *   group_id     int32 [n_v]          0 <= group_id < n_groups; the rows of a group need not be neighbours   (device)
+ *   out_row_ptr  int32 [n_groups + 1]                                                                         (device)
+ *   out_col      int32 [nnz_out], out_val fp32 [nnz_out]                                                      (device)
+ *   workspace    >= imrt_merge_rows_workspace_bytes(n_v, n_groups); the SAME workspace, unmodified, for both calls
+ * imrt_merge_rows_count sorts the rows by group, counts every merged row, fills out_row_ptr and returns nnz_out
+ * (synchronises); the caller allocates out_col / out_val and calls imrt_merge_rows_fill (asynchronous).
+ * Limits: n_b up to about 390,000 (the column bitmap of one group must fit 24 KB of shared memory).
+ */
+imrt_status imrt_merge_rows_workspace_bytes(int64_t n_v, int64_t n_groups, size_t* host_bytes);
+imrt_status imrt_merge_rows_count(int64_t n_v, int64_t n_b, const int32_t* row_ptr, const int32_t* col_idx, const int32_t* group_id,
+                                  int64_t n_groups, int32_t* out_row_ptr, int64_t* host_nnz_out, void* workspace, size_t workspace_bytes,
+                                  void* stream);
+imrt_status imrt_merge_rows_fill(int64_t n_v, int64_t n_b, const int32_t* row_ptr, const int32_t* col_idx, const float* val,
+                                 int64_t n_groups, const int32_t* out_row_ptr, int32_t* out_col, float* out_val, void* workspace,
+                                 size_t workspace_bytes, void* stream);
 
 /* Message of the last error on this plan (or of the last failed imrt_plan_create when plan is NULL).
  * Owned by the library, valid until the next call on the same plan / thread. */

@@ -58,6 +58,10 @@ def _load():
         lib.oracle_run_v.restype = ctypes.c_int
         lib.oracle_dvh.argtypes = [ctypes.c_int64, _P, _P, ctypes.c_int, _P, ctypes.c_int, _P, _P]
         lib.oracle_dvh.restype = None
+        lib.oracle_merge_rows_count.argtypes = [ctypes.c_int64, ctypes.c_int64, _P, _P, _P, ctypes.c_int64, _P]
+        lib.oracle_merge_rows_count.restype = None
+        lib.oracle_merge_rows_fill.argtypes = [ctypes.c_int64, ctypes.c_int64, _P, _P, _P, _P, ctypes.c_int64, _P, _P, _P]
+        lib.oracle_merge_rows_fill.restype = None
         _lib = lib
     return _lib
 
@@ -182,3 +186,17 @@ def dvh_points(sid, d, n_structures, pcts=DVH_PCTS):
     mean = np.empty(n_structures, np.float64)
     lib.oracle_dvh(sid.shape[0], _p(sid), _p(d), n_structures, _p(pc), pc.shape[0], _p(out), _p(mean))
     return out, mean
+
+
+def merge_rows(n_b, row_ptr, col, val, group, n_groups):
+    """Rows with the same group id replaced by their mean (reading R17): (row_ptr, col, val) of the merged
+    matrix, one row per group.  imrt_oracle.c: oracle_merge_rows_count / oracle_merge_rows_fill."""
+    lib = _load()
+    rp, c, v, g = _c(row_ptr, np.int32), _c(col, np.int32), _c(val, np.float32), _c(group, np.int32)
+    n_v = rp.shape[0] - 1
+    out_rp = np.zeros(n_groups + 1, np.int32)
+    lib.oracle_merge_rows_count(n_v, n_b, _p(rp), _p(c), _p(g), n_groups, _p(out_rp))
+    out_c = np.zeros(max(int(out_rp[-1]), 1), np.int32)
+    out_v = np.zeros(max(int(out_rp[-1]), 1), np.float32)
+    lib.oracle_merge_rows_fill(n_v, n_b, _p(rp), _p(c), _p(v), _p(g), n_groups, _p(out_rp), _p(out_c), _p(out_v))
+    return out_rp, out_c[:out_rp[-1]], out_v[:out_rp[-1]]

@@ -240,3 +240,59 @@ void oracle_dvh(int64_t n_v, const uint8_t *sid, const double *d, int n_structur
     }
     free(buf);
 }
+
+/*
+ * Mixed-resolution row merging (section 3.1: "for unspecified tissue we increased the voxel size in each
+ * dimension by a factor of 2"; reading R17): the rows of D that carry the same group id are replaced by ONE
+ * row, their MEAN (the dose of the coarse voxel is the mean dose of the fine voxels it contains).  Written out plainly:
+ * for every group, in ascending row order, add the rows into a dense fp64 accumulator over the n_b columns, divide by
+ * the number of rows of the group, and emit the touched columns in ascending order, rounded to fp32.  A column counts
+ * as touched if any row of the group stores it (a stored 0 is kept).
+ *
+ *   group[j]  in [0, n_groups) for every row j (groups need not be contiguous; a group without rows gives an empty row)
+ * Two calls, as a caller that allocates the output must make them: oracle_merge_rows_count fills out_row_ptr
+ * [n_groups + 1]; oracle_merge_rows_fill fills out_col / out_val [out_row_ptr[n_groups]].
+ */
+void oracle_merge_rows_count(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *col, const int32_t *group,
+                             int64_t n_groups, int32_t *out_row_ptr) {
+    unsigned char *mark = (unsigned char *)calloc((size_t)(n_b > 0 ? n_b : 1), 1);
+    out_row_ptr[0] = 0;
+    for (int64_t g = 0; g < n_groups; ++g) {
+        int32_t cnt = 0;
+        for (int64_t j = 0; j < n_v; ++j) {          /* plain and slow: every group scans every row */
+            if (group[j] != g) continue;
+            for (int64_t p = row_ptr[j]; p < row_ptr[j + 1]; ++p)
+                if (!mark[col[p]]) { mark[col[p]] = 1; ++cnt; }
+        }
+        for (int64_t j = 0; j < n_v; ++j)
+            if (group[j] == g)
+                for (int64_t p = row_ptr[j]; p < row_ptr[j + 1]; ++p) mark[col[p]] = 0;
+        out_row_ptr[g + 1] = out_row_ptr[g] + cnt;
+    }
+    free(mark);
+}
+
+void oracle_merge_rows_fill(int64_t n_v, int64_t n_b, const int32_t *row_ptr, const int32_t *col, const float *val,
+                            const int32_t *group, int64_t n_groups, const int32_t *out_row_ptr, int32_t *out_col, float *out_val) {
+    unsigned char *mark = (unsigned char *)calloc((size_t)(n_b > 0 ? n_b : 1), 1);
+    double *acc = (double *)calloc((size_t)(n_b > 0 ? n_b : 1), sizeof(double));
+    for (int64_t g = 0; g < n_groups; ++g) {
+        int64_t size = 0;
+        for (int64_t j = 0; j < n_v; ++j) {          /* ascending row order: the order of the fp64 additions */
+            if (group[j] != g) continue;
+            ++size;
+            for (int64_t p = row_ptr[j]; p < row_ptr[j + 1]; ++p) { mark[col[p]] = 1; acc[col[p]] += (double)val[p]; }
+        }
+        int64_t q = out_row_ptr[g];
+        for (int64_t c = 0; c < n_b; ++c) {
+            if (!mark[c]) continue;
+            out_col[q] = (int32_t)c;
+            out_val[q] = (float)(acc[c] / (double)size);
+            ++q;
+            mark[c] = 0;
+            acc[c] = 0.0;
+        }
+    }
+    free(mark);
+    free(acc);
+}

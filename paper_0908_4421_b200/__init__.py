@@ -18,17 +18,18 @@ import numpy as np
 
 from . import build as _build
 
-__all__ = ["Plan", "ImrtError", "lib", "Params", "STATUS_NAMES", "STOP_NAMES", "EXPORTS"]
+__all__ = ["Plan", "ImrtError", "lib", "Params", "Options", "STATUS_NAMES", "STOP_NAMES", "EXPORTS"]
 
 STATUS_NAMES = ("OK", "INVALID_ARG", "BAD_CSR", "BAD_STRUCTURE", "WORKSPACE_TOO_SMALL", "CUDA_ERROR",
                 "UNSUPPORTED_DEVICE", "UNSUPPORTED", "BAD_X", "NOT_READY")
-STOP_NAMES = ("MAX_ITERS", "TOLERANCE", "STATIONARY", "LINESEARCH_STALLED")
+STOP_NAMES = ("MAX_ITERS", "TOLERANCE", "STATIONARY", "LINESEARCH_STALLED", "TRACE_FULL")
 DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
 
 # every symbol include/imrtgp.h declares
 EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_set_voxel_limits", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
-           "imrt_plan_eval", "imrt_plan_gradient", "imrt_trial_point", "imrt_armijo_accepts", "imrt_stop_test", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
-           "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_last_error", "imrt_plan_destroy",
+           "imrt_plan_eval", "imrt_plan_eval_batch", "imrt_plan_gradient", "imrt_trial_point", "imrt_armijo_accepts", "imrt_stop_test", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
+           "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_plan_get_tuning", "imrt_plan_get_create_times",
+           "imrt_merge_rows_workspace_bytes", "imrt_merge_rows_count", "imrt_merge_rows_fill", "imrt_last_error", "imrt_plan_destroy",
            "imrt_version")
 
 
@@ -45,6 +46,17 @@ class Params(ctypes.Structure):
                 ("max_ls", ctypes.c_int32), ("max_iters", ctypes.c_int32), ("driver", ctypes.c_int32),
                 ("ls_batch", ctypes.c_int32)]
 
+
+class Options(ctypes.Structure):
+    """imrt_options: layout / tuning switches of imrt_plan_create (all 0 = defaults)."""
+    _fields_ = [("tune_level", ctypes.c_int32), ("dose_format", ctypes.c_int32), ("col_bits", ctypes.c_int32),
+                ("transpose_format", ctypes.c_int32), ("quad_cap", ctypes.c_int32), ("fused_gradient", ctypes.c_int32),
+                ("profile_create", ctypes.c_int32), ("reserved0", ctypes.c_int32),
+                ("host_tuning", ctypes.c_void_p), ("host_tuning_bytes", ctypes.c_size_t)]
+
+
+CREATE_PHASES = ("validate", "quad_unions", "record_layout", "pack_records", "transpose_sort", "pack_transpose", "state",
+                 "tune_dose", "tune_transpose", "graph")
 
 _lib = None
 _P = ctypes.c_void_p
@@ -65,13 +77,19 @@ def lib() -> ctypes.CDLL:
         i64, i32, dbl = ctypes.c_int64, ctypes.c_int32, ctypes.c_double
         L.imrt_workspace_bytes.argtypes = [i64, i64, i64, i32, i32, ctypes.POINTER(ctypes.c_size_t)]
         L.imrt_plan_create.argtypes = [ctypes.POINTER(_P), i64, i64, i64, _P, _P, _P, _P, i32, _P, _P, _P, _P,
-                                       ctypes.POINTER(Params), _P, ctypes.c_size_t, _P]
+                                       ctypes.POINTER(Params), ctypes.POINTER(Options), _P, ctypes.c_size_t, _P]
         L.imrt_plan_set_x.argtypes = [_P, _P]
         L.imrt_plan_set_voxel_limits.argtypes = [_P, _P, _P]
         L.imrt_plan_run_iters.argtypes = [_P, i32]
         L.imrt_plan_run_to_tol.argtypes = [_P, dbl, i32]
         L.imrt_plan_eval.argtypes = [_P, _P, _P, _P, _P, ctypes.POINTER(dbl)]
+        L.imrt_plan_eval_batch.argtypes = [_P, i32, _P, _P, _P]
         L.imrt_plan_gradient.argtypes = [_P, _P, _P]
+        L.imrt_plan_get_tuning.argtypes = [_P, _P, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t)]
+        L.imrt_plan_get_create_times.argtypes = [_P, _P, i32, ctypes.POINTER(i32)]
+        L.imrt_merge_rows_workspace_bytes.argtypes = [i64, i64, ctypes.POINTER(ctypes.c_size_t)]
+        L.imrt_merge_rows_count.argtypes = [i64, i64, _P, _P, _P, i64, _P, ctypes.POINTER(i64), _P, ctypes.c_size_t, _P]
+        L.imrt_merge_rows_fill.argtypes = [i64, i64, _P, _P, _P, i64, _P, _P, _P, _P, ctypes.c_size_t, _P]
         L.imrt_trial_point.argtypes = [_P, _P, dbl, i64, _P, _P, _P]
         L.imrt_armijo_accepts.argtypes = [dbl] * 5
         L.imrt_stop_test.argtypes = [dbl] * 3
@@ -132,7 +150,7 @@ def imrt_workspace_bytes(n_v: int, n_b: int, nnz: int, n_structures: int, max_it
 
 
 def imrt_plan_create(n_v, n_b, nnz, row_ptr, col_idx, val, structure_id, t_under, t_over, w_under, w_over, params: Params,
-                     workspace, stream_ptr: int = 0):
+                     workspace, stream_ptr: int = 0, options: Options = None):
     """Returns the opaque plan handle (a ctypes.c_void_p).  Tensors are borrowed: keep them alive."""
     import torch
     tabs = [np.ascontiguousarray(a, dtype=np.float32) for a in (t_under, t_over, w_under, w_over)]
@@ -141,7 +159,8 @@ def imrt_plan_create(n_v, n_b, nnz, row_ptr, col_idx, val, structure_id, t_under
     st = lib().imrt_plan_create(ctypes.byref(handle), n_v, n_b, nnz, _dptr(row_ptr, torch.int32, n_v + 1),
                                 _dptr(col_idx, torch.int32, nnz), _dptr(val, torch.float32, nnz),
                                 _dptr(structure_id, torch.uint8, n_v), n_s, _hptr(tabs[0]), _hptr(tabs[1]), _hptr(tabs[2]),
-                                _hptr(tabs[3]), ctypes.byref(params), _dptr(workspace), workspace.numel() * workspace.element_size(),
+                                _hptr(tabs[3]), ctypes.byref(params), ctypes.byref(options) if options is not None else None,
+                                _dptr(workspace), workspace.numel() * workspace.element_size(),
                                 ctypes.c_void_p(stream_ptr))
     _check(st, None)
     return handle
@@ -172,6 +191,51 @@ def imrt_plan_eval(plan, x, d=None, r=None, g=None) -> float:
     _check(lib().imrt_plan_eval(plan, _dptr(x, torch.float32), _dptr(d, torch.float32), _dptr(r, torch.float32),
                                 _dptr(g, torch.float32), ctypes.byref(obj)), plan)
     return obj.value
+
+
+def imrt_plan_eval_batch(plan, x, r=None):
+    """x: fp32 CUDA tensor [n_points, n_b] (n_points = 1, 2 or 4); r: optional fp32 [n_points, n_v].  Returns G [n_points]."""
+    import torch
+    n = int(x.shape[0])
+    obj = np.zeros(n, np.float64)
+    _check(lib().imrt_plan_eval_batch(plan, n, _dptr(x, torch.float32), _dptr(r, torch.float32), _hptr(obj)), plan)
+    return obj
+
+
+def imrt_plan_get_tuning(plan) -> bytes:
+    n = ctypes.c_size_t(0)
+    _check(lib().imrt_plan_get_tuning(plan, None, 0, ctypes.byref(n)), plan)
+    buf = ctypes.create_string_buffer(n.value)
+    _check(lib().imrt_plan_get_tuning(plan, buf, n.value, ctypes.byref(n)), plan)
+    return buf.raw
+
+
+def imrt_plan_get_create_times(plan) -> dict:
+    ms = np.zeros(16, np.float64)
+    n = ctypes.c_int32(0)
+    _check(lib().imrt_plan_get_create_times(plan, _hptr(ms), 16, ctypes.byref(n)), plan)
+    return dict(zip(CREATE_PHASES, (float(v) for v in ms[:n.value])))
+
+
+def imrt_merge_rows(n_b: int, row_ptr, col_idx, val, group_id, n_groups: int, stream_ptr: int = 0):
+    """Mixed-resolution row merging: (row_ptr, col, val) CUDA tensors of the matrix whose row g is the mean
+    of the rows of D with group_id == g.  Argument marshalling around imrt_merge_rows_count / imrt_merge_rows_fill."""
+    import torch
+    n_v = row_ptr.numel() - 1
+    nb = ctypes.c_size_t(0)
+    _check(lib().imrt_merge_rows_workspace_bytes(n_v, n_groups, ctypes.byref(nb)))
+    ws = torch.empty(nb.value, dtype=torch.uint8, device=row_ptr.device)
+    out_rp = torch.empty(n_groups + 1, dtype=torch.int32, device=row_ptr.device)
+    nnz = ctypes.c_int64(0)
+    st = ctypes.c_void_p(stream_ptr)
+    _check(lib().imrt_merge_rows_count(n_v, n_b, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32), _dptr(group_id, torch.int32, n_v),
+                                       n_groups, _dptr(out_rp), ctypes.byref(nnz), _dptr(ws), nb.value, st))
+    out_c = torch.empty(max(nnz.value, 4), dtype=torch.int32, device=row_ptr.device)
+    out_v = torch.empty(max(nnz.value, 4), dtype=torch.float32, device=row_ptr.device)
+    _check(lib().imrt_merge_rows_fill(n_v, n_b, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32), _dptr(val, torch.float32), n_groups,
+                                      _dptr(out_rp), _dptr(out_c), _dptr(out_v), _dptr(ws), nb.value, st))
+    torch.cuda.current_stream(row_ptr.device).synchronize()      # ws goes out of scope
+    return out_rp, out_c[:nnz.value], out_v[:nnz.value]
 
 
 def imrt_plan_gradient(plan, r, g):
@@ -279,7 +343,9 @@ class Plan:
     """
 
     def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None,
-                 ls_batch: int = 0):
+                 ls_batch: int = 0, tuning: bytes = None, **options):
+        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, fused_gradient,
+        profile_create); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_0908_4421_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -305,9 +371,15 @@ class Plan:
                              int(driver), int(ls_batch))
         nbytes = imrt_workspace_bytes(self.n_v, self.n_b, self.nnz, self.n_structures, self.max_iters)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.options = Options(**{k: int(v) for k, v in options.items()})
+        self._tuning = tuning
+        if tuning is not None:
+            self._tuning_buf = ctypes.create_string_buffer(tuning, len(tuning))
+            self.options.host_tuning = ctypes.cast(self._tuning_buf, ctypes.c_void_p)
+            self.options.host_tuning_bytes = len(tuning)
         self.handle = imrt_plan_create(self.n_v, self.n_b, self.nnz, self.row_ptr, self.col, self.val, self.sid,
                                        prob.t_under, prob.t_over, prob.w_under, prob.w_over, self.params, self.workspace,
-                                       self.stream.cuda_stream)
+                                       self.stream.cuda_stream, self.options)
         self._tvu = self._tvo = None
         if getattr(prob, "tv_under", None) is not None or getattr(prob, "tv_over", None) is not None:
             self.set_voxel_limits(getattr(prob, "tv_under", None), getattr(prob, "tv_over", None))
@@ -350,6 +422,30 @@ class Plan:
         g = torch.empty(self.n_b, dtype=torch.float32, device=self.device) if want_g else None
         G = imrt_plan_eval(self.handle, x, d, r, g)
         return d, r, g, G
+
+    def eval_batch(self, xs, want_r=True):
+        """(r [n, n_v] or None, G [n]) of n = 1, 2 or 4 points evaluated in one pass over D (the line search's batched pass)."""
+        import torch
+        x = torch.from_numpy(np.ascontiguousarray(xs, dtype=np.float32)).to(self.device) if not isinstance(xs, torch.Tensor) else xs
+        x = x.to(device=self.device, dtype=torch.float32).contiguous()
+        r = torch.empty((x.shape[0], self.n_v), dtype=torch.float32, device=self.device) if want_r else None
+        return r, imrt_plan_eval_batch(self.handle, x, r)
+
+    def gradient(self, r):
+        """g = D^T r for an arbitrary residual (one transpose pass)."""
+        import torch
+        if not isinstance(r, torch.Tensor):
+            r = torch.from_numpy(np.ascontiguousarray(r, dtype=np.float32))
+        r = r.to(device=self.device, dtype=torch.float32).contiguous()
+        g = torch.empty(self.n_b, dtype=torch.float32, device=self.device)
+        imrt_plan_gradient(self.handle, r, g)
+        return g
+
+    def tuning(self) -> bytes:
+        return imrt_plan_get_tuning(self.handle)
+
+    def create_times(self) -> dict:
+        return imrt_plan_get_create_times(self.handle)
 
     def get_x(self):
         import torch

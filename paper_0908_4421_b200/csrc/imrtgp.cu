@@ -15,9 +15,11 @@
 
 #include <cub/block/block_scan.cuh>
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 
 #include "dvh.cuh"
 #include "kernels.cuh"
+#include "merge.cuh"
 
 using namespace imrt;
 
@@ -27,6 +29,7 @@ static thread_local std::string g_create_error;
 struct imrt_plan {
     DevPlan P;
     imrt_params prm;
+    imrt_options opt;
     cudaStream_t stream;
     int n_sm;
     size_t smem_bytes;
@@ -46,6 +49,8 @@ struct imrt_plan {
     int* rowslot_w;
     int* cta_rng_w;
     double tune_spread[2];            // slowest / mean CTA time of the dose pass before and after tuning
+    std::vector<int> cta_blk_h;       // the dose-pass partition in use (host copy, for imrt_plan_get_tuning)
+    std::vector<double> create_ms;    // phase times of plan creation (imrt_options.profile_create)
     // borrowed inputs
     const int32_t* row_ptr;
     const uint8_t* sid;
@@ -201,6 +206,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.dvh.hist = w.take<unsigned int>((size_t)n_s * DVH_MAX_PCTS * DVH_BINS);
     L.dvh.cnt = w.take<unsigned int>((size_t)MAX_STRUCTURES);
     L.dvh.sum = w.take<double>((size_t)MAX_STRUCTURES);
+    L.dvh.part = w.take<double>((size_t)DVH_SUM_BLOCKS * n_s);
     L.dvh.query = w.take<DvhQuery>((size_t)MAX_STRUCTURES * DVH_MAX_PCTS);
     L.quadU = w.take<int>(n_v / 4 + 2);
     L.covered = w.take<unsigned char>(n_v + 4);
@@ -543,7 +549,7 @@ __global__ void k_reset_state(State* st) {
     st->iter = 0; st->iter_target = 0; st->m = 0; st->stop_reason = STOP_MAX_ITERS;
     st->xi = 0; st->ri = 0;   // the MODE_INIT dose pass reads xbuf[0], writes rbuf[1] and makes it current
     st->cont_outer = 0; st->cont_inner = 0; st->bad_x = 0;
-    st->ticket_f = 0u; st->ticket_t = 0u; st->gridbar = 0u;
+    st->ticket_f = 0u; st->ticket_t = 0u; st->gridbar = 0u; st->clamped = 0;
 }
 
 __global__ void k_copy_current_x(const DevPlan P, float* x) {
@@ -565,16 +571,20 @@ struct RecordCaps {
     int chunk_slots;   // row format: slots per record
     int max_rows;      // row format: rows per record
     int quad_cap;      // quad format: union columns per record
+    int quad_max;      // quad format: union columns of ONE quad at most (a longer one goes to row-format records)
 };
 // ring_est: roughly the bytes the dose pass's ring will have (what the gather array and g leave of shared memory).
-static RecordCaps record_caps(int64_t n_v, int64_t nnz, int64_t ring_est) {
+static RecordCaps record_caps(int64_t n_v, int64_t nnz, int64_t ring_est, int quad_cap_user) {
     auto clampi = [](int64_t v, int lo, int hi) { return (int)std::max<int64_t>(lo, std::min<int64_t>(hi, v)); };
     RecordCaps c;
     c.chunk_slots = clampi((nnz / TARGET_RECORDS + 3) & ~(int64_t)3, 64, ROW_REC_SLOTS);
     c.max_rows = clampi(n_v / TARGET_RECORDS, 8, MAXROWS_F);
     // quad records: at least one per consumer warp must fit in the ring (18 bytes per union column); measured on the
     // 9- and 15-field phantoms, 480 .. 576 columns (8 .. 10 KB, mostly 4 quads = 2 warp trips) is the sweet spot
-    c.quad_cap = clampi(std::min<int64_t>(nnz / 3 / TARGET_RECORDS, ring_est / (W_CONS * 18)), 32, QUAD_CAP);
+    const int cap = quad_cap_user > 0 ? std::max(32, std::min(quad_cap_user, 4096)) : QUAD_CAP;
+    c.quad_cap = clampi(std::min<int64_t>(nnz / 3 / TARGET_RECORDS, ring_est / (W_CONS * 18)), 32, cap);
+    // a single quad may exceed quad_cap (it then fills a record by itself), but two such records must fit in the ring
+    c.quad_max = clampi((ring_est / 2 - 256) / 18, 0, 65528);
     return c;
 }
 
@@ -625,9 +635,10 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
         }
         bool quads = !quadU.empty() && bytes_rows > 0;
         if (quads) {
+            bool fits = true;
             for (int q = seg0 / 4; q < (seg1 + 3) / 4; ++q)
-                if (quadU[q] > 0) bytes_quads += (long long)pad8(quadU[q]) * 18 + 8;
-            quads = bytes_quads < bytes_rows;
+                if (quadU[q] > 0) { bytes_quads += (long long)pad8(quadU[q]) * 18 + 8; fits = fits && quadU[q] <= caps.quad_max; }
+            quads = fits && bytes_quads < bytes_rows;
         }
         if (!quads) {
             // ---- row-format records
@@ -677,8 +688,6 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
                 if (quadU[q] == 0) { skip_quad(q); ++q; continue; }
                 const int q0 = q;
                 int cols = pad8(quadU[q]);
-                if (cols > 65528)
-                    return fail(pl, IMRT_STATUS_UNSUPPORTED, "rows %d..%d of D touch %d distinct columns; too many for one record", 4 * q, 4 * q + 3, quadU[q]);
                 int last = q, empties = 0, qq = q + 1;
                 while (qq < q_end && qq - q0 < QUAD_MAXQ) {
                     if (quadU[qq] == 0) {
@@ -693,7 +702,7 @@ imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::v
                     ++qq;
                 }
                 int q1 = last + 1, nq = q1 - q0;
-                constexpr int QROUND = 2 * TEAM;
+                constexpr int QROUND = 2;
                 if (nq > QROUND && nq % QROUND) {  // a warp takes two quads at a time: keep the pairs full
                     for (int t = q1 - nq % QROUND; t < q1; ++t) cols -= pad8(quadU[t]);
                     q1 -= nq % QROUND;
@@ -815,6 +824,7 @@ static imrt_status upload_partition(imrt_plan* pl, const std::vector<int>& cta_b
     k_ring_layout<<<pl->P.grid_f, 32, 0, st>>>(pl->blk_w, pl->cta_blk_w, pl->P.grid_f, (unsigned int)pl->P.ring_f_bytes);
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));   // cta_blk is a host vector the caller may drop
+    pl->cta_blk_h = cta_blk;
     return IMRT_STATUS_OK;
 }
 
@@ -835,7 +845,7 @@ static imrt_status timing_loop_run(imrt_plan* pl) {
     return IMRT_STATUS_OK;
 }
 constexpr int LOOP_MEASUREMENTS = 1;   // 3 gains 0.7 % of loop speed and costs 16 ms of plan creation (cfg3)
-static bool can_time_in_loop(const imrt_plan* pl) { return pl->prm.max_iters >= 3 && !getenv("IMRTGP_NO_LOOP_TUNE"); }
+static bool can_time_in_loop(const imrt_plan* pl) { return pl->prm.max_iters >= 3 && pl->opt.tune_level >= 2; }
 
 // The same for the transpose pass: equal shares of the D^T stream do not take equal time (the gathers of r hit the L2
 // differently from SM to SM), so measure every CTA's pass time and hand out shares in proportion to measured speed.
@@ -860,7 +870,7 @@ static imrt_status upload_shares(imrt_plan* pl, const std::vector<double>& share
 
 static imrt_status tune_transpose(imrt_plan* pl) {
     const int grid = pl->P.grid_t, n_b = pl->n_rows_tr;
-    if (getenv("IMRTGP_NO_TUNE") || grid < 2 || pl->rp_tr[n_b] < (long long)grid * 8 * CHUNK_T) return IMRT_STATUS_OK;
+    if (pl->opt.tune_level < 1 || grid < 2 || pl->rp_tr[n_b] < (long long)grid * 8 * CHUNK_T) return IMRT_STATUS_OK;
     cudaStream_t st = pl->stream;
     PassArgs A;
     memset(&A, 0, sizeof A);
@@ -917,7 +927,7 @@ static imrt_status tune_partition(imrt_plan* pl) {
     pl->tune_spread[0] = pl->tune_spread[1] = 0.0;
     const int grid = pl->P.grid_f;
     const size_t n_blk = pl->blk_cost.size();
-    if (getenv("IMRTGP_NO_TUNE") || n_blk < (size_t)grid * 8) return IMRT_STATUS_OK;
+    if (pl->opt.tune_level < 1 || n_blk < (size_t)grid * 8) return IMRT_STATUS_OK;
     cudaStream_t st = pl->stream;
     PassArgs A;              // the loop's own dose pass (R trial points) on x = 0
     memset(&A, 0, sizeof A);
@@ -967,6 +977,14 @@ static imrt_status tune_partition(imrt_plan* pl) {
     if (!best_blk.empty() && best_blk != cta_blk) return upload_partition(pl, best_blk);
     return IMRT_STATUS_OK;
 }
+
+// What imrt_plan_get_tuning hands out: this header, then cta_blk int[grid_f + 1], then tr_share double[grid_t].
+constexpr unsigned int TUNING_MAGIC = 0x696d7274u;
+struct TuningBlob {
+    unsigned int magic;
+    int grid_f, grid_t, pad;
+    int64_t n_blk, nnz_tr;
+};
 
 // graph:  k_begin -> WHILE(outer){ k_transpose -> WHILE(inner){ k_dose } }
 static imrt_status build_graph(imrt_plan* pl) {
@@ -1039,17 +1057,18 @@ static imrt_status build_graph(imrt_plan* pl) {
     return IMRT_STATUS_OK;
 }
 
-// Phase timer of plan creation (IMRTGP_PROFILE_CREATE=1 prints the phases to stderr).
+// Phase timer of plan creation (imrt_options.profile_create: a synchronisation after every phase; the times are read
+// with imrt_plan_get_create_times).
 struct PhaseTimer {
-    bool on;
+    std::vector<double>* out;
     cudaStream_t st;
     std::chrono::steady_clock::time_point t0;
-    PhaseTimer(cudaStream_t s) : on(getenv("IMRTGP_PROFILE_CREATE") != nullptr), st(s), t0(std::chrono::steady_clock::now()) {}
-    void mark(const char* what) {
-        if (!on) return;
+    PhaseTimer(std::vector<double>* o, cudaStream_t s) : out(o), st(s), t0(std::chrono::steady_clock::now()) {}
+    void mark() {
+        if (!out) return;
         cudaStreamSynchronize(st);
         const auto t1 = std::chrono::steady_clock::now();
-        fprintf(stderr, "imrt_plan_create: %-28s %8.3f ms\n", what, std::chrono::duration<double, std::milli>(t1 - t0).count());
+        out->push_back(std::chrono::duration<double, std::milli>(t1 - t0).count());
         t0 = t1;
     }
 };
@@ -1063,7 +1082,7 @@ const char* imrt_last_error(const imrt_plan* plan) { return plan ? plan->err.c_s
 
 imrt_status imrt_workspace_bytes(int64_t n_v, int64_t n_b, int64_t nnz, int32_t n_structures, int32_t max_iters,
                                  size_t* host_bytes) {
-    if (!host_bytes || n_v < 0 || n_b < 0 || nnz < 0 || n_structures < 1 || n_structures > MAX_STRUCTURES || max_iters < 0)
+    if (!host_bytes || n_v < 1 || n_b < 1 || nnz < 0 || n_structures < 1 || n_structures > MAX_STRUCTURES || max_iters < 0)
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_workspace_bytes: bad argument");
     if (nnz >= (1LL << 31) - 16 || n_v >= (1LL << 31) - 16 || n_b >= (1LL << 31) - 16)
         return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "sizes must fit int32");
@@ -1074,8 +1093,8 @@ imrt_status imrt_workspace_bytes(int64_t n_v, int64_t n_b, int64_t nnz, int32_t 
 imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t nnz, const int32_t* row_ptr,
                              const int32_t* col_idx, const float* val, const uint8_t* structure_id, int32_t n_structures,
                              const float* host_t_under, const float* host_t_over, const float* host_w_under,
-                             const float* host_w_over, const imrt_params* prm, void* workspace, size_t workspace_bytes,
-                             void* stream) {
+                             const float* host_w_over, const imrt_params* prm, const imrt_options* host_options,
+                             void* workspace, size_t workspace_bytes, void* stream) {
     if (out) *out = nullptr;
     if (!out || !row_ptr || !structure_id || !host_t_under || !host_t_over || !host_w_under || !host_w_over || !prm || !workspace)
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: null argument");
@@ -1108,8 +1127,16 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         return fail(nullptr, IMRT_STATUS_UNSUPPORTED_DEVICE, "device has compute capability %d.x; libimrtgp is built for sm_100a only", cc_major);
     if (n_sm > 1024) n_sm = 1024;
 
+    imrt_options opt;
+    memset(&opt, 0, sizeof opt);
+    if (host_options) opt = *host_options;
+    if (opt.tune_level < 0 || opt.tune_level > 2 || opt.dose_format < 0 || opt.dose_format > 1 || (opt.col_bits != 0 && opt.col_bits != 32) ||
+        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 || opt.fused_gradient < 0 || opt.fused_gradient > 1 ||
+        (opt.host_tuning && opt.host_tuning_bytes < sizeof(int) * 8))
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad imrt_options");
     imrt_plan* pl = new imrt_plan();
     pl->prm = *prm;
+    pl->opt = opt;
     pl->stream = (cudaStream_t)stream;
     pl->n_sm = n_sm;
     pl->has_x = false;
@@ -1121,7 +1148,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     // every early return below releases the handle
     struct Guard { imrt_plan* p; ~Guard() { if (p) { g_create_error = p->err; delete p; } } } guard{pl};
 
-    PhaseTimer phase(st);
+    PhaseTimer phase(opt.profile_create ? &pl->create_ms : nullptr, st);
     // ---- validate what the host can see: row_ptr and structure ids
     std::vector<int> rp((size_t)n_v + 1);
     std::vector<uint8_t> sid((size_t)n_v);
@@ -1147,7 +1174,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     for (int64_t j = 0; j < n_v; ++j)
         if (sid[j] >= n_structures) return fail(pl, IMRT_STATUS_BAD_STRUCTURE, "structure_id[%lld] = %d >= n_structures", (long long)j, sid[j]);
 
-    phase.mark("validate");
+    phase.mark();
     // ---- penalty table
     std::vector<float4> table_h(MAX_STRUCTURES, make_float4(0, 0, 0, 0));
     for (int s = 0; s < n_structures; ++s) table_h[s] = make_float4(host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]);
@@ -1158,17 +1185,17 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
 
     // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero); a block holds
     // ROW_REC_SLOTS slots unless a longer row forces more
-    const bool col16 = n_b <= 65536 && !getenv("IMRTGP_COL32");
+    const bool col16 = n_b <= 65536 && opt.col_bits != 32;
     int max_row = 0;
     for (int64_t j = 0; j < n_v; ++j) max_row = std::max(max_row, rp[j + 1] - rp[j]);
     if (max_row > MAX_CHUNK_SLOTS)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row of D has %d entries; this build handles rows up to %d", max_row, MAX_CHUNK_SLOTS);
     const int64_t nb_pad_est = (n_b + 31) & ~31LL;
-    const RecordCaps caps = record_caps(n_v, nnz, (int64_t)smem_optin - SMEM_HEADER - 256 - std::max(SMEM_WPART, SMEM_DSC) - nb_pad_est * 4 * (R_MAX + 1));
+    const RecordCaps caps = record_caps(n_v, nnz, (int64_t)smem_optin - SMEM_HEADER - 256 - std::max(SMEM_WPART, SMEM_DSC) - nb_pad_est * 4 * (R_MAX + 1), opt.quad_cap);
     // quad format on offer: count the distinct columns of every 4 consecutive rows on the device
     const int bm_words = (int)((n_b + 31) / 32);
     std::vector<int> quadU;
-    if (col16 && n_b <= QUAD_MAX_NB && nnz > 0 && !getenv("IMRTGP_NO_QUADS")) {
+    if (col16 && n_b <= QUAD_MAX_NB && nnz > 0 && opt.dose_format == 0) {
         const int n_quads = (int)((n_v + 3) / 4);
         quadU.resize(n_quads);
         k_quad_union<<<std::min(n_quads / 8 + 1, n_sm * 8), 256, 8 * bm_words * sizeof(uint32_t), st>>>(row_ptr, col_idx, (int)n_v, n_quads, bm_words, L.quadU);
@@ -1176,7 +1203,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaMemcpyAsync(quadU.data(), L.quadU, sizeof(int) * n_quads, cudaMemcpyDeviceToHost, st));
         CUDA_TRY(pl, cudaStreamSynchronize(st));
     }
-    phase.mark("quad union counts");
+    phase.mark();
     // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1).
     // Enqueued here, ahead of the record layout below: that runs on the host for a few ms and needs nothing of this, so
     // the device sorts meanwhile (no workspace region is shared between the two).
@@ -1208,7 +1235,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         return s;
     }
     CUDA_TRY(pl, cudaMemcpyAsync(L.covered, covered.data(), (size_t)n_v, cudaMemcpyHostToDevice, st));
-    phase.mark("build_blocks (host)");
+    phase.mark();
     const size_t n_blk = BP.blk.size();
     if ((int64_t)n_blk > B.max_blk || (int64_t)BP.meta.size() > B.max_meta || BP.pack_bytes > B.max_pack)
         return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %zu words, %zu bytes)",
@@ -1234,7 +1261,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaGetLastError());
     }
 
-    phase.mark("pack records");
+    phase.mark();
     // ---- the explicit transpose was enqueued before the record layout: fetch its row pointers
     if (nnz > 0) {
         CUDA_TRY(pl, cudaMemcpyAsync(rpT.data(), L.rowT_ptr, sizeof(int) * (n_b + 1), cudaMemcpyDeviceToHost, st));
@@ -1244,17 +1271,17 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     // ---- transpose-pass ranges and gradient slots
     std::vector<TrRange> ranges;
     std::vector<int> rowslot, cta_rng_h;
-    phase.mark("transpose (sort + gather)");
+    phase.mark();
     // ---- the stream the transpose pass reads.  First choice: row pairs with 16-bit voxel offsets, if that is smaller
     // than single rows; second: single rows with 16-bit offsets; last: the plain 32-bit CSR (a group of 32 entries
     // spanning more than 65,535 voxels rules the 16-bit forms out).
-    const bool can16 = nnz > 0 && !getenv("IMRTGP_NO_ID16") && nnz + 128 * n_b + 128 < (1LL << 31);
+    const bool can16 = nnz > 0 && opt.transpose_format != 2 && nnz + 128 * n_b + 128 < (1LL << 31);
     std::vector<int> rpP((size_t)n_b + 1, 0);
     if (can16)
         for (int64_t i = 0; i < n_b; ++i) rpP[i + 1] = rpP[i] + ((rpT[i + 1] - rpT[i] + 127) & ~127);
     const int n_pairs = (int)((n_b + 1) / 2);
     std::vector<int> rpPair((size_t)n_pairs + 1, 0);
-    bool pairs = can16 && n_b >= 2 && !getenv("IMRTGP_NO_PAIRS");
+    bool pairs = can16 && n_b >= 2 && opt.transpose_format == 0;
     if (pairs) {
         std::vector<int> U((size_t)n_pairs);
         k_pair_count<<<n_pairs, 256, 0, st>>>(L.rowT_ptr, L.colT, (int)n_b, L.pairU);
@@ -1307,7 +1334,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     pl->max_ranges = B.max_ranges; pl->max_slots = B.max_slots;
     pl->tr_range_w = L.tr_range; pl->rowslot_w = L.rowslot_ptr; pl->cta_rng_w = L.cta_rng;
 
-    phase.mark("pack D^T, ranges");
+    phase.mark();
     // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, dose
     // scratch, the R trial points, g, then the ring (dose pass) / stages (transpose pass).  R = the largest of 4, 2, 1
     // not above the request that leaves the ring room for 16 records of average size (one per consumer warp).
@@ -1315,7 +1342,6 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     const long long avg_rec = n_blk ? (long long)(BP.pack_bytes / n_blk) : 128;
     const int nb_pad = (int)((n_b + 31) & ~31LL);
     int R = prm->ls_batch == 0 ? R_MAX : prm->ls_batch;
-    if (getenv("IMRTGP_LS_BATCH")) R = atoi(getenv("IMRTGP_LS_BATCH"));
     if (R != 1 && R != 2 && R != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_params.ls_batch must be 0, 1, 2 or 4");
     const int stage_t = pairs ? CHUNK_T * 10 + CHUNK_T / 8 : id16 ? CHUNK_T * 6 + CHUNK_T / 8 : STAGE_T_BYTES;
     int off = 0, avail = 0, stt = 0;
@@ -1364,6 +1390,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaFuncSetAttribute(k_dose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
     CUDA_TRY(pl, cudaFuncSetAttribute(k_transpose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
     CUDA_TRY(pl, cudaFuncSetAttribute(k_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
+    CUDA_TRY(pl, cudaFuncSetAttribute(k_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
 
     // ---- device state, constant residual of the zero-dose rows
     State st_h;
@@ -1388,19 +1415,43 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
 
+    // ---- a caller-supplied partition (imrt_plan_get_tuning of an earlier plan of this problem) replaces the measurements
+    const TuningBlob* tb = static_cast<const TuningBlob*>(opt.host_tuning);
+    if (tb) {
+        if (tb->magic != TUNING_MAGIC || tb->n_blk != (int64_t)n_blk || tb->grid_f != grid_f || tb->grid_t != grid_t || tb->nnz_tr != pl->rp_tr[n_rows_tr] ||
+            opt.host_tuning_bytes < sizeof(TuningBlob) + sizeof(int) * (grid_f + 1) + sizeof(double) * grid_t)
+            return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_options.host_tuning does not belong to this problem / these options / this device");
+        const int* cb = reinterpret_cast<const int*>(tb + 1);
+        cta_blk.assign(cb, cb + grid_f + 1);
+        for (int c = 0; c < grid_f; ++c)
+            if (cta_blk[c] > cta_blk[c + 1] || cta_blk[0] != 0 || cta_blk[grid_f] != (int)n_blk)
+                return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_options.host_tuning: corrupt partition");
+    }
     s = upload_partition(pl, cta_blk);
     if (s != IMRT_STATUS_OK) return s;
-    phase.mark("state, first schedule");
-    s = tune_partition(pl);
-    if (s != IMRT_STATUS_OK) return s;
-    phase.mark("rebalance dose pass");
-    s = tune_transpose(pl);
-    if (s != IMRT_STATUS_OK) return s;
-    phase.mark("rebalance transpose pass");
+    phase.mark();
+    if (tb) {
+        std::vector<double> share(grid_t);
+        memcpy(share.data(), reinterpret_cast<const char*>(tb + 1) + sizeof(int) * (grid_f + 1), sizeof(double) * grid_t);
+        bool fits = true;
+        s = upload_shares(pl, share, fits);
+        if (s != IMRT_STATUS_OK) return s;
+        if (!fits) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_options.host_tuning: transpose shares do not fit");
+        phase.mark();
+        phase.mark();
+    } else {
+        s = tune_partition(pl);
+        if (s != IMRT_STATUS_OK) return s;
+        phase.mark();
+        s = tune_transpose(pl);
+        if (s != IMRT_STATUS_OK) return s;
+        phase.mark();
+    }
     if (prm->driver == 0) {
         s = build_graph(pl);
         if (s != IMRT_STATUS_OK) return s;
     }
+    phase.mark();
     guard.p = nullptr;
     *out = pl;
     return IMRT_STATUS_OK;
@@ -1522,6 +1573,33 @@ imrt_status imrt_plan_eval(imrt_plan* pl, const float* x, float* d, float* r, fl
     return IMRT_STATUS_OK;
 }
 
+imrt_status imrt_plan_eval_batch(imrt_plan* pl, int32_t n_points, const float* x, float* r, double* host_obj) {
+    if (!pl || !x || !host_obj) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_eval_batch: null argument");
+    if (n_points != 1 && n_points != 2 && n_points != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_eval_batch: n_points must be 1, 2 or 4");
+    if (n_points > pl->P.R)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "imrt_plan_eval_batch: this plan evaluates %d trial point(s) per pass (imrt_plan_get_info [10])", pl->P.R);
+    cudaStream_t st = pl->stream;
+    const int n_v = pl->P.n_v;
+    if (r) {      // constant residual of the rows no record covers
+        RPtrs rp;
+        memset(&rp, 0, sizeof rp);
+        for (int j = 0; j < n_points; ++j) rp.p[j] = r + (size_t)j * n_v;
+        k_fill_zero_dose_rows<<<(n_v + 255) / 256, 256, 0, st>>>(pl->sid, pl->P.table, pl->P.st, n_v, rp, nullptr);
+    }
+    PassArgs A;
+    memset(&A, 0, sizeof A);
+    A.mode = MODE_BATCH;
+    A.n_points = n_points;
+    A.x_in = x;
+    A.r_out = r;
+    CUDA_TRY(pl, launch_dose(pl, A));
+    double objs[4];
+    CUDA_TRY(pl, cudaMemcpyAsync(objs, pl->P.st->eval_objs, sizeof objs, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));
+    for (int j = 0; j < n_points; ++j) host_obj[j] = objs[j];
+    return IMRT_STATUS_OK;
+}
+
 imrt_status imrt_plan_gradient(imrt_plan* pl, const float* r, float* g) {
     if (!pl || !r || !g) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_gradient: null argument");
     PassArgs T;
@@ -1622,7 +1700,8 @@ imrt_status imrt_plan_get_trace(imrt_plan* pl, int32_t* host_n_iters_done, int32
     CUDA_TRY(pl, cudaStreamSynchronize(st));
     const int n = std::min(s.iter, capacity);
     if (host_n_iters_done) *host_n_iters_done = s.iter;
-    if (host_stop_reason) *host_stop_reason = s.stop_reason;
+    if (host_stop_reason)      // the trace filled up before the requested number of iterations was done
+        *host_stop_reason = (s.stop_reason == STOP_MAX_ITERS && s.clamped && s.iter >= s.trace_cap) ? STOP_TRACE_FULL : s.stop_reason;
     if (host_obj) CUDA_TRY(pl, cudaMemcpyAsync(host_obj, pl->P.tr_obj, sizeof(double) * (n + 1), cudaMemcpyDeviceToHost, st));
     if (host_lambda && n) CUDA_TRY(pl, cudaMemcpyAsync(host_lambda, pl->P.tr_lambda, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
     if (host_n_trials && n) CUDA_TRY(pl, cudaMemcpyAsync(host_n_trials, pl->P.tr_trials, sizeof(int) * n, cudaMemcpyDeviceToHost, st));
@@ -1654,6 +1733,127 @@ imrt_status imrt_plan_get_info(imrt_plan* pl, int64_t* host_info, int32_t n_info
     return IMRT_STATUS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- mixed resolution
+namespace {
+struct MergeLayout {
+    unsigned int *keysA, *keysB, *rowsA, *rowsB, *rows;
+    int *group_ptr, *cnt, *flags;
+    void* temp;
+    size_t temp_bytes, total;
+};
+MergeLayout merge_layout(void* base, int64_t n_v, int64_t n_groups) {
+    Bump w{static_cast<unsigned char*>(base), 0};
+    MergeLayout M;
+    M.keysA = w.take<unsigned int>(n_v + 4);
+    M.keysB = w.take<unsigned int>(n_v + 4);
+    M.rowsA = w.take<unsigned int>(n_v + 4);
+    M.rowsB = w.take<unsigned int>(n_v + 4);
+    M.rows = w.take<unsigned int>(n_v + 4);
+    M.group_ptr = w.take<int>(n_groups + 2);
+    M.cnt = w.take<int>(n_groups + 2);
+    M.flags = w.take<int>(16);
+    M.temp_bytes = (size_t)(16 << 20) + (size_t)(n_v + n_groups);
+    M.temp = w.take<unsigned char>(M.temp_bytes);
+    M.total = (w.off + 255) & ~(size_t)255;
+    return M;
+}
+// bitmap words per warp and warps per block that fit the default 48 KB of shared memory (copies: 1 count, 2 fill)
+bool merge_shape(int64_t n_b, int copies, int& words, int& warps) {
+    words = (int)((n_b + 31) / 32);
+    warps = MERGE_WARPS;
+    while (warps > 1 && (size_t)warps * copies * words * 4 > 48 * 1024) warps /= 2;
+    return (size_t)warps * copies * words * 4 <= 48 * 1024;
+}
+}  // namespace
+
+imrt_status imrt_merge_rows_workspace_bytes(int64_t n_v, int64_t n_groups, size_t* host_bytes) {
+    if (!host_bytes || n_v < 1 || n_groups < 1 || n_v >= (1LL << 31) - 16 || n_groups >= (1LL << 31) - 16)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_merge_rows_workspace_bytes: bad argument");
+    *host_bytes = merge_layout(nullptr, n_v, n_groups).total;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_merge_rows_count(int64_t n_v, int64_t n_b, const int32_t* row_ptr, const int32_t* col_idx, const int32_t* group_id,
+                                  int64_t n_groups, int32_t* out_row_ptr, int64_t* host_nnz_out, void* workspace, size_t workspace_bytes,
+                                  void* stream) {
+    if (!row_ptr || !group_id || !out_row_ptr || !host_nnz_out || !workspace || n_v < 1 || n_b < 1 || n_groups < 1 ||
+        n_v >= (1LL << 31) - 16 || n_groups >= (1LL << 31) - 16)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_merge_rows_count: bad argument");
+    const MergeLayout M = merge_layout(workspace, n_v, n_groups);
+    if (workspace_bytes < M.total) return fail(nullptr, IMRT_STATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", workspace_bytes, M.total);
+    int words, warps;
+    if (!merge_shape(n_b, 2, words, warps)) return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "imrt_merge_rows: n_b = %lld is too large for the column bitmap", (long long)n_b);
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(nullptr, cudaMemsetAsync(M.flags, 0, 16 * sizeof(int), st));
+    k_merge_keys<<<grid_for(n_v, 256), 256, 0, st>>>(group_id, (int)n_v, (int)n_groups, M.keysA, M.rowsA, M.flags);
+    cub::DoubleBuffer<unsigned int> dk(M.keysA, M.keysB), dv(M.rowsA, M.rowsB);
+    int end_bit = 1;
+    while ((1LL << end_bit) < n_groups) ++end_bit;
+    size_t temp = 0;
+    CUDA_TRY(nullptr, cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)n_v, 0, end_bit, st));
+    if (temp > M.temp_bytes) return fail(nullptr, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: sort needs %zu temp bytes", temp);
+    CUDA_TRY(nullptr, cub::DeviceRadixSort::SortPairs(M.temp, temp, dk, dv, (int)n_v, 0, end_bit, st));     // stable: rows stay ascending
+    CUDA_TRY(nullptr, cudaMemcpyAsync(M.rows, dv.Current(), sizeof(unsigned int) * n_v, cudaMemcpyDeviceToDevice, st));
+    k_merge_group_ptr<<<(int)((n_groups + 1 + 255) / 256), 256, 0, st>>>(dk.Current(), (int)n_v, (int)n_groups, M.group_ptr);
+    merge_shape(n_b, 1, words, warps);
+    CUDA_TRY(nullptr, cudaMemsetAsync(M.cnt, 0, sizeof(int) * (n_groups + 2), st));
+    int flags_h[16];
+    CUDA_TRY(nullptr, cudaMemcpyAsync(flags_h, M.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(nullptr, cudaStreamSynchronize(st));
+    if (flags_h[0]) return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_merge_rows_count: a group id is outside [0, n_groups)");
+    k_merge_count<<<(int)std::min<int64_t>((n_groups + warps - 1) / warps, 148 * 8), MERGE_WARPS * 32, (size_t)warps * words * 4, st>>>(
+        row_ptr, col_idx, M.rows, M.group_ptr, (int)n_groups, words, warps, M.cnt);
+    temp = 0;
+    CUDA_TRY(nullptr, cub::DeviceScan::ExclusiveSum(nullptr, temp, M.cnt, out_row_ptr, (int)(n_groups + 1), st));
+    if (temp > M.temp_bytes) return fail(nullptr, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: scan needs %zu temp bytes", temp);
+    CUDA_TRY(nullptr, cub::DeviceScan::ExclusiveSum(M.temp, temp, M.cnt, out_row_ptr, (int)(n_groups + 1), st));
+    int32_t total = 0;
+    CUDA_TRY(nullptr, cudaMemcpyAsync(&total, out_row_ptr + n_groups, sizeof total, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(nullptr, cudaStreamSynchronize(st));
+    *host_nnz_out = total;
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_merge_rows_fill(int64_t n_v, int64_t n_b, const int32_t* row_ptr, const int32_t* col_idx, const float* val,
+                                 int64_t n_groups, const int32_t* out_row_ptr, int32_t* out_col, float* out_val, void* workspace,
+                                 size_t workspace_bytes, void* stream) {
+    if (!row_ptr || !out_row_ptr || !workspace || n_v < 1 || n_b < 1 || n_groups < 1)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_merge_rows_fill: bad argument");
+    const MergeLayout M = merge_layout(workspace, n_v, n_groups);
+    if (workspace_bytes < M.total) return fail(nullptr, IMRT_STATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", workspace_bytes, M.total);
+    int words, warps;
+    if (!merge_shape(n_b, 2, words, warps)) return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "imrt_merge_rows: n_b = %lld is too large for the column bitmap", (long long)n_b);
+    if (!out_col || !out_val || !col_idx || !val) return IMRT_STATUS_OK;      // an empty merged matrix
+    k_merge_fill<<<(int)std::min<int64_t>((n_groups + warps - 1) / warps, 148 * 8), MERGE_WARPS * 32, (size_t)warps * 2 * words * 4, (cudaStream_t)stream>>>(
+        row_ptr, col_idx, val, M.rows, M.group_ptr, (int)n_groups, words, warps, out_row_ptr, out_col, out_val);
+    CUDA_TRY(nullptr, cudaGetLastError());
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_tuning(imrt_plan* pl, void* host_buf, size_t capacity, size_t* host_bytes) {
+    if (!pl || !host_bytes) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_tuning: null argument");
+    const int gf = pl->P.grid_f, gt = pl->P.grid_t;
+    const size_t need = sizeof(TuningBlob) + sizeof(int) * (gf + 1) + sizeof(double) * gt;
+    *host_bytes = need;
+    if (!host_buf) return IMRT_STATUS_OK;
+    if (capacity < need || (int)pl->cta_blk_h.size() != gf + 1 || (int)pl->tr_share.size() != gt)
+        return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_tuning: buffer too small (%zu needed)", need);
+    TuningBlob tb = {TUNING_MAGIC, gf, gt, 0, pl->n_blk, (int64_t)pl->rp_tr[pl->n_rows_tr]};
+    char* o = static_cast<char*>(host_buf);
+    memcpy(o, &tb, sizeof tb);
+    memcpy(o + sizeof tb, pl->cta_blk_h.data(), sizeof(int) * (gf + 1));
+    memcpy(o + sizeof tb + sizeof(int) * (gf + 1), pl->tr_share.data(), sizeof(double) * gt);
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_get_create_times(imrt_plan* pl, double* host_ms, int32_t capacity, int32_t* host_n) {
+    if (!pl || !host_n || capacity < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_create_times: bad argument");
+    const int n = std::min<int>((int)pl->create_ms.size(), capacity);
+    for (int i = 0; i < n && host_ms; ++i) host_ms[i] = pl->create_ms[i];
+    *host_n = n;
+    return IMRT_STATUS_OK;
+}
+
 imrt_status imrt_plan_get_pass_timing(imrt_plan* pl, int32_t kind, int64_t* host_start_ns, int64_t* host_end_ns, int32_t capacity,
                                       int32_t* host_n_ctas) {
     if (!pl || kind < 0 || kind > 1 || capacity < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_get_pass_timing: bad argument");
@@ -1670,8 +1870,16 @@ imrt_status imrt_plan_get_pass_timing(imrt_plan* pl, int32_t kind, int64_t* host
 }
 
 imrt_status imrt_plan_launch_pass(imrt_plan* pl, int32_t kind, int32_t n_repeat) {
-    if (!pl || kind < 0 || kind > 1 || n_repeat < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_launch_pass: bad argument");
+    if (!pl || kind < 0 || kind > 3 || n_repeat < 0) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_launch_pass: bad argument");
     if (!pl->has_x) return fail(pl, IMRT_STATUS_NOT_READY, "call imrt_plan_set_x first");
+    if (kind >= 2) {      // streaming ceilings: the pass's bytes through its ring / stages, no arithmetic
+        if (kind == 3 && pl->P.id16 != 2) return fail(pl, IMRT_STATUS_UNSUPPORTED, "the stream-only transpose pass exists for the row-pair stream only");
+        for (int i = 0; i < n_repeat; ++i) {
+            k_stream<<<kind == 2 ? pl->P.grid_f : pl->P.grid_t, NTHREADS, pl->smem_bytes, pl->stream>>>(pl->P, kind - 2);
+            CUDA_TRY(pl, cudaGetLastError());
+        }
+        return IMRT_STATUS_OK;
+    }
     PassArgs A;
     memset(&A, 0, sizeof A);
     A.mode = kind == 0 ? MODE_TIMING : MODE_EVAL;   // dose pass: the line search's pass, residuals to the trial buffers

@@ -30,9 +30,6 @@ namespace imrt {
 
 // ------------------------------------------------------------------------------------------------ constants
 constexpr int W_CONS = 16;                    // consumer warps per CTA
-constexpr int TEAM = 1;                       // consumer warps that split one dose-pass record (the block functions take
-                                              // (tw, TEAM); teams of 4 measured slower: profiles/r01_notes.md)
-constexpr int N_TEAMS = W_CONS / TEAM;
 constexpr int N_CONS = W_CONS * 32;           // consumer threads
 constexpr int N_PROD = 2;                     // producer warps of the dose pass (the transpose pass uses the first only)
 constexpr int NTHREADS = N_CONS + 32 * N_PROD;
@@ -55,14 +52,14 @@ constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a ra
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
 constexpr int RL_MAX = 32;                    // rows of D^T one transpose range may span
 constexpr int RING_ENTRIES = 64;              // dose-pass records in flight per CTA (a multiple of the team count)
-constexpr int MAX_STAGES_T = 12;
+constexpr int MAX_STAGES_T = 16;
 constexpr int MAX_STRUCTURES = 256;
 constexpr int SMEM_HEADER = 3072;             // barriers, flags, reduction scratch
 constexpr int SMEM_WPART = RL_MAX * W_CONS * 8 * 2;   // transpose pass: per-(row, warp) fp64 partials, two per row pair
 constexpr int SMEM_DSC = W_CONS * 32 * R_MAX * 4;   // per-warp scratch: dose of 32 rows x R trial points
 
-enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2, MODE_TIMING = 3 };
-enum { STOP_MAX_ITERS = 0, STOP_TOLERANCE = 1, STOP_STATIONARY = 2, STOP_LS_STALLED = 3 };
+enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2, MODE_TIMING = 3, MODE_BATCH = 4 };
+enum { STOP_MAX_ITERS = 0, STOP_TOLERANCE = 1, STOP_STATIONARY = 2, STOP_LS_STALLED = 3, STOP_TRACE_FULL = 4 };
 
 // ------------------------------------------------------------------------------------------------ device data
 struct State {                 // lives in the workspace; the single source of truth between launches
@@ -70,6 +67,7 @@ struct State {                 // lives in the workspace; the single source of t
     double lambda;             // step size of the first trial of the pending batch
     double eps, alpha, lambda0, delta_tol;
     double eval_obj;           // output of MODE_EVAL dose passes
+    double eval_objs[4];       // outputs of a MODE_BATCH dose pass (imrt_plan_eval_batch)
     double G_skip;             // objective of the rows no block covers (their dose is 0: a constant)
     const float* tvu;          // optional per-voxel limits T-_j / T+_j [n_v] (NULL: the structure's, reading R16)
     const float* tvo;
@@ -86,7 +84,7 @@ struct State {                 // lives in the workspace; the single source of t
     int bad_x;                 // set_x validation result
     unsigned int ticket_f, ticket_t;   // last-CTA tickets
     unsigned int gridbar;      // grid barrier counter of the persistent kernel
-    int pad;
+    int clamped;               // the last run's target was cut short by the trace capacity
 };
 
 struct TrRange {               // a contiguous piece of the D^T nnz stream, 32 bytes
@@ -175,6 +173,7 @@ struct PassArgs {
     float* d_out;              // dose pass, MODE_EVAL: dose out or NULL
     float* g_out;              // transpose pass MODE_EVAL: gradient out
     int mode;
+    int n_points;              // MODE_BATCH: points at x_in ([n_points][n_b]); residuals to r_out ([n_points][n_v]) or scratch
     int use_handles;           // 1 inside the conditional graph
     cudaGraphConditionalHandle h_outer, h_inner;
 };
@@ -198,7 +197,7 @@ __device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4
         for (int s = 0; s < RING_ENTRIES; ++s) mbar_init(&h->full_f[s], 1);
         for (int s = 0; s < MAX_STAGES_T; ++s) {
             mbar_init(&h->full_t[s], 1);
-            mbar_init(&h->empty_t[s], W_CONS / TGROUPS);
+            mbar_init(&h->empty_t[s], W_CONS);
         }
         mbar_fence_init();
     }
@@ -336,7 +335,7 @@ template <> struct XVec<4> { float v[4]; __device__ __forceinline__ void load(co
 template <bool COL16, int R>
 __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
                                            const float4* __restrict__ table_s, float* __restrict__ dsc,
-                                           float* const (&r_out)[R], float* __restrict__ d_out, const VoxelLimits vl, int tw, int lane,
+                                           float* const (&r_out)[R], float* __restrict__ d_out, const VoxelLimits vl, int lane,
                                            double (&Gacc)[R]) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nrows = (int)hdr.x, slots = (int)hdr.w;
@@ -346,11 +345,11 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
     const int grp = lane / VW, sub = lane % VW;
     constexpr int XB = 4 * R;   // bytes per beamlet in the gather array
     const int nbatch = (nrows + RB - 1) / RB;
-    // warp tw of the team takes the batches tw, tw + TEAM, ...; 8 of its batches (32 rows) make one penalty step
-    for (int q0 = tw; q0 < nbatch; q0 += 8 * TEAM) {
+    // 8 batches (32 rows) make one penalty step
+    for (int q0 = 0; q0 < nbatch; q0 += 8) {
 #pragma unroll 1
         for (int kq = 0; kq < 8; ++kq) {
-            const int q = q0 + kq * TEAM;
+            const int q = q0 + kq;
             if (q >= nbatch) break;
             const int row = q * RB + grp;
             uint32_t m0 = 0u, m1 = 0u;
@@ -395,7 +394,7 @@ __device__ __forceinline__ void dose_block(const unsigned char* __restrict__ rec
             }
         }
         __syncwarp();
-        const int row = (q0 + (lane / RB) * TEAM) * RB + (lane % RB);     // the row parked at position `lane`
+        const int row = (q0 + lane / RB) * RB + (lane % RB);     // the row parked at position `lane`
         if (row < nrows) {
             float4 t = table_s[(rows[row] >> 16) & 0xFFu];
             XVec<R> dv;
@@ -439,7 +438,7 @@ template <int R> __device__ __forceinline__ bool quad_owner(int lane) { return (
 template <int R>
 __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
                                                  const float4* __restrict__ table_s, float* __restrict__ my_r,
-                                                 float* __restrict__ d_out, const VoxelLimits vl, int tw, int lane, double& Gq) {
+                                                 float* __restrict__ d_out, const VoxelLimits vl, int lane, double& Gq) {
     const uint4 hdr = *reinterpret_cast<const uint4*>(rec);
     const int nq = (int)hdr.x, nbc = (int)hdr.w;
     const uint32_t* qt = reinterpret_cast<const uint32_t*>(rec) + META_HDR;
@@ -450,7 +449,7 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
     const bool hi8 = (lane & 8) != 0, hi4 = (lane & 4) != 0, hi2 = (lane & 2) != 0, hi1 = (lane & 1) != 0;
     const int rr = (hi8 ? 2 : 0) + (hi4 ? 1 : 0);          // the row this lane ends up with
     const bool owner = quad_owner<R>(lane);
-    for (int q0 = 2 * tw; q0 < nq; q0 += 2 * TEAM) {       // warp tw of the team takes the quad pairs tw, tw + TEAM, ...
+    for (int q0 = 0; q0 < nq; q0 += 2) {
         // A quad without a partner (the record's only or last one: typically a long quad that fills a record by itself)
         // is split between the halves instead, columns [s, mid) and [mid, e); their sums meet in one more xor step.
         const bool lone = q0 + 1 >= nq;
@@ -519,7 +518,9 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
 
 // All NTHREADS threads of the CTA call this.  xs: the R trial points in shared memory.  Writes the CTA's R objective
 // partials to Gpart[blockIdx.x * R ..] (thread 0).  Ends with a CTA-wide barrier.
-template <bool COL16, int R>
+// STREAM: the read-only streaming ceiling of the pass -- the producers move every record through the ring exactly as in
+// the real pass, the consumer warps wait for their records and hand them back untouched (imrt_plan_launch_pass kind 2).
+template <bool COL16, int R, bool STREAM = false>
 __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
                                             const float* xs, float* const (&r_out)[R], float* d_out, double* Gpart, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -535,15 +536,14 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
     const uint32_t full_a = smem_u32(&h->full_f[0]), ring_a = smem_u32(ring);
     volatile uint32_t* next_blk = h->next_blk;
     const unsigned int it0 = pipe.it_f;        // blocks are numbered over the CTA's life: this pass has it0 .. it0 + nb - 1
-    const int team = warp / TEAM, tw = warp % TEAM;
-    if (warp < W_CONS && lane == 0) next_blk[warp] = it0 + (unsigned int)team;
+    if (warp < W_CONS && lane == 0) next_blk[warp] = it0 + (unsigned int)warp;
     __syncthreads();
 
     // The ring: records keep their own size (128-byte multiples) and are laid end to end in a circular byte buffer;
     // a record that does not fit before the end starts over at 0.  Where each record goes, and how many of the CTA's
     // earlier blocks must have left the ring before its copy may be issued, depends only on the record sizes, so it is
     // computed once per partition (k_ring_layout) and travels with the block descriptors.  Block number `it` uses
-    // full barrier it % 64 in phase it / 64; a team's consecutive blocks are 4 apart, so the previous user of a
+    // full barrier it % 64 in phase it / 64; a warp's consecutive blocks are 16 apart, so the previous user of a
     // barrier is always a block the same warps have already finished.  Space is reclaimed in issue order: every
     // consumer warp publishes the number of the next block it will finish, and the minimum over the warps bounds
     // the blocks that are gone.
@@ -579,34 +579,33 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
             }
         }
     } else {
-        // ---------------- consumer warps: team t (4 warps) takes the CTA's blocks t, t + 4, ...; inside a record the
-        // team's warps split the quads / row batches
+        // ---------------- consumer warps: warp w takes the CTA's blocks w, w + 16, ...
         float* dsc = reinterpret_cast<float*>(smem + P.dsc_off) + warp * 32 * R_MAX;
         const unsigned char* xs_b = reinterpret_cast<const unsigned char*>(xs);
         float* my_r = r_out[0];
 #pragma unroll
         for (int r = 1; r < R; ++r) my_r = quad_trial<R>(lane) == r ? r_out[r] : my_r;
         const VoxelLimits vl = {P.st->tvu, P.st->tvo};
-        int at_next = (team < nb) ? __ldg(&P.blk[b0 + team].z) : 0;
-        for (int i = team; i < nb; i += N_TEAMS) {
+        int at_next = (warp < nb) ? __ldg(&P.blk[b0 + warp].z) : 0;
+        for (int i = warp; i < nb; i += W_CONS) {
             const int at = at_next;
-            if (i + N_TEAMS < nb) at_next = __ldg(&P.blk[b0 + i + N_TEAMS].z);
+            if (i + W_CONS < nb) at_next = __ldg(&P.blk[b0 + i + W_CONS].z);
             const unsigned int it = it0 + (unsigned int)i;
             mbar_wait_a(full_a + 8u * (it & (RING_ENTRIES - 1)), (it / RING_ENTRIES) & 1u);
-#ifndef IMRT_EXP_SKIP_COMPUTE
             const unsigned char* rec = ring + at;
-            if (COL16 && reinterpret_cast<const uint32_t*>(rec)[2] != 0u)      // header word 2: record format
-                dose_block_quads<R>(rec, xs_b, table_s, my_r, d_out, vl, tw, lane, Gq);
+            if (STREAM) {
+                // nothing: the record is only waited for
+            } else if (COL16 && reinterpret_cast<const uint32_t*>(rec)[2] != 0u)      // header word 2: record format
+                dose_block_quads<R>(rec, xs_b, table_s, my_r, d_out, vl, lane, Gq);
             else
-                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, vl, tw, lane, Gacc);
-#endif
+                dose_block<COL16, R>(rec, xs_b, table_s, dsc, r_out, d_out, vl, lane, Gacc);
             __syncwarp();
             if (lane == 0) {
                 __threadfence_block();
-                next_blk[warp] = it + (unsigned int)N_TEAMS;
+                next_blk[warp] = it + (unsigned int)W_CONS;
             }
         }
-        if (lane == 0) next_blk[warp] = it0 + (unsigned int)nb + (unsigned int)N_TEAMS;   // nothing left: never the minimum
+        if (lane == 0) next_blk[warp] = it0 + (unsigned int)nb + (unsigned int)W_CONS;   // nothing left: never the minimum
     }
     pipe.it_f += (unsigned int)nb;
     // the two kinds of partials are summed separately (each in an order that does not depend on R) and then added
@@ -626,11 +625,11 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
     __syncthreads();
 }
 
-template <int R>
+template <int R, bool STREAM = false>
 __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, const float4* table_s,
                                           const float* xs, float* const (&r_out)[R], float* d_out, double* Gpart, Pipe& pipe) {
-    if (P.col16) dose_pass_t<true, R>(P, h, smem, table_s, xs, r_out, d_out, Gpart, pipe);
-    else dose_pass_t<false, R>(P, h, smem, table_s, xs, r_out, d_out, Gpart, pipe);
+    if (P.col16) dose_pass_t<true, R, STREAM>(P, h, smem, table_s, xs, r_out, d_out, Gpart, pipe);
+    else dose_pass_t<false, R, STREAM>(P, h, smem, table_s, xs, r_out, d_out, Gpart, pipe);
 }
 
 // Objectives of a finished dose pass: fixed-order sums of the CTA partials + the constant of the skipped rows.
@@ -644,18 +643,139 @@ __device__ __forceinline__ void reduce_objective(const DevPlan& P, const double*
         for (int r = 0; r < R; ++r) G[r] += __ldcg(Gpart + c * R + r);
     }
     block_sum_vec<R>(G, h);
-#pragma unroll
     const double G_skip = P.st->G_skip;
 #pragma unroll
     for (int r = 0; r < R; ++r) G[r] += G_skip;
 }
 
 // ------------------------------------------------------------------------------------------------ transpose pass
-// Streams equal-nnz ranges of D^T; every consumer warp owns a contiguous slice of each stage, gathers r, and keeps
-// an fp64 running sum per row of D^T; per (warp,row) sums meet in shared memory and leave as one fp64 partial
-// per (range,row) slot.  All NTHREADS threads call this.  Ends with a CTA-wide barrier.
+// g = D^T r (PAPER.md:107 step 1, :128 kernel 3) on the explicit transpose.  One contiguous share of the D^T stream per
+// CTA, cut into ranges of at most RL_MAX rows; a producer warp streams fixed-size stages with bulk copies, the consumer
+// warps gather r, multiply-add in fp32 over short slices and keep fp64 running sums per row; per-(warp, row) sums meet
+// in shared memory and leave as one fp64 partial per (range, row) slot.  All NTHREADS threads call a pass; it ends with
+// a CTA-wide barrier.  Every consumer warp observes EVERY stage's full barrier and arrives on its empty barrier
+// (count W_CONS), so the producer can never refill a slot before all warps have seen its phase.
+
+// ---- plain 32-bit CSR stream (DevPlan::id16 == 0; rows are not padded, a slice may span several rows): the consumer
+// warps take the stages in two alternating groups of 8, each warp a contiguous 512-entry slice.
+__device__ __forceinline__ void transpose_pass_csr(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
+                                                   const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int S = P.n_stages_t;
+    unsigned char* stages = smem + P.stage_off;
+    unsigned int it = pipe.it_t;
+    const int rg0 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x] : 0;       // this CTA's ranges
+    const int rg1 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x + 1] : 0;
+    const unsigned long long t_start = global_ns();
+    int s = (int)(it % (unsigned int)S);
+    unsigned int ph = (it / (unsigned int)S) & 1u;
+
+    if (warp >= W_CONS) {
+        const uint64_t pol = policy_evict_first();
+        for (int rg = rg0; rg < rg1; ++rg) {
+            const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
+            for (int cs = e0; cs < e1; cs += CHUNK_T, ++it) {
+                if (warp == W_CONS && lane == 0) {
+                    mbar_wait(&h->empty_t[s], ph ^ 1u);
+                    int n = e1 - cs;
+                    n = n > CHUNK_T ? CHUNK_T : n;
+                    unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
+                    const int shift = e0 & 3;   // 16-byte source alignment: start the copy up to 3 entries early
+                    const uint32_t bytes = (uint32_t)((n + shift + 3) & ~3) * 4u;   // D^T is padded: always in bounds
+                    int* col_s = reinterpret_cast<int*>(st);
+                    float* val_s = reinterpret_cast<float*>(col_s + CHUNK_T_PAD);
+                    mbar_expect_tx(&h->full_t[s], 2u * bytes);
+                    bulk_g2s(col_s, P.colT + (cs - shift), bytes, &h->full_t[s], pol);
+                    bulk_g2s(val_s, P.valT + (cs - shift), bytes, &h->full_t[s], pol);
+                }
+                if (++s == S) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else {
+        const uint64_t keep = policy_evict_last();
+        for (int rg = rg0; rg < rg1; ++rg) {
+            const TrRange R = P.tr_range[rg];
+            for (int i = threadIdx.x; i < RL_MAX * W_CONS; i += N_CONS) wpart[i] = 0.0;
+            named_bar_sync(1, N_CONS);
+            int cur_row = R.first_row;
+            int cur_end = __ldg(P.rowT_ptr + cur_row + 1);
+            double dacc = 0.0;
+            bool touched = false;
+            for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
+                mbar_wait(&h->full_t[s], ph);
+                if ((int)(it % TGROUPS) == warp / (W_CONS / TGROUPS)) {      // this group's stage
+                    const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
+                    const int* col_s = reinterpret_cast<const int*>(st) + (R.e_begin & 3);
+                    const float* val_s = reinterpret_cast<const float*>(st) + CHUNK_T_PAD + (R.e_begin & 3);
+                    const int ce = min(cs + CHUNK_T, R.e_end);
+                    int pos = cs + (warp % (W_CONS / TGROUPS)) * SLICE_T;
+                    const int b = min(pos + SLICE_T, ce);
+                    while (pos < b) {
+                        while (cur_end <= pos) {   // the slice moved past the end of the current row (warp-uniform)
+                            if (touched) {
+                                const double sum = warp_sum(dacc);
+                                if (lane == 0) wpart[(cur_row - R.first_row) * W_CONS + warp] = sum;
+                                dacc = 0.0;
+                                touched = false;
+                            }
+                            ++cur_row;
+                            cur_end = __ldg(P.rowT_ptr + cur_row + 1);
+                        }
+                        const int seg_end = min(b, cur_end);
+                        const int* cp = col_s + (pos - cs);
+                        const float* vp = val_s + (pos - cs);
+                        float acc = 0.0f;
+                        if (seg_end - pos == SLICE_T) {
+                            int c[SLICE_T / 32];
+                            float rr[SLICE_T / 32];
+#pragma unroll
+                            for (int u = 0; u < SLICE_T / 32; ++u) c[u] = cp[lane + 32 * u];
+#pragma unroll
+                            for (int u = 0; u < SLICE_T / 32; ++u) rr[u] = ld_keep(r_in + c[u], keep);
+#pragma unroll
+                            for (int u = 0; u < SLICE_T / 32; ++u) acc = fmaf(vp[lane + 32 * u], rr[u], acc);
+                        } else {
+                            for (int k = lane; k < seg_end - pos; k += 32) acc = fmaf(vp[k], ld_keep(r_in + cp[k], keep), acc);
+                        }
+                        dacc += (double)acc;
+                        touched = true;
+                        pos = seg_end;
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&h->empty_t[s]);    // consumed or only observed: either way this warp is done with it
+                if (++s == S) { s = 0; ph ^= 1u; }
+            }
+            if (touched) {
+                const double sum = warp_sum(dacc);
+                if (lane == 0) wpart[(cur_row - R.first_row) * W_CONS + warp] = sum;
+            }
+            named_bar_sync(1, N_CONS);
+            for (int t = threadIdx.x; t < R.n_rows; t += N_CONS) {
+                double sum = 0.0;
+#pragma unroll
+                for (int w = 0; w < W_CONS; ++w) sum += wpart[t * W_CONS + w];
+                gslot[R.slot_base + t] = sum;
+            }
+            named_bar_sync(1, N_CONS);
+        }
+    }
+    pipe.it_t = it;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
+        P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
+    }
+}
+
+// ---- packed streams: voxel ids as 16-bit offsets from one 32-bit base per aligned group of 32 entries, rows padded to 128
+// entries, 4,096-entry stages taken by the consumer warps in two alternating groups of 8 (a contiguous 512-entry slice and
+// 16 gathers of r in flight per lane).  A software-pipelined variant (every warp a 128-entry slice of every stage, values
+// parked in registers, multiply-adds four stages later) measured no faster in isolation and slower inside the persistent
+// kernel (register pressure): the pass is bound by L2 throughput -- the stream plus the r gathers -- not by latency.
 template <bool ID16>
-__device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
+__device__ __forceinline__ void transpose_pass_rows(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
                                                const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = P.n_stages_t;
@@ -713,10 +833,11 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
             double dacc = 0.0;
             bool touched = false;
             for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
-                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage: not consumed here,
-                    mbar_wait(&h->full_t[s], ph);      // but its phase must be seen to complete -- a warp that skipped it
-                    if (++s == S) { s = 0; ph ^= 1u; } // could otherwise mistake the slot's NEXT phase for complete
-                    continue;                          // (phase parity; matters when the stage count is odd)
+                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage: not consumed here, but
+                    mbar_wait(&h->full_t[s], ph);      // its phase must be OBSERVED and the observation reported: the empty
+                    if (lane == 0) mbar_arrive(&h->empty_t[s]);   // barrier counts all W_CONS warps, so the producer cannot
+                    if (++s == S) { s = 0; ph ^= 1u; } // refill a slot before every warp has seen its phase complete
+                    continue;
                 }
                 mbar_wait(&h->full_t[s], ph);
                 const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
@@ -752,11 +873,7 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
                             unsigned int c[SLICE_T / 32];
                             float rr[SLICE_T / 32];
 #pragma unroll
-#ifdef IMRT_EXP_NOGATHER
-                            for (int u = 0; u < SLICE_T / 32; ++u) c[u] = (bp[u] + ip[lane + 32 * u]) & 1023u;
-#else
                             for (int u = 0; u < SLICE_T / 32; ++u) c[u] = bp[u] + ip[lane + 32 * u];
-#endif
 #pragma unroll
                             for (int u = 0; u < SLICE_T / 32; ++u) rr[u] = ld_keep(r_in + c[u], keep);
 #pragma unroll
@@ -809,6 +926,7 @@ __device__ __forceinline__ void transpose_pass_t(const DevPlan& P, SmemHeader* h
 
 // The same pass over the ROW-PAIR stream (DevPlan::id16 == 2): an entry is one voxel of the union of two rows with a
 // float2 of values, so one gather of r feeds two multiply-adds and every sum, partial and slot comes in twos.
+template <bool STREAM = false>
 __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
                                                      const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -850,10 +968,11 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
             double dacc0 = 0.0, dacc1 = 0.0;
             bool touched = false;
             for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
-                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage: not consumed here,
-                    mbar_wait(&h->full_t[s], ph);      // but its phase must be seen to complete -- a warp that skipped it
-                    if (++s == S) { s = 0; ph ^= 1u; } // could otherwise mistake the slot's NEXT phase for complete
-                    continue;                          // (phase parity; matters when the stage count is odd)
+                if ((int)(it % TGROUPS) != warp / (W_CONS / TGROUPS)) {      // another group's stage: not consumed here, but
+                    mbar_wait(&h->full_t[s], ph);      // its phase must be OBSERVED and the observation reported: the empty
+                    if (lane == 0) mbar_arrive(&h->empty_t[s]);   // barrier counts all W_CONS warps, so the producer cannot
+                    if (++s == S) { s = 0; ph ^= 1u; } // refill a slot before every warp has seen its phase complete
+                    continue;
                 }
                 mbar_wait(&h->full_t[s], ph);
                 const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
@@ -863,7 +982,7 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
                 const int ce = min(cs + CHUNK_T, R.e_end);
                 int pos = cs + (warp % (W_CONS / TGROUPS)) * SLICE_T;
                 const int b = min(pos + SLICE_T, ce);
-                while (pos < b) {
+                while (!STREAM && pos < b) {
                     while (cur_end <= pos) {   // the slice moved past the end of the current row pair (warp-uniform)
                         if (touched) {
                             const double s0 = warp_sum(dacc0), s1 = warp_sum(dacc1);
@@ -941,9 +1060,9 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
 
 __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
                                                const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
-    if (P.id16 == 2) transpose_pass_pairs(P, h, smem, wpart, r_in, gslot, pipe);
-    else if (P.id16) transpose_pass_t<true>(P, h, smem, wpart, r_in, gslot, pipe);
-    else transpose_pass_t<false>(P, h, smem, wpart, r_in, gslot, pipe);
+    if (P.id16 == 2) transpose_pass_pairs<false>(P, h, smem, wpart, r_in, gslot, pipe);
+    else if (P.id16) transpose_pass_rows<true>(P, h, smem, wpart, r_in, gslot, pipe);
+    else transpose_pass_csr(P, h, smem, wpart, r_in, gslot, pipe);
 }
 
 // g_i = sum of the slots of row i, in slot order (fixed).  All NTHREADS threads; g_out shared or global.
@@ -1204,6 +1323,33 @@ __device__ __forceinline__ void dose_timing(const DevPlan& P, SmemHeader* h, con
     dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[(int)(st->fwd_passes & 1)], pipe);
 }
 
+// imrt_plan_eval_batch: the loop's R-point dose pass on R GIVEN points (A.x_in, [R][n_b]); residuals to A.r_out
+// ([R][n_v]) or to the trial buffers; objectives to State::eval_objs.  No decision, no state change.
+template <int R>
+__device__ __forceinline__ void dose_batch(const DevPlan& P, const PassArgs& A, SmemHeader* h, const float4* table_s, float* xs) {
+    State* st = P.st;
+    const int ri = st->ri;
+    for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) xs[(size_t)i * R + r] = A.x_in[(size_t)r * P.n_b + i];
+    }
+    __syncthreads();
+    float* r_out[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) r_out[j] = A.r_out ? A.r_out + (size_t)j * P.n_v : P.rbuf[(ri + 1 + j) % (P.R + 1)];
+    Pipe pipe = {0u, 0u};
+    const int par = (int)(st->fwd_passes & 1);
+    dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[par], pipe);
+    __threadfence();
+    if (!cta_is_last(&st->ticket_f, h)) return;
+    double G[R];
+    reduce_objective<R>(P, P.Gpart[par], h, G);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) st->eval_objs[r] = G[r];
+    }
+}
+
 // Dose pass as a kernel of its own (graph / host drivers, set_x, eval, get_dose).
 __global__ void __launch_bounds__(NTHREADS, 1) k_dose(const __grid_constant__ DevPlan P, const PassArgs A) {
     SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
@@ -1214,10 +1360,30 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dose(const __grid_constant__ De
         if (P.R == 4) dose_timing<4>(P, h, table_s, xs);
         else if (P.R == 2) dose_timing<2>(P, h, table_s, xs);
         else dose_timing<1>(P, h, table_s, xs);
+    } else if (A.mode == MODE_BATCH) {
+        if (A.n_points == 4) dose_batch<4>(P, A, h, table_s, xs);
+        else if (A.n_points == 2) dose_batch<2>(P, A, h, table_s, xs);
+        else dose_batch<1>(P, A, h, table_s, xs);
     } else if (A.mode != MODE_TRIAL) dose_single(P, A, h, table_s, xs);
     else if (P.R == 4) dose_trials<4>(P, A, h, table_s, xs);
     else if (P.R == 2) dose_trials<2>(P, A, h, table_s, xs);
     else dose_trials<1>(P, A, h, table_s, xs);
+}
+
+// The streaming ceilings of the two passes (imrt_plan_launch_pass kinds 2 and 3): every byte a pass reads travels
+// through the same ring / stages, nobody computes.  kind 0: the dose pass's records; 1: the row-pair D^T stream.
+__global__ void __launch_bounds__(NTHREADS, 1) k_stream(const __grid_constant__ DevPlan P, int kind) {
+    SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
+    float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
+    float* xs = reinterpret_cast<float*>(imrt_smem + P.x_off);
+    cta_init(h, P, table_s);
+    Pipe pipe = {0u, 0u};
+    if (kind == 0) {
+        float* r_out[1] = {nullptr};
+        dose_pass<1, true>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[0], pipe);
+    } else if (P.id16 == 2) {
+        transpose_pass_pairs<true>(P, h, imrt_smem, reinterpret_cast<double*>(imrt_smem + P.wpart_off), P.rbuf[0], P.gslot[0], pipe);
+    }
 }
 
 // Transpose pass as a kernel of its own.
@@ -1266,6 +1432,7 @@ __global__ void k_begin(State* st, int use_handles, cudaGraphConditionalHandle h
 // Plain launch before a run: how far to go and with which tolerance.
 __global__ void k_set_target(State* st, int n_more, double delta_tol) {
     int target = st->iter + n_more;
+    st->clamped = target > st->trace_cap;
     if (target > st->trace_cap) target = st->trace_cap;
     st->iter_target = target;
     st->delta_tol = delta_tol;

@@ -236,6 +236,26 @@ def make_random(seed: int, n_v: int, n_b: int, density: float = 0.3, n_structure
     return prob
 
 
+def mixed_resolution_groups(prob: Problem, body_sid: int = 3):
+    """Group id per row for the paper's mixed-resolution problem: every target / OAR voxel is a group of
+    its own (ids 0 .. n_fine-1, in row order), the body voxels of one 2x2x2 block share a group (ids n_fine ..., in
+    ascending block key).  Returns (group int32 [n_v], n_groups, structure id per group uint8 [n_groups]).  Index
+    arithmetic only: the merging itself is imrt_merge_rows (library) / oracle.merge_rows (oracle)."""
+    nx, ny, nz = prob.meta["grid"]
+    vid = prob.voxel_ids
+    ix, iy, iz = vid % nx, (vid // nx) % ny, vid // (nx * ny)
+    body = prob.sid == body_sid
+    key = (ix // 2) + ((nx + 1) // 2) * ((iy // 2) + ((ny + 1) // 2) * (iz // 2))
+    n_fine = int((~body).sum())
+    uniq, inv = np.unique(key[body], return_inverse=True)
+    group = np.empty(prob.n_v, np.int32)
+    group[~body] = np.arange(n_fine, dtype=np.int32)
+    group[body] = n_fine + inv.astype(np.int32)
+    n_groups = n_fine + int(uniq.shape[0])
+    sid_g = np.concatenate([prob.sid[~body], np.full(uniq.shape[0], body_sid, np.uint8)])
+    return group, n_groups, sid_g
+
+
 def mixed_resolution(prob: Problem, body_sid: int = 3) -> Problem:
     """The paper's mixed-resolution problem: voxels of unspecified tissue (structure `body_sid`) are
     doubled in each dimension, targets and OARs keep the full resolution.  A coarse voxel's row of D is the mean of

@@ -74,7 +74,7 @@ def test_null_and_undersized_arguments_are_refused_with_a_message():
     L = imrt.lib()
     out = ctypes.c_void_p()
     prm = imrt.Params(0.2, 2.0, 1e-3, 30, 10, imrt.DRIVER_PERSISTENT, 0)
-    s = L.imrt_plan_create(ctypes.byref(out), 10, 2, 5, None, None, None, None, 1, None, None, None, None, ctypes.byref(prm), None, 0, None)
+    s = L.imrt_plan_create(ctypes.byref(out), 10, 2, 5, None, None, None, None, 1, None, None, None, None, ctypes.byref(prm), None, None, 0, None)
     assert imrt.STATUS_NAMES[s] == "INVALID_ARG" and b"null" in L.imrt_last_error(None) and out.value is None
     assert imrt.STATUS_NAMES[L.imrt_plan_run_iters(None, 3)] == "INVALID_ARG"
     assert imrt.STATUS_NAMES[L.imrt_plan_destroy(None)] == "INVALID_ARG"
@@ -83,7 +83,7 @@ def test_null_and_undersized_arguments_are_refused_with_a_message():
     rp, ci, v, sid = np.array([0, 1, 2], np.int32), np.zeros(2, np.int32), np.ones(2, np.float32), np.zeros(2, np.uint8)
     t, ws = np.ones(1, np.float32), np.zeros(1 << 16, np.uint8)
     s = L.imrt_plan_create(ctypes.byref(out), 2, 1, 2, hp(rp), hp(ci), hp(v), hp(sid), 1, hp(t), hp(t), hp(t), hp(t), ctypes.byref(prm),
-                           hp(ws), ws.nbytes, None)
+                           None, hp(ws), ws.nbytes, None)
     assert imrt.STATUS_NAMES[s] == "WORKSPACE_TOO_SMALL" and b"needed" in L.imrt_last_error(None)
 
 
@@ -99,7 +99,7 @@ def test_no_device_is_an_error_not_a_fallback():
     t = np.ones(1, np.float32)
     ws = np.zeros(imrt.imrt_workspace_bytes(2, 1, 2, 1, 10), np.uint8)
     s = L.imrt_plan_create(ctypes.byref(out), 2, 1, 2, hp(rp), hp(ci), hp(v), hp(sid), 1, hp(t), hp(t), hp(t), hp(t), ctypes.byref(prm),
-                           hp(ws), ws.nbytes, None)
+                           None, hp(ws), ws.nbytes, None)
     assert imrt.STATUS_NAMES[s] in ("CUDA_ERROR", "UNSUPPORTED_DEVICE") and out.value is None
     assert L.imrt_last_error(None)
 

@@ -52,12 +52,43 @@ def check_eval(m, plan, prob, x):
     x64 = np.asarray(x, np.float32).astype(np.float64)
     d_o, r_o, G_o = oracle.eval_objective(prob, x64)
     g_o = oracle.gradient(prob, r_o)
-    assert relerr(d.cpu().numpy(), d_o) <= TOL_KERNEL
+    dn = d.cpu().numpy().astype(np.float64)
+    assert relerr(dn, d_o) <= TOL_KERNEL
+    # d is a one-signed sum: also element by element, relative to the element itself (floor: 1e-3 of the largest dose), so
+    # that a wrong short row at a field edge cannot hide behind the 70 Gy core
+    floor = 1e-3 * np.abs(d_o).max() if d_o.size else 0.0
+    assert (np.abs(dn - d_o) <= TOL_KERNEL * np.maximum(np.abs(d_o), floor)).all(), \
+        "dose row %d off by %.3e" % (int(np.argmax(np.abs(dn - d_o) / np.maximum(np.abs(d_o), floor + 1e-300))), np.abs(dn - d_o).max())
     assert relerr(r.cpu().numpy(), r_o) <= TOL_KERNEL
     assert relerr(g.cpu().numpy(), g_o) <= TOL_KERNEL
     assert abs(G - G_o) <= TOL_KERNEL * abs(G_o) + 1e-300
-    # the transpose kernel alone: feed it the ORACLE's residual (rounded to fp32) instead of the GPU's
+    # the transpose kernel ALONE (a4 isolated from a2 / a3): it is fed the ORACLE's residual, rounded to fp32, and compared
+    # with the oracle's gradient of that same rounded residual -- a compensating error in the penalty and the transpose
+    # pass cannot pass this
+    r32 = r_o.astype(np.float32)
+    g_alone = plan.gradient(r32).cpu().numpy()
+    assert relerr(g_alone, oracle.gradient(prob, r32.astype(np.float64))) <= TOL_KERNEL
     return d, r, g, G
+
+
+def check_eval_batch(m, plan, prob, xs):
+    """The line search's batched pass (the R = len(xs) kernels bench.py times) on given points: every residual vector
+    and every objective against the oracle."""
+    xs = np.ascontiguousarray(xs, np.float32)
+    r, G = plan.eval_batch(xs)
+    r = r.cpu().numpy()
+    for j in range(xs.shape[0]):
+        d_o, r_o, G_o = oracle.eval_objective(prob, xs[j].astype(np.float64))
+        assert relerr(r[j], r_o) <= TOL_KERNEL, j
+        assert abs(G[j] - G_o) <= TOL_KERNEL * abs(G_o) + 1e-300, j
+
+
+def trial_points(prob, x, n):
+    """The first n trial points of the line search at x, computed by the oracle."""
+    x64 = np.asarray(x, np.float32).astype(np.float64)
+    _, r_o, _ = oracle.eval_objective(prob, x64)
+    g_o = oracle.gradient(prob, r_o)
+    return np.stack([oracle.trial_point(x64, g_o, prob.lambda0 / prob.alpha ** j)[0] for j in range(n)]).astype(np.float32)
 
 
 # ---------------------------------------------------------------------------------------------- D^T construction
@@ -87,6 +118,28 @@ def test_eval_parity_phantoms(m, cfg):
     for n in (1, 10):
         xo = oracle.run(prob, n_iters=n).x.astype(np.float32)
         check_eval(m, plan, prob, xo)
+    # the batched pass: the four trial points of the first line search, then two
+    check_eval_batch(m, plan, prob, trial_points(prob, prob.x0, 4))
+    check_eval_batch(m, plan, prob, trial_points(prob, xo, 2))
+    plan.close()
+
+
+def test_penalty_alone_on_identity_matrix(m):
+    # a3 isolated from a2: with D = I the dose IS x (exactly, in fp32), so r and G test Eq. (1) / its gradient factor alone
+    n = 5003
+    rng = np.random.default_rng(3)
+    base = synth_inputs.make_random(1, n_v=50, n_b=8)
+    sid = rng.integers(0, 3, n).astype(np.uint8)
+    prob = synth_inputs.Problem("ident-n", n, n, np.arange(n + 1, dtype=np.int32), np.arange(n, dtype=np.int32), np.ones(n, np.float32),
+                                sid, base.t_under, base.t_over, base.w_under, base.w_over, np.ones(n, np.float32))
+    plan = m.Plan(prob, max_iters=2)
+    x = rng.uniform(0, 90, n).astype(np.float32)
+    d, r, g, G = plan.eval(x)
+    np.testing.assert_array_equal(d.cpu().numpy(), x)
+    d_o, r_o, G_o = oracle.eval_objective(prob, x.astype(np.float64))
+    assert np.abs(r.cpu().numpy() - r_o).max() <= 1e-6 * np.abs(r_o).max()      # one fp32 rounding or two per element
+    assert abs(G - G_o) <= 1e-6 * G_o                                           # fp64 accumulation of fp32 u, o
+    check_eval_batch(m, plan, prob, np.stack([x, 0.5 * x, 2 * x, np.zeros_like(x)]))
     plan.close()
 
 
@@ -128,8 +181,8 @@ def test_eval_all_rows_empty_and_leading_trailing_empty(m):
 
 
 # ---------------------------------------------------------------------------------------------- the loop
-def run_gpu(m, prob, n_iters, driver, delta=0.0, ls_batch=0):
-    plan = m.Plan(prob, max_iters=max(n_iters, 1), driver=driver, ls_batch=ls_batch)
+def run_gpu(m, prob, n_iters, driver, delta=0.0, ls_batch=0, **options):
+    plan = m.Plan(prob, max_iters=max(n_iters, 1), driver=driver, ls_batch=ls_batch, **options)
     plan.set_x(prob.x0)
     if delta > 0:
         plan.run_to_tol(delta, n_iters)
@@ -142,8 +195,8 @@ def run_gpu(m, prob, n_iters, driver, delta=0.0, ls_batch=0):
     return plan, tr, x, d, cnt
 
 
-def test_three_drivers_are_bit_identical(m, monkeypatch):
-    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")     # plans are compared with each other: they must share one partition
+def test_three_drivers_are_bit_identical(m):
+    # plans are compared with each other: tune_level 0 (the default) gives every plan of a problem the same partition
     prob = phantom(0)
     res = [run_gpu(m, prob, 25, drv) for drv in (m.DRIVER_HOST, m.DRIVER_GRAPH, m.DRIVER_PERSISTENT)]
     _, tr0, x0, d0, c0 = res[0]
@@ -162,10 +215,9 @@ def test_three_drivers_are_bit_identical(m, monkeypatch):
 
 
 @pytest.mark.parametrize("cfg,n", [(0, 50), (2, 40)])
-def test_batched_line_search_is_bit_identical_to_sequential(m, cfg, n, monkeypatch):
+def test_batched_line_search_is_bit_identical_to_sequential(m, cfg, n):
     # Plans are compared with each other, so they must share one CTA partition: the measured rebalancing of plan
-    # creation (timing dependent; it changes the order in which objective partials are summed) is switched off.
-    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")
+    # creation (timing dependent; it changes the order in which objective partials are summed) stays off (tune_level 0).
     # imrt_params.ls_batch: 1 = one trial point per pass over D (steps 2-4 of PAPER.md:109-111 literally), 2 / 4 = the
     # next 2 / 4 trial points in one pass.  Same iterates, objectives, step sizes and trial counts, bit for bit.
     prob = phantom(cfg)
@@ -186,8 +238,7 @@ def test_batched_line_search_is_bit_identical_to_sequential(m, cfg, n, monkeypat
         r[0].close()
 
 
-def test_runs_are_reproducible_and_resumable(m, monkeypatch):
-    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")     # two plans are compared: they must share one partition
+def test_runs_are_reproducible_and_resumable(m):
     prob = phantom(0)
     p1, tr1, x1, _, _ = run_gpu(m, prob, 20, m.DRIVER_PERSISTENT)
     plan = m.Plan(prob, max_iters=20, driver=m.DRIVER_PERSISTENT)
@@ -197,20 +248,26 @@ def test_runs_are_reproducible_and_resumable(m, monkeypatch):
     tr2 = plan.trace()
     np.testing.assert_array_equal(tr2.obj, tr1.obj)
     np.testing.assert_array_equal(plan.get_x().cpu().numpy(), x1)
-    plan.run_iters(5)    # trace capacity reached: nothing more happens
-    assert plan.trace().n_iters == 20
+    plan.run_iters(5)    # trace capacity reached: nothing more happens, and the caller is told why
+    assert plan.trace().n_iters == 20 and m.STOP_NAMES[plan.trace().stop_reason] == "TRACE_FULL"
     p1.close()
     plan.close()
 
 
-@pytest.mark.parametrize("cfg,driver", [(0, 2), (0, 0), (1, 2)])
+@pytest.mark.parametrize("cfg,driver", [(0, 2), (0, 0), (1, 2), (2, 2), (2, 0)])
 def test_trajectory_parity_follow_mode(m, cfg, driver):
+    # Every config at ITS OWN run length (SURVEY.md 8(d) "Run lengths"): cfg0 50 and cfg1 200 fixed iterations; cfg2 under its
+    # rule "delta = 1e-6 or 500 iterations", compared at the GPU's own stopping count.  (cfg3 / cfg4: test_full_size_parity.)
     prob = phantom(cfg)
-    n = prob.n_iters
-    plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, n, driver)
-    assert tr.n_iters == n and tr.stop_reason == oracle.STOP_MAX_ITERS
+    plan, tr, x, d, (fwd, trp) = run_gpu(m, prob, prob.n_iters, driver, delta=prob.delta)
+    n = tr.n_iters
+    if prob.delta > 0:
+        print("cfg%d: GPU stopped after %d iterations (%s)" % (cfg, n, m.STOP_NAMES[tr.stop_reason]))
+        assert tr.stop_reason in (oracle.STOP_MAX_ITERS, oracle.STOP_TOLERANCE) and n > 100
+    else:
+        assert n == prob.n_iters and tr.stop_reason == oracle.STOP_MAX_ITERS
     R = plan.info()["ls_batch"]     # one dose pass evaluates up to R trial points
-    assert fwd == 1 + np.ceil(tr.n_trials / R).sum() and trp == n
+    assert fwd == 1 + np.ceil(tr.n_trials / R).sum()
     assert (np.diff(tr.obj) < 0).all() and (x >= 0).all()
     fol = oracle.run(prob, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert fol.n_follow_violations == 0, "GPU accepted/rejected a trial the oracle would not (first at iteration %d)" % fol.first_violation
@@ -235,14 +292,19 @@ def test_trajectory_parity_follow_mode(m, cfg, driver):
     plan.close()
 
 
-def test_run_to_tolerance_matches_oracle_stop(m):
-    prob = phantom(0)
-    plan, tr, x, d, _ = run_gpu(m, prob, 400, m.DRIVER_PERSISTENT, delta=1e-3)
-    ref = oracle.run(prob, n_iters=400, delta=1e-3)
-    assert tr.stop_reason == oracle.STOP_TOLERANCE
+@pytest.mark.parametrize("cfg,delta", [(0, 1e-3), (1, 1e-3), (2, 3e-3), (2, 1e-3)])
+def test_run_to_tolerance_matches_oracle_stop(m, cfg, delta):
+    # step 5 (reading R5): the TOLERANCE exit fires on both sides, at the same iteration (+-1: the two
+    # relative changes are compared with delta in different precisions)
+    prob = phantom(cfg)
+    plan, tr, x, d, _ = run_gpu(m, prob, 500, m.DRIVER_PERSISTENT, delta=delta)
+    ref = oracle.run(prob, n_iters=500, delta=delta)
+    assert tr.stop_reason == oracle.STOP_TOLERANCE and ref.stop_reason == oracle.STOP_TOLERANCE
     rel = np.abs(np.diff(tr.obj)) / tr.obj[1:]
-    assert rel[-1] < 1e-3 and (rel[:-1] >= 1e-3).all()
-    assert abs(tr.n_iters - ref.n_iters) <= 1
+    assert rel[-1] < delta and (rel[:-1] >= delta).all()
+    assert abs(tr.n_iters - ref.n_iters) <= 1, (tr.n_iters, ref.n_iters)
+    fol = oracle.run(prob, n_iters=tr.n_iters, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert fol.n_follow_violations == 0 and abs(tr.obj[-1] - fol.obj[-1]) <= TOL_G_FINAL * fol.obj[-1]
     plan.close()
 
 
@@ -309,20 +371,28 @@ def test_linesearch_stall_and_bad_inputs(m):
 # BASELINE.json configs[3] (headline) and configs[4] (stress), in the launch configuration bench.py times (persistent
 # driver, one CTA per SM, tuned partition).  The oracle's eval / gradient take well under a second per call even at
 # these sizes, so every output element is compared, not a sample.
-@pytest.mark.parametrize("cfg,n_iters", [(3, 30), (4, 10)])
-def test_full_size_parity(m, cfg, n_iters):
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_parity(m, cfg):
+    # the configs' own run lengths: cfg3 "delta = 1e-6 or 500 iterations", cfg4 300 fixed iterations -- the oracle replays
+    # the GPU's iteration count in follow mode (about 2 and 4 minutes of serial fp64 work)
     prob = phantom(cfg)
-    plan = m.Plan(prob, max_iters=n_iters, driver=m.DRIVER_PERSISTENT)
+    plan = m.Plan(prob, max_iters=prob.n_iters, driver=m.DRIVER_PERSISTENT, tune_level=2)     # as bench.py creates it
     info = plan.info()
     assert info["fwd_grid"] == info["n_sm"] and info["tr_grid"] == info["n_sm"]   # what bench.py launches
     check_eval(m, plan, prob, prob.x0)
     xo = oracle.run(prob, n_iters=3).x.astype(np.float32)
     check_eval(m, plan, prob, xo)
-    # trajectory: n_iters accepted iterations from x0, oracle in follow mode
+    check_eval_batch(m, plan, prob, trial_points(prob, xo, 4))     # the R = 4 pass bench.py times, on four trial points
+    # trajectory from x0 under the config's own rule, oracle in follow mode
     plan.set_x(prob.x0)
-    plan.run_iters(n_iters)
+    if prob.delta > 0:
+        plan.run_to_tol(prob.delta, prob.n_iters)
+    else:
+        plan.run_iters(prob.n_iters)
     tr = plan.trace()
-    assert tr.n_iters == n_iters and tr.stop_reason == oracle.STOP_MAX_ITERS
+    n_iters = tr.n_iters
+    print("cfg%d: GPU stopped after %d iterations (%s)" % (cfg, n_iters, m.STOP_NAMES[tr.stop_reason]))
+    assert tr.stop_reason in (oracle.STOP_MAX_ITERS, oracle.STOP_TOLERANCE) and n_iters >= min(300, prob.n_iters)
     assert (np.diff(tr.obj) < 0).all()
     fol = oracle.run(prob, n_iters=n_iters, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert fol.n_follow_violations == 0, "first violation at iteration %d" % fol.first_violation
@@ -336,8 +406,12 @@ def test_full_size_parity(m, cfg, n_iters):
     dp_o, mean_o = oracle.dvh_points(prob.sid, d_o, prob.n_structures)
     dp_g, mean_g = plan.dvh(oracle.DVH_PCTS)
     assert np.nanmax(np.abs(dp_g - dp_o)) <= TOL_DVH_GY and np.nanmax(np.abs(mean_g - mean_o)) <= TOL_DVH_GY
-    assert relerr(d, d_o) <= 5e-4   # dose of the two final plans (same trial counts, fp32 vs fp64 trajectories): a sanity
-                                    # bound only -- the north star's criteria are the objective and the DVH points above
+    # dose of the two final plans, voxel by voxel: the DVH tolerance (0.5 % of the prescription) applied to EVERY voxel.
+    # (The minimiser is not unique -- reading R14 -- so the fp32 and fp64 trajectories may drift apart along directions
+    # the objective does not see; DESIGN.md section 6 records the measured drift per iteration.)
+    print("cfg%d: dose drift after %d iterations: normwise %.2e, largest voxel %.4f Gy" % (cfg, n_iters, relerr(d, d_o), np.abs(d - d_o).max()))
+    assert np.abs(d - d_o).max() <= TOL_DVH_GY
+    assert relerr(d, d_o) <= 1e-4      # the bound of round 1's first version, at the full run length
     plan.close()
     _phantoms.pop(cfg, None)        # free ~1-3 GB of host memory
 
@@ -375,24 +449,24 @@ def test_per_voxel_limits_parity(m, cfg):
 
 
 # ---------------------------------------------------------------------------------------------- the fallback layouts
-@pytest.mark.parametrize("env", ["IMRTGP_NO_QUADS", "IMRTGP_COL32", "IMRTGP_NO_PAIRS", "IMRTGP_NO_ID16", "IMRTGP_NO_TUNE"])
-def test_fallback_layouts_parity(m, env, monkeypatch):
+@pytest.mark.parametrize("opt", [{"dose_format": 1}, {"col_bits": 32}, {"transpose_format": 1}, {"transpose_format": 2},
+                                 {"tune_level": 1}, {"tune_level": 2}, {"quad_cap": 64}, {"fused_gradient": 1}])
+def test_fallback_layouts_parity(m, opt):
     # the layouts a plan falls back to when the matrix does not suit the packed ones: row-format records everywhere,
     # 32-bit column indices (n_b > 65,536), single rows of D^T instead of row pairs, the 32-bit D^T stream (a group of 32
-    # entries wider than 65,535 voxels), and the modelled (unmeasured) partitions -- forced here through the library's
-    # environment switches
-    monkeypatch.setenv(env, "1")
+    # entries wider than 65,535 voxels); the measured partitions; small records; the loop without the fused gradient --
+    # forced here through imrt_options
     for prob in (phantom(0), phantom(1),
                  synth_inputs.make_random(21, n_v=4099, n_b=130, density=0.5, empty_row_frac=0.15, full_rows=2)):
-        plan = m.Plan(prob, max_iters=12)
+        plan = m.Plan(prob, max_iters=12, **opt)
         info = plan.info()
-        if env == "IMRTGP_NO_QUADS":
+        if opt.get("dose_format") == 1:
             assert info["quad_rows"] == 0
-        if env == "IMRTGP_COL32":
+        if opt.get("col_bits") == 32:
             assert info["col16"] == 0 and info["quad_rows"] == 0
-        if env == "IMRTGP_NO_PAIRS":
+        if opt.get("transpose_format") == 1:
             assert info["tr_format"] == 1
-        if env == "IMRTGP_NO_ID16":
+        if opt.get("transpose_format") == 2:
             assert info["tr_format"] == 0
         x = np.random.default_rng(5).uniform(0, 60, prob.n_b).astype(np.float32)
         check_eval(m, plan, prob, x)
@@ -407,10 +481,9 @@ def test_fallback_layouts_parity(m, env, monkeypatch):
 
 @pytest.mark.parametrize("seed,n_quads,n_b,tail", [(1, 1, 40, 0), (2, 2, 64, 1), (3, 3, 300, 2), (4, 257, 512, 3), (5, 4001, 900, 0),
                                                      (6, 1500, 2304, 1)])
-def test_quad_pairs_edge_cases(m, seed, n_quads, n_b, tail, monkeypatch):
+def test_quad_pairs_edge_cases(m, seed, n_quads, n_b, tail):
     # The dose pass takes the quads of a record two at a time (one per half-warp): single quads, odd counts, an
     # incomplete last group, empty groups between long ones, neighbours of very different length, rows without entries.
-    monkeypatch.setenv("IMRTGP_NO_TUNE", "1")
     prob = synth_inputs.make_quad_blocks(seed, n_quads, n_b, tail)
     x = np.random.default_rng(seed).uniform(0, 3, prob.n_b).astype(np.float32)
     ref = None
@@ -419,6 +492,7 @@ def test_quad_pairs_edge_cases(m, seed, n_quads, n_b, tail, monkeypatch):
         if n_quads >= 100:
             assert plan.info()["quad_rows"] > 0          # the case really exercises the quad records
         check_eval(m, plan, prob, x)
+        check_eval_batch(m, plan, prob, np.stack([x * f for f in (1.0, 0.5, 0.25, 0.0)][:R]))
         plan.set_x(prob.x0)
         plan.run_iters(8)
         tr = plan.trace()
@@ -467,9 +541,22 @@ def test_mixed_resolution_workflow(m):
     # "For unspecified tissue we increased the voxel size in each dimension by a factor of 2 ... The full resolution was
     # used when evaluating the treatment quality": optimise on the mixed-resolution matrix, evaluate dose and DVH with a
     # second plan on the full-resolution matrix.  (The row merging is input preparation: synth_inputs.mixed_resolution.)
+    import copy
+    import torch
     fine = phantom(1)
-    mixed = synth_inputs.mixed_resolution(fine)
-    assert mixed.n_v < fine.n_v // 4 and mixed.meta["fine_rows"] == int((fine.sid != 3).sum())
+    # the merge is a library call (imrt_merge_rows_count / _fill): bit-exact against the oracle's plain merge
+    group, n_groups, sid_g = synth_inputs.mixed_resolution_groups(fine)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    m_rp, m_col, m_val = m.imrt_merge_rows(fine.n_b, dev(fine.row_ptr), dev(fine.col), dev(fine.val), dev(group), n_groups)
+    o_rp, o_col, o_val = oracle.merge_rows(fine.n_b, fine.row_ptr, fine.col, fine.val, group, n_groups)
+    np.testing.assert_array_equal(m_rp.cpu().numpy(), o_rp)
+    np.testing.assert_array_equal(m_col.cpu().numpy(), o_col)
+    np.testing.assert_array_equal(m_val.cpu().numpy(), o_val)
+    mixed = copy.copy(fine)
+    mixed.name, mixed.n_v, mixed.sid, mixed.voxel_ids = fine.name + "-mixed", n_groups, sid_g, None
+    mixed.row_ptr, mixed.col, mixed.val = m_rp.cpu().numpy(), m_col.cpu().numpy(), m_val.cpu().numpy()
+    mixed.lambda0, _ = synth_inputs.pick_lambda0(mixed.row_ptr, mixed.col, mixed.val, mixed.sid, mixed.w_under, mixed.w_over)
+    assert mixed.n_v < fine.n_v // 4 and int((sid_g != 3).sum()) == int((fine.sid != 3).sum())
     n = 40
     plan = m.Plan(mixed, max_iters=n)
     check_eval(m, plan, mixed, mixed.x0)
@@ -522,3 +609,49 @@ def test_randomised_shapes_layouts_batches_and_drivers(m):
         tr = plan.trace()
         assert (np.diff(tr.obj) < 0).all() and (plan.get_x().cpu().numpy() >= 0).all(), prob.name
         plan.close()
+
+
+# ---------------------------------------------------------------------------------------------- tuning blobs, dense quads
+def test_tuned_partition_can_be_exported_and_reinjected(m):
+    # tune_level >= 1 balances the passes from measured times, so two tuned plans may differ in the last bits; a plan
+    # created from the first one's blob (imrt_plan_get_tuning -> imrt_options.host_tuning) reproduces it bit for bit
+    prob = phantom(2)
+    p1, tr1, x1, d1, _ = run_gpu(m, prob, 30, m.DRIVER_PERSISTENT, tune_level=2)
+    blob = p1.tuning()
+    p2 = m.Plan(prob, max_iters=30, tuning=blob)
+    p2.set_x(prob.x0)
+    p2.run_iters(30)
+    tr2 = p2.trace()
+    np.testing.assert_array_equal(tr2.obj, tr1.obj)
+    np.testing.assert_array_equal(p2.get_x().cpu().numpy(), x1)
+    with pytest.raises(m.ImrtError):
+        m.Plan(phantom(0), max_iters=4, tuning=blob)          # another problem's blob is refused
+    p1.close()
+    p2.close()
+
+
+def test_dense_quads_fall_back_to_row_records(m):
+    # 4 full rows of a wide matrix: one quad record would not fit in the ring twice, so those rows go to row-format records
+    prob = synth_inputs.make_random(31, n_v=64, n_b=8000, density=0.02, empty_row_frac=0.0, full_rows=4)
+    plan = m.Plan(prob, max_iters=4)
+    x = np.random.default_rng(1).uniform(0, 2, prob.n_b).astype(np.float32)
+    check_eval(m, plan, prob, x)
+    plan.close()
+
+
+@pytest.mark.parametrize("seed,n_v,n_b,n_groups", [(1, 300, 40, 37), (2, 5000, 700, 1200), (3, 64, 30000, 9), (4, 2000, 5, 2500)])
+def test_merge_rows_matches_oracle_bit_for_bit(m, seed, n_v, n_b, n_groups):
+    # rows scattered over the groups at random (not neighbours), groups without rows, empty rows, one very wide matrix
+    import torch
+    prob = synth_inputs.make_random(seed, n_v=n_v, n_b=n_b, density=0.1 if n_b < 1000 else 0.003, empty_row_frac=0.2, full_rows=1)
+    group = np.random.default_rng(seed).integers(0, n_groups, n_v).astype(np.int32)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    m_rp, m_col, m_val = m.imrt_merge_rows(n_b, dev(prob.row_ptr), dev(prob.col), dev(prob.val), dev(group), n_groups)
+    o_rp, o_col, o_val = oracle.merge_rows(n_b, prob.row_ptr, prob.col, prob.val, group, n_groups)
+    np.testing.assert_array_equal(m_rp.cpu().numpy(), o_rp)
+    np.testing.assert_array_equal(m_col.cpu().numpy(), o_col)
+    np.testing.assert_array_equal(m_val.cpu().numpy(), o_val)
+    bad = group.copy()
+    bad[0] = n_groups
+    with pytest.raises(m.ImrtError):
+        m.imrt_merge_rows(n_b, dev(prob.row_ptr), dev(prob.col), dev(prob.val), dev(bad), n_groups)

@@ -350,3 +350,22 @@ def test_mixed_resolution_rows_are_block_means(phantom0):
     assert mixed.n_v == n_fine + expect.shape[0] and mixed.n_b == phantom0.n_b
     np.testing.assert_allclose(d_mixed[n_fine:], expect, rtol=1e-5, atol=1e-7)     # fp32 rounding of the merged values
     assert (mixed.sid[n_fine:] == 3).all() and (mixed.sid[:n_fine] != 3).all()
+
+
+def test_merge_rows_hand_case_and_block_means(phantom0):
+    # oracle.merge_rows (reading R17) pinned by (i) a hand case, (ii) the independently built scipy block
+    # means of synth_inputs.mixed_resolution: same structure, values within one fp32 ulp (scipy adds in another order)
+    rp = np.array([0, 2, 3, 4, 4], np.int32)
+    col = np.array([0, 2, 0, 1], np.int32)
+    val = np.array([1.0, 3.0, 3.0, 5.0], np.float32)
+    group = np.array([0, 0, 2, 0], np.int32)             # rows 0, 1 and the empty row 3 -> group 0; group 1 has no rows
+    orp, oc, ov = oracle.merge_rows(3, rp, col, val, group, 3)
+    assert orp.tolist() == [0, 2, 2, 3] and oc.tolist() == [0, 2, 1]
+    np.testing.assert_array_equal(ov, np.array([4.0 / 3.0, 1.0, 5.0], np.float32))      # (1 + 3) / 3, 3 / 3, 5 / 1
+    group, n_groups, sid_g = synth_inputs.mixed_resolution_groups(phantom0)
+    orp, oc, ov = oracle.merge_rows(phantom0.n_b, phantom0.row_ptr, phantom0.col, phantom0.val, group, n_groups)
+    mixed = synth_inputs.mixed_resolution(phantom0)
+    np.testing.assert_array_equal(sid_g, mixed.sid)
+    np.testing.assert_array_equal(orp, mixed.row_ptr)
+    np.testing.assert_array_equal(oc, mixed.col)
+    assert (np.abs(ov - mixed.val) <= np.spacing(np.abs(mixed.val))).all()
