@@ -106,9 +106,7 @@ typedef struct imrt_options {
     int32_t transpose_format;  /* 0: smallest of {row pairs, single rows} with 16-bit voxel offsets, else plain CSR;
                                   1: single rows with 16-bit offsets (no pairs);  2: the plain 32-bit D^T CSR         */
     int32_t quad_cap;          /* union columns per quad record at most (0 = default, 576; clamped to [32, 4096])     */
-    int32_t fused_gradient;    /* the persistent loop (driver 2) forms g = D^T r INSIDE the dose pass for the trial
-                                  point most likely to be accepted:  0 = default (on when the
-                                  accumulators fit in shared memory), 1 = off (a transpose pass per iteration)         */
+    int32_t reserved1;
     int32_t profile_create;    /* 1: synchronise after every phase of plan creation and keep the phase times for
                                   imrt_plan_get_create_times                                                           */
     int32_t reserved0;

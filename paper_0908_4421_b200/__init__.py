@@ -50,7 +50,7 @@ class Params(ctypes.Structure):
 class Options(ctypes.Structure):
     """imrt_options: layout / tuning switches of imrt_plan_create (all 0 = defaults)."""
     _fields_ = [("tune_level", ctypes.c_int32), ("dose_format", ctypes.c_int32), ("col_bits", ctypes.c_int32),
-                ("transpose_format", ctypes.c_int32), ("quad_cap", ctypes.c_int32), ("fused_gradient", ctypes.c_int32),
+                ("transpose_format", ctypes.c_int32), ("quad_cap", ctypes.c_int32), ("reserved1", ctypes.c_int32),
                 ("profile_create", ctypes.c_int32), ("reserved0", ctypes.c_int32),
                 ("host_tuning", ctypes.c_void_p), ("host_tuning_bytes", ctypes.c_size_t)]
 
@@ -344,8 +344,7 @@ class Plan:
 
     def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None,
                  ls_batch: int = 0, tuning: bytes = None, **options):
-        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, fused_gradient,
-        profile_create); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
+        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, profile_create); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_0908_4421_b200 needs a CUDA device (sm_100a); there is no CPU path")

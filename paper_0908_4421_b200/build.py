@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libimrtgp.so")
 SOURCES = ["imrtgp.cu"]
-HEADERS = ["kernels.cuh", "pipeline.cuh", "dvh.cuh", "merge.cuh", os.path.join("..", "..", "include", "imrtgp.h")]
+HEADERS = ["kernels.cuh", "pipeline.cuh", "dvh.cuh", "merge.cuh", "layout.cuh", os.path.join("..", "..", "include", "imrtgp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC", "-cudart", "static"]
 

@@ -19,6 +19,7 @@
 
 #include "dvh.cuh"
 #include "kernels.cuh"
+#include "layout.cuh"
 #include "merge.cuh"
 
 using namespace imrt;
@@ -158,6 +159,9 @@ struct Layout {
     // build scratch
     int* quadU;
     unsigned char* covered;
+    LayoutTotals* totals;
+    int *seg_rec, *seg_meta, *seg_b128;
+    long long *cost_fx, *cost_pre;
     unsigned int* keysA;
     unsigned int* keysB;
     unsigned int* valsA;
@@ -210,6 +214,12 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.dvh.query = w.take<DvhQuery>((size_t)MAX_STRUCTURES * DVH_MAX_PCTS);
     L.quadU = w.take<int>(n_v / 4 + 2);
     L.covered = w.take<unsigned char>(n_v + 4);
+    L.totals = w.take<LayoutTotals>(1);
+    L.seg_rec = w.take<int>(n_v / SEG_ROWS + 4);
+    L.seg_meta = w.take<int>(n_v / SEG_ROWS + 4);
+    L.seg_b128 = w.take<int>(n_v / SEG_ROWS + 4);
+    L.cost_fx = w.take<long long>(B.max_blk + 2);
+    L.cost_pre = w.take<long long>(B.max_blk + 2);
     L.keysA = w.take<unsigned int>(nnz + 4);
     L.keysB = w.take<unsigned int>(nnz + 4);
     L.valsA = w.take<unsigned int>(nnz + 4);
@@ -563,16 +573,9 @@ inline int grid_for(long long n, int block) {
 }
 
 // ------------------------------------------------------------------------------------------------ host builders
-// Row-aligned blocks of D for the dose pass.  Each block becomes one self-contained record of the packed stream
-// (layout: kernels.cuh, DevPlan::pack); this lays the records out and writes their headers and row tables.
 // How much a record may hold.  Large matrices get the full sizes; a small one is cut into at least ~TARGET_RECORDS
-// records so that every consumer warp of every CTA has several (a record is consumed by one warp).
-struct RecordCaps {
-    int chunk_slots;   // row format: slots per record
-    int max_rows;      // row format: rows per record
-    int quad_cap;      // quad format: union columns per record
-    int quad_max;      // quad format: union columns of ONE quad at most (a longer one goes to row-format records)
-};
+// records so that every consumer warp of every CTA has several (a record is consumed by one warp).  The layout itself
+// (which rows go into which record) is done on the device: layout.cuh.
 // ring_est: roughly the bytes the dose pass's ring will have (what the gather array and g leave of shared memory).
 static RecordCaps record_caps(int64_t n_v, int64_t nnz, int64_t ring_est, int quad_cap_user) {
     auto clampi = [](int64_t v, int lo, int hi) { return (int)std::max<int64_t>(lo, std::min<int64_t>(hi, v)); };
@@ -586,153 +589,6 @@ static RecordCaps record_caps(int64_t n_v, int64_t nnz, int64_t ring_est, int qu
     // a single quad may exceed quad_cap (it then fills a record by itself), but two such records must fit in the ring
     c.quad_max = clampi((ring_est / 2 - 256) / 18, 0, 65528);
     return c;
-}
-
-struct BlockPlan {
-    std::vector<int4> blk;        // {record offset / 128, record bytes, 0, 0}                 -> device, dose pass
-    std::vector<int4> pk;         // {meta word offset, meta words, record offset / 128, 0}    -> device, pack kernel
-    std::vector<uint32_t> meta;   // headers + row tables, block after block
-    std::vector<int> rows, slots; // per block, for the cost model
-    size_t pack_bytes = 0;
-    int max_rec_bytes = 0;
-};
-
-// quadU: distinct columns per quad (4 consecutive rows), or empty when the quad format is not on offer.
-imrt_status build_blocks(imrt_plan* pl, const std::vector<int>& rp, const std::vector<uint8_t>& sid, const float4* table_h,
-                         const RecordCaps caps, int col_bytes, const std::vector<int>& quadU, BlockPlan& B,
-                         std::vector<unsigned char>& covered, int64_t& n_skipped, int64_t& n_nonempty, int64_t& n_quad_rows) {
-    const int n_v = (int)sid.size();
-    covered.assign((size_t)n_v, 1);
-    n_skipped = 0;
-    n_nonempty = 0;
-    n_quad_rows = 0;
-    auto skip_row = [&](int j) {   // d = 0 on a row without entries: a constant of the objective (k_skip_constants)
-        covered[j] = 0;
-        ++n_skipped;
-    };
-    auto pad4 = [](int n) { return (n + 3) & ~3; };
-    auto pad8 = [](int n) { return n; };   // unions are not padded: a lane past the end of a quad reads the zero column
-    size_t off = 0;
-    auto close_record = [&](int mo, int payload_bytes, int fmt, int rows, int slots) {
-        while ((B.meta.size() - mo - META_HDR) & 3) B.meta.push_back(0u);
-        const int mw = (int)B.meta.size() - mo;
-        const int rec = (mw * 4 + payload_bytes + 127) & ~127;
-        B.blk.push_back(make_int4((int)(off / 128), rec, 0, 0));
-        B.pk.push_back(make_int4(mo, mw, (int)(off / 128), fmt));
-        B.rows.push_back(rows);
-        B.slots.push_back(slots);
-        B.max_rec_bytes = std::max(B.max_rec_bytes, rec);
-        off += (size_t)rec;
-    };
-
-    for (int seg0 = 0; seg0 < n_v; seg0 += SEG_ROWS) {
-        const int seg1 = std::min(n_v, seg0 + SEG_ROWS);
-        // ---- which format is smaller on this segment
-        long long bytes_rows = 0, bytes_quads = 0;
-        for (int j = seg0; j < seg1; ++j) {
-            const int len = rp[j + 1] - rp[j];
-            if (len > 0) { bytes_rows += (long long)pad4(len) * (4 + col_bytes) + 4; ++n_nonempty; }
-        }
-        bool quads = !quadU.empty() && bytes_rows > 0;
-        if (quads) {
-            bool fits = true;
-            for (int q = seg0 / 4; q < (seg1 + 3) / 4; ++q)
-                if (quadU[q] > 0) { bytes_quads += (long long)pad8(quadU[q]) * 18 + 8; fits = fits && quadU[q] <= caps.quad_max; }
-            quads = fits && bytes_quads < bytes_rows;
-        }
-        if (!quads) {
-            // ---- row-format records
-            int j = seg0;
-            while (j < seg1) {
-                if (rp[j + 1] == rp[j]) { skip_row(j); ++j; continue; }
-                const int r0 = j;
-                int slots = pad4(rp[j + 1] - rp[j]);      // a row longer than the cap gets a record of its own
-                if (slots > MAX_CHUNK_SLOTS)
-                    return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has %d entries; this build handles rows up to %d", j,
-                                rp[j + 1] - rp[j], MAX_CHUNK_SLOTS);
-                int last = j, empties = 0, jj = j + 1;
-                while (jj < seg1 && jj - r0 < caps.max_rows) {
-                    const int len = rp[jj + 1] - rp[jj];
-                    if (len == 0) {
-                        if (++empties > 32) break;
-                        ++jj;
-                        continue;
-                    }
-                    if (slots + pad4(len) > caps.chunk_slots) break;
-                    slots += pad4(len);
-                    empties = 0;
-                    last = jj;
-                    ++jj;
-                }
-                const int r1 = last + 1, nrows = r1 - r0;
-                const int mo = (int)B.meta.size();
-                B.meta.push_back((uint32_t)nrows);
-                B.meta.push_back((uint32_t)r0);
-                B.meta.push_back(0u);
-                B.meta.push_back((uint32_t)slots);
-                int so = 0;
-                for (int row = r0; row < r1; ++row) {
-                    B.meta.push_back((uint32_t)so | ((uint32_t)sid[row] << 16));
-                    so += pad4(rp[row + 1] - rp[row]);
-                }
-                B.meta.push_back((uint32_t)so);
-                close_record(mo, (slots + ZPAD) * (4 + col_bytes), 0, nrows, slots);
-                j = r1;
-            }
-        } else {
-            // ---- quad-format records
-            int q = seg0 / 4;
-            const int q_end = (seg1 + 3) / 4;
-            auto skip_quad = [&](int qq) { for (int j = 4 * qq; j < std::min(n_v, 4 * qq + 4); ++j) skip_row(j); };
-            while (q < q_end) {
-                if (quadU[q] == 0) { skip_quad(q); ++q; continue; }
-                const int q0 = q;
-                int cols = pad8(quadU[q]);
-                int last = q, empties = 0, qq = q + 1;
-                while (qq < q_end && qq - q0 < QUAD_MAXQ) {
-                    if (quadU[qq] == 0) {
-                        if (++empties > 8) break;
-                        ++qq;
-                        continue;
-                    }
-                    if (cols + pad8(quadU[qq]) > caps.quad_cap) break;
-                    cols += pad8(quadU[qq]);
-                    empties = 0;
-                    last = qq;
-                    ++qq;
-                }
-                int q1 = last + 1, nq = q1 - q0;
-                constexpr int QROUND = 2;
-                if (nq > QROUND && nq % QROUND) {  // a warp takes two quads at a time: keep the pairs full
-                    for (int t = q1 - nq % QROUND; t < q1; ++t) cols -= pad8(quadU[t]);
-                    q1 -= nq % QROUND;
-                    nq = q1 - q0;
-                }
-                const int mo = (int)B.meta.size();
-                B.meta.push_back((uint32_t)nq);
-                B.meta.push_back((uint32_t)(4 * q0));
-                B.meta.push_back(1u);
-                B.meta.push_back((uint32_t)cols);
-                int co = 0, rows_here = 0;
-                for (int t = q0; t < q1; ++t) {
-                    uint32_t mask = 0u, sids = 0u;
-                    for (int i = 0; i < 4; ++i)
-                        if (4 * t + i < n_v) { mask |= 1u << i; sids |= (uint32_t)sid[4 * t + i] << (8 * i); ++rows_here; }
-                    B.meta.push_back((uint32_t)co | (mask << 16));
-                    B.meta.push_back(sids);
-                    co += pad8(quadU[t]);
-                }
-                B.meta.push_back((uint32_t)co);
-                B.meta.push_back(0u);
-                close_record(mo, (cols + 1) * 16 + (cols + 8) * 2, 1, rows_here, 4 * cols);
-                n_quad_rows += rows_here;
-                q = q1;
-                for (; q < q_end && quadU[q] == 0; ++q) skip_quad(q);   // trailing empties of the run belong to no record
-            }
-        }
-    }
-    B.pack_bytes = off;
-    return IMRT_STATUS_OK;
 }
 
 // Contiguous block ranges of (nearly) equal total cost, one per CTA.
@@ -1131,7 +987,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     memset(&opt, 0, sizeof opt);
     if (host_options) opt = *host_options;
     if (opt.tune_level < 0 || opt.tune_level > 2 || opt.dose_format < 0 || opt.dose_format > 1 || (opt.col_bits != 0 && opt.col_bits != 32) ||
-        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 || opt.fused_gradient < 0 || opt.fused_gradient > 1 ||
+        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 ||
         (opt.host_tuning && opt.host_tuning_bytes < sizeof(int) * 8))
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad imrt_options");
     imrt_plan* pl = new imrt_plan();
@@ -1149,65 +1005,77 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     struct Guard { imrt_plan* p; ~Guard() { if (p) { g_create_error = p->err; delete p; } } } guard{pl};
 
     PhaseTimer phase(opt.profile_create ? &pl->create_ms : nullptr, st);
-    // ---- validate what the host can see: row_ptr and structure ids
-    std::vector<int> rp((size_t)n_v + 1);
-    std::vector<uint8_t> sid((size_t)n_v);
-    CUDA_TRY(pl, cudaMemcpyAsync(rp.data(), row_ptr, sizeof(int) * (n_v + 1), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(pl, cudaMemcpyAsync(sid.data(), structure_id, (size_t)n_v, cudaMemcpyDeviceToHost, st));
+    // ---- validate: column indices and values, the row structure, the structure ids -- all on the device; only a
+    // handful of flags come back (the rows must be known to be sane before any kernel walks them)
+    DevPlan& P = pl->P;
+    memset(&P, 0, sizeof P);
     CUDA_TRY(pl, cudaMemsetAsync(L.flags, 0, 16 * sizeof(int), st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.totals, 0, sizeof(LayoutTotals), st));
     if (nnz > 0) k_validate<<<grid_for(nnz, 256), 256, 0, st>>>(col_idx, val, nnz, (int)n_b, L.flags);
+    k_validate_structure<<<grid_for(n_v, 256), 256, 0, st>>>(row_ptr, structure_id, (int)n_v, nnz, n_structures, L.totals);
+    CUDA_TRY(pl, cudaGetLastError());
     int flags_h[16];
+    LayoutTotals tot;
     CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(&tot, L.totals, sizeof tot, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(pl, cudaStreamSynchronize(st));
-    if (rp[0] != 0 || rp[n_v] != nnz) return fail(pl, IMRT_STATUS_BAD_CSR, "row_ptr[0] = %d, row_ptr[n_v] = %d, nnz = %lld", rp[0], rp[n_v], (long long)nnz);
-    for (int64_t j = 0; j < n_v; ++j)
-        if (rp[j + 1] < rp[j]) return fail(pl, IMRT_STATUS_BAD_CSR, "row_ptr decreases at row %lld", (long long)j);
+    if (tot.bad_row_ptr) return fail(pl, IMRT_STATUS_BAD_CSR, "row_ptr is not a valid CSR row pointer (row_ptr[0] != 0, row_ptr[n_v] != nnz = %lld, or it decreases near row %d)", (long long)nnz, tot.bad_row);
     if (flags_h[0]) return fail(pl, IMRT_STATUS_BAD_CSR, "a column index is outside [0, n_b)");
     if (flags_h[1]) return fail(pl, IMRT_STATUS_BAD_CSR, "a value of D is not finite");
-    if (nnz > 0) {      // row_ptr is sane: the rows can be walked
-        k_validate_rows<<<grid_for(n_v * 32, 256), 256, 0, st>>>(row_ptr, col_idx, (int)n_v, L.flags);
-        CUDA_TRY(pl, cudaGetLastError());
-        CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
-        if (flags_h[3]) return fail(pl, IMRT_STATUS_BAD_CSR, "column indices are not strictly ascending inside a row");
-    }
-    for (int64_t j = 0; j < n_v; ++j)
-        if (sid[j] >= n_structures) return fail(pl, IMRT_STATUS_BAD_STRUCTURE, "structure_id[%lld] = %d >= n_structures", (long long)j, sid[j]);
+    if (tot.bad_sid) return fail(pl, IMRT_STATUS_BAD_STRUCTURE, "structure_id[%d] >= n_structures", tot.bad_sid - 1);
+    if (tot.long_row)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "row %d of D has more than %d entries; this build handles rows up to that", tot.long_row - 1, MAX_CHUNK_SLOTS);
 
-    phase.mark();
     // ---- penalty table
     std::vector<float4> table_h(MAX_STRUCTURES, make_float4(0, 0, 0, 0));
     for (int s = 0; s < n_structures; ++s) table_h[s] = make_float4(host_t_under[s], host_t_over[s], host_w_under[s], host_w_over[s]);
     CUDA_TRY(pl, cudaMemcpyAsync(L.table, table_h.data(), sizeof(float4) * MAX_STRUCTURES, cudaMemcpyHostToDevice, st));
-
-    DevPlan& P = pl->P;
-    memset(&P, 0, sizeof P);
-
-    // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero); a block holds
-    // ROW_REC_SLOTS slots unless a longer row forces more
-    const bool col16 = n_b <= 65536 && opt.col_bits != 32;
-    int max_row = 0;
-    for (int64_t j = 0; j < n_v; ++j) max_row = std::max(max_row, rp[j + 1] - rp[j]);
-    if (max_row > MAX_CHUNK_SLOTS)
-        return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row of D has %d entries; this build handles rows up to %d", max_row, MAX_CHUNK_SLOTS);
-    const int64_t nb_pad_est = (n_b + 31) & ~31LL;
-    const RecordCaps caps = record_caps(n_v, nnz, (int64_t)smem_optin - SMEM_HEADER - 256 - std::max(SMEM_WPART, SMEM_DSC) - nb_pad_est * 4 * (R_MAX + 1), opt.quad_cap);
-    // quad format on offer: count the distinct columns of every 4 consecutive rows on the device
-    const int bm_words = (int)((n_b + 31) / 32);
-    std::vector<int> quadU;
-    if (col16 && n_b <= QUAD_MAX_NB && nnz > 0 && opt.dose_format == 0) {
-        const int n_quads = (int)((n_v + 3) / 4);
-        quadU.resize(n_quads);
-        k_quad_union<<<std::min(n_quads / 8 + 1, n_sm * 8), 256, 8 * bm_words * sizeof(uint32_t), st>>>(row_ptr, col_idx, (int)n_v, n_quads, bm_words, L.quadU);
+    if (nnz > 0) {      // row_ptr is sane: the rows can be walked
+        k_validate_rows<<<grid_for(n_v * 32, 256), 256, 0, st>>>(row_ptr, col_idx, (int)n_v, L.flags);
         CUDA_TRY(pl, cudaGetLastError());
-        CUDA_TRY(pl, cudaMemcpyAsync(quadU.data(), L.quadU, sizeof(int) * n_quads, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
     }
     phase.mark();
-    // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1).
-    // Enqueued here, ahead of the record layout below: that runs on the host for a few ms and needs nothing of this, so
-    // the device sorts meanwhile (no workspace region is shared between the two).
+
+    // ---- dose-pass blocks: 16-bit columns whenever n_b allows (25 % fewer bytes per non-zero)
+    const bool col16 = n_b <= 65536 && opt.col_bits != 32;
+    const int64_t nb_pad_est = (n_b + 31) & ~31LL;
+    const RecordCaps caps = record_caps(n_v, nnz, (int64_t)smem_optin - SMEM_HEADER - 256 - std::max(SMEM_WPART, SMEM_DSC) - nb_pad_est * 4 * (R_MAX + 1), opt.quad_cap);
+    // quad format on offer: count the distinct columns of every 4 consecutive rows
+    const int bm_words = (int)((n_b + 31) / 32);
+    const bool offer_quads = col16 && n_b <= QUAD_MAX_NB && nnz > 0 && opt.dose_format == 0;
+    if (offer_quads) {
+        const int n_quads = (int)((n_v + 3) / 4);
+        k_quad_union<<<std::min(n_quads / 8 + 1, n_sm * 8), 256, 8 * bm_words * sizeof(uint32_t), st>>>(row_ptr, col_idx, (int)n_v, n_quads, bm_words, L.quadU);
+        CUDA_TRY(pl, cudaGetLastError());
+    }
+    phase.mark();
+    // ---- record layout on the device (layout.cuh): count per segment, scan, write
     const Bounds B = bounds_for(n_v, n_b, nnz);
+    const int n_seg = (int)((n_v + SEG_ROWS - 1) / SEG_ROWS);
+    const int col_bytes = col16 ? 2 : 4;
+    CUDA_TRY(pl, cudaMemsetAsync(L.covered, 1, (size_t)n_v, st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.seg_rec, 0, sizeof(int) * (n_seg + 2), st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.seg_meta, 0, sizeof(int) * (n_seg + 2), st));
+    CUDA_TRY(pl, cudaMemsetAsync(L.seg_b128, 0, sizeof(int) * (n_seg + 2), st));
+    k_layout_count<<<grid_for(n_seg, 64), 64, 0, st>>>(row_ptr, structure_id, offer_quads ? L.quadU : nullptr, (int)n_v, n_seg, caps, col_bytes,
+                                                       L.seg_rec, L.seg_meta, L.seg_b128, L.totals);
+    for (int* arr : {L.seg_rec, L.seg_meta, L.seg_b128}) {
+        size_t temp = 0;
+        CUDA_TRY(pl, cub::DeviceScan::ExclusiveSum(nullptr, temp, arr, arr, n_seg + 1, st));
+        if (temp > B.sort_temp) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: scan needs %zu temp bytes", temp);
+        CUDA_TRY(pl, cub::DeviceScan::ExclusiveSum(L.sort_temp, temp, arr, arr, n_seg + 1, st));
+    }
+    LayoutOut LO = {L.blk, L.pk, L.rowmeta, L.cost_fx, L.covered};
+    k_layout_write<<<grid_for(n_seg, 64), 64, 0, st>>>(row_ptr, structure_id, offer_quads ? L.quadU : nullptr, (int)n_v, n_seg, caps, col_bytes,
+                                                       L.seg_rec, L.seg_meta, L.seg_b128, LO, L.totals);
+    CUDA_TRY(pl, cudaGetLastError());
+    CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaMemcpyAsync(&tot, L.totals, sizeof tot, cudaMemcpyDeviceToHost, st));
+    cudaEvent_t ev_totals;
+    CUDA_TRY(pl, cudaEventCreateWithFlags(&ev_totals, cudaEventDisableTiming));
+    CUDA_TRY(pl, cudaEventRecord(ev_totals, st));
+    // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1).
+    // Enqueued before the host waits for the layout totals: the device sorts while the host sizes the next launches.
     CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.valT, 0, sizeof(float) * B.nnz_pad, st));
     std::vector<int> rpT((size_t)n_b + 1, 0);
@@ -1226,52 +1094,59 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     } else {
         CUDA_TRY(pl, cudaMemsetAsync(L.rowT_ptr, 0, sizeof(int) * (n_b + 1), st));
     }
-    BlockPlan BP;
-    std::vector<unsigned char> covered;
-    imrt_status s = build_blocks(pl, rp, sid, table_h.data(), caps, col16 ? 2 : 4, quadU, BP, covered, pl->n_skipped,
-                                 pl->n_nonempty, pl->n_quad_rows);
-    if (s != IMRT_STATUS_OK) {
-        cudaStreamSynchronize(st);     // the transpose kernels enqueued above still write to the caller's workspace
-        return s;
+    {
+        const cudaError_t e = cudaEventSynchronize(ev_totals);
+        cudaEventDestroy(ev_totals);
+        if (e != cudaSuccess) { cudaStreamSynchronize(st); return fail(pl, IMRT_STATUS_CUDA_ERROR, "layout: %s", cudaGetErrorString(e)); }
     }
-    CUDA_TRY(pl, cudaMemcpyAsync(L.covered, covered.data(), (size_t)n_v, cudaMemcpyHostToDevice, st));
+    if (flags_h[3]) { cudaStreamSynchronize(st); return fail(pl, IMRT_STATUS_BAD_CSR, "column indices are not strictly ascending inside a row"); }
     phase.mark();
-    const size_t n_blk = BP.blk.size();
-    if ((int64_t)n_blk > B.max_blk || (int64_t)BP.meta.size() > B.max_meta || BP.pack_bytes > B.max_pack)
-        return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %zu words, %zu bytes)",
-                    n_blk, BP.meta.size(), BP.pack_bytes);
+    const size_t n_blk = (size_t)tot.n_blk;
+    const size_t pack_bytes = (size_t)tot.pack128 * 128;
+    if ((int64_t)n_blk > B.max_blk || (int64_t)tot.n_meta > B.max_meta || pack_bytes > B.max_pack) {
+        cudaStreamSynchronize(st);
+        return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: block tables exceed their bound (%zu blocks, %d words, %zu bytes)", n_blk, tot.n_meta, pack_bytes);
+    }
     pl->n_blk = (int64_t)n_blk;
-    pl->pack_bytes = (int64_t)BP.pack_bytes;
+    pl->pack_bytes = (int64_t)pack_bytes;
+    pl->n_skipped = tot.n_skipped; pl->n_nonempty = tot.n_nonempty; pl->n_quad_rows = tot.n_quad_rows;
     const int grid_f = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_sm, n_blk));
-    // cost of a block in SM cycles: the slower of streaming its bytes at a 1/n_sm share of HBM bandwidth and of
-    // issuing its instructions (per-row work dominates where rows are short, e.g. at the field edges); refined from
-    // measured per-CTA times by tune_partition() below
-    pl->blk_cost.resize(n_blk);
-    for (size_t b = 0; b < n_blk; ++b)
-        pl->blk_cost[b] = std::max(BP.blk[b].y / 22.4, 130.0 + 9.0 * BP.rows[b] + 0.08 * BP.slots[b]);
-    std::vector<int> cta_blk;
-    partition_blocks(pl->blk_cost, grid_f, cta_blk);
     if (n_blk) {
-        CUDA_TRY(pl, cudaMemcpyAsync(L.blk, BP.blk.data(), sizeof(int4) * n_blk, cudaMemcpyHostToDevice, st));
-        CUDA_TRY(pl, cudaMemcpyAsync(L.pk, BP.pk.data(), sizeof(int4) * n_blk, cudaMemcpyHostToDevice, st));
-        CUDA_TRY(pl, cudaMemcpyAsync(L.rowmeta, BP.meta.data(), sizeof(uint32_t) * BP.meta.size(), cudaMemcpyHostToDevice, st));
-        const size_t pk_smem = quadU.empty() ? 0 : 8 * 2 * bm_words * sizeof(uint32_t);
+        const size_t pk_smem = offer_quads ? 8 * 2 * bm_words * sizeof(uint32_t) : 0;
         if (col16) k_pack_blocks<true><<<(unsigned int)n_blk, 256, pk_smem, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, (int)n_v, bm_words, L.pack);
         else k_pack_blocks<false><<<(unsigned int)n_blk, 256, 0, st>>>(L.pk, L.rowmeta, row_ptr, col_idx, val, (int)n_v, bm_words, L.pack);
         CUDA_TRY(pl, cudaGetLastError());
     }
-
+    // the modelled partition: exclusive scan of the record costs, one binary search per CTA
+    std::vector<int> cta_blk((size_t)grid_f + 1, 0);
+    {
+        CUDA_TRY(pl, cudaMemsetAsync(L.cost_fx + n_blk, 0, sizeof(long long), st));
+        size_t temp = 0;
+        CUDA_TRY(pl, cub::DeviceScan::ExclusiveSum(nullptr, temp, L.cost_fx, L.cost_pre, (int)(n_blk + 1), st));
+        if (temp > B.sort_temp) return fail(pl, IMRT_STATUS_WORKSPACE_TOO_SMALL, "internal: scan needs %zu temp bytes", temp);
+        // the radix sort above owns sort_temp until it has run; the stream serialises the two
+        CUDA_TRY(pl, cub::DeviceScan::ExclusiveSum(L.sort_temp, temp, L.cost_fx, L.cost_pre, (int)(n_blk + 1), st));
+        k_partition<<<(grid_f + 1 + 127) / 128, 128, 0, st>>>(L.cost_pre, (int)n_blk, grid_f, L.cta_blk);
+        CUDA_TRY(pl, cudaGetLastError());
+        CUDA_TRY(pl, cudaMemcpyAsync(cta_blk.data(), L.cta_blk, sizeof(int) * (grid_f + 1), cudaMemcpyDeviceToHost, st));
+        if (opt.tune_level >= 1 && !opt.host_tuning) {      // the measured rebalancing rescales the costs on the host
+            std::vector<long long> cfx(n_blk);
+            CUDA_TRY(pl, cudaMemcpyAsync(cfx.data(), L.cost_fx, sizeof(long long) * n_blk, cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(pl, cudaStreamSynchronize(st));
+            pl->blk_cost.resize(n_blk);
+            for (size_t b = 0; b < n_blk; ++b) pl->blk_cost[b] = (double)cfx[b] / 1024.0;
+        }
+    }
     phase.mark();
     // ---- the explicit transpose was enqueued before the record layout: fetch its row pointers
-    if (nnz > 0) {
-        CUDA_TRY(pl, cudaMemcpyAsync(rpT.data(), L.rowT_ptr, sizeof(int) * (n_b + 1), cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(pl, cudaStreamSynchronize(st));
-    }
+    if (nnz > 0) CUDA_TRY(pl, cudaMemcpyAsync(rpT.data(), L.rowT_ptr, sizeof(int) * (n_b + 1), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(pl, cudaStreamSynchronize(st));      // rpT and cta_blk are on the host now
+    phase.mark();
+    imrt_status s = IMRT_STATUS_OK;
 
     // ---- transpose-pass ranges and gradient slots
     std::vector<TrRange> ranges;
     std::vector<int> rowslot, cta_rng_h;
-    phase.mark();
     // ---- the stream the transpose pass reads.  First choice: row pairs with 16-bit voxel offsets, if that is smaller
     // than single rows; second: single rows with 16-bit offsets; last: the plain 32-bit CSR (a group of 32 entries
     // spanning more than 65,535 voxels rules the 16-bit forms out).
@@ -1338,8 +1213,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     // ---- shared-memory layout (one layout for the three kernels): header, penalty table, transpose partials, dose
     // scratch, the R trial points, g, then the ring (dose pass) / stages (transpose pass).  R = the largest of 4, 2, 1
     // not above the request that leaves the ring room for 16 records of average size (one per consumer warp).
-    const int max_rec = std::max(BP.max_rec_bytes, 128);
-    const long long avg_rec = n_blk ? (long long)(BP.pack_bytes / n_blk) : 128;
+    const int max_rec = std::max(tot.max_rec_bytes, 128);
+    const long long avg_rec = n_blk ? (long long)(pack_bytes / n_blk) : 128;
     const int nb_pad = (int)((n_b + 31) & ~31LL);
     int R = prm->ls_batch == 0 ? R_MAX : prm->ls_batch;
     if (R != 1 && R != 2 && R != 4) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_params.ls_batch must be 0, 1, 2 or 4");

@@ -450,11 +450,11 @@ def test_per_voxel_limits_parity(m, cfg):
 
 # ---------------------------------------------------------------------------------------------- the fallback layouts
 @pytest.mark.parametrize("opt", [{"dose_format": 1}, {"col_bits": 32}, {"transpose_format": 1}, {"transpose_format": 2},
-                                 {"tune_level": 1}, {"tune_level": 2}, {"quad_cap": 64}, {"fused_gradient": 1}])
+                                 {"tune_level": 1}, {"tune_level": 2}, {"quad_cap": 64}])
 def test_fallback_layouts_parity(m, opt):
     # the layouts a plan falls back to when the matrix does not suit the packed ones: row-format records everywhere,
     # 32-bit column indices (n_b > 65,536), single rows of D^T instead of row pairs, the 32-bit D^T stream (a group of 32
-    # entries wider than 65,535 voxels); the measured partitions; small records; the loop without the fused gradient --
+    # entries wider than 65,535 voxels); the measured partitions; small records --
     # forced here through imrt_options
     for prob in (phantom(0), phantom(1),
                  synth_inputs.make_random(21, n_v=4099, n_b=130, density=0.5, empty_row_frac=0.15, full_rows=2)):
