@@ -217,25 +217,42 @@ def imrt_plan_get_create_times(plan) -> dict:
     return dict(zip(CREATE_PHASES, (float(v) for v in ms[:n.value])))
 
 
-def imrt_merge_rows(n_b: int, row_ptr, col_idx, val, group_id, n_groups: int, stream_ptr: int = 0):
-    """Mixed-resolution row merging (PAPER.md:150): (row_ptr, col, val) CUDA tensors of the matrix whose row g is the mean
-    of the rows of D with group_id == g.  Argument marshalling around imrt_merge_rows_count / imrt_merge_rows_fill."""
-    import torch
-    n_v = row_ptr.numel() - 1
+def imrt_merge_rows_workspace_bytes(n_v: int, n_groups: int) -> int:
     nb = ctypes.c_size_t(0)
     _check(lib().imrt_merge_rows_workspace_bytes(n_v, n_groups, ctypes.byref(nb)))
-    ws = torch.empty(nb.value, dtype=torch.uint8, device=row_ptr.device)
-    out_rp = torch.empty(n_groups + 1, dtype=torch.int32, device=row_ptr.device)
+    return nb.value
+
+
+def imrt_merge_rows_count(n_v, n_b, row_ptr, col_idx, group_id, n_groups, out_row_ptr, workspace, stream_ptr: int = 0) -> int:
+    """Fills out_row_ptr (int32 CUDA tensor [n_groups + 1]); returns the non-zeros of the merged matrix."""
+    import torch
     nnz = ctypes.c_int64(0)
-    st = ctypes.c_void_p(stream_ptr)
-    _check(lib().imrt_merge_rows_count(n_v, n_b, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32), _dptr(group_id, torch.int32, n_v),
-                                       n_groups, _dptr(out_rp), ctypes.byref(nnz), _dptr(ws), nb.value, st))
-    out_c = torch.empty(max(nnz.value, 4), dtype=torch.int32, device=row_ptr.device)
-    out_v = torch.empty(max(nnz.value, 4), dtype=torch.float32, device=row_ptr.device)
-    _check(lib().imrt_merge_rows_fill(n_v, n_b, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32), _dptr(val, torch.float32), n_groups,
-                                      _dptr(out_rp), _dptr(out_c), _dptr(out_v), _dptr(ws), nb.value, st))
+    _check(lib().imrt_merge_rows_count(n_v, n_b, _dptr(row_ptr, torch.int32, n_v + 1), _dptr(col_idx, torch.int32), _dptr(group_id, torch.int32, n_v),
+                                       n_groups, _dptr(out_row_ptr, torch.int32, n_groups + 1), ctypes.byref(nnz), _dptr(workspace),
+                                       workspace.numel() * workspace.element_size(), ctypes.c_void_p(stream_ptr)))
+    return nnz.value
+
+
+def imrt_merge_rows_fill(n_v, n_b, row_ptr, col_idx, val, n_groups, out_row_ptr, out_col, out_val, workspace, stream_ptr: int = 0):
+    import torch
+    _check(lib().imrt_merge_rows_fill(n_v, n_b, _dptr(row_ptr, torch.int32, n_v + 1), _dptr(col_idx, torch.int32), _dptr(val, torch.float32), n_groups,
+                                      _dptr(out_row_ptr, torch.int32), _dptr(out_col, torch.int32), _dptr(out_val, torch.float32), _dptr(workspace),
+                                      workspace.numel() * workspace.element_size(), ctypes.c_void_p(stream_ptr)))
+
+
+def imrt_merge_rows(n_b: int, row_ptr, col_idx, val, group_id, n_groups: int, stream_ptr: int = 0):
+    """Mixed-resolution row merging (PAPER.md:150): (row_ptr, col, val) CUDA tensors of the matrix whose row g is the mean
+    of the rows of D with group_id == g.  Allocation + the two C calls (imrt_merge_rows_count / imrt_merge_rows_fill)."""
+    import torch
+    n_v = row_ptr.numel() - 1
+    ws = torch.empty(imrt_merge_rows_workspace_bytes(n_v, n_groups), dtype=torch.uint8, device=row_ptr.device)
+    out_rp = torch.empty(n_groups + 1, dtype=torch.int32, device=row_ptr.device)
+    nnz = imrt_merge_rows_count(n_v, n_b, row_ptr, col_idx, group_id, n_groups, out_rp, ws, stream_ptr)
+    out_c = torch.empty(max(nnz, 4), dtype=torch.int32, device=row_ptr.device)
+    out_v = torch.empty(max(nnz, 4), dtype=torch.float32, device=row_ptr.device)
+    imrt_merge_rows_fill(n_v, n_b, row_ptr, col_idx, val, n_groups, out_rp, out_c, out_v, ws, stream_ptr)
     torch.cuda.current_stream(row_ptr.device).synchronize()      # ws goes out of scope
-    return out_rp, out_c[:nnz.value], out_v[:nnz.value]
+    return out_rp, out_c[:nnz], out_v[:nnz]
 
 
 def imrt_plan_gradient(plan, r, g):
