@@ -11,8 +11,10 @@ steps run inside ONE imrt_plan_run_iters(K) call: the loop is device-resident, t
 
 Workload: BASELINE.json configs[3], the headline 9-field / 5 mm beamlet / 2.5 mm voxel phantom (the config the
 metric's 60 %-of-HBM target is quoted on); it fits one GPU.  Inputs are seeded and synthetic (synth_inputs).
-N > 1: the path is single-GPU (replicas only) -- every rank optimises its own replica, no
-collective on the data path; value is the sum over ranks, time the max over ranks.
+N > 1: `value` is replicas (every rank optimises its own plan -- the unit of production throughput is one patient's
+plan; no collective on the data path; sum over ranks / max time), and the line's "sharded" object is the SAME single
+workload row-sharded over the N GPUs with the in-kernel exchange (strong scaling).  At N = 1 "sharded" runs
+--virtual-ranks ranks co-resident on the one GPU.
 """
 from __future__ import annotations
 
@@ -172,6 +174,7 @@ def run_ours(args):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")        # the ranks' transport log (NVLink / NVLS) goes to stderr
         dist.init_process_group("nccl", device_id=dev)
 
     def barrier():
@@ -181,8 +184,6 @@ def run_ours(args):
 
     K, W = args.steps, max(args.warmup, 3)
     prob = synth_inputs.make_phantom(args.config)
-    if args.sharded:
-        return run_sharded(args, prob, dev, rank, world, dist, barrier)
     driver = DRIVERS[args.driver]
     stream = torch.cuda.current_stream(dev)
 
@@ -240,6 +241,11 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     value = world * K / (ms * 1e-3)
+
+    # ---------------- the same workload row-sharded over ranks (all ranks take part): the in-kernel exchange path
+    sharded_res = None
+    if world > 1 or args.virtual_ranks > 1:
+        sharded_res = run_sharded(args, prob, dev, rank, world, dist, barrier)
 
     extra = {}
     if rank == 0:
@@ -376,6 +382,7 @@ def run_ours(args):
                 "clocks": clocks, "gpu_launches": n_launch, "plan_create_s": plan_create_s,
                 "objective": {"first": float(tr.obj[0]), "after_warmup": float(tr.obj[W]), "last": float(tr.obj[-1])}}
         line.update({k: v for k, v in extra.items() if k != "flush"})
+        line["sharded"] = sharded_res
         print(json.dumps(line))
     plan.close()
     if world > 1:
@@ -385,46 +392,45 @@ def run_ours(args):
 
 
 def run_sharded(args, prob, dev, rank, world, dist, barrier):
-    """--sharded: ONE problem over all ranks, rows of D in contiguous slabs (paper_0908_4421_b200/sharded.py): partial
-    objectives and gradients are summed with NCCL all-reduces; host-driven loop, one dose pass per trial.  Strong
-    scaling of a fixed workload -- the mode for matrices beyond one GPU's memory, not the headline."""
+    """ONE problem over several ranks, rows of D in contiguous slabs (paper_0908_4421_b200/sharded.py): the partial
+    gradients and objectives are summed INSIDE the persistent kernel through peer-memory inboxes.  world > 1: one rank per
+    GPU (torch symmetric memory over NVLink), strong scaling of the fixed workload; world == 1: --virtual-ranks V ranks
+    co-resident on the one GPU, each on SMs / V CTAs, one cooperative launch.  Returns a dict (rank 0) for the JSON line."""
     import torch
     from paper_0908_4421_b200 import sharded
     K, W = args.steps, max(args.warmup, 3)
-    sub, (r0, r1) = sharded.shard_rows(prob, world, rank)
-    opt = sharded.ShardedOptimizer(prob, sharded.GpuShard(sub, dev))
-    opt.run(prob.x0, W)
+    virtual = world == 1
+    n_ranks = args.virtual_ranks if virtual else world
+    try:
+        if virtual:
+            sp = sharded.CoResidentRanks(prob, n_ranks, max_iters=W + K, device=dev, tune_level=args.tune_level)
+        else:
+            sp = sharded.PeerRank(prob, max_iters=W + K, device=dev, tune_level=args.tune_level)
+    except Exception as exc:       # e.g. no peer access / symmetric memory on this box
+        return {"error": "%s: %s" % (type(exc).__name__, exc)}
+    sp.set_x(prob.x0)
+    sp.run_iters(W)
     barrier()
-    sampler = ClockSampler(dev.index or 0)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stream = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
-    tr = opt.run(opt.shard.to_numpy(opt.x), K)
+    sp.run_iters(K)
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
-    clocks = sampler.stop()
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    if rank == 0:
-        passes = int(tr.n_trials.sum())
-        print(json.dumps({"metric": METRIC, "value": tr.n_iters / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": tr.n_iters, "warmup": W,
-                          "ms_per_step": ms / max(tr.n_iters, 1), "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-                          "dtype": "f32", "data": "synthetic",
-                          "config": {"workload": prob.name, "n_v": prob.n_v, "n_b": prob.n_b, "nnz": prob.nnz,
-                                     "parallelism": "row slabs x%d, all-reduce of g per iteration and of G per trial" % world,
-                                     "driver": "host (sharded)", "rows_of_rank0": [r0, r1], "trials_per_iter": passes / max(tr.n_iters, 1)},
-                          "clocks": clocks, "gpu_launches": 1 + tr.n_iters + 2 * passes,     # gradient, dose and trial-point kernels
-                          "e2e": None, "roofline": None, "cpu_baseline": None,
-                          "objective": {"first": float(tr.obj[0]), "last": float(tr.obj[-1])}}))
-    if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
-    return 0
+    tr = sp.trace()
+    out = {"value": (tr.n_iters - W) / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / max(tr.n_iters - W, 1), "scaling": "strong",
+           "ranks": n_ranks, "placement": "co-resident on one GPU (%d CTAs each, one cooperative launch)" % sp.plans[0].info()["fwd_grid"] if virtual
+           else "one rank per GPU, inboxes in symmetric memory (NVLink peer stores)",
+           "exchange": "in-kernel: g (n_b fp32) per iteration, R objectives per batch; fixed rank-order sums",
+           "iterations": tr.n_iters - W, "stop_reason": tr.stop_reason, "objective_last": float(tr.obj[-1])}
+    sp.close()
+    return out
 
 
 def main():
@@ -441,8 +447,8 @@ def main():
                     help="imrt_options.tune_level: 0 modelled partitions, 1 + isolated measurements, 2 + measurements inside the loop")
     ap.add_argument("--cpu-iters", type=int, default=60, help="oracle iterations timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sharded", action="store_true",
-                    help="one problem over all ranks (row slabs of D, NCCL all-reduces) instead of one replica per rank")
+    ap.add_argument("--virtual-ranks", type=int, default=2,
+                    help="ranks of the row-sharded run that share the GPU when there is only one (0 = skip the sharded run)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

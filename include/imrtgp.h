@@ -106,7 +106,8 @@ typedef struct imrt_options {
     int32_t transpose_format;  /* 0: smallest of {row pairs, single rows} with 16-bit voxel offsets, else plain CSR;
                                   1: single rows with 16-bit offsets (no pairs);  2: the plain 32-bit D^T CSR         */
     int32_t quad_cap;          /* union columns per quad record at most (0 = default, 576; clamped to [32, 4096])     */
-    int32_t reserved1;
+    int32_t n_ctas;            /* CTAs of the persistent passes: 0 = one per SM of the device; fewer leaves SMs to other work
+                                  (or to other ranks of a row-sharded problem sharing the device, imrt_plan_run_ranks)   */
     int32_t profile_create;    /* 1: synchronise after every phase of plan creation and keep the phase times for
                                   imrt_plan_get_create_times                                                           */
     int32_t reserved0;
@@ -307,6 +308,30 @@ imrt_status imrt_plan_get_tuning(imrt_plan* plan, void* host_buf, size_t capacit
  *   [5] D^T stream packing, ranges  [6] state, first schedule  [7] dose-pass tuning  [8] transpose-pass tuning  [9] graph
  */
 imrt_status imrt_plan_get_create_times(imrt_plan* plan, double* host_ms, int32_t capacity, int32_t* host_n);
+
+/*
+ * Row-sharded problems (the paper is single-GPU): rank q of `world` holds a contiguous slab
+ * of rows of D -- one plan per rank, created from the slab's CSR with the FULL beamlet count -- and the loop sums the
+ * partial gradients (once per iteration) and the partial objectives (once per batch of trial points) over the ranks
+ * INSIDE the persistent kernel: every rank pushes its partial into every rank's inbox (peer memory; NVLink stores), raises
+ * a sequence flag, and adds what its own inbox holds in rank order, so all ranks compute the same bits and take the same
+ * Armijo decisions with no broadcast.
+ *   imrt_shard_inbox_bytes  size of one rank's inbox for n_b beamlets and `world` ranks (host arithmetic)
+ *   imrt_plan_set_shard     host_inboxes [world]: device pointers to EVERY rank's inbox as this rank's device can address
+ *                           them (its own included; peers' through peer access / IPC / symmetric memory), 16-byte
+ *                           aligned, zero-filled once before the first run and never touched by the caller afterwards.
+ *                           world = 1 returns to a stand-alone plan.  Persistent driver only.  Call imrt_plan_set_x after.
+ * Every rank then calls imrt_plan_set_x (the same x0) and imrt_plan_run_iters / _run_to_tol (the same arguments); the
+ * traces of all ranks are identical and hold the objective of the WHOLE problem; imrt_plan_get_dose / _eval / _dvh stay
+ * per slab.
+ *   imrt_plan_run_ranks     the same for ranks that are CO-RESIDENT on one device (plans created with
+ *                           imrt_options.n_ctas = SMs / ranks on one stream): ONE cooperative launch runs all of them --
+ *                           ranks wait on one another, so separate launches on one device could deadlock.  host_plans [n_ranks]
+ *                           in rank order.  Asynchronous.
+ */
+imrt_status imrt_shard_inbox_bytes(int64_t n_b, int32_t world, size_t* host_bytes);
+imrt_status imrt_plan_set_shard(imrt_plan* plan, int32_t rank, int32_t world, void* const* host_inboxes);
+imrt_status imrt_plan_run_ranks(imrt_plan* const* host_plans, int32_t n_ranks, int32_t n_iters, double delta);
 
 /*
  * Mixed-resolution row merging (section 3.1: "for unspecified tissue we increased the voxel size in each

@@ -29,6 +29,7 @@ DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
 EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_plan_set_voxel_limits", "imrt_plan_run_iters", "imrt_plan_run_to_tol",
            "imrt_plan_eval", "imrt_plan_eval_batch", "imrt_plan_gradient", "imrt_trial_point", "imrt_armijo_accepts", "imrt_stop_test", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
            "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_plan_get_tuning", "imrt_plan_get_create_times",
+           "imrt_shard_inbox_bytes", "imrt_plan_set_shard", "imrt_plan_run_ranks",
            "imrt_merge_rows_workspace_bytes", "imrt_merge_rows_count", "imrt_merge_rows_fill", "imrt_last_error", "imrt_plan_destroy",
            "imrt_version")
 
@@ -50,7 +51,7 @@ class Params(ctypes.Structure):
 class Options(ctypes.Structure):
     """imrt_options: layout / tuning switches of imrt_plan_create (all 0 = defaults)."""
     _fields_ = [("tune_level", ctypes.c_int32), ("dose_format", ctypes.c_int32), ("col_bits", ctypes.c_int32),
-                ("transpose_format", ctypes.c_int32), ("quad_cap", ctypes.c_int32), ("reserved1", ctypes.c_int32),
+                ("transpose_format", ctypes.c_int32), ("quad_cap", ctypes.c_int32), ("n_ctas", ctypes.c_int32),
                 ("profile_create", ctypes.c_int32), ("reserved0", ctypes.c_int32),
                 ("host_tuning", ctypes.c_void_p), ("host_tuning_bytes", ctypes.c_size_t)]
 
@@ -87,6 +88,9 @@ def lib() -> ctypes.CDLL:
         L.imrt_plan_gradient.argtypes = [_P, _P, _P]
         L.imrt_plan_get_tuning.argtypes = [_P, _P, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t)]
         L.imrt_plan_get_create_times.argtypes = [_P, _P, i32, ctypes.POINTER(i32)]
+        L.imrt_shard_inbox_bytes.argtypes = [i64, i32, ctypes.POINTER(ctypes.c_size_t)]
+        L.imrt_plan_set_shard.argtypes = [_P, i32, i32, ctypes.POINTER(_P)]
+        L.imrt_plan_run_ranks.argtypes = [ctypes.POINTER(_P), i32, i32, dbl]
         L.imrt_merge_rows_workspace_bytes.argtypes = [i64, i64, ctypes.POINTER(ctypes.c_size_t)]
         L.imrt_merge_rows_count.argtypes = [i64, i64, _P, _P, _P, i64, _P, ctypes.POINTER(i64), _P, ctypes.c_size_t, _P]
         L.imrt_merge_rows_fill.argtypes = [i64, i64, _P, _P, _P, i64, _P, _P, _P, _P, ctypes.c_size_t, _P]
@@ -215,6 +219,24 @@ def imrt_plan_get_create_times(plan) -> dict:
     n = ctypes.c_int32(0)
     _check(lib().imrt_plan_get_create_times(plan, _hptr(ms), 16, ctypes.byref(n)), plan)
     return dict(zip(CREATE_PHASES, (float(v) for v in ms[:n.value])))
+
+
+def imrt_shard_inbox_bytes(n_b: int, world: int) -> int:
+    nb = ctypes.c_size_t(0)
+    _check(lib().imrt_shard_inbox_bytes(n_b, world, ctypes.byref(nb)))
+    return nb.value
+
+
+def imrt_plan_set_shard(plan, rank: int, world: int, inbox_ptrs):
+    """inbox_ptrs: device addresses (ints) of every rank's inbox as this rank's device addresses them."""
+    arr = (_P * max(world, 1))(*[ctypes.c_void_p(int(p)) for p in inbox_ptrs]) if world > 1 else None
+    _check(lib().imrt_plan_set_shard(plan, rank, world, arr), plan)
+
+
+def imrt_plan_run_ranks(plans, n_iters: int, delta: float = 0.0):
+    """Run the co-resident ranks `plans` (handles, in rank order) in one cooperative launch."""
+    arr = (_P * len(plans))(*plans)
+    _check(lib().imrt_plan_run_ranks(arr, len(plans), int(n_iters), float(delta)), plans[0])
 
 
 def imrt_merge_rows_workspace_bytes(n_v: int, n_groups: int) -> int:
@@ -361,7 +383,7 @@ class Plan:
 
     def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None,
                  ls_batch: int = 0, tuning: bytes = None, **options):
-        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, profile_create); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
+        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, n_ctas, profile_create); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_0908_4421_b200 needs a CUDA device (sm_100a); there is no CPU path")

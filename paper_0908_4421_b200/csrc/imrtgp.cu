@@ -32,7 +32,8 @@ struct imrt_plan {
     imrt_params prm;
     imrt_options opt;
     cudaStream_t stream;
-    int n_sm;
+    int n_sm;                         // CTAs of this plan's persistent passes (the SM count, or imrt_options.n_ctas)
+    int n_sm_device;                  // SMs of the device
     size_t smem_bytes;
     int grid_p;                       // persistent kernel grid
     bool has_x;
@@ -63,6 +64,7 @@ struct imrt_plan {
     int* colT_w;
     float* valT_w;
     DvhWork dvh;
+    DevPlan* rank_plans_w;            // device copies of the plans of co-resident ranks (imrt_plan_run_ranks)
     // conditional graph (driver 0)
     cudaGraph_t graph;
     cudaGraphExec_t graph_exec;
@@ -160,6 +162,7 @@ struct Layout {
     int* quadU;
     unsigned char* covered;
     LayoutTotals* totals;
+    DevPlan* rank_plans;
     int *seg_rec, *seg_meta, *seg_b128;
     long long *cost_fx, *cost_pre;
     unsigned int* keysA;
@@ -215,6 +218,7 @@ Layout make_layout(void* base, int64_t n_v, int64_t n_b, int64_t nnz, int n_s, i
     L.quadU = w.take<int>(n_v / 4 + 2);
     L.covered = w.take<unsigned char>(n_v + 4);
     L.totals = w.take<LayoutTotals>(1);
+    L.rank_plans = w.take<DevPlan>(MAX_WORLD);
     L.seg_rec = w.take<int>(n_v / SEG_ROWS + 4);
     L.seg_meta = w.take<int>(n_v / SEG_ROWS + 4);
     L.seg_b128 = w.take<int>(n_v / SEG_ROWS + 4);
@@ -982,12 +986,14 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     if (cc_major != 10)
         return fail(nullptr, IMRT_STATUS_UNSUPPORTED_DEVICE, "device has compute capability %d.x; libimrtgp is built for sm_100a only", cc_major);
     if (n_sm > 1024) n_sm = 1024;
+    const int n_sm_device = n_sm;
+    if (host_options && host_options->n_ctas > 0) n_sm = std::min(n_sm, host_options->n_ctas);      // a share of the device
 
     imrt_options opt;
     memset(&opt, 0, sizeof opt);
     if (host_options) opt = *host_options;
     if (opt.tune_level < 0 || opt.tune_level > 2 || opt.dose_format < 0 || opt.dose_format > 1 || (opt.col_bits != 0 && opt.col_bits != 32) ||
-        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 ||
+        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 || opt.n_ctas < 0 ||
         (opt.host_tuning && opt.host_tuning_bytes < sizeof(int) * 8))
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad imrt_options");
     imrt_plan* pl = new imrt_plan();
@@ -995,6 +1001,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     pl->opt = opt;
     pl->stream = (cudaStream_t)stream;
     pl->n_sm = n_sm;
+    pl->n_sm_device = n_sm_device;
     pl->has_x = false;
     pl->graph = nullptr;
     pl->graph_exec = nullptr;
@@ -1260,6 +1267,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     pl->blk_w = L.blk;
     pl->rowT_ptr_w = L.rowT_ptr; pl->colT_w = L.colT; pl->valT_w = L.valT;
     pl->dvh = L.dvh;
+    pl->rank_plans_w = L.rank_plans;
     pl->grid_p = n_sm;
 
     CUDA_TRY(pl, cudaFuncSetAttribute(k_dose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes));
@@ -1381,6 +1389,8 @@ static imrt_status run_common(imrt_plan* pl, int32_t n_iters, double delta) {
     cudaStream_t st = pl->stream;
     k_set_target<<<1, 1, 0, st>>>(pl->P.st, n_iters, delta);
     CUDA_TRY(pl, cudaGetLastError());
+    if (pl->P.world > 1 && pl->prm.driver != 2)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row-sharded plan runs with the persistent driver (imrt_params.driver = 2) only");
     if (pl->prm.driver == 0) {
         CUDA_TRY(pl, cudaGraphLaunch(pl->graph_exec, st));
     } else if (pl->prm.driver == 2) {
@@ -1411,6 +1421,72 @@ static imrt_status run_common(imrt_plan* pl, int32_t n_iters, double delta) {
 }
 
 imrt_status imrt_plan_run_iters(imrt_plan* pl, int32_t n_iters) { return run_common(pl, n_iters, 0.0); }
+
+// ---------------------------------------------------------------------------------------------- row-sharded plans
+imrt_status imrt_shard_inbox_bytes(int64_t n_b, int32_t world, size_t* host_bytes) {
+    if (!host_bytes || n_b < 1 || n_b >= (1LL << 31) - 64 || world < 1 || world > MAX_WORLD)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_shard_inbox_bytes: bad argument (1 <= world <= %d)", MAX_WORLD);
+    *host_bytes = inbox_bytes((int)n_b, world);
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_set_shard(imrt_plan* pl, int32_t rank, int32_t world, void* const* host_inboxes) {
+    if (!pl || world < 1 || world > MAX_WORLD || rank < 0 || rank >= world || (world > 1 && !host_inboxes))
+        return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_shard: bad argument (0 <= rank < world <= %d)", MAX_WORLD);
+    if (world > 1 && pl->prm.driver != 2)
+        return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row-sharded plan runs with the persistent driver (imrt_params.driver = 2) only");
+    pl->P.rank = rank;
+    pl->P.world = world;
+    for (int q = 0; q < MAX_WORLD; ++q) {
+        pl->P.inbox[q] = (world > 1 && q < world) ? static_cast<unsigned char*>(host_inboxes[q]) : nullptr;
+        if (world > 1 && q < world && (!host_inboxes[q] || ((uintptr_t)host_inboxes[q] & 15)))
+            return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_shard: inbox %d is null or misaligned", q);
+    }
+    pl->has_x = false;         // G(x_1) has to be formed again, and summed over the ranks
+    return IMRT_STATUS_OK;
+}
+
+imrt_status imrt_plan_run_ranks(imrt_plan* const* host_plans, int32_t n_ranks, int32_t n_iters, double delta) {
+    if (!host_plans || n_ranks < 1 || n_ranks > MAX_WORLD || n_iters < 0 || !(delta >= 0.0))
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_ranks: bad argument");
+    imrt_plan* p0 = host_plans[0];
+    if (!p0) return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_ranks: null plan");
+    std::vector<DevPlan> plans(n_ranks);
+    int total = 0;
+    size_t smem = 0;
+    for (int q = 0; q < n_ranks; ++q) {
+        imrt_plan* pl = host_plans[q];
+        if (!pl) return fail(p0, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_ranks: null plan");
+        if (!pl->has_x) return fail(p0, IMRT_STATUS_NOT_READY, "rank %d: call imrt_plan_set_x first", q);
+        if (pl->prm.driver != 2 || pl->stream != p0->stream || pl->grid_p != p0->grid_p || pl->P.world != n_ranks || pl->P.rank != q)
+            return fail(p0, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_ranks: plan %d must be rank %d of %d (imrt_plan_set_shard), use the persistent "
+                        "driver, the stream and the number of CTAs (imrt_options.n_ctas) of plan 0", q, q, n_ranks);
+        plans[q] = pl->P;
+        total += pl->grid_p;
+        smem = std::max(smem, pl->smem_bytes);
+    }
+    if (total > p0->n_sm_device)
+        return fail(p0, IMRT_STATUS_UNSUPPORTED, "%d ranks of %d CTAs do not fit the device's %d SMs at one CTA per SM (imrt_options.n_ctas)", n_ranks, p0->grid_p, p0->n_sm_device);
+    cudaStream_t st = p0->stream;
+    for (int q = 0; q < n_ranks; ++q) k_set_target<<<1, 1, 0, st>>>(host_plans[q]->P.st, n_iters, delta);
+    CUDA_TRY(p0, cudaMemcpyAsync(p0->rank_plans_w, plans.data(), sizeof(DevPlan) * n_ranks, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(p0, cudaStreamSynchronize(st));       // `plans` is a host vector
+    CUDA_TRY(p0, cudaFuncSetAttribute(k_persistent_ranks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3(total);
+    cfg.blockDim = dim3(NTHREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;      // the ranks wait on one another: all their CTAs must be co-resident
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    const DevPlan* dp = p0->rank_plans_w;
+    CUDA_TRY(p0, cudaLaunchKernelEx(&cfg, k_persistent_ranks, dp, p0->grid_p));
+    return IMRT_STATUS_OK;
+}
 
 imrt_status imrt_plan_run_to_tol(imrt_plan* pl, double delta, int32_t max_iters) {
     if (pl && !(delta > 0.0)) return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_to_tol: delta must be > 0");

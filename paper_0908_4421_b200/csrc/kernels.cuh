@@ -54,6 +54,7 @@ constexpr int RL_MAX = 32;                    // rows of D^T one transpose range
 constexpr int RING_ENTRIES = 64;              // dose-pass records in flight per CTA (a multiple of the team count)
 constexpr int MAX_STAGES_T = 16;
 constexpr int MAX_STRUCTURES = 256;
+constexpr int MAX_WORLD = 16;                 // ranks of a row-sharded problem (one GPU each, or co-resident on one device)
 constexpr int SMEM_HEADER = 3072;             // barriers, flags, reduction scratch
 constexpr int SMEM_WPART = RL_MAX * W_CONS * 8 * 2;   // transpose pass: per-(row, warp) fp64 partials, two per row pair
 constexpr int SMEM_DSC = W_CONS * 32 * R_MAX * 4;   // per-warp scratch: dose of 32 rows x R trial points
@@ -85,6 +86,9 @@ struct State {                 // lives in the workspace; the single source of t
     unsigned int ticket_f, ticket_t;   // last-CTA tickets
     unsigned int gridbar;      // grid barrier counter of the persistent kernel
     int clamped;               // the last run's target was cut short by the trace capacity
+    unsigned long long seq_g, seq_G;   // row-sharded plans: exchanges of the gradient / of objectives done so far (never reset)
+    int G_is_local;            // row-sharded plans: G_k is this slab's share only (after set_x), not yet the sum over the ranks
+    int pad2;
 };
 
 struct TrRange {               // a contiguous piece of the D^T nnz stream, 32 bytes
@@ -160,6 +164,10 @@ struct DevPlan {
     double* tr_lambda;         // [cap]
     double* tr_step_sq;        // [cap]
     int* tr_trials;            // [cap]
+    // row-sharded problems: this plan holds the rows of rank `rank` of `world`; inbox[q] is rank q's
+    // exchange buffer (peer memory over NVLink, or plain device memory when the ranks share one device)
+    int rank, world;
+    unsigned char* inbox[MAX_WORLD];
     int wpart_off;             // byte offsets into dynamic shared memory: transpose per-(row, warp) partials,
     int dsc_off;               // dose-pass per-warp scratch,
     int x_off, g_off;          // the trial points x+ [n_b][R] (gathered by the dose pass) and the gradient (persistent kernel)
@@ -185,6 +193,8 @@ struct SmemHeader {
     double red[32 * R_MAX];    // block-reduction scratch
     double bcast[4];
     int flag;
+    int cta, n_cta;            // this CTA's index among the CTAs of ITS plan and their number: h->cta / gridDim.x, except when
+                               // several plans (ranks) share one cooperative launch (k_persistent_ranks)
 };
 static_assert(sizeof(SmemHeader) <= SMEM_HEADER, "header");
 
@@ -192,8 +202,10 @@ struct Pipe {                  // running stage counters; identical in producer 
     unsigned int it_f, it_t;
 };
 
-__device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4* table_s) {
+__device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4* table_s, int cta = (int)blockIdx.x, int n_cta = (int)gridDim.x) {
     if (threadIdx.x == 0) {
+        h->cta = cta;
+        h->n_cta = n_cta;
         for (int s = 0; s < RING_ENTRIES; ++s) mbar_init(&h->full_f[s], 1);
         for (int s = 0; s < MAX_STAGES_T; ++s) {
             mbar_init(&h->full_t[s], 1);
@@ -525,8 +537,8 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
                                             const float* xs, float* const (&r_out)[R], float* d_out, double* Gpart, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned char* ring = smem + P.stage_off;
-    const int b0 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x] : 0;
-    const int b1 = (blockIdx.x < P.grid_f) ? P.cta_blk[blockIdx.x + 1] : 0;
+    const int b0 = (h->cta < P.grid_f) ? P.cta_blk[h->cta] : 0;
+    const int b1 = (h->cta < P.grid_f) ? P.cta_blk[h->cta + 1] : 0;
     const int nb = b1 - b0;
     double Gacc[R];              // objective partials of the row-format records (every lane, every trial) ...
 #pragma unroll
@@ -616,11 +628,11 @@ __device__ __forceinline__ void dose_pass_t(const DevPlan& P, SmemHeader* h, uns
     block_sum_vec<R>(Gqv, h);
 #pragma unroll
     for (int r = 0; r < R; ++r) Gacc[r] += Gqv[r];
-    if (threadIdx.x == 0 && blockIdx.x < P.grid_f) {
+    if (threadIdx.x == 0 && h->cta < P.grid_f) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) Gpart[blockIdx.x * R + r] = Gacc[r];
-        P.cta_ns[2 * blockIdx.x] = t_start;            // when this CTA's share of the pass began and ended: lets the
-        P.cta_ns[2 * blockIdx.x + 1] = global_ns();    // host see (and rebalance) the static partition
+        for (int r = 0; r < R; ++r) Gpart[h->cta * R + r] = Gacc[r];
+        P.cta_ns[2 * h->cta] = t_start;            // when this CTA's share of the pass began and ended: lets the
+        P.cta_ns[2 * h->cta + 1] = global_ns();    // host see (and rebalance) the static partition
     }
     __syncthreads();
 }
@@ -664,8 +676,8 @@ __device__ __forceinline__ void transpose_pass_csr(const DevPlan& P, SmemHeader*
     const int S = P.n_stages_t;
     unsigned char* stages = smem + P.stage_off;
     unsigned int it = pipe.it_t;
-    const int rg0 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x] : 0;       // this CTA's ranges
-    const int rg1 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x + 1] : 0;
+    const int rg0 = (h->cta < P.grid_t) ? P.cta_rng[h->cta] : 0;       // this CTA's ranges
+    const int rg1 = (h->cta < P.grid_t) ? P.cta_rng[h->cta + 1] : 0;
     const unsigned long long t_start = global_ns();
     int s = (int)(it % (unsigned int)S);
     unsigned int ph = (it / (unsigned int)S) & 1u;
@@ -764,8 +776,8 @@ __device__ __forceinline__ void transpose_pass_csr(const DevPlan& P, SmemHeader*
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {
-        P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
-        P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
+        P.cta_ns[2048 + 2 * h->cta] = t_start;
+        P.cta_ns[2048 + 2 * h->cta + 1] = global_ns();
     }
 }
 
@@ -781,8 +793,8 @@ __device__ __forceinline__ void transpose_pass_rows(const DevPlan& P, SmemHeader
     const int S = P.n_stages_t;
     unsigned char* stages = smem + P.stage_off;
     unsigned int it = pipe.it_t;
-    const int rg0 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x] : 0;       // this CTA's ranges
-    const int rg1 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x + 1] : 0;
+    const int rg0 = (h->cta < P.grid_t) ? P.cta_rng[h->cta] : 0;       // this CTA's ranges
+    const int rg1 = (h->cta < P.grid_t) ? P.cta_rng[h->cta + 1] : 0;
     const unsigned long long t_start = global_ns();
     int s = (int)(it % (unsigned int)S);
     unsigned int ph = (it / (unsigned int)S) & 1u;
@@ -919,8 +931,8 @@ __device__ __forceinline__ void transpose_pass_rows(const DevPlan& P, SmemHeader
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {
-        P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
-        P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
+        P.cta_ns[2048 + 2 * h->cta] = t_start;
+        P.cta_ns[2048 + 2 * h->cta + 1] = global_ns();
     }
 }
 
@@ -933,8 +945,8 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
     const int S = P.n_stages_t;
     unsigned char* stages = smem + P.stage_off;
     unsigned int it = pipe.it_t;
-    const int rg0 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x] : 0;
-    const int rg1 = (blockIdx.x < P.grid_t) ? P.cta_rng[blockIdx.x + 1] : 0;
+    const int rg0 = (h->cta < P.grid_t) ? P.cta_rng[h->cta] : 0;
+    const int rg1 = (h->cta < P.grid_t) ? P.cta_rng[h->cta + 1] : 0;
     const unsigned long long t_start = global_ns();
     int s = (int)(it % (unsigned int)S);
     unsigned int ph = (it / (unsigned int)S) & 1u;
@@ -1053,8 +1065,8 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {
-        P.cta_ns[2048 + 2 * blockIdx.x] = t_start;
-        P.cta_ns[2048 + 2 * blockIdx.x + 1] = global_ns();
+        P.cta_ns[2048 + 2 * h->cta] = t_start;
+        P.cta_ns[2048 + 2 * h->cta + 1] = global_ns();
     }
 }
 
@@ -1092,11 +1104,88 @@ __device__ __forceinline__ void reduce_gradient(const DevPlan& P, const double* 
     }
 }
 
+// ------------------------------------------------------------------------------------------------ row-sharded exchange
+// rank q holds a slab of rows of D, computes a partial gradient over ALL beamlets and a partial
+// objective; the path's two exchange steps are the sums of those over the ranks.  Every rank owns an INBOX; a rank
+// PUSHES its partial into slot [rank] of every rank's inbox (remote stores over NVLink peer memory), then raises a
+// sequence flag there with a system-scope release; every CTA of a rank spins on its OWN inbox's flags (local memory)
+// and adds the world's partials in rank order -- the same order on every rank, so all ranks hold the same bits and take
+// the same decisions without any broadcast.  Two buffers per exchange kind, selected by the sequence number's parity: a
+// rank can be at most one exchange ahead of its slowest peer (it needs that peer's push to finish the current one).
+//   inbox: flags_g u64[MAX_WORLD] | flags_G u64[MAX_WORLD] | G double[2][MAX_WORLD][R_MAX] | g float[2][world][nb_pad]
+constexpr int INBOX_FLAGS_G = 0, INBOX_FLAGS_BIGG = 8 * MAX_WORLD, INBOX_BIGG = 16 * MAX_WORLD;
+constexpr int INBOX_G = INBOX_BIGG + 8 * 2 * MAX_WORLD * R_MAX;
+__host__ __device__ inline int inbox_nb_pad(int n_b) { return (n_b + 31) & ~31; }
+__host__ __device__ inline size_t inbox_bytes(int n_b, int world) { return (size_t)INBOX_G + (size_t)2 * world * inbox_nb_pad(n_b) * 4; }
+
+__device__ __forceinline__ void st_release_sys(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_acquire_sys(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// g_s: this slab's partial gradient on entry (every CTA of the rank holds the same), the sum over the ranks on exit.
+// fp32 partials, added in fp64 in rank order, rounded once.  All NTHREADS threads call it.
+__device__ __forceinline__ void shard_sum_gradient(const DevPlan& P, SmemHeader* h, float* g_s, unsigned long long seq) {
+    const int nbp = inbox_nb_pad(P.n_b), par = (int)(seq & 1ull);
+    if (h->cta == 0) {
+        for (int q = 0; q < P.world; ++q) {
+            float* dst = reinterpret_cast<float*>(P.inbox[q] + INBOX_G) + (size_t)(par * P.world + P.rank) * nbp;
+            for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) dst[i] = g_s[i];
+        }
+        __threadfence_system();
+        __syncthreads();
+        if ((int)threadIdx.x < P.world)
+            st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[threadIdx.x] + INBOX_FLAGS_G) + P.rank, seq);
+    }
+    if ((int)threadIdx.x < P.world) {
+        const unsigned long long* f = reinterpret_cast<const unsigned long long*>(P.inbox[P.rank] + INBOX_FLAGS_G) + threadIdx.x;
+        while (ld_acquire_sys(f) < seq) {}
+    }
+    __syncthreads();
+    const float* src = reinterpret_cast<const float*>(P.inbox[P.rank] + INBOX_G) + (size_t)par * P.world * nbp;
+    for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) {
+        double sum = 0.0;
+        for (int q = 0; q < P.world; ++q) sum += (double)__ldcg(src + (size_t)q * nbp + i);       // rank order
+        g_s[i] = (float)sum;
+    }
+    __syncthreads();
+}
+
+// G: this slab's R partial objectives on entry (the same in every thread of every CTA of the rank), the sums on exit.
+template <int R>
+__device__ __forceinline__ void shard_sum_objective(const DevPlan& P, SmemHeader* h, double (&G)[R], unsigned long long seq) {
+    const int par = (int)(seq & 1ull);
+    if (h->cta == 0 && (int)threadIdx.x < P.world) {
+        const int q = threadIdx.x;
+        double* dst = reinterpret_cast<double*>(P.inbox[q] + INBOX_BIGG) + (size_t)(par * MAX_WORLD + P.rank) * R_MAX;
+#pragma unroll
+        for (int r = 0; r < R; ++r) dst[r] = G[r];
+        st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[q] + INBOX_FLAGS_BIGG) + P.rank, seq);   // the same thread wrote the data
+    }
+    if ((int)threadIdx.x < P.world) {
+        const unsigned long long* f = reinterpret_cast<const unsigned long long*>(P.inbox[P.rank] + INBOX_FLAGS_BIGG) + threadIdx.x;
+        while (ld_acquire_sys(f) < seq) {}
+    }
+    __syncthreads();
+    const double* src = reinterpret_cast<const double*>(P.inbox[P.rank] + INBOX_BIGG) + (size_t)par * MAX_WORLD * R_MAX;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        double sum = 0.0;
+        for (int q = 0; q < P.world; ++q) sum += __ldcg(src + (size_t)q * R_MAX + r);              // rank order
+        G[r] = sum;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ scalar logic
 struct Loop {                  // the loop's scalar state, replicated in registers by the persistent kernel
     double G_k, lambda;
     int iter, m, stop_reason, xi, ri;
     long long fwd, tr;
+    unsigned long long seq_g, seq_G;
 };
 
 // After a transpose pass of the loop: start the line search (PAPER.md:109 step 2).  Returns true if trials are pending.
@@ -1158,11 +1247,13 @@ __device__ __forceinline__ void loop_load(const State* st, Loop& L) {
     L.G_k = st->G_k; L.lambda = st->lambda;
     L.iter = st->iter; L.m = st->m; L.stop_reason = st->stop_reason; L.xi = st->xi; L.ri = st->ri;
     L.fwd = st->fwd_passes; L.tr = st->tr_passes;
+    L.seq_g = st->seq_g; L.seq_G = st->seq_G;
 }
 __device__ __forceinline__ void loop_store(State* st, const Loop& L) {
     st->G_k = L.G_k; st->lambda = L.lambda;
     st->iter = L.iter; st->m = L.m; st->stop_reason = L.stop_reason; st->xi = L.xi; st->ri = L.ri;
     st->fwd_passes = L.fwd; st->tr_passes = L.tr;
+    st->seq_g = L.seq_g; st->seq_G = L.seq_G;
 }
 
 // Last-CTA election (threadfence reduction pattern).  Every thread has fenced its global writes before the call.
@@ -1171,7 +1262,7 @@ __device__ __forceinline__ bool cta_is_last(unsigned int* ticket, SmemHeader* h)
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned int t = atomicAdd(ticket, 1u);
-        const int last = (t == gridDim.x - 1);
+        const int last = (t == (unsigned int)h->n_cta - 1u);
         if (last) { *ticket = 0u; __threadfence(); }
         h->flag = last;
     }
@@ -1261,6 +1352,7 @@ __device__ __forceinline__ void dose_single(const DevPlan& P, const PassArgs& A,
         st->eval_obj = G[0];            // not counted: fwd_passes / tr_passes count the loop's passes
     } else {
         st->G_k = G[0]; st->fwd_passes += 1; st->ri = r_next;   // xbuf[xi] already holds x_1
+        st->G_is_local = P.world > 1;
         P.tr_obj[0] = G[0];
     }
 }
@@ -1444,29 +1536,37 @@ __global__ void k_set_target(State* st, int n_more, double delta_tol) {
 // fixed-order reductions, so CTAs never exchange anything but the pass partials; CTA 0 records the trace and
 // publishes the accepted iterate.
 template <int R>
-__device__ __forceinline__ void persistent_loop(const DevPlan& P) {
+__device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n_cta) {
     SmemHeader* h = reinterpret_cast<SmemHeader*>(imrt_smem);
     float4* table_s = reinterpret_cast<float4*>(imrt_smem + SMEM_HEADER);
     double* wpart = reinterpret_cast<double*>(imrt_smem + P.wpart_off);
     float* xs = reinterpret_cast<float*>(imrt_smem + P.x_off);     // the R trial points (the dose pass gathers from them)
     float* g_s = reinterpret_cast<float*>(imrt_smem + P.g_off);
     State* st = P.st;
-    cta_init(h, P, table_s);
+    cta_init(h, P, table_s, cta, n_cta);
     Loop L;
     loop_load(st, L);
     const int iter_target = st->iter_target;
     const double alpha = st->alpha;
     L.stop_reason = STOP_MAX_ITERS;
+    const bool sharded = P.world > 1;
+    if (sharded && st->G_is_local) {       // G(x_1) of imrt_plan_set_x is this slab's share: make it the sum over the ranks
+        double G1[1] = {L.G_k};
+        shard_sum_objective<1>(P, h, G1, ++L.seq_G);
+        L.G_k = G1[0];
+        if (h->cta == 0 && threadIdx.x == 0) P.tr_obj[0] = G1[0];
+    }
     Pipe pipe = {0u, 0u};
     unsigned int epoch = 0;
-    const bool rec = (blockIdx.x == 0) && (threadIdx.x == 0);
+    const bool rec = (h->cta == 0) && (threadIdx.x == 0);
 
     while (L.iter < iter_target) {
         const int tpar = (int)(L.tr & 1);
         transpose_pass(P, h, imrt_smem, wpart, P.rbuf[L.ri], P.gslot[tpar], pipe);
-        grid_barrier(&st->gridbar, epoch);
+        grid_barrier(&st->gridbar, epoch, h->n_cta);
         reduce_gradient(P, P.gslot[tpar], g_s);
         __syncthreads();
+        if (sharded) shard_sum_gradient(P, h, g_s, ++L.seq_g);      // exchange step 1: g = sum over the row slabs
         // start of the line search (PAPER.md:109 step 2; the same decisions begin_line_search takes, with the first
         // trial's Delta taken from the batch that is built anyway).  x_k lives in global memory.
         L.tr += 1;
@@ -1484,12 +1584,13 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P) {
             for (int j = 0; j < R; ++j) r_out[j] = P.rbuf[(L.ri + 1 + j) % (R + 1)];
             const int fpar = (int)(L.fwd & 1);
             dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[fpar], pipe);
-            grid_barrier(&st->gridbar, epoch);
+            grid_barrier(&st->gridbar, epoch, h->n_cta);
             reduce_objective<R>(P, P.Gpart[fpar], h, G_new);
+            if (sharded) shard_sum_objective<R>(P, h, G_new, ++L.seq_G);      // exchange step 2: G = sum over the row slabs
             dec = armijo_decide<R>(P, st, L, G_new, step_sq, rec, j_acc);
             if (dec != DEC_REJECT_RETRY) break;
         }
-        if (j_acc >= 0 && blockIdx.x == 0) {
+        if (j_acc >= 0 && h->cta == 0) {
             // x_{k+1}: publish it (L.xi already points at the new buffer); the other CTAs read it only after the
             // next grid barrier
             publish_x<R>(xs, j_acc, P.xbuf[L.xi], P.n_b);
@@ -1497,21 +1598,42 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P) {
         if (dec != DEC_ACCEPT_CONTINUE) break;
     }
     // every CTA has passed the last grid barrier before CTA 0 gets here with a changed state
-    grid_barrier(&st->gridbar, epoch);
-    if (blockIdx.x == 0) {
+    grid_barrier(&st->gridbar, epoch, h->n_cta);
+    if (h->cta == 0) {
         for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) P.g[i] = g_s[i];
         if (threadIdx.x == 0) {
             loop_store(st, L);
             st->cont_outer = 0;
             st->cont_inner = 0;
+            st->G_is_local = 0;
         }
     }
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) k_persistent(const __grid_constant__ DevPlan P) {
-    if (P.R == 4) persistent_loop<4>(P);
-    else if (P.R == 2) persistent_loop<2>(P);
-    else persistent_loop<1>(P);
+    if (P.R == 4) persistent_loop<4>(P, (int)blockIdx.x, (int)gridDim.x);
+    else if (P.R == 2) persistent_loop<2>(P, (int)blockIdx.x, (int)gridDim.x);
+    else persistent_loop<1>(P, (int)blockIdx.x, (int)gridDim.x);
+}
+
+// Several ranks of a row-sharded problem CO-RESIDENT on one device: one cooperative launch, rank q = the CTAs
+// [q ctas_per_rank, (q + 1) ctas_per_rank), each running the loop of its own plan and exchanging with the others through
+// their inboxes exactly as ranks on different GPUs do.  (Ranks that wait on one another must share ONE cooperative
+// launch on a single device: separate launches are not guaranteed to run at the same time.)
+static_assert(sizeof(SmemHeader) + sizeof(DevPlan) <= SMEM_HEADER, "the header region also holds a plan");
+__global__ void __launch_bounds__(NTHREADS, 1) k_persistent_ranks(const DevPlan* __restrict__ plans, int ctas_per_rank) {
+    DevPlan* Ps = reinterpret_cast<DevPlan*>(imrt_smem + sizeof(SmemHeader));
+    const int rank = (int)blockIdx.x / ctas_per_rank, cta = (int)blockIdx.x % ctas_per_rank;
+    {
+        const int* src = reinterpret_cast<const int*>(plans + rank);
+        int* dst = reinterpret_cast<int*>(Ps);
+        for (int i = threadIdx.x; i < (int)(sizeof(DevPlan) / 4); i += NTHREADS) dst[i] = src[i];
+        __syncthreads();
+    }
+    const DevPlan& P = *Ps;
+    if (P.R == 4) persistent_loop<4>(P, cta, ctas_per_rank);
+    else if (P.R == 2) persistent_loop<2>(P, cta, ctas_per_rank);
+    else persistent_loop<1>(P, cta, ctas_per_rank);
 }
 
 }  // namespace imrt

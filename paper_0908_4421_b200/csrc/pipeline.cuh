@@ -107,15 +107,16 @@ __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
 }
 
 // ---------------------------------------------------------------------------------------------- grid barrier
-// Monotone-counter barrier for a cooperative (co-resident) launch.  Every CTA calls it the same number of times;
+// Monotone-counter barrier for a cooperative (co-resident) launch over the n_cta CTAs that share `counter` (the whole
+// grid, or one rank's CTAs when several plans share a launch).  Every CTA calls it the same number of times;
 // `epoch` counts the calls (kept in a register by the caller).  counter must be 0 at kernel start.
-__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch) {
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, int n_cta) {
     __syncthreads();
     ++epoch;
     if (threadIdx.x == 0) {
         __threadfence();
         atomicAdd(counter, 1u);
-        const unsigned int target = epoch * gridDim.x;
+        const unsigned int target = epoch * (unsigned int)n_cta;
         unsigned int seen;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");

@@ -1,48 +1,55 @@
-"""Row-sharded gradient projection over several GPUs (one process per GPU, torch.distributed).
+"""Row-sharded gradient projection: slab selection and the set-up of the device-resident sharded loop.
 
 Rank q holds a contiguous slab of rows of D (voxels) -- and with it the matching columns of D^T --, the full x,
 and computes local dose, residual, a partial objective and a partial gradient over ALL beamlets.  The exchange
-steps of the method are then
+steps of the method are
 
-    G(x)  = sum over ranks of G_q(x)            one scalar per line-search trial      (all-reduce, SUM)
-    g     = sum over ranks of D_q^T r_q         n_b fp32 (9-15 KB) per iteration      (all-reduce, SUM)
+    g     = sum over ranks of D_q^T r_q         n_b fp32 (9-15 KB) per iteration
+    G(x+) = sum over ranks of G_q(x+)           R scalars per batch of line-search trial points
 
-and every rank takes the same Armijo decisions from the same reduced numbers (readings R4-R7 of
-DESIGN.md), so the iterates stay replicated without ever being broadcast.
+and every rank takes the same Armijo decisions from the same sums (readings R4-R7 of DESIGN.md),
+so the iterates stay replicated without ever being broadcast.
 
-This module is host logic only: slab selection, the loop, the two collectives.  All arithmetic of the path runs in
-the library's kernels through three C-ABI calls per shard -- imrt_plan_eval (dose, penalty, residual, partial
-objective), imrt_plan_gradient (partial D^T r) and imrt_trial_point (projection and step norm); the two scalar
-decisions are the library's host functions imrt_armijo_accepts / imrt_stop_test.  The loop is
-host-driven (a synchronisation per trial, one dose pass per trial): it is the way to run matrices that do not fit
-one GPU, not the fast path -- on one GPU use Plan.run_iters, which keeps the whole loop on the device.
+BOTH exchange steps run INSIDE the library's persistent kernel (csrc/kernels.cuh: shard_sum_gradient /
+shard_sum_objective): a rank pushes its partial into every rank's inbox with peer-memory stores, raises a sequence
+flag, and adds its own inbox's entries in rank order.  This module only marshals: it cuts the slabs, allocates the
+inboxes, hands every plan the inbox addresses (imrt_plan_set_shard) and calls the run functions.  None of the
+method's arithmetic or control flow lives here.
 
-The local shard is an object with eval_partial / grad_partial / trial_point (GpuShard below); tests substitute a
-CPU stand-in to exercise slab selection, loop and collectives under the gloo backend.
+  CoResidentRanks   all ranks on ONE device, each on its share of the SMs, one cooperative launch
+                    (imrt_plan_run_ranks) -- how the sharded loop is exercised where a single GPU is available
+  PeerRank          one rank per process / GPU (torchrun): the inboxes live in torch symmetric memory, whose rendezvous
+                    returns every peer's buffer address as this device maps it (NVLink peer access)
 """
 from __future__ import annotations
 
 import copy
-from dataclasses import dataclass
 
 import numpy as np
 
-STOP_MAX_ITERS, STOP_TOLERANCE, STOP_STATIONARY, STOP_LS_STALLED = 0, 1, 2, 3
-
 
 def slab_bounds(row_ptr: np.ndarray, world: int) -> np.ndarray:
-    """Row boundaries [world + 1] of contiguous slabs with (nearly) equal numbers of non-zeros."""
+    """Row boundaries [world + 1] of contiguous slabs with (nearly) equal numbers of non-zeros; every slab gets at least
+    one row as long as there are at least `world` rows (a plan cannot be created from zero rows)."""
     row_ptr = np.asarray(row_ptr, dtype=np.int64)
     n_v, nnz = row_ptr.shape[0] - 1, int(row_ptr[-1])
     b = np.zeros(world + 1, dtype=np.int64)
     for q in range(1, world):
         b[q] = int(np.searchsorted(row_ptr, nnz * q // world, side="left"))
     b[world] = n_v
-    return np.maximum.accumulate(np.minimum(b, n_v))
+    b = np.maximum.accumulate(np.minimum(b, n_v))
+    if n_v >= world:
+        for q in range(1, world):                    # push boundaries apart where a slab came out empty
+            b[q] = max(b[q], b[q - 1] + 1)
+        for q in range(world - 1, 0, -1):
+            b[q] = min(b[q], b[q + 1] - 1)
+    return b
 
 
 def shard_rows(prob, world: int, rank: int):
     """The sub-problem of `rank`: rows [r0, r1) of D with their structure ids (and per-voxel limits, if any)."""
+    if prob.n_v < world:             # the same refusal on every rank, before any collective
+        raise ValueError("%d ranks for a %d-row matrix: some rank would hold no rows; use fewer ranks" % (world, prob.n_v))
     b = slab_bounds(prob.row_ptr, world)
     r0, r1 = int(b[rank]), int(b[rank + 1])
     p0, p1 = int(prob.row_ptr[r0]), int(prob.row_ptr[r1])
@@ -59,113 +66,88 @@ def shard_rows(prob, world: int, rank: int):
     return sub, (r0, r1)
 
 
-@dataclass
-class ShardedTrace:
-    n_iters: int
-    stop_reason: int
-    obj: np.ndarray        # float64 [n+1]
-    lam: np.ndarray        # float64 [n]
-    n_trials: np.ndarray   # int32 [n]
-    step_sq: np.ndarray    # float64 [n]
+class CoResidentRanks:
+    """`world` ranks of one problem on ONE device: plan q gets slab q and SMs / world CTAs; all of them run in one
+    cooperative launch and exchange through inboxes in that device's memory, exactly as ranks on different GPUs do."""
 
-
-class GpuShard:
-    """One slab on one GPU: a Plan of the sub-problem; every method is one C-ABI call (argument marshalling only)."""
-
-    def __init__(self, sub_prob, device):
+    def __init__(self, prob, world: int, max_iters: int = 1000, device="cuda:0", **options):
         import torch
-        from . import Plan, imrt_plan_eval, imrt_plan_gradient, imrt_trial_point
-        self._eval, self._grad, self._trial = imrt_plan_eval, imrt_plan_gradient, imrt_trial_point
+        from . import Plan, imrt_plan_set_shard, imrt_shard_inbox_bytes
         self.device = torch.device(device)
-        self.n_b = int(sub_prob.n_b)
-        self.plan = Plan(sub_prob, max_iters=1, device=self.device)
-        self.r = torch.empty(max(int(sub_prob.n_v), 1), dtype=torch.float32, device=self.device)
-        self.step = torch.zeros(1, dtype=torch.float64, device=self.device)
+        self.world = int(world)
+        n_sm = torch.cuda.get_device_properties(self.device).multi_processor_count
+        self.rows = []
+        self.plans = []
+        for q in range(self.world):
+            sub, rows = shard_rows(prob, self.world, q)
+            self.rows.append(rows)
+            self.plans.append(Plan(sub, max_iters=max_iters, device=self.device, n_ctas=n_sm // self.world, **options))
+        nbytes = imrt_shard_inbox_bytes(int(prob.n_b), self.world)
+        self.inboxes = [torch.zeros(nbytes, dtype=torch.uint8, device=self.device) for _ in range(self.world)]
+        ptrs = [t.data_ptr() for t in self.inboxes]
+        for q, p in enumerate(self.plans):
+            imrt_plan_set_shard(p.handle, q, self.world, ptrs)
 
-    def vector(self, x0):
+    def set_x(self, x0):
+        for p in self.plans:
+            p.set_x(x0)
+
+    def run_iters(self, n: int):
+        from . import imrt_plan_run_ranks
+        imrt_plan_run_ranks([p.handle for p in self.plans], int(n), 0.0)
+
+    def run_to_tol(self, delta: float, max_iters: int):
+        from . import imrt_plan_run_ranks
+        imrt_plan_run_ranks([p.handle for p in self.plans], int(max_iters), float(delta))
+
+    def trace(self, rank: int = 0):
+        return self.plans[rank].trace()
+
+    def get_x(self, rank: int = 0):
+        return self.plans[rank].get_x()
+
+    def get_dose(self):
+        """Dose of the whole problem: the slabs' doses in row order."""
         import torch
-        return torch.from_numpy(np.ascontiguousarray(x0, dtype=np.float32)).to(self.device)
+        return torch.cat([p.get_dose() for p in self.plans])
 
-    def eval_partial(self, x) -> float:
-        """G_q(x); leaves r_q(x) in self.r."""
-        return self._eval(self.plan.handle, x, None, self.r, None)
+    def close(self):
+        for p in self.plans:
+            p.close()
 
-    def grad_partial(self):
-        """D_q^T r_q for the residual of the last eval_partial (fp32 [n_b])."""
+
+class PeerRank:
+    """This process's rank of a row-sharded problem, one GPU per process (torch.distributed initialised, NCCL).  The inbox
+    is allocated in torch symmetric memory; its rendezvous maps every peer's inbox into this device's address space."""
+
+    def __init__(self, prob, max_iters: int = 1000, device=None, group=None, **options):
         import torch
-        g = torch.empty(self.n_b, dtype=torch.float32, device=self.device)
-        self._grad(self.plan.handle, self.r, g)
-        return g
-
-    def trial_point(self, x, g, lam: float):
-        import torch
-        x_new = torch.empty_like(x)
-        self._trial(x, g, lam, x_new, self.step, self.plan.stream.cuda_stream)
-        return x_new, float(self.step.item())
-
-    def to_numpy(self, x):
-        return x.detach().cpu().numpy()
-
-
-class ShardedOptimizer:
-    """The Main Iterative Loop of PAPER.md:99-114 over row slabs; `shard` is this rank's local shard."""
-
-    def __init__(self, prob, shard, group=None, accepts=None, stop_test=None):
         import torch.distributed as dist
-        self.dist, self.group, self.shard = dist, group, shard
-        if accepts is None or stop_test is None:      # the library's own scalar decisions (pure host C functions)
-            from . import imrt_armijo_accepts, imrt_stop_test
-            accepts, stop_test = accepts or imrt_armijo_accepts, stop_test or imrt_stop_test
-        self.accepts, self.stop_test = accepts, stop_test
-        self.eps, self.alpha, self.lambda0, self.max_ls = float(prob.eps), float(prob.alpha), float(prob.lambda0), int(prob.max_ls)
+        import torch.distributed._symmetric_memory as symm_mem
+        from . import Plan, imrt_plan_set_shard, imrt_shard_inbox_bytes
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.device = torch.device(device if device is not None else "cuda:%d" % torch.cuda.current_device())
+        sub, self.rows = shard_rows(prob, self.world, self.rank)
+        self.plan = Plan(sub, max_iters=max_iters, device=self.device, **options)
+        nbytes = imrt_shard_inbox_bytes(int(prob.n_b), self.world)
+        self.inbox = symm_mem.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.inbox.zero_()
+        self.handle = symm_mem.rendezvous(self.inbox, group=(group.group_name if group is not None else dist.group.WORLD.group_name))
+        torch.cuda.synchronize(self.device)
+        dist.barrier(group)                          # every inbox is zero before anybody pushes
+        imrt_plan_set_shard(self.plan.handle, self.rank, self.world, [int(p) for p in self.handle.buffer_ptrs])
 
-    # -- the two exchange steps
-    def _sum_scalar(self, v: float) -> float:
-        import torch
-        t = torch.tensor([v], dtype=torch.float64, device=getattr(self.shard, "device", "cpu"))
-        if self.dist.is_initialized() and self.dist.get_world_size(self.group) > 1:
-            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
-        return float(t.item())
+    def set_x(self, x0):
+        self.plan.set_x(x0)
 
-    def _sum_vector(self, g):
-        if self.dist.is_initialized() and self.dist.get_world_size(self.group) > 1:
-            self.dist.all_reduce(g, op=self.dist.ReduceOp.SUM, group=self.group)
-        return g
+    def run_iters(self, n: int):
+        self.plan.run_iters(n)
 
-    def run(self, x0, n_iters: int, delta: float = 0.0):
-        sh = self.shard
-        x = sh.vector(x0)
-        G_k = self._sum_scalar(sh.eval_partial(x))
-        obj, lams, trials, steps = [G_k], [], [], []
-        reason = STOP_MAX_ITERS
-        while len(lams) < n_iters:
-            g = self._sum_vector(sh.grad_partial())                     # step 1
-            if G_k == 0.0:
-                reason = STOP_STATIONARY
-                break
-            lam, m, accepted = self.lambda0, 0, False                   # step 2
-            while True:
-                x_new, step_sq = sh.trial_point(x, g, lam)
-                if m == 0 and step_sq == 0.0:
-                    reason = STOP_STATIONARY
-                    break
-                G_new = self._sum_scalar(sh.eval_partial(x_new))
-                if self.accepts(G_k, G_new, step_sq, self.eps, lam):    # step 3, Eq. (5)
-                    accepted = True
-                    break
-                m += 1                                                  # step 4
-                if m > self.max_ls:
-                    reason = STOP_LS_STALLED
-                    break
-                lam = lam / self.alpha
-            if not accepted:
-                if reason == STOP_LS_STALLED:
-                    sh.eval_partial(x)                                  # restore r(x_k) (x_k is kept)
-                break
-            G_old, G_k, x = G_k, G_new, x_new
-            obj.append(G_new); lams.append(lam); trials.append(m + 1); steps.append(step_sq)
-            if self.stop_test(G_old, G_new, delta):                     # step 5
-                reason = STOP_TOLERANCE
-                break
-        self.x = x
-        return ShardedTrace(len(lams), reason, np.asarray(obj), np.asarray(lams), np.asarray(trials, np.int32), np.asarray(steps))
+    def run_to_tol(self, delta: float, max_iters: int):
+        self.plan.run_to_tol(delta, max_iters)
+
+    def trace(self):
+        return self.plan.trace()
+
+    def close(self):
+        self.plan.close()

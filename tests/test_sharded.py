@@ -10,6 +10,7 @@ import pytest
 import oracle
 import synth_inputs
 from paper_0908_4421_b200 import sharded
+import host_sharded_loop as host_loop
 
 
 class OracleShard:
@@ -65,7 +66,7 @@ def _worker(rank, world, port, n_iters, out):
     try:
         prob = synth_inputs.make_phantom(0)
         sub, _ = sharded.shard_rows(prob, world, rank)
-        opt = sharded.ShardedOptimizer(prob, OracleShard(sub))
+        opt = host_loop.ShardedOptimizer(prob, OracleShard(sub))
         tr = opt.run(prob.x0, n_iters)
         out[rank] = (tr.n_iters, tr.stop_reason, tr.obj.tolist(), tr.lam.tolist(), tr.n_trials.tolist(), opt.x.numpy().tolist())
     finally:
@@ -94,25 +95,25 @@ def test_two_ranks_gloo_reproduce_the_single_process_loop():
 
 def test_stationary_and_tolerance_exits_without_a_process_group():
     prob = synth_inputs.make_phantom(0)
-    opt = sharded.ShardedOptimizer(prob, OracleShard(prob))
+    opt = host_loop.ShardedOptimizer(prob, OracleShard(prob))
     tr = opt.run(prob.x0, 400, delta=1e-3)
     ref = oracle.run(prob, n_iters=400, delta=1e-3)
-    assert tr.stop_reason == sharded.STOP_TOLERANCE == ref.stop_reason and tr.n_iters == ref.n_iters
+    assert tr.stop_reason == host_loop.STOP_TOLERANCE == ref.stop_reason and tr.n_iters == ref.n_iters
     np.testing.assert_array_equal(tr.obj, ref.obj)                    # one slab: the very same arithmetic
     T = np.array([10.0, 20.0, 30.0], np.float32)
     ident = synth_inputs.Problem("ident", 3, 3, np.array([0, 1, 2, 3], np.int32), np.array([0, 1, 2], np.int32), np.ones(3, np.float32),
                                  np.array([0, 1, 2], np.uint8), T, T, np.ones(3, np.float32), np.ones(3, np.float32),
                                  np.array([12.0, 16.0, 30.0], np.float32), eps=0.2, alpha=2.0, lambda0=1.0)
-    tr = sharded.ShardedOptimizer(ident, OracleShard(ident)).run(ident.x0, 5)
-    assert tr.n_iters == 1 and tr.stop_reason == sharded.STOP_STATIONARY and tr.obj.tolist() == [20.0, 0.0] and tr.n_trials.tolist() == [2]
+    tr = host_loop.ShardedOptimizer(ident, OracleShard(ident)).run(ident.x0, 5)
+    assert tr.n_iters == 1 and tr.stop_reason == host_loop.STOP_STATIONARY and tr.obj.tolist() == [20.0, 0.0] and tr.n_trials.tolist() == [2]
 
 
 class _TwoSlabs:
     """Two GpuShards on one device whose partials are added here: what the all-reduce does across two GPUs."""
 
     def __init__(self, prob, device):
-        self.a = sharded.GpuShard(sharded.shard_rows(prob, 2, 0)[0], device)
-        self.b = sharded.GpuShard(sharded.shard_rows(prob, 2, 1)[0], device)
+        self.a = host_loop.GpuShard(sharded.shard_rows(prob, 2, 0)[0], device)
+        self.b = host_loop.GpuShard(sharded.shard_rows(prob, 2, 1)[0], device)
         self.device = self.a.device
 
     def vector(self, x0):
@@ -141,8 +142,8 @@ def test_two_slabs_of_the_cuda_path_add_up(cfg):
     plan.set_x(prob.x0)
     plan.run_iters(n)
     tr1 = plan.trace()
-    one = sharded.ShardedOptimizer(prob, sharded.GpuShard(prob, "cuda:0")).run(prob.x0, n)
-    two = sharded.ShardedOptimizer(prob, _TwoSlabs(prob, "cuda:0")).run(prob.x0, n)
+    one = host_loop.ShardedOptimizer(prob, host_loop.GpuShard(prob, "cuda:0")).run(prob.x0, n)
+    two = host_loop.ShardedOptimizer(prob, _TwoSlabs(prob, "cuda:0")).run(prob.x0, n)
     for tr in (one, two):
         assert tr.n_iters == n
         np.testing.assert_array_equal(tr.n_trials, tr1.n_trials)
@@ -151,3 +152,78 @@ def test_two_slabs_of_the_cuda_path_add_up(cfg):
     fol = oracle.run(prob, n_iters=n, follow_trials=two.n_trials, tau_rel=1e-6)
     assert fol.n_follow_violations == 0 and abs(two.obj[-1] - fol.obj[-1]) <= 1e-4 * fol.obj[-1]
     plan.close()
+
+
+def test_no_rank_is_left_without_rows():
+    # a few rows hold most of the non-zeros: equal-nnz cuts would leave ranks empty; every rank still gets >= 1 row
+    rp = np.array([0, 1000, 1000, 1001, 1002, 1003, 1004], np.int64)
+    for world in (2, 3, 6):
+        b = sharded.slab_bounds(rp, world)
+        assert b[0] == 0 and b[-1] == 6 and (np.diff(b) >= 1).all(), b
+    prob = synth_inputs.make_phantom(0)
+    small = synth_inputs.Problem("two-rows", 2, 3, np.array([0, 1, 2], np.int32), np.array([0, 1], np.int32), np.ones(2, np.float32),
+                                 np.zeros(2, np.uint8), prob.t_under, prob.t_over, prob.w_under, prob.w_over, np.ones(3, np.float32))
+    with pytest.raises(ValueError):
+        sharded.shard_rows(small, 3, 2)              # more ranks than rows: refused on every rank alike, before any collective
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,world,n", [(0, 2, 30), (2, 2, 60), (2, 4, 60), (1, 3, 40)])
+def test_device_resident_sharded_loop_co_resident_ranks(cfg, world, n):
+    # The row-sharded loop INSIDE the persistent kernel (exchange of g per iteration and of the R objectives per batch through
+    # the ranks' inboxes): `world` ranks co-resident on one device, one cooperative launch (imrt_plan_run_ranks).
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_0908_4421_b200 as m
+    prob = synth_inputs.make_phantom(cfg)
+    ranks = sharded.CoResidentRanks(prob, world, max_iters=n)
+    ranks.set_x(prob.x0)
+    ranks.run_iters(n // 2)
+    ranks.run_iters(n - n // 2)                      # resumable: sequence numbers and inboxes carry over between launches
+    traces = [ranks.trace(q) for q in range(world)]
+    tr = traces[0]
+    assert tr.n_iters == n and tr.stop_reason == oracle.STOP_MAX_ITERS
+    for q in range(1, world):                        # the ranks hold the same bits: same sums, same order, same decisions
+        np.testing.assert_array_equal(traces[q].obj, tr.obj)
+        np.testing.assert_array_equal(traces[q].n_trials, tr.n_trials)
+        np.testing.assert_array_equal(traces[q].step_sq, tr.step_sq)
+        np.testing.assert_array_equal(ranks.get_x(q).cpu().numpy(), ranks.get_x(0).cpu().numpy())
+    # against the oracle on the WHOLE problem, follow mode
+    fol = oracle.run(prob, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
+    assert fol.n_follow_violations == 0
+    np.testing.assert_array_equal(tr.lam, fol.lam)
+    assert np.abs(tr.obj - fol.obj).max() <= 1e-4 * fol.obj.max() and abs(tr.obj[-1] - fol.obj[-1]) <= 1e-4 * fol.obj[-1]
+    d = ranks.get_dose().cpu().numpy().astype(np.float64)
+    d_o = oracle.eval_objective(prob, fol.x)[0]
+    assert np.abs(d - d_o).max() <= 0.005 * 70.0
+    # and against the single-plan loop of the same library: same trial counts
+    plan = m.Plan(prob, max_iters=n)
+    plan.set_x(prob.x0)
+    plan.run_iters(n)
+    np.testing.assert_array_equal(plan.trace().n_trials, tr.n_trials)
+    np.testing.assert_allclose(plan.trace().obj, tr.obj, rtol=2e-5)
+    plan.close()
+    ranks.close()
+
+
+@pytest.mark.gpu
+def test_sharded_run_to_tolerance_and_refusals():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_0908_4421_b200 as m
+    prob = synth_inputs.make_phantom(0)
+    ranks = sharded.CoResidentRanks(prob, 2, max_iters=400)
+    ranks.set_x(prob.x0)
+    ranks.run_to_tol(1e-3, 400)
+    tr = ranks.trace()
+    ref = oracle.run(prob, n_iters=400, delta=1e-3)
+    assert tr.stop_reason == oracle.STOP_TOLERANCE and abs(tr.n_iters - ref.n_iters) <= 1
+    with pytest.raises(m.ImrtError):                 # a rank of a sharded problem cannot run alone on this device's stream
+        m.imrt_plan_run_ranks([ranks.plans[0].handle], 1)
+    ranks.close()
+    solo = m.Plan(prob, max_iters=4, driver=m.DRIVER_GRAPH)
+    with pytest.raises(m.ImrtError):
+        m.imrt_plan_set_shard(solo.handle, 0, 2, [16, 32])           # persistent driver only
+    solo.close()
