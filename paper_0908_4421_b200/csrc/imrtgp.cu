@@ -380,8 +380,10 @@ __global__ void k_pack_blocks(const int4* __restrict__ pk, const uint32_t* __res
                 const int q0 = row_ptr[row], q1 = row_ptr[row + 1];
                 for (int p = q0 + lane; p < q1; p += 32) {
                     const int c = col[p];
-                    const int pos = off + (int)pre[c >> 5] + __popc(bm[c >> 5] & ((1u << (c & 31)) - 1u));
-                    val_o[(size_t)pos * 4 + (row - ra)] = val[p];
+                    const int rank = (int)pre[c >> 5] + __popc(bm[c >> 5] & ((1u << (c & 31)) - 1u));     // position inside the quad
+                    const int pos = off + rank;
+                    // rows rotated by bits 3 and 2 of the position: the dose pass's row-splitting butterfly needs no selects
+                    val_o[(size_t)pos * 4 + ((row - ra) ^ (((rank >> 3) & 1) * 2 + ((rank >> 2) & 1)))] = val[p];
                     col_o[pos] = (unsigned short)c;
                 }
             }

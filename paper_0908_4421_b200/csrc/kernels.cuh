@@ -113,7 +113,8 @@ struct DevPlan {
     //   header  uint32[4]  {quads, first row (a multiple of 4), 1, union columns}
     //   quads   uint32[2 (quads + 1)]  {column offset of the quad (low 16 bits) | row-exists mask << 16,
     //                                   the 4 structure ids}; the last pair holds the total; padded to 4 words
-    //   val     fp32[columns + 1][4]   per union column the 4 rows' values; one zero column at the end
+    //   val     fp32[columns + 1][4]   per union column the 4 rows' values, slot j = row j ^ (2 b3 + b2) with b3 b2 = bits 3, 2
+    //                                  of the column's position inside its quad (dose_block_quads); one zero column at the end
     //   col     uint16[columns + 8]
     // One record is consumed by ONE warp.
     const unsigned char* pack;
@@ -445,7 +446,8 @@ template <int R> __device__ __forceinline__ bool quad_owner(int lane) { return (
 // The reduction is one xor butterfly over the 16 lanes of a half-warp for every (row, trial) sum -- the same tree of
 // additions whatever R is -- but at each step a lane keeps only half of what it holds: xor 8 splits the rows
 // {0,1} | {2,3}, xor 4 leaves one row, xor 2 / xor 1 split the trial points (R = 4; xor 2 only for R = 2).  4 R - 1
-// shuffles for two quads, and lane (b4 b3 b2 b1 b0) ends with row 2 b3 + b2 of trial 2 b1 + b0 of quad b4.
+// shuffles for two quads, and lane (b4 b3 b2 b1 b0) ends with row 2 b3 + b2 of trial 2 b1 + b0 of quad b4.  The
+// packing rotates the rows of every column so that the two row-splitting steps need no selects (see below).
 // my_r: the residual buffer of this lane's trial.  Gq: this lane's objective partial (of its own trial).
 template <int R>
 __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict__ rec, const unsigned char* __restrict__ xs_b,
@@ -469,18 +471,38 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
         const uint2 w = *reinterpret_cast<const uint2*>(qt + 2 * qi);
         int s = (int)(w.x & 0xFFFFu), e = (int)(qt[2 * qi + 2] & 0xFFFFu);
         if (lone) {
-            const int mid = s + ((e - s + 1) >> 1);
+            // the cut is a multiple of 16 columns after s: lane l16 then takes the columns at positions = l16 (mod 16) of
+            // the quad in BOTH halves, which is what the packed row rotation (below) is keyed to
+            const int mid = min(e, s + 16 * ((e - s + 31) >> 5));
             if (half) s = mid; else e = mid;
         }
         const int len = e - s;
-        const int trips = max(len, __shfl_xor_sync(0xffffffffu, len, 16));
+        const int olen = __shfl_xor_sync(0xffffffffu, len, 16);
+        const int trips = max(len, olen);
+        const int n_fast = min(len, olen) >> 4;            // trips in which BOTH halves have a full 16 columns: no clamping
         // rows {0,1} and {2,3} of a trial are kept as register pairs: one packed multiply-add (FFMA2, the trial value as
         // its broadcast operand) does two rows -- 2 R instead of 4 R issue slots per column, each half an IEEE fma
         float2 acc01[R], acc23[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) acc01[r] = acc23[r] = make_float2(0.0f, 0.0f);
+        {
+            const unsigned char* vp = val_b + 16 * (s + l16);
+            const unsigned char* cp = col_b + 2 * (s + l16);
 #pragma unroll 2
-        for (int t0 = 0; t0 < trips; t0 += 16) {
+            for (int i = 0; i < n_fast; ++i, vp += 256, cp += 32) {
+                const float4 v = *reinterpret_cast<const float4*>(vp);
+                const uint32_t c = *reinterpret_cast<const unsigned short*>(cp);
+                XVec<R> x;
+                x.load(xs_b + c * XB);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float2 xr = make_float2(x.v[r], x.v[r]);
+                    acc01[r] = __ffma2_rn(make_float2(v.x, v.y), xr, acc01[r]);
+                    acc23[r] = __ffma2_rn(make_float2(v.z, v.w), xr, acc23[r]);
+                }
+            }
+        }
+        for (int t0 = 16 * n_fast; t0 < trips; t0 += 16) {      // the ragged end: at most a few trips per pair
             const int k = s + t0 + l16;
             const int kk = k < e ? k : nbc;                // past the quad's end: the zero column
             const float4 v = *reinterpret_cast<const float4*>(val_b + 16 * kk);
@@ -494,12 +516,16 @@ __device__ __forceinline__ void dose_block_quads(const unsigned char* __restrict
                 acc23[r] = __ffma2_rn(make_float2(v.z, v.w), xr, acc23[r]);
             }
         }
+        // The record stores the 4 rows' values of the column at position p of its quad ROTATED: slot j holds row
+        // j ^ (2 b3 + b2), b3 b2 = bits 3 and 2 of p -- and p = l16 (mod 16) for the lane that takes the column.  So in every
+        // lane slot 0 already holds the row the lane ends up with (2 b3 + b2), slot 1 its xor-4 partner's row, slots 2, 3 its
+        // xor-8 partner's rows: the row-splitting steps keep the low slots and send the high ones, with no selects.
         float h[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float a0 = (hi8 ? acc23[r].x : acc01[r].x) + __shfl_xor_sync(0xffffffffu, hi8 ? acc01[r].x : acc23[r].x, 8);
-            const float a1 = (hi8 ? acc23[r].y : acc01[r].y) + __shfl_xor_sync(0xffffffffu, hi8 ? acc01[r].y : acc23[r].y, 8);
-            h[r] = (hi4 ? a1 : a0) + __shfl_xor_sync(0xffffffffu, hi4 ? a0 : a1, 4);
+            const float a0 = acc01[r].x + __shfl_xor_sync(0xffffffffu, acc23[r].x, 8);
+            const float a1 = acc01[r].y + __shfl_xor_sync(0xffffffffu, acc23[r].y, 8);
+            h[r] = a0 + __shfl_xor_sync(0xffffffffu, a1, 4);
         }
         float d;
         if (R == 4) {
