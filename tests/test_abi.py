@@ -130,3 +130,11 @@ def test_product_and_oracle_share_nothing():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_0908_4421_b200" not in text and "from paper_0908_4421_b200" not in text, f
             assert "imrtgp.h" not in text and "libimrtgp" not in text, f
+
+
+def test_the_library_reads_no_environment_variables():
+    # every switch of the library is a field of imrt_params / imrt_options (include/imrtgp.h): no getenv in csrc/
+    import glob
+    for path in glob.glob(os.path.join(ROOT, "paper_0908_4421_b200", "csrc", "*")):
+        with open(path) as f:
+            assert "getenv" not in f.read(), path
