@@ -17,6 +17,7 @@ from dataclasses import dataclass
 import numpy as np
 
 from . import build as _build
+from . import sharded  # noqa: E402,F401  (row-sharded set-up: slab selection, inboxes)
 
 __all__ = ["Plan", "ImrtError", "lib", "Params", "Options", "STATUS_NAMES", "STOP_NAMES", "EXPORTS"]
 
