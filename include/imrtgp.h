@@ -363,7 +363,7 @@ const char* imrt_last_error(const imrt_plan* plan);
 /* Release host-side resources (graph, events).  Device memory belongs to the caller. */
 imrt_status imrt_plan_destroy(imrt_plan* plan);
 
-/* Library version string, e.g. "imrtgp 0.1 (sm_100a)". */
+/* Library version string, e.g. "imrtgp 0.2 (sm_100a)". */
 const char* imrt_version(void);
 
 #ifdef __cplusplus

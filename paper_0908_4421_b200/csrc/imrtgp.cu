@@ -938,7 +938,7 @@ struct PhaseTimer {
 // ------------------------------------------------------------------------------------------------ C-ABI
 extern "C" {
 
-const char* imrt_version(void) { return "imrtgp 0.1 (sm_100a)"; }
+const char* imrt_version(void) { return "imrtgp 0.2 (sm_100a)"; }
 
 const char* imrt_last_error(const imrt_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
 

@@ -694,122 +694,10 @@ __device__ __forceinline__ void reduce_objective(const DevPlan& P, const double*
 // a CTA-wide barrier.  Every consumer warp observes EVERY stage's full barrier and arrives on its empty barrier
 // (count W_CONS), so the producer can never refill a slot before all warps have seen its phase.
 
-// ---- plain 32-bit CSR stream (DevPlan::id16 == 0; rows are not padded, a slice may span several rows): the consumer
-// warps take the stages in two alternating groups of 8, each warp a contiguous 512-entry slice.
-__device__ __forceinline__ void transpose_pass_csr(const DevPlan& P, SmemHeader* h, unsigned char* smem, double* wpart,
-                                                   const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int S = P.n_stages_t;
-    unsigned char* stages = smem + P.stage_off;
-    unsigned int it = pipe.it_t;
-    const int rg0 = (h->cta < P.grid_t) ? P.cta_rng[h->cta] : 0;       // this CTA's ranges
-    const int rg1 = (h->cta < P.grid_t) ? P.cta_rng[h->cta + 1] : 0;
-    const unsigned long long t_start = global_ns();
-    int s = (int)(it % (unsigned int)S);
-    unsigned int ph = (it / (unsigned int)S) & 1u;
-
-    if (warp >= W_CONS) {
-        const uint64_t pol = policy_evict_first();
-        for (int rg = rg0; rg < rg1; ++rg) {
-            const int e0 = P.tr_range[rg].e_begin, e1 = P.tr_range[rg].e_end;
-            for (int cs = e0; cs < e1; cs += CHUNK_T, ++it) {
-                if (warp == W_CONS && lane == 0) {
-                    mbar_wait(&h->empty_t[s], ph ^ 1u);
-                    int n = e1 - cs;
-                    n = n > CHUNK_T ? CHUNK_T : n;
-                    unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
-                    const int shift = e0 & 3;   // 16-byte source alignment: start the copy up to 3 entries early
-                    const uint32_t bytes = (uint32_t)((n + shift + 3) & ~3) * 4u;   // D^T is padded: always in bounds
-                    int* col_s = reinterpret_cast<int*>(st);
-                    float* val_s = reinterpret_cast<float*>(col_s + CHUNK_T_PAD);
-                    mbar_expect_tx(&h->full_t[s], 2u * bytes);
-                    bulk_g2s(col_s, P.colT + (cs - shift), bytes, &h->full_t[s], pol);
-                    bulk_g2s(val_s, P.valT + (cs - shift), bytes, &h->full_t[s], pol);
-                }
-                if (++s == S) { s = 0; ph ^= 1u; }
-            }
-        }
-    } else {
-        const uint64_t keep = policy_evict_last();
-        for (int rg = rg0; rg < rg1; ++rg) {
-            const TrRange R = P.tr_range[rg];
-            for (int i = threadIdx.x; i < RL_MAX * W_CONS; i += N_CONS) wpart[i] = 0.0;
-            named_bar_sync(1, N_CONS);
-            int cur_row = R.first_row;
-            int cur_end = __ldg(P.rowT_ptr + cur_row + 1);
-            double dacc = 0.0;
-            bool touched = false;
-            for (int cs = R.e_begin; cs < R.e_end; cs += CHUNK_T, ++it) {
-                mbar_wait(&h->full_t[s], ph);
-                if ((int)(it % TGROUPS) == warp / (W_CONS / TGROUPS)) {      // this group's stage
-                    const unsigned char* st = stages + (size_t)s * (size_t)P.stage_t_bytes;
-                    const int* col_s = reinterpret_cast<const int*>(st) + (R.e_begin & 3);
-                    const float* val_s = reinterpret_cast<const float*>(st) + CHUNK_T_PAD + (R.e_begin & 3);
-                    const int ce = min(cs + CHUNK_T, R.e_end);
-                    int pos = cs + (warp % (W_CONS / TGROUPS)) * SLICE_T;
-                    const int b = min(pos + SLICE_T, ce);
-                    while (pos < b) {
-                        while (cur_end <= pos) {   // the slice moved past the end of the current row (warp-uniform)
-                            if (touched) {
-                                const double sum = warp_sum(dacc);
-                                if (lane == 0) wpart[(cur_row - R.first_row) * W_CONS + warp] = sum;
-                                dacc = 0.0;
-                                touched = false;
-                            }
-                            ++cur_row;
-                            cur_end = __ldg(P.rowT_ptr + cur_row + 1);
-                        }
-                        const int seg_end = min(b, cur_end);
-                        const int* cp = col_s + (pos - cs);
-                        const float* vp = val_s + (pos - cs);
-                        float acc = 0.0f;
-                        if (seg_end - pos == SLICE_T) {
-                            int c[SLICE_T / 32];
-                            float rr[SLICE_T / 32];
-#pragma unroll
-                            for (int u = 0; u < SLICE_T / 32; ++u) c[u] = cp[lane + 32 * u];
-#pragma unroll
-                            for (int u = 0; u < SLICE_T / 32; ++u) rr[u] = ld_keep(r_in + c[u], keep);
-#pragma unroll
-                            for (int u = 0; u < SLICE_T / 32; ++u) acc = fmaf(vp[lane + 32 * u], rr[u], acc);
-                        } else {
-                            for (int k = lane; k < seg_end - pos; k += 32) acc = fmaf(vp[k], ld_keep(r_in + cp[k], keep), acc);
-                        }
-                        dacc += (double)acc;
-                        touched = true;
-                        pos = seg_end;
-                    }
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&h->empty_t[s]);    // consumed or only observed: either way this warp is done with it
-                if (++s == S) { s = 0; ph ^= 1u; }
-            }
-            if (touched) {
-                const double sum = warp_sum(dacc);
-                if (lane == 0) wpart[(cur_row - R.first_row) * W_CONS + warp] = sum;
-            }
-            named_bar_sync(1, N_CONS);
-            for (int t = threadIdx.x; t < R.n_rows; t += N_CONS) {
-                double sum = 0.0;
-#pragma unroll
-                for (int w = 0; w < W_CONS; ++w) sum += wpart[t * W_CONS + w];
-                gslot[R.slot_base + t] = sum;
-            }
-            named_bar_sync(1, N_CONS);
-        }
-    }
-    pipe.it_t = it;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        P.cta_ns[2048 + 2 * h->cta] = t_start;
-        P.cta_ns[2048 + 2 * h->cta + 1] = global_ns();
-    }
-}
-
-// ---- packed streams: voxel ids as 16-bit offsets from one 32-bit base per aligned group of 32 entries, rows padded to 128
-// entries, 4,096-entry stages taken by the consumer warps in two alternating groups of 8 (a contiguous 512-entry slice and
-// 16 gathers of r in flight per lane).  A software-pipelined variant (every warp a 128-entry slice of every stage, values
+// ---- single rows.  ID16 = false: the plain 32-bit CSR (rows are not padded, a slice may span several rows, a range may
+// start at any multiple of 4 entries).  ID16 = true: the packed stream -- voxel ids as 16-bit offsets from one 32-bit
+// base per aligned group of 32 entries, rows padded to 128 entries.  4,096-entry stages taken by the consumer warps in
+// two alternating groups of 8 (a contiguous 512-entry slice and 16 gathers of r in flight per lane).  A software-pipelined variant (every warp a 128-entry slice of every stage, values
 // parked in registers, multiply-adds four stages later) measured no faster in isolation and slower inside the persistent
 // kernel (register pressure): the pass is bound by L2 throughput -- the stream plus the r gathers -- not by latency.
 template <bool ID16>
@@ -1100,7 +988,7 @@ __device__ __forceinline__ void transpose_pass(const DevPlan& P, SmemHeader* h, 
                                                const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
     if (P.id16 == 2) transpose_pass_pairs<false>(P, h, smem, wpart, r_in, gslot, pipe);
     else if (P.id16) transpose_pass_rows<true>(P, h, smem, wpart, r_in, gslot, pipe);
-    else transpose_pass_csr(P, h, smem, wpart, r_in, gslot, pipe);
+    else transpose_pass_rows<false>(P, h, smem, wpart, r_in, gslot, pipe);
 }
 
 // g_i = sum of the slots of row i, in slot order (fixed).  All NTHREADS threads; g_out shared or global.
