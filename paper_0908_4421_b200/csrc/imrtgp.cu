@@ -520,14 +520,18 @@ __global__ void k_fill_zero_dose_rows(const uint8_t* __restrict__ sid, const flo
     if (d) d[j] = 0.0f;
 }
 
-// The constants of the rows no record covers (dose 0 whatever x is): their objective, State::G_skip, summed in a fixed
-// order by ONE block, and their residual in every residual buffer of the loop.  Runs at plan creation and whenever
-// the per-voxel limits change.
-__global__ void k_skip_constants(const uint8_t* __restrict__ sid, const unsigned char* __restrict__ covered,
-                                 const float4* __restrict__ table, State* st, int n_v, const RPtrs R) {
+// The constants of the rows no record covers (dose 0 whatever x is): their objective, State::G_skip, and their residual
+// in every residual buffer of the loop.  Runs at plan creation and whenever the per-voxel limits change.  The objective
+// is summed in a fixed order: every block adds its rows (thread-strided, warp butterfly, warps in order) into part[block],
+// k_skip_final adds the blocks' partials in block order.
+constexpr int SKIP_BLOCKS = 128;
+__global__ void __launch_bounds__(1024) k_skip_constants(const uint8_t* __restrict__ sid, const unsigned char* __restrict__ covered,
+                                                         const float4* __restrict__ table, const State* st, int n_v, const RPtrs R, double* part) {
     __shared__ double red[32];
     double acc = 0.0;
-    for (int j = threadIdx.x; j < n_v; j += blockDim.x) {
+    const int per = (n_v + gridDim.x - 1) / gridDim.x;            // a contiguous chunk of rows per block
+    const int j0 = blockIdx.x * per, j1 = min(n_v, j0 + per);
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         if (covered[j]) continue;
         float4 t = table[sid[j]];
         if (st->tvu) t.x = st->tvu[j];
@@ -546,8 +550,13 @@ __global__ void k_skip_constants(const uint8_t* __restrict__ sid, const unsigned
     if (threadIdx.x == 0) {
         double s = 0.0;
         for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += red[w];
-        st->G_skip = s;
+        part[blockIdx.x] = s;
     }
+}
+__global__ void k_skip_final(const double* __restrict__ part, int n, State* st) {
+    double s = 0.0;
+    for (int b = 0; b < n; ++b) s += part[b];
+    st->G_skip = s;
 }
 
 __global__ void k_check_x(const float* __restrict__ x, int n_b, State* st) {
@@ -1295,7 +1304,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         RPtrs rp_all;
         for (int i = 0; i <= R_MAX; ++i) rp_all.p[i] = L.rbuf[i];
         k_fill_zero_dose_rows<<<(int)((n_v + 255) / 256), 256, 0, st>>>(structure_id, L.table, L.st, (int)n_v, rp_all, nullptr);
-        k_skip_constants<<<1, 1024, 0, st>>>(structure_id, L.covered, L.table, L.st, (int)n_v, rp_all);
+        k_skip_constants<<<SKIP_BLOCKS, 1024, 0, st>>>(structure_id, L.covered, L.table, L.st, (int)n_v, rp_all, L.Gpart[1]);
+        k_skip_final<<<1, 1, 0, st>>>(L.Gpart[1], SKIP_BLOCKS, L.st);
     }
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaStreamSynchronize(st));
@@ -1378,7 +1388,8 @@ imrt_status imrt_plan_set_voxel_limits(imrt_plan* pl, const float* t_under_v, co
     k_set_limits<<<1, 1, 0, st>>>(pl->P.st, t_under_v, t_over_v);
     RPtrs rp_all;
     for (int i = 0; i <= R_MAX; ++i) rp_all.p[i] = pl->P.rbuf[i];
-    k_skip_constants<<<1, 1024, 0, st>>>(pl->sid, pl->P.covered, pl->P.table, pl->P.st, pl->P.n_v, rp_all);
+    k_skip_constants<<<SKIP_BLOCKS, 1024, 0, st>>>(pl->sid, pl->P.covered, pl->P.table, pl->P.st, pl->P.n_v, rp_all, pl->P.Gpart[1]);
+    k_skip_final<<<1, 1, 0, st>>>(pl->P.Gpart[1], SKIP_BLOCKS, pl->P.st);
     CUDA_TRY(pl, cudaGetLastError());
     pl->has_x = false;     // G(x_1), r(x_1) belong to the old limits
     return IMRT_STATUS_OK;
