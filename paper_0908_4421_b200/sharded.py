@@ -132,7 +132,7 @@ class PeerRank:
         nbytes = imrt_shard_inbox_bytes(int(prob.n_b), self.world)
         self.inbox = symm_mem.empty(nbytes, dtype=torch.uint8, device=self.device)
         self.inbox.zero_()
-        self.handle = symm_mem.rendezvous(self.inbox, group=(group.group_name if group is not None else dist.group.WORLD.group_name))
+        self.handle = symm_mem.rendezvous(self.inbox, group if group is not None else dist.group.WORLD)
         torch.cuda.synchronize(self.device)
         dist.barrier(group)                          # every inbox is zero before anybody pushes
         imrt_plan_set_shard(self.plan.handle, self.rank, self.world, [int(p) for p in self.handle.buffer_ptrs])
