@@ -45,8 +45,10 @@ constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int TARGET_RECORDS = 8192;          // a small matrix is cut into at least about this many records (imrtgp.cu)
 constexpr int ZPAD = 4;                       // zero slots after a block's last row: where lanes past a row's end read
 constexpr int R_MAX = 4;                      // line-search trial points evaluated per dose pass (1, 2 or 4)
-constexpr int CHUNK_T = 4096;                 // nnz per transpose-pass stage (pure streaming)
-constexpr int TGROUPS = 2;                    // the consumer warps take the stages in turns, in this many groups:
+constexpr int CHUNK_T = 2048;                 // entries per transpose-pass stage: 4 groups x 4 warps x 512-entry slices.  (Stages of
+                                              // 4,096 entries for 2 groups of 8 warps hold the same 16 slices but hand the ring back in
+                                              // 41 KB steps: 4 % slower; 1,024 entries for 8 groups of 2: 20 % slower.)
+constexpr int TGROUPS = 4;                    // the consumer warps take the stages in turns, in this many groups:
 constexpr int SLICE_T = CHUNK_T / (W_CONS / TGROUPS);   // contiguous nnz per warp of a stage's group (gathers in flight)
 constexpr int CHUNK_T_PAD = CHUNK_T + 4;            // + alignment shift of a range start (<= 3 entries)
 constexpr int STAGE_T_BYTES = CHUNK_T_PAD * 8;
@@ -696,8 +698,9 @@ __device__ __forceinline__ void reduce_objective(const DevPlan& P, const double*
 
 // ---- single rows.  ID16 = false: the plain 32-bit CSR (rows are not padded, a slice may span several rows, a range may
 // start at any multiple of 4 entries).  ID16 = true: the packed stream -- voxel ids as 16-bit offsets from one 32-bit
-// base per aligned group of 32 entries, rows padded to 128 entries.  4,096-entry stages taken by the consumer warps in
-// two alternating groups of 8 (a contiguous 512-entry slice and 16 gathers of r in flight per lane).  A software-pipelined variant (every warp a 128-entry slice of every stage, values
+// base per aligned group of 32 entries, rows padded to 128 entries.  2,048-entry stages taken in turns by four groups
+// of 4 consumer warps (a contiguous 512-entry slice and 16 gathers of r in flight per lane): 4 stages are being
+// consumed while the other 4 of the ring are in flight, and the ring is handed back to the producer in 20 KB steps.  A software-pipelined variant (every warp a 128-entry slice of every stage, values
 // parked in registers, multiply-adds four stages later) measured no faster in isolation and slower inside the persistent
 // kernel (register pressure): the pass is bound by L2 throughput -- the stream plus the r gathers -- not by latency.
 template <bool ID16>
