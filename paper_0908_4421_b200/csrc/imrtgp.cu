@@ -1249,7 +1249,8 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         P.stage_off = off;
         avail = smem_optin - off;
         avail = (smem_optin - off) & ~127;
-        stt = avail > 0 ? std::min(MAX_STAGES_T, avail / stage_t) : 0;
+        P.tr_stage_off = (P.x_off + 127) & ~127;
+        stt = avail > 0 ? std::min(MAX_STAGES_T, (off + avail - P.tr_stage_off) / stage_t) : 0;
         if (R == 1 || (avail >= 2 * max_rec && avail >= (W_CONS / 2) * avg_rec && stt >= 2)) break;
     }
     if (avail < 2 * max_rec || stt < 2)

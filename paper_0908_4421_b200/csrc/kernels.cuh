@@ -174,7 +174,9 @@ struct DevPlan {
     int wpart_off;             // byte offsets into dynamic shared memory: transpose per-(row, warp) partials,
     int dsc_off;               // dose-pass per-warp scratch,
     int x_off, g_off;          // the trial points x+ [n_b][R] (gathered by the dose pass) and the gradient (persistent kernel)
-    int stage_off;             // byte offset of the stage ring
+    int stage_off;             // byte offset of the dose pass's ring
+    int tr_stage_off;          // byte offset of the transpose pass's stages: they also cover the trial points and g, which are
+                               // dead while a transpose pass runs (both are rebuilt right after it)
 };
 
 struct PassArgs {
@@ -708,7 +710,7 @@ __device__ __forceinline__ void transpose_pass_rows(const DevPlan& P, SmemHeader
                                                const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = P.n_stages_t;
-    unsigned char* stages = smem + P.stage_off;
+    unsigned char* stages = smem + P.tr_stage_off;
     unsigned int it = pipe.it_t;
     const int rg0 = (h->cta < P.grid_t) ? P.cta_rng[h->cta] : 0;       // this CTA's ranges
     const int rg1 = (h->cta < P.grid_t) ? P.cta_rng[h->cta + 1] : 0;
@@ -860,7 +862,7 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
                                                      const float* __restrict__ r_in, double* gslot, Pipe& pipe) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = P.n_stages_t;
-    unsigned char* stages = smem + P.stage_off;
+    unsigned char* stages = smem + P.tr_stage_off;
     unsigned int it = pipe.it_t;
     const int rg0 = (h->cta < P.grid_t) ? P.cta_rng[h->cta] : 0;
     const int rg1 = (h->cta < P.grid_t) ? P.cta_rng[h->cta + 1] : 0;
