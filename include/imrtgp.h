@@ -105,7 +105,7 @@ typedef struct imrt_options {
     int32_t col_bits;          /* 0: 16-bit column indices when n_b <= 65,536;  32: always 32-bit                     */
     int32_t transpose_format;  /* 0: smallest of {row pairs, single rows} with 16-bit voxel offsets, else plain CSR;
                                   1: single rows with 16-bit offsets (no pairs);  2: the plain 32-bit D^T CSR         */
-    int32_t quad_cap;          /* union columns per quad record at most (0 = default, 576; clamped to [32, 4096])     */
+    int32_t quad_cap;          /* union columns per quad record at most (0 = default, 384; clamped to [32, 4096])     */
     int32_t n_ctas;            /* CTAs of the persistent passes: 0 = one per SM of the device; fewer leaves SMs to other work
                                   (or to other ranks of a row-sharded problem sharing the device, imrt_plan_run_ranks)   */
     int32_t profile_create;    /* 1: synchronise after every phase of plan creation and keep the phase times for

@@ -598,7 +598,8 @@ static RecordCaps record_caps(int64_t n_v, int64_t nnz, int64_t ring_est, int qu
     c.chunk_slots = clampi((nnz / TARGET_RECORDS + 3) & ~(int64_t)3, 64, ROW_REC_SLOTS);
     c.max_rows = clampi(n_v / TARGET_RECORDS, 8, MAXROWS_F);
     // quad records: at least one per consumer warp must fit in the ring (18 bytes per union column); measured on the
-    // 9- and 15-field phantoms, 480 .. 576 columns (8 .. 10 KB, mostly 4 quads = 2 warp trips) is the sweet spot
+    // 9- and 15-field phantoms, 384 .. 448 columns (~7 KB) is the sweet spot: 16 records being consumed then hold ~110 KB
+    // of the ring and ~60 KB stay in flight (576 columns, best with round 1's heavier quad loop, leave ~30 KB: 3 % slower)
     const int cap = quad_cap_user > 0 ? std::max(32, std::min(quad_cap_user, 4096)) : QUAD_CAP;
     c.quad_cap = clampi(std::min<int64_t>(nnz / 3 / TARGET_RECORDS, ring_est / (W_CONS * 18)), 32, cap);
     // a single quad may exceed quad_cap (it then fills a record by itself), but two such records must fit in the ring

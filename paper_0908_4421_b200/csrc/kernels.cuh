@@ -39,7 +39,7 @@ constexpr int ROW_REC_SLOTS = 1024;           // slots per row-format record (fe
 constexpr int MAX_CHUNK_SLOTS = 8192;         // longest row of D this build handles (slot offsets are 16-bit)
 constexpr int MAXROWS_F = 256;                // rows per block
 constexpr int QUAD_MAX_NB = 16384;            // quad-format records are offered up to this many beamlets (pack-kernel bitmap)
-constexpr int QUAD_CAP = 576;                 // union columns per quad record, at most (see record_caps)
+constexpr int QUAD_CAP = 384;                 // union columns per quad record, at most (see record_caps)
 constexpr int QUAD_MAXQ = 64;                 // quads per record
 constexpr int SEG_ROWS = 256;                 // rows per format decision
 constexpr int TARGET_RECORDS = 8192;          // a small matrix is cut into at least about this many records (imrtgp.cu)
