@@ -1090,9 +1090,12 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     CUDA_TRY(pl, cudaGetLastError());
     CUDA_TRY(pl, cudaMemcpyAsync(flags_h, L.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(pl, cudaMemcpyAsync(&tot, L.totals, sizeof tot, cudaMemcpyDeviceToHost, st));
-    cudaEvent_t ev_totals;
-    CUDA_TRY(pl, cudaEventCreateWithFlags(&ev_totals, cudaEventDisableTiming));
-    CUDA_TRY(pl, cudaEventRecord(ev_totals, st));
+    struct Event {             // released on every path out of this function
+        cudaEvent_t e = nullptr;
+        ~Event() { if (e) cudaEventDestroy(e); }
+    } ev_totals;
+    CUDA_TRY(pl, cudaEventCreateWithFlags(&ev_totals.e, cudaEventDisableTiming));
+    CUDA_TRY(pl, cudaEventRecord(ev_totals.e, st));
     // ---- explicit transpose: stable radix sort of (column, position) pairs, then gather (north star choice 1).
     // Enqueued before the host waits for the layout totals: the device sorts while the host sizes the next launches.
     CUDA_TRY(pl, cudaMemsetAsync(L.colT, 0, sizeof(int) * B.nnz_pad, st));
@@ -1114,8 +1117,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
         CUDA_TRY(pl, cudaMemsetAsync(L.rowT_ptr, 0, sizeof(int) * (n_b + 1), st));
     }
     {
-        const cudaError_t e = cudaEventSynchronize(ev_totals);
-        cudaEventDestroy(ev_totals);
+        const cudaError_t e = cudaEventSynchronize(ev_totals.e);
         if (e != cudaSuccess) { cudaStreamSynchronize(st); return fail(pl, IMRT_STATUS_CUDA_ERROR, "layout: %s", cudaGetErrorString(e)); }
     }
     if (flags_h[3]) { cudaStreamSynchronize(st); return fail(pl, IMRT_STATUS_BAD_CSR, "column indices are not strictly ascending inside a row"); }
