@@ -138,3 +138,17 @@ def test_the_library_reads_no_environment_variables():
     for path in glob.glob(os.path.join(ROOT, "paper_0908_4421_b200", "csrc", "*")):
         with open(path) as f:
             assert "getenv" not in f.read(), path
+
+
+def test_shard_inbox_size_and_refusals_host_only():
+    # imrt_shard_inbox_bytes is host arithmetic: flags for 16 ranks (2 x 128 B), the objective slots
+    # (2 parities x 16 ranks x 4 trial points x 8 B) and 2 parities x world x n_b (padded to 32) fp32 gradient partials
+    assert imrt.imrt_shard_inbox_bytes(2304, 2) == 256 + 1024 + 2 * 2 * 2304 * 4
+    assert imrt.imrt_shard_inbox_bytes(5, 3) == 256 + 1024 + 2 * 3 * 32 * 4
+    L = imrt.lib()
+    n = ctypes.c_size_t(0)
+    assert imrt.STATUS_NAMES[L.imrt_shard_inbox_bytes(100, 17, ctypes.byref(n))] == "INVALID_ARG"      # at most 16 ranks
+    assert imrt.STATUS_NAMES[L.imrt_plan_set_shard(None, 0, 2, None)] == "INVALID_ARG"
+    assert imrt.STATUS_NAMES[L.imrt_plan_run_ranks(None, 2, 1, 0.0)] == "INVALID_ARG"
+    assert imrt.STATUS_NAMES[L.imrt_merge_rows_workspace_bytes(0, 1, ctypes.byref(n))] == "INVALID_ARG"
+    assert imrt.imrt_merge_rows_workspace_bytes(1000, 10) > 5 * 4 * 1000
