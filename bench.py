@@ -391,7 +391,7 @@ def run_ours(args):
                 "data": "synthetic",
                 "config": {"workload": prob.name, "n_v": prob.n_v, "n_b": prob.n_b, "nnz": prob.nnz,
                            "nonempty_rows": info["nonempty_rows"], "lambda0": prob.lambda0, "eps": prob.eps, "alpha": prob.alpha,
-                           "driver": args.driver, "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
+                           "driver": args.driver, "tune_level": args.tune_level, "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
                            "l2": extra.get("flush"), "trials_per_iter": trials_timed / K, "ls_batch": R,
                            "fwd_passes_timed": passes_timed, "tr_passes_timed": K},
                 "clocks": clocks, "gpu_launches": n_launch, "plan_create_s": plan_create_s,
