@@ -207,9 +207,8 @@ imrt_status imrt_plan_eval_batch(imrt_plan* plan, int32_t n_points, const float*
 
 /*
  * g = D^T r for an arbitrary r (fp32 [n_v], device) -> g (fp32 [n_b], device): one transpose pass, the optimiser state is
- * not touched.  With imrt_plan_eval (which leaves r(x)) and imrt_trial_point this is what a host-driven loop over
- * several plans -- one per row slab of D, on one GPU each -- is made of: the partial objectives and gradients of the
- * slabs add up (paper_0908_4421_b200/sharded.py).  Asynchronous.
+ * not touched.  A parity hook (the transpose pass in isolation); with imrt_plan_eval and imrt_trial_point it is also all a
+ * host-driven loop over row slabs needs (tests/host_sharded_loop.py restates the sharded protocol that way).  Asynchronous.
  */
 imrt_status imrt_plan_gradient(imrt_plan* plan, const float* r, float* g);
 
