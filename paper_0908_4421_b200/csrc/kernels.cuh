@@ -847,7 +847,7 @@ __device__ __forceinline__ void transpose_pass_rows(const DevPlan& P, SmemHeader
         }
     }
     pipe.it_t = it;
-    __threadfence();
+    // (the slots become visible to the other CTAs through the release that follows: the grid barrier's, or the ticket's)
     __syncthreads();
     if (threadIdx.x == 0) {
         P.cta_ns[2048 + 2 * h->cta] = t_start;
@@ -981,7 +981,7 @@ __device__ __forceinline__ void transpose_pass_pairs(const DevPlan& P, SmemHeade
         }
     }
     pipe.it_t = it;
-    __threadfence();
+    // (the slots become visible to the other CTAs through the release that follows: the grid barrier's, or the ticket's)
     __syncthreads();
     if (threadIdx.x == 0) {
         P.cta_ns[2048 + 2 * h->cta] = t_start;
@@ -1175,7 +1175,9 @@ __device__ __forceinline__ void loop_store(State* st, const Loop& L) {
     st->seq_g = L.seq_g; st->seq_G = L.seq_G;
 }
 
-// Last-CTA election (threadfence reduction pattern).  Every thread has fenced its global writes before the call.
+// Last-CTA election (threadfence reduction pattern).  The CTA's global writes are ordered before thread 0's fence by
+// the bar.sync (the fence is cumulative), so no other thread needs a fence of its own; the last CTA's second fence is
+// the acquire side (it also invalidates L1) before it reads the other CTAs' partials.
 __device__ __forceinline__ bool cta_is_last(unsigned int* ticket, SmemHeader* h) {
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -1262,7 +1264,6 @@ __device__ __forceinline__ void dose_single(const DevPlan& P, const PassArgs& A,
     Pipe pipe = {0u, 0u};
     const int par = (int)(st->fwd_passes & 1);
     dose_pass<1>(P, h, imrt_smem, table_s, xs, r_out, A.mode == MODE_EVAL ? A.d_out : nullptr, P.Gpart[par], pipe);
-    __threadfence();
     if (!cta_is_last(&st->ticket_f, h)) return;
     double G[1];
     reduce_objective<1>(P, P.Gpart[par], h, G);
@@ -1290,7 +1291,6 @@ __device__ __forceinline__ void dose_trials(const DevPlan& P, const PassArgs& A,
     Pipe pipe = {0u, 0u};
     const int par = (int)(st->fwd_passes & 1);
     dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[par], pipe);
-    __threadfence();
     if (!cta_is_last(&st->ticket_f, h)) return;
 
     // ---- the last CTA to finish takes the decision
@@ -1351,7 +1351,6 @@ __device__ __forceinline__ void dose_batch(const DevPlan& P, const PassArgs& A, 
     Pipe pipe = {0u, 0u};
     const int par = (int)(st->fwd_passes & 1);
     dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[par], pipe);
-    __threadfence();
     if (!cta_is_last(&st->ticket_f, h)) return;
     double G[R];
     reduce_objective<R>(P, P.Gpart[par], h, G);

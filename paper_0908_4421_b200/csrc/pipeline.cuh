@@ -110,18 +110,19 @@ __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
 // Monotone-counter barrier for a cooperative (co-resident) launch over the n_cta CTAs that share `counter` (the whole
 // grid, or one rank's CTAs when several plans share a launch).  Every CTA calls it the same number of times;
 // `epoch` counts the calls (kept in a register by the caller).  counter must be 0 at kernel start.
+// Release / acquire at gpu scope: the arrival is a red.release (the CTA's earlier writes, ordered before it by the
+// bar.sync, become visible to whoever acquires the count), the wait an ld.acquire spin (SASS: LDG.STRONG.GPU followed by
+// CCTL.IVALL, so the other threads' plain loads after the closing bar.sync cannot hit stale L1 lines).  No full fences.
 __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, int n_cta) {
     __syncthreads();
     ++epoch;
     if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(counter, 1u);
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
         const unsigned int target = epoch * (unsigned int)n_cta;
         unsigned int seen;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
         } while (seen < target);
-        __threadfence();
     }
     __syncthreads();
 }
