@@ -1508,10 +1508,13 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
             dec = armijo_decide<R>(P, st, L, G_new, step_sq, rec, j_acc);
             if (dec != DEC_REJECT_RETRY) break;
         }
-        if (j_acc >= 0 && h->cta == 0) {
-            // x_{k+1}: publish it (L.xi already points at the new buffer); the other CTAs read it only after the
-            // next grid barrier
-            publish_x<R>(xs, j_acc, P.xbuf[L.xi], P.n_b);
+        if (j_acc >= 0) {
+            // x_{k+1}: publish it (L.xi already points at the new buffer).  Every CTA holds all of it and writes one slice,
+            // so no CTA enters the next pass late; the others read it only after the next grid barrier.
+            const int per = ((P.n_b + h->n_cta - 1) / h->n_cta + 31) & ~31;
+            const int i0 = h->cta * per, i1 = min(P.n_b, i0 + per);
+            float* x_out = P.xbuf[L.xi];
+            for (int i = i0 + (int)threadIdx.x; i < i1; i += NTHREADS) x_out[i] = xs[(size_t)i * R + j_acc];
         }
         if (dec != DEC_ACCEPT_CONTINUE) break;
     }
