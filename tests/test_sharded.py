@@ -168,7 +168,7 @@ def test_no_rank_is_left_without_rows():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg,world,n", [(0, 2, 30), (2, 2, 60), (2, 4, 60), (1, 3, 40)])
+@pytest.mark.parametrize("cfg,world,n", [(0, 2, 30), (2, 2, 60), (2, 4, 60), (1, 3, 40), (3, 2, 30)])      # (3, ...): the headline size
 def test_device_resident_sharded_loop_co_resident_ranks(cfg, world, n):
     # The row-sharded loop INSIDE the persistent kernel (exchange of g per iteration and of the R objectives per batch through
     # the ranks' inboxes): `world` ranks co-resident on one device, one cooperative launch (imrt_plan_run_ranks).
