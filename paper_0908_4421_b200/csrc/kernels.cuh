@@ -191,6 +191,19 @@ struct PassArgs {
     cudaGraphConditionalHandle h_outer, h_inner;
 };
 
+// The loop's constants: State fields that do not change during a run.  The persistent kernel keeps a copy in shared
+// memory (the scalar phases between the passes are chains of latencies; every global read they do not make is ~0.3 us).
+struct LoopConst {
+    double eps, alpha, lambda0, delta_tol, G_skip;
+    int max_ls, iter_target;
+};
+__device__ __forceinline__ LoopConst loop_const(const State* st) {
+    LoopConst C;
+    C.eps = st->eps; C.alpha = st->alpha; C.lambda0 = st->lambda0; C.delta_tol = st->delta_tol; C.G_skip = st->G_skip;
+    C.max_ls = st->max_ls; C.iter_target = st->iter_target;
+    return C;
+}
+
 // ------------------------------------------------------------------------------------------------ shared memory
 struct SmemHeader {
     uint64_t full_f[RING_ENTRIES], full_t[MAX_STAGES_T], empty_t[MAX_STAGES_T];
@@ -198,6 +211,7 @@ struct SmemHeader {
     double red[32 * R_MAX];    // block-reduction scratch
     double bcast[4];
     int flag;
+    LoopConst lc;              // persistent kernel: the run's constants
     int cta, n_cta;            // this CTA's index among the CTAs of ITS plan and their number: h->cta / gridDim.x, except when
                                // several plans (ranks) share one cooperative launch (k_persistent_ranks)
 };
@@ -677,7 +691,7 @@ __device__ __forceinline__ void dose_pass(const DevPlan& P, SmemHeader* h, unsig
 // Objectives of a finished dose pass: fixed-order sums of the CTA partials + the constant of the skipped rows.
 // Every thread of the calling CTA gets the values.
 template <int R>
-__device__ __forceinline__ void reduce_objective(const DevPlan& P, const double* Gpart, SmemHeader* h, double (&G)[R]) {
+__device__ __forceinline__ void reduce_objective(const DevPlan& P, const double* Gpart, SmemHeader* h, double (&G)[R], double G_skip) {
 #pragma unroll
     for (int r = 0; r < R; ++r) G[r] = 0.0;
     for (int c = threadIdx.x; c < P.grid_f; c += NTHREADS) {
@@ -685,7 +699,6 @@ __device__ __forceinline__ void reduce_objective(const DevPlan& P, const double*
         for (int r = 0; r < R; ++r) G[r] += __ldcg(Gpart + c * R + r);
     }
     block_sum_vec<R>(G, h);
-    const double G_skip = P.st->G_skip;
 #pragma unroll
     for (int r = 0; r < R; ++r) G[r] += G_skip;
 }
@@ -1125,14 +1138,14 @@ enum { DEC_ACCEPT_CONTINUE = 0, DEC_ACCEPT_STOP = 1, DEC_REJECT_RETRY = 2, DEC_R
 // trial that passes is accepted (j_acc) and the later ones are ignored; each failure is one step 4.  Scalar work only.
 // write_trace: only one CTA records.
 template <int R>
-__device__ __forceinline__ int armijo_decide(const DevPlan& P, const State* st, Loop& L, const double (&G_new)[R],
+__device__ __forceinline__ int armijo_decide(const DevPlan& P, const LoopConst& st, Loop& L, const double (&G_new)[R],
                                              const double (&step_sq)[R], bool write_trace, int& j_acc) {
     L.fwd += 1;
     j_acc = -1;
     double lam = L.lambda;
 #pragma unroll
     for (int j = 0; j < R; ++j) {
-        const double C = L.G_k - (st->eps / lam) * step_sq[j];       // Eq. (5)
+        const double C = L.G_k - (st.eps / lam) * step_sq[j];       // Eq. (5)
         if (G_new[j] < C) {                                           // step 3, strict as printed
             const int k = L.iter;
             if (write_trace) {
@@ -1147,16 +1160,16 @@ __device__ __forceinline__ int armijo_decide(const DevPlan& P, const State* st, 
             L.xi ^= 1;
             L.ri = (L.ri + 1 + j) % (R + 1);
             j_acc = j;
-            if (st->delta_tol > 0.0 && (G_new[j] == 0.0 || fabs(G_new[j] - G_old) / G_new[j] < st->delta_tol)) {   // step 5
+            if (st.delta_tol > 0.0 && (G_new[j] == 0.0 || fabs(G_new[j] - G_old) / G_new[j] < st.delta_tol)) {   // step 5
                 L.stop_reason = STOP_TOLERANCE;
                 return DEC_ACCEPT_STOP;
             }
-            if (L.iter >= st->iter_target) { L.stop_reason = STOP_MAX_ITERS; return DEC_ACCEPT_STOP; }
+            if (L.iter >= st.iter_target) { L.stop_reason = STOP_MAX_ITERS; return DEC_ACCEPT_STOP; }
             return DEC_ACCEPT_CONTINUE;
         }
         L.m += 1;                                                     // step 4
-        if (L.m > st->max_ls) { L.stop_reason = STOP_LS_STALLED; return DEC_REJECT_STOP; }
-        lam = lam / st->alpha;
+        if (L.m > st.max_ls) { L.stop_reason = STOP_LS_STALLED; return DEC_REJECT_STOP; }
+        lam = lam / st.alpha;
     }
     L.lambda = lam;            // first step size of the next batch
     return DEC_REJECT_RETRY;
@@ -1266,7 +1279,7 @@ __device__ __forceinline__ void dose_single(const DevPlan& P, const PassArgs& A,
     dose_pass<1>(P, h, imrt_smem, table_s, xs, r_out, A.mode == MODE_EVAL ? A.d_out : nullptr, P.Gpart[par], pipe);
     if (!cta_is_last(&st->ticket_f, h)) return;
     double G[1];
-    reduce_objective<1>(P, P.Gpart[par], h, G);
+    reduce_objective<1>(P, P.Gpart[par], h, G, st->G_skip);
     if (threadIdx.x != 0) return;
     if (A.mode == MODE_EVAL) {
         st->eval_obj = G[0];            // not counted: fwd_passes / tr_passes count the loop's passes
@@ -1295,11 +1308,12 @@ __device__ __forceinline__ void dose_trials(const DevPlan& P, const PassArgs& A,
 
     // ---- the last CTA to finish takes the decision
     double G_new[R];
-    reduce_objective<R>(P, P.Gpart[par], h, G_new);
+    const LoopConst C = loop_const(st);
+    reduce_objective<R>(P, P.Gpart[par], h, G_new, C.G_skip);
     Loop L;
     loop_load(st, L);
     int j_acc;
-    const int dec = armijo_decide<R>(P, st, L, G_new, step_sq, threadIdx.x == 0, j_acc);
+    const int dec = armijo_decide<R>(P, C, L, G_new, step_sq, threadIdx.x == 0, j_acc);
     if (j_acc >= 0) publish_x<R>(xs, j_acc, P.xbuf[xi ^ 1], P.n_b);
     if (threadIdx.x == 0) {
         loop_store(st, L);
@@ -1353,7 +1367,7 @@ __device__ __forceinline__ void dose_batch(const DevPlan& P, const PassArgs& A, 
     dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[par], pipe);
     if (!cta_is_last(&st->ticket_f, h)) return;
     double G[R];
-    reduce_objective<R>(P, P.Gpart[par], h, G);
+    reduce_objective<R>(P, P.Gpart[par], h, G, st->G_skip);
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int r = 0; r < R; ++r) st->eval_objs[r] = G[r];
@@ -1462,10 +1476,13 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
     float* g_s = reinterpret_cast<float*>(imrt_smem + P.g_off);
     State* st = P.st;
     cta_init(h, P, table_s, cta, n_cta);
+    if (threadIdx.x == 0) h->lc = loop_const(st);
+    __syncthreads();
+    const LoopConst& C = h->lc;
     Loop L;
     loop_load(st, L);
-    const int iter_target = st->iter_target;
-    const double alpha = st->alpha;
+    const int iter_target = C.iter_target;
+    const double alpha = C.alpha;
     L.stop_reason = STOP_MAX_ITERS;
     const bool sharded = P.world > 1;
     if (sharded && st->G_is_local) {       // G(x_1) of imrt_plan_set_x is this slab's share: make it the sum over the ranks
@@ -1489,7 +1506,7 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
         // trial's Delta taken from the batch that is built anyway).  x_k lives in global memory.
         L.tr += 1;
         if (L.G_k == 0.0) { L.stop_reason = STOP_STATIONARY; break; }          // reading R4
-        L.lambda = st->lambda0;
+        L.lambda = C.lambda0;
         L.m = 0;
         int dec, j_acc = -1;
         for (;;) {
@@ -1503,9 +1520,9 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
             const int fpar = (int)(L.fwd & 1);
             dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[fpar], pipe);
             grid_barrier(&st->gridbar, epoch, h->n_cta);
-            reduce_objective<R>(P, P.Gpart[fpar], h, G_new);
+            reduce_objective<R>(P, P.Gpart[fpar], h, G_new, C.G_skip);
             if (sharded) shard_sum_objective<R>(P, h, G_new, ++L.seq_G);      // exchange step 2: G = sum over the row slabs
-            dec = armijo_decide<R>(P, st, L, G_new, step_sq, rec, j_acc);
+            dec = armijo_decide<R>(P, C, L, G_new, step_sq, rec, j_acc);
             if (dec != DEC_REJECT_RETRY) break;
         }
         if (j_acc >= 0) {
