@@ -355,6 +355,33 @@ imrt_status imrt_merge_rows_fill(int64_t n_v, int64_t n_b, const int32_t* row_pt
                                  int64_t n_groups, const int32_t* out_row_ptr, int32_t* out_col, float* out_val, void* workspace,
                                  size_t workspace_bytes, void* stream);
 
+/*
+ * Dose-volume-histogram points of ANY dose on the device, for callers that cannot give the library memory to work in.
+ * Same definition and same kernels as imrt_plan_dvh (D_p = the ceil(p n_s / 100)-th largest dose of
+ * a structure's n_s voxels, plus the mean dose), but no plan and no workspace: the histograms, counters and partial sums
+ * live in an array that is part of the library image itself.  The call and everything under it makes no cudaMalloc,
+ * cudaFree or other allocating CUDA call.  Who needs that: an application that has already handed all device memory to
+ * its own pool (a planning server that sizes its buffers once, a process sharing the GPU under a fixed memory budget),
+ * so that a further cudaMalloc would fail; and code in a latency-sensitive stretch, where the device-wide
+ * synchronisation hidden in cudaMalloc / cudaFree would stall work on other streams.
+ *   dose          fp32  [n_v]   any finite doses, e.g. from imrt_plan_get_dose or a full-resolution D x      (device)
+ *   structure_id  uint8 [n_v]   < n_structures (checked: IMRT_STATUS_BAD_STRUCTURE)                           (device)
+ *   host_pcts     fp64  [n_pcts] percent of the structure's volume;  host_dp [n_structures][n_pcts], host_mean
+ *                 [n_structures] as for imrt_plan_dvh (NaN for a structure without voxels)                    (host)
+ *   stream        a cudaStream_t as void* of the CURRENT device (NULL = the legacy default stream)
+ * Limits (IMRT_STATUS_UNSUPPORTED, with the numbers in imrt_last_error(NULL)): n_structures <= 16, n_pcts <= 16,
+ * n_structures * n_pcts <= 128, n_v <= 2^30.  The built-in array is 1,128,704 bytes (about 1.1 MB); every device on
+ * which the library's code is loaded keeps that much until the process exits, whether or not this call is ever made.
+ * Larger problems: imrt_plan_dvh, whose scratch is in the caller's workspace.
+ * First call on a device: looks up the array's address on that device (once; the device must be current) -- make that
+ * first call before starting any stream capture.
+ * Sharing: all calls on a device use the one array, and it still holds what the previous call left behind; the call
+ * clears what has to start from zero.  Two calls running on the GPU at the same time would corrupt each other's
+ * histograms, so the call holds a library-wide lock and returns only after its stream has drained (it synchronises).
+ */
+imrt_status imrt_dvh_static(const float* dose, const uint8_t* structure_id, int64_t n_v, int32_t n_structures,
+                            const double* host_pcts, int32_t n_pcts, double* host_dp, double* host_mean, void* stream);
+
 /* Message of the last error on this plan (or of the last failed imrt_plan_create when plan is NULL).
  * Owned by the library, valid until the next call on the same plan / thread. */
 const char* imrt_last_error(const imrt_plan* plan);

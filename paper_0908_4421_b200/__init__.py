@@ -31,7 +31,7 @@ EXPORTS = ("imrt_workspace_bytes", "imrt_plan_create", "imrt_plan_set_x", "imrt_
            "imrt_plan_eval", "imrt_plan_eval_batch", "imrt_plan_gradient", "imrt_trial_point", "imrt_armijo_accepts", "imrt_stop_test", "imrt_plan_get_x", "imrt_plan_get_dose", "imrt_plan_dvh", "imrt_plan_get_trace",
            "imrt_plan_get_counters", "imrt_plan_get_info", "imrt_plan_launch_pass", "imrt_plan_get_pass_timing", "imrt_plan_get_tuning", "imrt_plan_get_create_times",
            "imrt_shard_inbox_bytes", "imrt_plan_set_shard", "imrt_plan_run_ranks",
-           "imrt_merge_rows_workspace_bytes", "imrt_merge_rows_count", "imrt_merge_rows_fill", "imrt_last_error", "imrt_plan_destroy",
+           "imrt_merge_rows_workspace_bytes", "imrt_merge_rows_count", "imrt_merge_rows_fill", "imrt_dvh_static", "imrt_last_error", "imrt_plan_destroy",
            "imrt_version")
 
 
@@ -101,6 +101,7 @@ def lib() -> ctypes.CDLL:
         L.imrt_plan_get_x.argtypes = [_P, _P]
         L.imrt_plan_get_dose.argtypes = [_P, _P]
         L.imrt_plan_dvh.argtypes = [_P, _P, i32, _P, _P]
+        L.imrt_dvh_static.argtypes = [_P, _P, i64, i32, _P, i32, _P, _P, _P]
         L.imrt_plan_get_trace.argtypes = [_P, ctypes.POINTER(i32), ctypes.POINTER(i32), _P, _P, _P, _P, i32]
         L.imrt_plan_get_counters.argtypes = [_P, ctypes.POINTER(i64), ctypes.POINTER(i64)]
         L.imrt_plan_get_info.argtypes = [_P, _P, i32, _P, _P, _P]
@@ -313,6 +314,20 @@ def imrt_plan_dvh(plan, pcts, n_structures: int):
     dp = np.empty((n_structures, pc.shape[0]), np.float64)
     mean = np.empty(n_structures, np.float64)
     _check(lib().imrt_plan_dvh(plan, _hptr(pc), pc.shape[0], _hptr(dp), _hptr(mean)), plan)
+    return dp, mean
+
+
+def imrt_dvh_static(dose, structure_id, n_structures: int, pcts, stream_ptr: int = 0):
+    """DVH points and mean dose of an fp32 CUDA dose tensor without a plan or a workspace: the scratch is an array built
+    into libimrtgp.so, so nothing is allocated on the device (for processes whose memory pool already owns the GPU).
+    At most 16 structures and 128 structure x percentage pairs; one call at a time per process (the call synchronises)."""
+    import torch
+    pc = np.ascontiguousarray(pcts, dtype=np.float64)
+    dp = np.empty((n_structures, pc.shape[0]), np.float64)
+    mean = np.empty(n_structures, np.float64)
+    n_v = dose.numel()
+    _check(lib().imrt_dvh_static(_dptr(dose, torch.float32), _dptr(structure_id, torch.uint8, n_v), n_v, n_structures, _hptr(pc),
+                                 pc.shape[0], _hptr(dp), _hptr(mean), ctypes.c_void_p(stream_ptr)))
     return dp, mean
 
 

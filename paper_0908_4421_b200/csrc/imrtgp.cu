@@ -1857,3 +1857,102 @@ imrt_status imrt_plan_launch_pass(imrt_plan* pl, int32_t kind, int32_t n_repeat)
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ DVH without a workspace
+// imrt_dvh_static (include/imrtgp.h): the dose-volume-histogram kernels of dvh.cuh run on scratch that lives inside the
+// library image instead of in memory the caller hands over.  Meant for code that has a dose on the device but may not
+// allocate: a planning service whose own pool already owns all of HBM (a raw cudaMalloc would simply fail), or a section
+// that must not take the device-wide stall a cudaMalloc / cudaFree brings with it.
+//
+// g_dvh_static is ONE array per device for the life of the process (every device that loads the library keeps its
+// IMRT_DVH_STATIC_BYTES until exit).  In host code the name g_dvh_static is only a handle for the runtime, never an address
+// a kernel can use; the address on the current device comes from cudaGetSymbolAddress below, once per device.
+#include <mutex>
+
+namespace {
+
+constexpr int DVH_STATIC_MAX_STRUCTURES = 16;                                // part[] and the documented limit
+constexpr int DVH_STATIC_MAX_QUERIES = 128;                                  // n_structures * n_pcts: one 2,048-bin histogram each
+constexpr size_t DVH_STATIC_HIST = sizeof(unsigned int) * DVH_STATIC_MAX_QUERIES * DVH_BINS;     // 1 MiB
+constexpr size_t DVH_STATIC_CNT = sizeof(unsigned int) * 256;                // dvh_points clears 256 counters / sums
+constexpr size_t DVH_STATIC_SUM = sizeof(double) * 256;
+constexpr size_t DVH_STATIC_PART = sizeof(double) * DVH_SUM_BLOCKS * DVH_STATIC_MAX_STRUCTURES;
+constexpr size_t DVH_STATIC_QUERY = sizeof(DvhQuery) * DVH_STATIC_MAX_QUERIES;
+constexpr size_t DVH_STATIC_FLAG = 256;                                      // largest structure id seen (input check)
+constexpr size_t DVH_STATIC_OFF_CNT = DVH_STATIC_HIST;
+constexpr size_t DVH_STATIC_OFF_SUM = DVH_STATIC_OFF_CNT + DVH_STATIC_CNT;
+constexpr size_t DVH_STATIC_OFF_PART = DVH_STATIC_OFF_SUM + DVH_STATIC_SUM;
+constexpr size_t DVH_STATIC_OFF_QUERY = DVH_STATIC_OFF_PART + DVH_STATIC_PART;
+constexpr size_t DVH_STATIC_OFF_FLAG = DVH_STATIC_OFF_QUERY + DVH_STATIC_QUERY;
+constexpr size_t DVH_STATIC_BYTES = DVH_STATIC_OFF_FLAG + DVH_STATIC_FLAG;   // 1,128,704 bytes
+static_assert(DVH_STATIC_OFF_CNT % 256 == 0 && DVH_STATIC_OFF_SUM % 256 == 0 && DVH_STATIC_OFF_PART % 256 == 0 &&
+              DVH_STATIC_OFF_QUERY % 256 == 0 && DVH_STATIC_OFF_FLAG % 256 == 0, "pieces of the static scratch stay 256-byte aligned");
+
+constexpr int DVH_STATIC_MAX_DEVICES = 64;
+std::mutex g_dvh_static_lock;                                                // one call at a time: the array is shared
+unsigned char* g_dvh_static_addr[DVH_STATIC_MAX_DEVICES] = {nullptr};       // device address of g_dvh_static, per device ordinal
+
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_dvh_static[DVH_STATIC_BYTES];
+
+// Largest structure id among the n_v voxels -> the flag word of the static scratch (device code may name the array).
+__global__ void k_dvh_static_max_sid(const uint8_t* __restrict__ sid, int n_v) {
+    unsigned int m = 0u;
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n_v; j += gridDim.x * blockDim.x) m = max(m, (unsigned int)sid[j]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(reinterpret_cast<unsigned int*>(g_dvh_static + DVH_STATIC_OFF_FLAG), m);
+}
+
+extern "C" imrt_status imrt_dvh_static(const float* dose, const uint8_t* structure_id, int64_t n_v, int32_t n_structures,
+                                       const double* host_pcts, int32_t n_pcts, double* host_dp, double* host_mean, void* stream) {
+    if (!dose || !structure_id || !host_pcts || !host_dp || !host_mean || n_v < 1 || n_structures < 1 || n_pcts < 1)
+        return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_dvh_static: null pointer or non-positive size");
+    if (n_structures > DVH_STATIC_MAX_STRUCTURES || n_pcts > DVH_MAX_PCTS || n_structures * n_pcts > DVH_STATIC_MAX_QUERIES || n_v > (1LL << 30))
+        return fail(nullptr, IMRT_STATUS_UNSUPPORTED,
+                    "imrt_dvh_static: the built-in scratch (%zu bytes) holds at most %d structures, %d percentages per structure, %d "
+                    "structure x percentage pairs and 2^30 voxels; got n_structures = %d, n_pcts = %d, n_v = %lld -- use imrt_plan_dvh "
+                    "(caller-provided workspace) for more", DVH_STATIC_BYTES, DVH_STATIC_MAX_STRUCTURES, DVH_MAX_PCTS, DVH_STATIC_MAX_QUERIES,
+                    (int)n_structures, (int)n_pcts, (long long)n_v);
+    cudaStream_t st = (cudaStream_t)stream;
+    std::lock_guard<std::mutex> hold(g_dvh_static_lock);      // held until the stream has drained: calls never overlap on the GPU
+
+    // Set-up, once per device, with that device current: ask the runtime where this device keeps the array.
+    int dev = -1;
+    CUDA_TRY(nullptr, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= DVH_STATIC_MAX_DEVICES) return fail(nullptr, IMRT_STATUS_UNSUPPORTED, "imrt_dvh_static: device ordinal %d >= %d", dev, DVH_STATIC_MAX_DEVICES);
+    if (!g_dvh_static_addr[dev]) {
+        unsigned char* p = nullptr;
+        CUDA_TRY(nullptr, cudaGetSymbolAddress((void**)&p, g_dvh_static));
+        if (!p) return fail(nullptr, IMRT_STATUS_CUDA_ERROR, "imrt_dvh_static: cudaGetSymbolAddress returned a null address");
+        g_dvh_static_addr[dev] = p;
+    }
+    unsigned char* base = g_dvh_static_addr[dev];
+
+    // The array still holds the previous call's histograms, sums and flag.  dvh_points clears cnt, sum and (per round) hist
+    // and overwrites every part / query entry it reads; the flag is cleared here.
+    unsigned int* flag = reinterpret_cast<unsigned int*>(base + DVH_STATIC_OFF_FLAG);
+    CUDA_TRY(nullptr, cudaMemsetAsync(flag, 0, sizeof(unsigned int), st));
+    k_dvh_static_max_sid<<<std::max(1, (int)std::min<int64_t>((n_v + 255) / 256, 148 * 8)), 256, 0, st>>>(structure_id, (int)n_v);
+    CUDA_TRY(nullptr, cudaGetLastError());
+    unsigned int max_sid = 0u;
+    CUDA_TRY(nullptr, cudaMemcpyAsync(&max_sid, flag, sizeof max_sid, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(nullptr, cudaStreamSynchronize(st));
+    if (max_sid >= (unsigned int)n_structures)
+        return fail(nullptr, IMRT_STATUS_BAD_STRUCTURE, "imrt_dvh_static: structure_id %u >= n_structures %d", max_sid, (int)n_structures);
+
+    DvhWork W;
+    W.hist = reinterpret_cast<unsigned int*>(base);
+    W.cnt = reinterpret_cast<unsigned int*>(base + DVH_STATIC_OFF_CNT);
+    W.sum = reinterpret_cast<double*>(base + DVH_STATIC_OFF_SUM);
+    W.part = reinterpret_cast<double*>(base + DVH_STATIC_OFF_PART);
+    W.query = reinterpret_cast<DvhQuery*>(base + DVH_STATIC_OFF_QUERY);
+    const char* what = nullptr;
+    cudaError_t e = dvh_points(W, dose, structure_id, (int)n_v, n_structures, host_pcts, n_pcts, host_dp, host_mean, st, &what);
+    if (e != cudaSuccess) {
+        cudaStreamSynchronize(st);                            // nothing of this call may still be using the array when the lock drops
+        return fail(nullptr, IMRT_STATUS_CUDA_ERROR, "imrt_dvh_static: %s (%s)", cudaGetErrorString(e), what ? what : "");
+    }
+    return IMRT_STATUS_OK;
+}
