@@ -1495,11 +1495,18 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
     unsigned int epoch = 0;
     const bool rec = (h->cta == 0) && (threadIdx.x == 0);
 
+    bool g_valid = false;                  // g_s holds the gradient of the current iterate (a transpose pass ran in this launch)
     while (L.iter < iter_target) {
         const int tpar = (int)(L.tr & 1);
+        // The transpose stages overlay xs and g_s (DevPlan::tr_stage_off = x_off).  Everybody is done with both -- the
+        // publish loop below read xs, trial_batch / reduce_gradient wrote them through the generic proxy -- before the
+        // producer warp lets the TMA unit write over them: proxy fence in every thread, then a CTA barrier.
+        fence_proxy_async_smem();
+        __syncthreads();
         transpose_pass(P, h, imrt_smem, wpart, P.rbuf[L.ri], P.gslot[tpar], pipe);
         grid_barrier(&st->gridbar, epoch, h->n_cta);
         reduce_gradient(P, P.gslot[tpar], g_s);
+        g_valid = true;
         __syncthreads();
         if (sharded) shard_sum_gradient(P, h, g_s, ++L.seq_g);      // exchange step 1: g = sum over the row slabs
         // start of the line search (PAPER.md:109 step 2; the same decisions begin_line_search takes, with the first
@@ -1538,7 +1545,8 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
     // every CTA has passed the last grid barrier before CTA 0 gets here with a changed state
     grid_barrier(&st->gridbar, epoch, h->n_cta);
     if (h->cta == 0) {
-        for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) P.g[i] = g_s[i];
+        if (g_valid)                       // a launch that did no iteration leaves P.g as it was
+            for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) P.g[i] = g_s[i];
         if (threadIdx.x == 0) {
             loop_store(st, L);
             st->cont_outer = 0;

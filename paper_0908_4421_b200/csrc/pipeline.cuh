@@ -59,6 +59,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {}
 }
 
+// Orders this thread's earlier generic-proxy accesses to shared memory (plain ld / st) before later async-proxy accesses
+// (the TMA unit's writes of a bulk copy) to the same bytes.  Issued by every thread that touched the bytes, then a CTA
+// barrier, then the producer may issue its bulk copies over them.
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // ---------------------------------------------------------------------------------------------- L2 policies
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;

@@ -273,7 +273,7 @@ def test_trajectory_parity_follow_mode(m, cfg, driver):
     assert fol.n_follow_violations == 0, "GPU accepted/rejected a trial the oracle would not (first at iteration %d)" % fol.first_violation
     np.testing.assert_array_equal(tr.lam, fol.lam)
     assert abs(tr.obj[-1] - fol.obj[-1]) <= TOL_G_FINAL * fol.obj[-1]
-    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    assert (np.abs(tr.obj - fol.obj) <= TOL_G_FINAL * fol.obj).all()
     # DVH points of the final plans
     d_o, _, _ = oracle.eval_objective(prob, fol.x)
     dp_o, mean_o = oracle.dvh_points(prob.sid, d_o, prob.n_structures)
@@ -367,53 +367,7 @@ def test_linesearch_stall_and_bad_inputs(m):
     assert torch.cuda.is_available()
 
 
-# ---------------------------------------------------------------------------------------------- full size (bench configuration)
-# BASELINE.json configs[3] (headline) and configs[4] (stress), in the launch configuration bench.py times (persistent
-# driver, one CTA per SM, tuned partition).  The oracle's eval / gradient take well under a second per call even at
-# these sizes, so every output element is compared, not a sample.
-@pytest.mark.parametrize("cfg", [3, 4])
-def test_full_size_parity(m, cfg):
-    # the configs' own run lengths: cfg3 "delta = 1e-6 or 500 iterations", cfg4 300 fixed iterations -- the oracle replays
-    # the GPU's iteration count in follow mode (about 2 and 4 minutes of serial fp64 work)
-    prob = phantom(cfg)
-    plan = m.Plan(prob, max_iters=prob.n_iters, driver=m.DRIVER_PERSISTENT, tune_level=2)     # as bench.py creates it
-    info = plan.info()
-    assert info["fwd_grid"] == info["n_sm"] and info["tr_grid"] == info["n_sm"]   # what bench.py launches
-    check_eval(m, plan, prob, prob.x0)
-    xo = oracle.run(prob, n_iters=3).x.astype(np.float32)
-    check_eval(m, plan, prob, xo)
-    check_eval_batch(m, plan, prob, trial_points(prob, xo, 4))     # the R = 4 pass bench.py times, on four trial points
-    # trajectory from x0 under the config's own rule, oracle in follow mode
-    plan.set_x(prob.x0)
-    if prob.delta > 0:
-        plan.run_to_tol(prob.delta, prob.n_iters)
-    else:
-        plan.run_iters(prob.n_iters)
-    tr = plan.trace()
-    n_iters = tr.n_iters
-    print("cfg%d: GPU stopped after %d iterations (%s)" % (cfg, n_iters, m.STOP_NAMES[tr.stop_reason]))
-    assert tr.stop_reason in (oracle.STOP_MAX_ITERS, oracle.STOP_TOLERANCE) and n_iters >= min(300, prob.n_iters)
-    assert (np.diff(tr.obj) < 0).all()
-    fol = oracle.run(prob, n_iters=n_iters, follow_trials=tr.n_trials, tau_rel=1e-6)
-    assert fol.n_follow_violations == 0, "first violation at iteration %d" % fol.first_violation
-    np.testing.assert_array_equal(tr.lam, fol.lam)
-    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
-    assert abs(tr.obj[-1] - fol.obj[-1]) <= TOL_G_FINAL * fol.obj[-1]
-    x = plan.get_x().cpu().numpy()
-    assert (x >= 0).all()
-    d = plan.get_dose().cpu().numpy()
-    d_o, _, _ = oracle.eval_objective(prob, fol.x)
-    dp_o, mean_o = oracle.dvh_points(prob.sid, d_o, prob.n_structures)
-    dp_g, mean_g = plan.dvh(oracle.DVH_PCTS)
-    assert np.nanmax(np.abs(dp_g - dp_o)) <= TOL_DVH_GY and np.nanmax(np.abs(mean_g - mean_o)) <= TOL_DVH_GY
-    # dose of the two final plans, voxel by voxel: the DVH tolerance (0.5 % of the prescription) applied to EVERY voxel.
-    # (The minimiser is not unique -- reading R14 -- so the fp32 and fp64 trajectories may drift apart along directions
-    # the objective does not see; DESIGN.md section 6 records the measured drift per iteration.)
-    print("cfg%d: dose drift after %d iterations: normwise %.2e, largest voxel %.4f Gy" % (cfg, n_iters, relerr(d, d_o), np.abs(d - d_o).max()))
-    assert np.abs(d - d_o).max() <= TOL_DVH_GY
-    assert relerr(d, d_o) <= 1e-4      # the bound of round 1's first version, at the full run length
-    plan.close()
-    _phantoms.pop(cfg, None)        # free ~1-3 GB of host memory
+# (the full-size cases, cfg3 and cfg4, live in tests/test_zz_full_size.py: they take minutes and sort after the cheap tests)
 
 
 # ---------------------------------------------------------------------------------------------- per-voxel limits
@@ -433,7 +387,7 @@ def test_per_voxel_limits_parity(m, cfg):
     tr = plan.trace()
     fol = oracle.run(prob, n_iters=20, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert tr.n_iters == 20 and fol.n_follow_violations == 0
-    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    assert (np.abs(tr.obj - fol.obj) <= TOL_G_FINAL * fol.obj).all()
     # back to per-structure limits: the plan behaves as if the call had never happened
     plan.set_voxel_limits(None, None)
     base = phantom(cfg)
@@ -475,7 +429,7 @@ def test_fallback_layouts_parity(m, opt):
         tr = plan.trace()
         fol = oracle.run(prob, n_iters=12, follow_trials=tr.n_trials, tau_rel=1e-6)
         assert tr.n_iters == fol.n_iters and fol.n_follow_violations == 0
-        assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+        assert (np.abs(tr.obj - fol.obj) <= TOL_G_FINAL * fol.obj).all()
         plan.close()
 
 
@@ -532,7 +486,7 @@ def test_wide_transpose_groups_use_the_32_bit_stream(m):
     plan.run_iters(8)
     tr = plan.trace()
     fol = oracle.run(prob, n_iters=8, follow_trials=tr.n_trials, tau_rel=1e-6)
-    assert fol.n_follow_violations == 0 and np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    assert fol.n_follow_violations == 0 and (np.abs(tr.obj - fol.obj) <= TOL_G_FINAL * fol.obj).all()
     plan.close()
 
 
@@ -565,7 +519,7 @@ def test_mixed_resolution_workflow(m):
     tr = plan.trace()
     fol = oracle.run(mixed, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert tr.n_iters == n and fol.n_follow_violations == 0
-    assert np.abs(tr.obj - fol.obj).max() <= TOL_G_FINAL * fol.obj.max()
+    assert (np.abs(tr.obj - fol.obj) <= TOL_G_FINAL * fol.obj).all()
     x = plan.get_x()
     # full-resolution evaluation of that plan
     full = m.Plan(fine, max_iters=1)

@@ -193,7 +193,7 @@ def test_device_resident_sharded_loop_co_resident_ranks(cfg, world, n):
     fol = oracle.run(prob, n_iters=n, follow_trials=tr.n_trials, tau_rel=1e-6)
     assert fol.n_follow_violations == 0
     np.testing.assert_array_equal(tr.lam, fol.lam)
-    assert np.abs(tr.obj - fol.obj).max() <= 1e-4 * fol.obj.max() and abs(tr.obj[-1] - fol.obj[-1]) <= 1e-4 * fol.obj[-1]
+    assert (np.abs(tr.obj - fol.obj) <= 1e-4 * fol.obj).all()      # every entry of the trace, relative to itself
     d = ranks.get_dose().cpu().numpy().astype(np.float64)
     d_o = oracle.eval_objective(prob, fol.x)[0]
     assert np.abs(d - d_o).max() <= 0.005 * 70.0
