@@ -65,8 +65,14 @@ typedef enum imrt_stop_reason {
     IMRT_STOP_TOLERANCE = 1,             /* |G_new - G_old| / G_new < delta (or G_new == 0)                      */
     IMRT_STOP_STATIONARY = 2,            /* G(x_k) == 0, or the first trial point equals x_k                     */
     IMRT_STOP_LINESEARCH_STALLED = 3,    /* more than max_ls backtracking steps; x_k kept                        */
-    IMRT_STOP_TRACE_FULL = 4             /* the trace (imrt_params.max_iters accepted iterations since imrt_plan_set_x)
+    IMRT_STOP_TRACE_FULL = 4,            /* the trace (imrt_params.max_iters accepted iterations since imrt_plan_set_x)
                                             filled up before the requested number of iterations was done          */
+    IMRT_STOP_PEER_TIMEOUT = 5           /* persistent driver: a wait inside the kernel -- on the other CTAs of the launch or,
+                                            for a row-sharded plan, on a peer rank's partial sums -- was not answered within
+                                            imrt_options.spin_timeout_ms.  The kernel left its loop instead of hanging the
+                                            device; the iterate is no longer valid.  Runs are refused (they return at once
+                                            with this stop reason) until the next imrt_plan_set_x; the inboxes of a sharded
+                                            group must be zero-filled and imrt_plan_set_shard called again first.        */
 } imrt_stop_reason;
 
 /* Line-search / loop parameters (PAPER.md:92 "two parameters 0 < eps < 1 and alpha > 1", :103, :114). */
@@ -110,7 +116,8 @@ typedef struct imrt_options {
                                   (or to other ranks of a row-sharded problem sharing the device, imrt_plan_run_ranks)   */
     int32_t profile_create;    /* 1: synchronise after every phase of plan creation and keep the phase times for
                                   imrt_plan_get_create_times                                                           */
-    int32_t reserved0;
+    int32_t spin_timeout_ms;   /* bound, in milliseconds, on every wait inside the persistent kernel (grid barrier, peer
+                                  ranks' flags): 0 = default, 2000.  On expiry the run ends with IMRT_STOP_PEER_TIMEOUT          */
     const void* host_tuning;   /* a blob written by imrt_plan_get_tuning for the same problem, options and device: the
                                   plan takes its partitions from it instead of measuring (tune_level is ignored)       */
     size_t host_tuning_bytes;
@@ -318,7 +325,10 @@ imrt_status imrt_plan_get_create_times(imrt_plan* plan, double* host_ms, int32_t
  *   imrt_shard_inbox_bytes  size of one rank's inbox for n_b beamlets and `world` ranks (host arithmetic)
  *   imrt_plan_set_shard     host_inboxes [world]: device pointers to EVERY rank's inbox as this rank's device can address
  *                           them (its own included; peers' through peer access / IPC / symmetric memory), 16-byte
- *                           aligned, zero-filled once before the first run and never touched by the caller afterwards.
+ *                           aligned, zero-filled before EVERY imrt_plan_set_shard (the call restarts the plan's exchange
+ *                           counters at zero; all ranks of a group must be set up against the same freshly zeroed inboxes)
+ *                           and never touched by the caller afterwards.  All arguments are validated before anything is
+ *                           changed: a refused call leaves the plan as it was.
  *                           world = 1 returns to a stand-alone plan.  Persistent driver only.  Call imrt_plan_set_x after.
  * Every rank then calls imrt_plan_set_x (the same x0) and imrt_plan_run_iters / _run_to_tol (the same arguments); the
  * traces of all ranks are identical and hold the objective of the WHOLE problem; imrt_plan_get_dose / _eval / _dvh stay
@@ -326,7 +336,11 @@ imrt_status imrt_plan_get_create_times(imrt_plan* plan, double* host_ms, int32_t
  *   imrt_plan_run_ranks     the same for ranks that are CO-RESIDENT on one device (plans created with
  *                           imrt_options.n_ctas = SMs / ranks on one stream): ONE cooperative launch runs all of them --
  *                           ranks wait on one another, so separate launches on one device could deadlock.  host_plans [n_ranks]
- *                           in rank order.  Asynchronous.
+ *                           in rank order; they must agree in ls_batch, max_iters and n_b (checked) and must all be at the
+ *                           same iteration (every rank got the same imrt_plan_set_x / run calls; not checked).  Asynchronous.
+ * Failure detection: no wait inside the kernel is unbounded.  A peer that never launched, died, or runs a different number
+ * of exchanges makes the waiting rank give up after imrt_options.spin_timeout_ms, mark the exchange as failed in every
+ * rank's inbox (so the surviving ranks stop at once as well) and end its run with IMRT_STOP_PEER_TIMEOUT.
  */
 imrt_status imrt_shard_inbox_bytes(int64_t n_b, int32_t world, size_t* host_bytes);
 imrt_status imrt_plan_set_shard(imrt_plan* plan, int32_t rank, int32_t world, void* const* host_inboxes);
@@ -343,7 +357,9 @@ imrt_status imrt_plan_run_ranks(imrt_plan* const* host_plans, int32_t n_ranks, i
  *   out_row_ptr  int32 [n_groups + 1]                                                                         (device)
  *   out_col      int32 [nnz_out], out_val fp32 [nnz_out]                                                      (device)
  *   workspace    >= imrt_merge_rows_workspace_bytes(n_v, n_groups); the SAME workspace, unmodified, for both calls
- * imrt_merge_rows_count sorts the rows by group, counts every merged row, fills out_row_ptr and returns nnz_out
+ * imrt_merge_rows_count checks the raw input first -- group ids in range (IMRT_STATUS_INVALID_ARG), row_ptr[0] = 0 and
+ * non-decreasing, every column in [0, n_b) (IMRT_STATUS_BAD_CSR): this call runs BEFORE imrt_plan_create has seen the
+ * matrix --, then sorts the rows by group, counts every merged row, fills out_row_ptr and returns nnz_out
  * (synchronises); the caller allocates out_col / out_val and calls imrt_merge_rows_fill (asynchronous).
  * Limits: n_b up to about 390,000 (the column bitmap of one group must fit 24 KB of shared memory).
  */

@@ -23,7 +23,7 @@ __all__ = ["Plan", "ImrtError", "lib", "Params", "Options", "STATUS_NAMES", "STO
 
 STATUS_NAMES = ("OK", "INVALID_ARG", "BAD_CSR", "BAD_STRUCTURE", "WORKSPACE_TOO_SMALL", "CUDA_ERROR",
                 "UNSUPPORTED_DEVICE", "UNSUPPORTED", "BAD_X", "NOT_READY")
-STOP_NAMES = ("MAX_ITERS", "TOLERANCE", "STATIONARY", "LINESEARCH_STALLED", "TRACE_FULL")
+STOP_NAMES = ("MAX_ITERS", "TOLERANCE", "STATIONARY", "LINESEARCH_STALLED", "TRACE_FULL", "PEER_TIMEOUT")
 DRIVER_GRAPH, DRIVER_HOST, DRIVER_PERSISTENT = 0, 1, 2
 
 # every symbol include/imrtgp.h declares
@@ -53,7 +53,7 @@ class Options(ctypes.Structure):
     """imrt_options: layout / tuning switches of imrt_plan_create (all 0 = defaults)."""
     _fields_ = [("tune_level", ctypes.c_int32), ("dose_format", ctypes.c_int32), ("col_bits", ctypes.c_int32),
                 ("transpose_format", ctypes.c_int32), ("quad_cap", ctypes.c_int32), ("n_ctas", ctypes.c_int32),
-                ("profile_create", ctypes.c_int32), ("reserved0", ctypes.c_int32),
+                ("profile_create", ctypes.c_int32), ("spin_timeout_ms", ctypes.c_int32),
                 ("host_tuning", ctypes.c_void_p), ("host_tuning_bytes", ctypes.c_size_t)]
 
 
@@ -399,7 +399,7 @@ class Plan:
 
     def __init__(self, prob, max_iters: int = 1000, driver: int = DRIVER_PERSISTENT, device="cuda:0", stream=None,
                  ls_batch: int = 0, tuning: bytes = None, **options):
-        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, n_ctas, profile_create); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
+        """options: fields of imrt_options (tune_level, dose_format, col_bits, transpose_format, quad_cap, n_ctas, profile_create, spin_timeout_ms); tuning: a blob from Plan.tuning() of an earlier plan of the same problem."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_0908_4421_b200 needs a CUDA device (sm_100a); there is no CPU path")

@@ -574,7 +574,7 @@ __global__ void k_reset_state(State* st) {
     st->iter = 0; st->iter_target = 0; st->m = 0; st->stop_reason = STOP_MAX_ITERS;
     st->xi = 0; st->ri = 0;   // the MODE_INIT dose pass reads xbuf[0], writes rbuf[1] and makes it current
     st->cont_outer = 0; st->cont_inner = 0; st->bad_x = 0;
-    st->ticket_f = 0u; st->ticket_t = 0u; st->gridbar = 0u; st->clamped = 0;
+    st->ticket_f = 0u; st->ticket_t = 0u; st->gridbar = 0u; st->clamped = 0; st->fault = 0;
 }
 
 __global__ void k_copy_current_x(const DevPlan P, float* x) {
@@ -1005,7 +1005,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     memset(&opt, 0, sizeof opt);
     if (host_options) opt = *host_options;
     if (opt.tune_level < 0 || opt.tune_level > 2 || opt.dose_format < 0 || opt.dose_format > 1 || (opt.col_bits != 0 && opt.col_bits != 32) ||
-        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 || opt.n_ctas < 0 ||
+        opt.transpose_format < 0 || opt.transpose_format > 2 || opt.quad_cap < 0 || opt.n_ctas < 0 || opt.spin_timeout_ms < 0 ||
         (opt.host_tuning && opt.host_tuning_bytes < sizeof(int) * 8))
         return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_plan_create: bad imrt_options");
     imrt_plan* pl = new imrt_plan();
@@ -1295,6 +1295,7 @@ imrt_status imrt_plan_create(imrt_plan** out, int64_t n_v, int64_t n_b, int64_t 
     memset(&st_h, 0, sizeof st_h);
     st_h.eps = prm->eps; st_h.alpha = prm->alpha; st_h.lambda0 = prm->lambda0; st_h.lambda = prm->lambda0;
     st_h.max_ls = prm->max_ls; st_h.trace_cap = prm->max_iters; st_h.xi = 0; st_h.ri = 0;
+    st_h.spin_timeout_ns = (unsigned long long)(pl->opt.spin_timeout_ms > 0 ? pl->opt.spin_timeout_ms : 2000) * 1000000ull;
     CUDA_TRY(pl, cudaMemcpyAsync(L.st, &st_h, sizeof st_h, cudaMemcpyHostToDevice, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.gslot[0], 0, sizeof(double) * 2 * B.max_slots, st));
     CUDA_TRY(pl, cudaMemsetAsync(L.gslot[1], 0, sizeof(double) * 2 * B.max_slots, st));
@@ -1447,18 +1448,22 @@ imrt_status imrt_shard_inbox_bytes(int64_t n_b, int32_t world, size_t* host_byte
     return IMRT_STATUS_OK;
 }
 
+__global__ void k_reset_shard_seq(State* st) { st->seq_g = 0ull; st->seq_G = 0ull; }
+
 imrt_status imrt_plan_set_shard(imrt_plan* pl, int32_t rank, int32_t world, void* const* host_inboxes) {
     if (!pl || world < 1 || world > MAX_WORLD || rank < 0 || rank >= world || (world > 1 && !host_inboxes))
         return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_shard: bad argument (0 <= rank < world <= %d)", MAX_WORLD);
     if (world > 1 && pl->prm.driver != 2)
         return fail(pl, IMRT_STATUS_UNSUPPORTED, "a row-sharded plan runs with the persistent driver (imrt_params.driver = 2) only");
+    for (int q = 0; world > 1 && q < world; ++q)             // validate everything first: a refused call changes nothing
+        if (!host_inboxes[q] || ((uintptr_t)host_inboxes[q] & 15))
+            return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_shard: inbox %d is null or misaligned", q);
     pl->P.rank = rank;
     pl->P.world = world;
-    for (int q = 0; q < MAX_WORLD; ++q) {
-        pl->P.inbox[q] = (world > 1 && q < world) ? static_cast<unsigned char*>(host_inboxes[q]) : nullptr;
-        if (world > 1 && q < world && (!host_inboxes[q] || ((uintptr_t)host_inboxes[q] & 15)))
-            return fail(pl, IMRT_STATUS_INVALID_ARG, "imrt_plan_set_shard: inbox %d is null or misaligned", q);
-    }
+    for (int q = 0; q < MAX_WORLD; ++q) pl->P.inbox[q] = (world > 1 && q < world) ? static_cast<unsigned char*>(host_inboxes[q]) : nullptr;
+    // the exchange counters restart with the (zero-filled) inboxes: every rank of a group counts from the same number
+    k_reset_shard_seq<<<1, 1, 0, pl->stream>>>(pl->P.st);
+    CUDA_TRY(pl, cudaGetLastError());
     pl->has_x = false;         // G(x_1) has to be formed again, and summed over the ranks
     return IMRT_STATUS_OK;
 }
@@ -1478,6 +1483,10 @@ imrt_status imrt_plan_run_ranks(imrt_plan* const* host_plans, int32_t n_ranks, i
         if (pl->prm.driver != 2 || pl->stream != p0->stream || pl->grid_p != p0->grid_p || pl->P.world != n_ranks || pl->P.rank != q)
             return fail(p0, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_ranks: plan %d must be rank %d of %d (imrt_plan_set_shard), use the persistent "
                         "driver, the stream and the number of CTAs (imrt_options.n_ctas) of plan 0", q, q, n_ranks);
+        // ranks that disagree on the batch size or on the trace capacity would count their exchanges differently
+        if (pl->P.R != p0->P.R || pl->prm.max_iters != p0->prm.max_iters || pl->P.n_b != p0->P.n_b)
+            return fail(p0, IMRT_STATUS_INVALID_ARG, "imrt_plan_run_ranks: plan %d differs from plan 0 in ls_batch (%d / %d), max_iters (%d / %d) or "
+                        "n_b (%d / %d)", q, pl->P.R, p0->P.R, pl->prm.max_iters, p0->prm.max_iters, pl->P.n_b, p0->P.n_b);
         plans[q] = pl->P;
         total += pl->grid_p;
         smem = std::max(smem, pl->smem_bytes);
@@ -1754,6 +1763,8 @@ imrt_status imrt_merge_rows_count(int64_t n_v, int64_t n_b, const int32_t* row_p
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(nullptr, cudaMemsetAsync(M.flags, 0, 16 * sizeof(int), st));
     k_merge_keys<<<grid_for(n_v, 256), 256, 0, st>>>(group_id, (int)n_v, (int)n_groups, M.keysA, M.rowsA, M.flags);
+    k_merge_check_row_ptr<<<grid_for(n_v, 256), 256, 0, st>>>(row_ptr, (int)n_v, M.flags);
+    if (col_idx) k_merge_check_cols<<<grid_for(n_v * 32, 256), 256, 0, st>>>(row_ptr, col_idx, (int)n_v, (int)n_b, M.flags);
     cub::DoubleBuffer<unsigned int> dk(M.keysA, M.keysB), dv(M.rowsA, M.rowsB);
     int end_bit = 1;
     while ((1LL << end_bit) < n_groups) ++end_bit;
@@ -1769,6 +1780,8 @@ imrt_status imrt_merge_rows_count(int64_t n_v, int64_t n_b, const int32_t* row_p
     CUDA_TRY(nullptr, cudaMemcpyAsync(flags_h, M.flags, sizeof flags_h, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(nullptr, cudaStreamSynchronize(st));
     if (flags_h[0]) return fail(nullptr, IMRT_STATUS_INVALID_ARG, "imrt_merge_rows_count: a group id is outside [0, n_groups)");
+    if (flags_h[1]) return fail(nullptr, IMRT_STATUS_BAD_CSR, "imrt_merge_rows_count: row_ptr[0] != 0 or row_ptr decreases");
+    if (flags_h[2]) return fail(nullptr, IMRT_STATUS_BAD_CSR, "imrt_merge_rows_count: a column index is outside [0, n_b)");
     k_merge_count<<<(int)std::min<int64_t>((n_groups + warps - 1) / warps, 148 * 8), MERGE_WARPS * 32, (size_t)warps * words * 4, st>>>(
         row_ptr, col_idx, M.rows, M.group_ptr, (int)n_groups, words, warps, M.cnt);
     temp = 0;

@@ -62,7 +62,7 @@ constexpr int SMEM_WPART = RL_MAX * W_CONS * 8 * 2;   // transpose pass: per-(ro
 constexpr int SMEM_DSC = W_CONS * 32 * R_MAX * 4;   // per-warp scratch: dose of 32 rows x R trial points
 
 enum { MODE_TRIAL = 0, MODE_INIT = 1, MODE_EVAL = 2, MODE_TIMING = 3, MODE_BATCH = 4 };
-enum { STOP_MAX_ITERS = 0, STOP_TOLERANCE = 1, STOP_STATIONARY = 2, STOP_LS_STALLED = 3, STOP_TRACE_FULL = 4 };
+enum { STOP_MAX_ITERS = 0, STOP_TOLERANCE = 1, STOP_STATIONARY = 2, STOP_LS_STALLED = 3, STOP_TRACE_FULL = 4, STOP_PEER_TIMEOUT = 5 };
 
 // ------------------------------------------------------------------------------------------------ device data
 struct State {                 // lives in the workspace; the single source of truth between launches
@@ -90,7 +90,8 @@ struct State {                 // lives in the workspace; the single source of t
     int clamped;               // the last run's target was cut short by the trace capacity
     unsigned long long seq_g, seq_G;   // row-sharded plans: exchanges of the gradient / of objectives done so far (never reset)
     int G_is_local;            // row-sharded plans: G_k is this slab's share only (after set_x), not yet the sum over the ranks
-    int pad2;
+    int fault;                 // sticky: a wait of the persistent loop timed out (STOP_PEER_TIMEOUT); cleared by imrt_plan_set_x
+    unsigned long long spin_timeout_ns;   // bound on every in-kernel wait (grid barrier, inbox flags); imrt_options.spin_timeout_ms
 };
 
 struct TrRange {               // a contiguous piece of the D^T nnz stream, 32 bytes
@@ -195,12 +196,13 @@ struct PassArgs {
 // memory (the scalar phases between the passes are chains of latencies; every global read they do not make is ~0.3 us).
 struct LoopConst {
     double eps, alpha, lambda0, delta_tol, G_skip;
+    unsigned long long spin_timeout_ns;
     int max_ls, iter_target;
 };
 __device__ __forceinline__ LoopConst loop_const(const State* st) {
     LoopConst C;
     C.eps = st->eps; C.alpha = st->alpha; C.lambda0 = st->lambda0; C.delta_tol = st->delta_tol; C.G_skip = st->G_skip;
-    C.max_ls = st->max_ls; C.iter_target = st->iter_target;
+    C.max_ls = st->max_ls; C.iter_target = st->iter_target; C.spin_timeout_ns = st->spin_timeout_ns;
     return C;
 }
 
@@ -211,6 +213,7 @@ struct SmemHeader {
     double red[32 * R_MAX];    // block-reduction scratch
     double bcast[4];
     int flag;
+    int fault;                 // persistent kernel: a bounded wait gave up (grid_barrier / shard_wait); 0 at kernel start
     LoopConst lc;              // persistent kernel: the run's constants
     int cta, n_cta;            // this CTA's index among the CTAs of ITS plan and their number: h->cta / gridDim.x, except when
                                // several plans (ranks) share one cooperative launch (k_persistent_ranks)
@@ -225,6 +228,7 @@ __device__ __forceinline__ void cta_init(SmemHeader* h, const DevPlan& P, float4
     if (threadIdx.x == 0) {
         h->cta = cta;
         h->n_cta = n_cta;
+        h->fault = 0;
         for (int s = 0; s < RING_ENTRIES; ++s) mbar_init(&h->full_f[s], 1);
         for (int s = 0; s < MAX_STAGES_T; ++s) {
             mbar_init(&h->full_t[s], 1);
@@ -1059,9 +1063,46 @@ __device__ __forceinline__ unsigned long long ld_acquire_sys(const unsigned long
     return v;
 }
 
+// Failure detection: a peer that never launched, died, or was given a different iteration count
+// never raises its flag.  Every wait on an inbox flag is therefore bounded by State::spin_timeout_ns; a rank that gives
+// up POISONS the exchange -- SHARD_POISON into its slot of every rank's flags and into all flags of its own inbox, so
+// that its peers and its own other CTAs fall out of their waits at once instead of each sitting out the full timeout --
+// and sets BAR_FAULT in its grid-barrier counter.  The inboxes must be zero-filled again before they are reused.
+constexpr unsigned long long SHARD_POISON = ~0ull;
+// true: the flag reached seq in time and is not poisoned
+__device__ __forceinline__ bool shard_wait(const unsigned long long* f, unsigned long long seq, unsigned long long timeout_ns) {
+    unsigned int polls = 0u;
+    unsigned long long t0 = 0ull;
+    for (;;) {
+        const unsigned long long v = ld_acquire_sys(f);
+        if (v >= seq) return v != SHARD_POISON;
+        if ((++polls & 63u) == 0u) {
+            const unsigned long long now = spin_clock_ns();
+            if (t0 == 0ull) t0 = now;
+            else if (now - t0 > timeout_ns) return false;
+        }
+    }
+}
+// Called by all threads of a CTA whose wait failed (block-uniform): tell everybody, remember it in h->fault.
+__device__ __forceinline__ void shard_give_up(const DevPlan& P, SmemHeader* h) {
+    if ((int)threadIdx.x < P.world) {
+        const int q = threadIdx.x;
+        st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[q] + INBOX_FLAGS_G) + P.rank, SHARD_POISON);
+        st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[q] + INBOX_FLAGS_BIGG) + P.rank, SHARD_POISON);
+        st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[P.rank] + INBOX_FLAGS_G) + q, SHARD_POISON);
+        st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[P.rank] + INBOX_FLAGS_BIGG) + q, SHARD_POISON);
+    }
+    if (threadIdx.x == 0) {
+        atomicOr(&P.st->gridbar, BAR_FAULT);
+        h->fault = 1;
+    }
+    __syncthreads();
+}
+
 // g_s: this slab's partial gradient on entry (every CTA of the rank holds the same), the sum over the ranks on exit.
-// fp32 partials, added in fp64 in rank order, rounded once.  All NTHREADS threads call it.
-__device__ __forceinline__ void shard_sum_gradient(const DevPlan& P, SmemHeader* h, float* g_s, unsigned long long seq) {
+// fp32 partials, added in fp64 in rank order, rounded once.  All NTHREADS threads call it.  false: a peer did not answer.
+__device__ __forceinline__ bool shard_sum_gradient(const DevPlan& P, SmemHeader* h, float* g_s, unsigned long long seq,
+                                                   unsigned long long timeout_ns) {
     const int nbp = inbox_nb_pad(P.n_b), par = (int)(seq & 1ull);
     if (h->cta == 0) {
         for (int q = 0; q < P.world; ++q) {
@@ -1073,11 +1114,12 @@ __device__ __forceinline__ void shard_sum_gradient(const DevPlan& P, SmemHeader*
         if ((int)threadIdx.x < P.world)
             st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[threadIdx.x] + INBOX_FLAGS_G) + P.rank, seq);
     }
+    bool ok = true;
     if ((int)threadIdx.x < P.world) {
         const unsigned long long* f = reinterpret_cast<const unsigned long long*>(P.inbox[P.rank] + INBOX_FLAGS_G) + threadIdx.x;
-        while (ld_acquire_sys(f) < seq) {}
+        ok = shard_wait(f, seq, timeout_ns);
     }
-    __syncthreads();
+    if (__syncthreads_or(!ok)) { shard_give_up(P, h); return false; }
     const float* src = reinterpret_cast<const float*>(P.inbox[P.rank] + INBOX_G) + (size_t)par * P.world * nbp;
     for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) {
         double sum = 0.0;
@@ -1085,11 +1127,14 @@ __device__ __forceinline__ void shard_sum_gradient(const DevPlan& P, SmemHeader*
         g_s[i] = (float)sum;
     }
     __syncthreads();
+    return true;
 }
 
 // G: this slab's R partial objectives on entry (the same in every thread of every CTA of the rank), the sums on exit.
+// false: a peer did not answer.
 template <int R>
-__device__ __forceinline__ void shard_sum_objective(const DevPlan& P, SmemHeader* h, double (&G)[R], unsigned long long seq) {
+__device__ __forceinline__ bool shard_sum_objective(const DevPlan& P, SmemHeader* h, double (&G)[R], unsigned long long seq,
+                                                    unsigned long long timeout_ns) {
     const int par = (int)(seq & 1ull);
     if (h->cta == 0 && (int)threadIdx.x < P.world) {
         const int q = threadIdx.x;
@@ -1098,11 +1143,12 @@ __device__ __forceinline__ void shard_sum_objective(const DevPlan& P, SmemHeader
         for (int r = 0; r < R; ++r) dst[r] = G[r];
         st_release_sys(reinterpret_cast<unsigned long long*>(P.inbox[q] + INBOX_FLAGS_BIGG) + P.rank, seq);   // the same thread wrote the data
     }
+    bool ok = true;
     if ((int)threadIdx.x < P.world) {
         const unsigned long long* f = reinterpret_cast<const unsigned long long*>(P.inbox[P.rank] + INBOX_FLAGS_BIGG) + threadIdx.x;
-        while (ld_acquire_sys(f) < seq) {}
+        ok = shard_wait(f, seq, timeout_ns);
     }
-    __syncthreads();
+    if (__syncthreads_or(!ok)) { shard_give_up(P, h); return false; }
     const double* src = reinterpret_cast<const double*>(P.inbox[P.rank] + INBOX_BIGG) + (size_t)par * MAX_WORLD * R_MAX;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -1110,6 +1156,7 @@ __device__ __forceinline__ void shard_sum_objective(const DevPlan& P, SmemHeader
         for (int q = 0; q < P.world; ++q) sum += __ldcg(src + (size_t)q * R_MAX + r);              // rank order
         G[r] = sum;
     }
+    return true;
 }
 
 // ------------------------------------------------------------------------------------------------ scalar logic
@@ -1475,10 +1522,12 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
     float* xs = reinterpret_cast<float*>(imrt_smem + P.x_off);     // the R trial points (the dose pass gathers from them)
     float* g_s = reinterpret_cast<float*>(imrt_smem + P.g_off);
     State* st = P.st;
+    if (st->fault) return;                 // a wait of an earlier launch gave up: nothing runs until imrt_plan_set_x
     cta_init(h, P, table_s, cta, n_cta);
     if (threadIdx.x == 0) h->lc = loop_const(st);
     __syncthreads();
     const LoopConst& C = h->lc;
+    // h->fault (shared, block-uniform after every wait): a bounded wait gave up -- leave without touching another barrier
     Loop L;
     loop_load(st, L);
     const int iter_target = C.iter_target;
@@ -1487,16 +1536,16 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
     const bool sharded = P.world > 1;
     if (sharded && st->G_is_local) {       // G(x_1) of imrt_plan_set_x is this slab's share: make it the sum over the ranks
         double G1[1] = {L.G_k};
-        shard_sum_objective<1>(P, h, G1, ++L.seq_G);
+        const bool ok = shard_sum_objective<1>(P, h, G1, ++L.seq_G, C.spin_timeout_ns);
         L.G_k = G1[0];
-        if (h->cta == 0 && threadIdx.x == 0) P.tr_obj[0] = G1[0];
+        if (ok && h->cta == 0 && threadIdx.x == 0) P.tr_obj[0] = G1[0];
     }
     Pipe pipe = {0u, 0u};
     unsigned int epoch = 0;
     const bool rec = (h->cta == 0) && (threadIdx.x == 0);
 
     bool g_valid = false;                  // g_s holds the gradient of the current iterate (a transpose pass ran in this launch)
-    while (L.iter < iter_target) {
+    while (!h->fault && L.iter < iter_target) {
         const int tpar = (int)(L.tr & 1);
         // The transpose stages overlay xs and g_s (DevPlan::tr_stage_off = x_off).  Everybody is done with both -- the
         // publish loop below read xs, trial_batch / reduce_gradient wrote them through the generic proxy -- before the
@@ -1504,11 +1553,11 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
         fence_proxy_async_smem();
         __syncthreads();
         transpose_pass(P, h, imrt_smem, wpart, P.rbuf[L.ri], P.gslot[tpar], pipe);
-        grid_barrier(&st->gridbar, epoch, h->n_cta);
+        if (grid_barrier(&st->gridbar, epoch, h->n_cta, C.spin_timeout_ns, &h->fault)) break;
         reduce_gradient(P, P.gslot[tpar], g_s);
         g_valid = true;
         __syncthreads();
-        if (sharded) shard_sum_gradient(P, h, g_s, ++L.seq_g);      // exchange step 1: g = sum over the row slabs
+        if (sharded && !shard_sum_gradient(P, h, g_s, ++L.seq_g, C.spin_timeout_ns)) break;   // exchange step 1: g = sum over the row slabs
         // start of the line search (PAPER.md:109 step 2; the same decisions begin_line_search takes, with the first
         // trial's Delta taken from the batch that is built anyway).  x_k lives in global memory.
         L.tr += 1;
@@ -1526,9 +1575,11 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
             for (int j = 0; j < R; ++j) r_out[j] = P.rbuf[(L.ri + 1 + j) % (R + 1)];
             const int fpar = (int)(L.fwd & 1);
             dose_pass<R>(P, h, imrt_smem, table_s, xs, r_out, nullptr, P.Gpart[fpar], pipe);
-            grid_barrier(&st->gridbar, epoch, h->n_cta);
+            if (grid_barrier(&st->gridbar, epoch, h->n_cta, C.spin_timeout_ns, &h->fault)) { dec = DEC_REJECT_STOP; break; }
             reduce_objective<R>(P, P.Gpart[fpar], h, G_new, C.G_skip);
-            if (sharded) shard_sum_objective<R>(P, h, G_new, ++L.seq_G);      // exchange step 2: G = sum over the row slabs
+            if (sharded && !shard_sum_objective<R>(P, h, G_new, ++L.seq_G, C.spin_timeout_ns)) {      // exchange step 2: G = sum over the row slabs
+                dec = DEC_REJECT_STOP; break;
+            }
             dec = armijo_decide<R>(P, C, L, G_new, step_sq, rec, j_acc);
             if (dec != DEC_REJECT_RETRY) break;
         }
@@ -1543,7 +1594,18 @@ __device__ __forceinline__ void persistent_loop(const DevPlan& P, int cta, int n
         if (dec != DEC_ACCEPT_CONTINUE) break;
     }
     // every CTA has passed the last grid barrier before CTA 0 gets here with a changed state
-    grid_barrier(&st->gridbar, epoch, h->n_cta);
+    if (!h->fault) grid_barrier(&st->gridbar, epoch, h->n_cta, C.spin_timeout_ns, &h->fault);
+    if (h->fault) {
+        // Failure exit: some CTA of this rank, or a peer rank, did not show up within the bound.  The
+        // iterate buffers may be half written: the plan refuses to run until the next imrt_plan_set_x (State::fault).
+        if (h->cta == 0 && threadIdx.x == 0) {
+            st->fault = 1;
+            st->stop_reason = STOP_PEER_TIMEOUT;
+            st->cont_outer = 0;
+            st->cont_inner = 0;
+        }
+        return;
+    }
     if (h->cta == 0) {
         if (g_valid)                       // a launch that did no iteration leaves P.g as it was
             for (int i = threadIdx.x; i < P.n_b; i += NTHREADS) P.g[i] = g_s[i];

@@ -29,6 +29,23 @@ __global__ void k_merge_keys(const int* __restrict__ group, int n_v, int n_group
     if (bad) flags[0] = 1;
 }
 
+// The raw CSR is checked here, BEFORE imrt_plan_create ever sees it (merging runs first): flags[1] = row_ptr does not start at
+// 0 or decreases somewhere; flags[2] = a column outside [0, n_b) (it would index past the shared-memory bitmap below).
+__global__ void k_merge_check_row_ptr(const int* __restrict__ row_ptr, int n_v, int* flags) {
+    int bad = 0;
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n_v; j += gridDim.x * blockDim.x)
+        bad |= (row_ptr[j] > row_ptr[j + 1]) | (j == 0 && row_ptr[0] != 0);
+    if (bad) flags[1] = 1;
+}
+__global__ void k_merge_check_cols(const int* __restrict__ row_ptr, const int* __restrict__ col, int n_v, int n_b, int* flags) {
+    if (flags[1]) return;                            // row_ptr cannot be trusted: do not follow it
+    const int lane = threadIdx.x & 31, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    int bad = 0;
+    for (int j = warp; j < n_v; j += n_warps)
+        for (int p = row_ptr[j] + lane; p < row_ptr[j + 1]; p += 32) bad |= (col[p] < 0) | (col[p] >= n_b);
+    if (bad) flags[2] = 1;
+}
+
 // group_ptr[g] = first position of the sorted keys that is >= g
 __global__ void k_merge_group_ptr(const unsigned int* __restrict__ keys, int n_v, int n_groups, int* group_ptr) {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;

@@ -112,24 +112,47 @@ __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
 }
 
 // ---------------------------------------------------------------------------------------------- grid barrier
+__device__ __forceinline__ unsigned long long spin_clock_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
 // Monotone-counter barrier for a cooperative (co-resident) launch over the n_cta CTAs that share `counter` (the whole
 // grid, or one rank's CTAs when several plans share a launch).  Every CTA calls it the same number of times;
 // `epoch` counts the calls (kept in a register by the caller).  counter must be 0 at kernel start.
 // Release / acquire at gpu scope: the arrival is a red.release (the CTA's earlier writes, ordered before it by the
 // bar.sync, become visible to whoever acquires the count), the wait an ld.acquire spin (SASS: LDG.STRONG.GPU followed by
 // CCTL.IVALL, so the other threads' plain loads after the closing bar.sync cannot hit stale L1 lines).  No full fences.
-__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, int n_cta) {
+//
+// The wait is BOUNDED: after timeout_ns without the count being reached, the waiter sets BAR_FAULT in the counter --
+// which makes every present and future wait on it return at once -- and the call returns true ("the run is faulted") in
+// every thread of every CTA that passes the barrier from then on.  Anybody else who detects a fault (a lost peer rank,
+// shard_wait) sets the same bit.  The caller leaves its loop without touching another barrier.  *fault_s: one int of
+// shared memory, 0 at kernel start.  The counter stays far below 2^31 in a fault-free launch (barriers x CTAs).
+constexpr unsigned int BAR_FAULT = 0x80000000u;
+__device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int& epoch, int n_cta, unsigned long long timeout_ns,
+                                             volatile int* fault_s) {
     __syncthreads();
     ++epoch;
     if (threadIdx.x == 0) {
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
         const unsigned int target = epoch * (unsigned int)n_cta;
-        unsigned int seen;
-        do {
+        unsigned int seen, polls = 0u;
+        unsigned long long t0 = 0ull;
+        for (;;) {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
-        } while (seen < target);
+            if (seen >= target) break;                       // also true once BAR_FAULT is set
+            if ((++polls & 255u) == 0u) {                    // look at the clock once in a while only
+                const unsigned long long now = spin_clock_ns();
+                if (t0 == 0ull) t0 = now;
+                else if (now - t0 > timeout_ns) { atomicOr(counter, BAR_FAULT); seen = BAR_FAULT; break; }
+            }
+        }
+        if (seen & BAR_FAULT) *fault_s = 1;
     }
     __syncthreads();
+    return *fault_s != 0;
 }
 
 }  // namespace imrt

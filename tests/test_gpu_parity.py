@@ -609,3 +609,20 @@ def test_merge_rows_matches_oracle_bit_for_bit(m, seed, n_v, n_b, n_groups):
     bad[0] = n_groups
     with pytest.raises(m.ImrtError):
         m.imrt_merge_rows(n_b, dev(prob.row_ptr), dev(prob.col), dev(prob.val), dev(bad), n_groups)
+    # the raw CSR is validated here too (merging runs before imrt_plan_create): a column outside [0, n_b) must not reach the
+    # shared-memory column bitmap, a decreasing row_ptr must not be followed
+    if prob.col.size:
+        bad_col = prob.col.copy()
+        bad_col[bad_col.size // 2] = n_b
+        with pytest.raises(m.ImrtError) as e:
+            m.imrt_merge_rows(n_b, dev(prob.row_ptr), dev(bad_col), dev(prob.val), dev(group), n_groups)
+        assert e.value.status_name == "BAD_CSR"
+        bad_col[bad_col.size // 2] = -1
+        with pytest.raises(m.ImrtError) as e:
+            m.imrt_merge_rows(n_b, dev(prob.row_ptr), dev(bad_col), dev(prob.val), dev(group), n_groups)
+        assert e.value.status_name == "BAD_CSR"
+    bad_rp = prob.row_ptr.copy()
+    bad_rp[n_v // 2] = bad_rp[-1] + 7
+    with pytest.raises(m.ImrtError) as e:
+        m.imrt_merge_rows(n_b, dev(bad_rp), dev(prob.col), dev(prob.val), dev(group), n_groups)
+    assert e.value.status_name == "BAD_CSR"

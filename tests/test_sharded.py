@@ -227,3 +227,59 @@ def test_sharded_run_to_tolerance_and_refusals():
     with pytest.raises(m.ImrtError):
         m.imrt_plan_set_shard(solo.handle, 0, 2, [16, 32])           # persistent driver only
     solo.close()
+
+
+@pytest.mark.gpu
+def test_a_lost_peer_ends_the_run_with_a_status_instead_of_hanging_the_device():
+    # SURVEY.md section 5 (failure detection): every wait inside the persistent kernel is bounded (imrt_options.spin_timeout_ms).
+    # Rank 0 of a 2-rank group is launched ALONE (imrt_plan_run_iters on one plan of the pair): its peer never pushes a partial
+    # sum, so rank 0 must give up after the bound, report IMRT_STOP_PEER_TIMEOUT and refuse to run on until it is set up again.
+    import time
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_0908_4421_b200 as m
+    prob = synth_inputs.make_phantom(0)
+    ranks = sharded.CoResidentRanks(prob, 2, max_iters=20, spin_timeout_ms=300)
+    ranks.set_x(prob.x0)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ranks.plans[0].run_iters(5)                          # the peer's CTAs are not in this launch
+    tr = ranks.plans[0].trace()                          # synchronises
+    waited = time.perf_counter() - t0
+    assert m.STOP_NAMES[tr.stop_reason] == "PEER_TIMEOUT" and tr.n_iters == 0
+    assert 0.25 <= waited < 5.0, waited
+    ranks.plans[0].run_iters(5)                          # refused on the device, at once: the iterate is not valid any more
+    t1 = time.perf_counter()
+    tr = ranks.plans[0].trace()
+    assert m.STOP_NAMES[tr.stop_reason] == "PEER_TIMEOUT" and tr.n_iters == 0 and time.perf_counter() - t1 < 0.2
+    # the give-up was written into the peer's inbox as well: launched now, rank 1 stops at once rather than after its own bound
+    t2 = time.perf_counter()
+    ranks.plans[1].run_iters(5)
+    tr1 = ranks.plans[1].trace()
+    assert m.STOP_NAMES[tr1.stop_reason] == "PEER_TIMEOUT" and time.perf_counter() - t2 < 0.2
+    # recovery: zero the inboxes, set the group up again, set x -- and the pair runs as if nothing had happened
+    for box in ranks.inboxes:
+        box.zero_()
+    ptrs = [t.data_ptr() for t in ranks.inboxes]
+    for q, p in enumerate(ranks.plans):
+        m.imrt_plan_set_shard(p.handle, q, 2, ptrs)
+    ranks.set_x(prob.x0)
+    ranks.run_iters(20)
+    tr = ranks.trace()
+    fresh = sharded.CoResidentRanks(prob, 2, max_iters=20)
+    fresh.set_x(prob.x0)
+    fresh.run_iters(20)
+    assert tr.n_iters == 20 and tr.stop_reason == oracle.STOP_MAX_ITERS
+    np.testing.assert_array_equal(tr.obj, fresh.trace().obj)
+    np.testing.assert_array_equal(ranks.get_x().cpu().numpy(), fresh.get_x().cpu().numpy())
+    # a refused imrt_plan_set_shard (misaligned inbox) changes nothing: the group still runs
+    with pytest.raises(m.ImrtError):
+        m.imrt_plan_set_shard(ranks.plans[0].handle, 0, 2, [ptrs[0], ptrs[1] + 4])
+    # ranks that disagree on the trace capacity are refused before anything is launched
+    odd = sharded.CoResidentRanks(prob, 2, max_iters=21)
+    odd.set_x(prob.x0)
+    with pytest.raises(m.ImrtError):
+        m.imrt_plan_run_ranks([fresh.plans[0].handle, odd.plans[1].handle], 1)
+    for r in (ranks, fresh, odd):
+        r.close()
